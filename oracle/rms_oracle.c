@@ -1,0 +1,519 @@
+/*
+ * rms_oracle.c -- TEST INFRASTRUCTURE, NOT THE PRODUCT.
+ *
+ * Plain, slow, single-walker-at-a-time fp64 CPU oracle of the hot path of the
+ * Realistic Microstructure Simulator (arXiv 2012.06478): the Monte Carlo random
+ * walk through a 3d voxelised label lattice with elastic reflection / permeation,
+ * PGSE phase, T2 weight and the final signal / moment sums.
+ *
+ * Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / reference
+ * legs may call this.  It shares no code, header, table or constant generator
+ * with the CUDA path under paper_2012_06478_b200/csrc; the two only agree on
+ * the counter scheme of the random numbers.
+ *
+ * Citations: "P:<n>" is a line of /root/reference/PAPER.md, with the section /
+ * equation it falls in.  "R<n>" is a numbered reading in DESIGN.md (where the
+ * paper is silent).
+ *
+ * Pins (tests/test_oracle_*.py, all "-m 'not gpu'"):
+ *   philox4x32_10        known-answer vectors (tests/golden/philox4x32_10_kat.txt)
+ *   direction            <u>=0, <u_k^2>=1/3, <u_k^4>=1/5, |u|=1, z<->-z symmetry
+ *   tables               ds=0.049 um, Eq.3 = Eq.2a/(1+alpha),
+ *                        P12/P21 = sqrt(D2/D1)
+ *   step                 brute-force sub-stepped ray march on tiny random lattices,
+ *                        all reflect/pass outcomes forced
+ *   run, free            <X^2>=2Dt exactly in expectation, K=-6/(5N), S=prod sinc
+ *   run, plates          closed-form narrow-pulse S(q,t) and <X^2>(t)
+ *   run, equilibrium     uniform density kept with D contrast and permeable walls
+ *                        (P:78), exchange between slabs vs. the eigen-series
+ *   run, T2              alpha = exp(-t/T2) exactly for a single compartment (Eq.5)
+ * Parity unpinned: wide-pulse signals inside voxelised cylinders / axons have
+ *   no closed form; they are pinned only through the pieces above.
+ */
+#include <math.h>
+#include <pthread.h>
+#include <stdint.h>
+#include <stdlib.h>
+#include <string.h>
+
+#define ORC_OK 0
+#define ORC_ERR_ARG -1
+#define ORC_ERR_STEP_TOO_LARGE -2
+#define ORC_ERR_P_RANGE -3
+#define ORC_ERR_NO_SPACE -4
+#define ORC_ERR_OOM -5
+
+#define ORC_MAX_INIT_ATTEMPTS (1u << 20)
+
+/* ------------------------------------------------------------------------- */
+/* Philox4x32-10 (Salmon, Moraes, Dror, Shaw, SC'11).  R2: the paper names no  */
+/* generator; north_star fixes this one, keyed on (seed, walker, step).        */
+/* ------------------------------------------------------------------------- */
+void rms_oracle_philox4x32_10(const uint32_t ctr[4], const uint32_t key[2], uint32_t out[4])
+{
+    uint32_t c0 = ctr[0], c1 = ctr[1], c2 = ctr[2], c3 = ctr[3];
+    uint32_t k0 = key[0], k1 = key[1];
+    for (int round = 0; round < 10; ++round) {
+        uint64_t p0 = (uint64_t)0xD2511F53u * c0; /* hi0:lo0 */
+        uint64_t p1 = (uint64_t)0xCD9E8D57u * c2; /* hi1:lo1 */
+        uint32_t hi0 = (uint32_t)(p0 >> 32), lo0 = (uint32_t)p0;
+        uint32_t hi1 = (uint32_t)(p1 >> 32), lo1 = (uint32_t)p1;
+        uint32_t n0 = hi1 ^ c1 ^ k0;
+        uint32_t n1 = lo1;
+        uint32_t n2 = hi0 ^ c3 ^ k1;
+        uint32_t n3 = lo0;
+        c0 = n0; c1 = n1; c2 = n2; c3 = n3;
+        k0 += 0x9E3779B9u;
+        k1 += 0xBB67AE85u;
+    }
+    out[0] = c0; out[1] = c1; out[2] = c2; out[3] = c3;
+}
+
+/* Counter layout (R2): key = (seed_lo, seed_hi); ctr = (walker_lo, walker_hi, index, stream). */
+enum { STREAM_INIT = 0, STREAM_DIR = 1, STREAM_PERM = 2, STREAM_INIT_OFFSET = 3 };
+
+static void draw(uint64_t seed, uint64_t walker, uint32_t index, uint32_t stream, uint32_t out[4])
+{
+    uint32_t ctr[4] = { (uint32_t)walker, (uint32_t)(walker >> 32), index, stream };
+    uint32_t key[2] = { (uint32_t)seed, (uint32_t)(seed >> 32) };
+    rms_oracle_philox4x32_10(ctr, key, out);
+}
+
+/* R3: words -> reals, all exactly representable in fp32 as well as fp64.
+ * sym(w) = (2*(w>>9) + 1 - 2^23) * 2^-23  in (-1,1), symmetric, never 0 or +-1.
+ * uni(w) = (w>>8) * 2^-24                 in [0,1). */
+static double sym(uint32_t w) { return ((double)(2 * (int64_t)(w >> 9) + 1 - 8388608)) / 8388608.0; }
+static double uni(uint32_t w) { return (double)(w >> 8) / 16777216.0; }
+
+/* R4 ("random direction in 3d"): z uniform in (-1,1), azimuth psi = pi*sym(wb)
+ * (Archimedes' hat-box theorem => uniform on the sphere). */
+void rms_oracle_direction(uint32_t wa, uint32_t wb, double u[3])
+{
+    const double pi = 3.14159265358979323846;
+    double z = sym(wa);
+    double psi = pi * sym(wb);
+    double rho = sqrt(1.0 - z * z);
+    u[0] = rho * cos(psi);
+    u[1] = rho * sin(psi);
+    u[2] = z;
+}
+
+/* Direction words of absolute 1-based step i (R2): one Philox call serves two steps. */
+static void direction_words(uint64_t seed, uint64_t walker, int64_t step, uint32_t* wa, uint32_t* wb)
+{
+    uint32_t w[4];
+    draw(seed, walker, (uint32_t)((step - 1) >> 1), STREAM_DIR, w);
+    if (step & 1) { *wa = w[0]; *wb = w[1]; } else { *wa = w[2]; *wb = w[3]; }
+}
+
+/* Permeation uniforms of step i (R5): 33-bit uniforms u_e = (c_e + uni(v_e)) / 512 for the
+ * e-th unlike-label encounter of the step, e = 0,1,2.  The 9 coarse bits c_0, c_1 are the
+ * low 9 bits of the step's two direction words (unused by sym); c_2 = v_3 & 511.
+ * v_0..v_3 = Philox(walker, index = step, stream PERM). */
+static void permeation_uniforms(uint64_t seed, uint64_t walker, int64_t step, uint32_t wa, uint32_t wb, double u[3])
+{
+    uint32_t v[4];
+    draw(seed, walker, (uint32_t)step, STREAM_PERM, v);
+    u[0] = ((double)(wa & 511u) + uni(v[0])) / 512.0;
+    u[1] = ((double)(wb & 511u) + uni(v[1])) / 512.0;
+    u[2] = ((double)(v[3] & 511u) + uni(v[2])) / 512.0;
+}
+
+/* ------------------------------------------------------------------------- */
+/* Tables (Eq.1, Eq.2-3, P:678-681 Eq.C.15).                    */
+/* s[L]  = sqrt(6 D_L dt) / l_p : hop length in voxel units (d = 3).           */
+/* P[a][b] permeation probability from label a into label b.                   */
+/* Both are rounded once to fp32-representable values (R6).                    */
+/* ------------------------------------------------------------------------- */
+int rms_oracle_tables(int n_labels, const float* D, const float* kappa, double voxel_um, double dt_ms,
+                      double* s_out, double* P_out)
+{
+    const double C3 = 2.0 / 3.0; /* Eq.2b, d = 3 */
+    if (n_labels <= 0 || !D || !(voxel_um > 0) || !(dt_ms > 0)) return ORC_ERR_ARG;
+    for (int a = 0; a < n_labels; ++a) {
+        if (!(D[a] > 0)) return ORC_ERR_ARG;
+        double s = sqrt(6.0 * (double)D[a] * dt_ms) / voxel_um; /* Eq.1 */
+        s_out[a] = (double)(float)s;
+        if (!(s_out[a] < 1.0)) return ORC_ERR_STEP_TOO_LARGE;   /* ds < l_p */
+    }
+    if (!P_out) return ORC_OK;
+    for (int a = 0; a < n_labels; ++a) {
+        for (int b = 0; b < n_labels; ++b) {
+            double P;
+            if (a == b) {
+                P = 1.0;
+            } else {
+                double k = kappa ? (double)kappa[a * n_labels + b] : 0.0;
+                double Da = D[a], Db = D[b];
+                if (k < 0 || k != k) return ORC_ERR_ARG;
+                if (k == 0.0) {
+                    P = 0.0;
+                } else if (isinf(k)) {
+                    /* no membrane between media of different D: Eq.C.15 with c1 = c2 */
+                    P = sqrt(Db / Da);
+                    if (P > 1.0) P = 1.0;
+                } else {
+                    double Aab = k * sqrt(6.0 * dt_ms / Da) * C3; /* kappa ds_a / D_a C_d, Eq.2a */
+                    double Aba = k * sqrt(6.0 * dt_ms / Db) * C3;
+                    P = Aab / (1.0 + 0.5 * (Aab + Aba));          /* Eq.3 */
+                    if (P > 1.0) return ORC_ERR_P_RANGE;          /* R9 */
+                }
+            }
+            P_out[a * n_labels + b] = (double)(float)P;
+        }
+    }
+    return ORC_OK;
+}
+
+/* ------------------------------------------------------------------------- */
+/* One Monte Carlo step (P:152-159 steps 2-4; Fig.2).         */
+/* Coordinates in voxel units: unwrapped voxel vox[3], offset off[3] in [0,1). */
+/* u[3] unit direction, up[3] permeation uniforms for encounters 0,1,2.        */
+/* ------------------------------------------------------------------------- */
+typedef struct {
+    int nx, ny, nz;
+    const uint16_t* labels;
+    int n_labels;
+    const double* s; /* [n_labels] */
+    const double* P; /* [n_labels^2] */
+} lattice_t;
+
+static int wrap(int64_t a, int n) { int64_t m = a % n; return (int)(m < 0 ? m + n : m); }
+
+static uint16_t label_at(const lattice_t* lat, const int32_t v[3])
+{
+    int x = wrap(v[0], lat->nx), y = wrap(v[1], lat->ny), z = wrap(v[2], lat->nz); /* R1: periodic box */
+    return lat->labels[((size_t)z * lat->ny + y) * lat->nx + x];
+}
+
+/* permeation uniforms are drawn only when a membrane with 0 < P < 1 is met (same values either way) */
+typedef struct { uint64_t seed, walker; int64_t step; uint32_t wa, wb; int have; double u[3]; } perm_src_t;
+
+static double perm_uniform(perm_src_t* ps, int e)
+{
+    if (!ps->have) { permeation_uniforms(ps->seed, ps->walker, ps->step, ps->wa, ps->wb, ps->u); ps->have = 1; }
+    return ps->u[e < 3 ? e : 2];
+}
+
+static void step_core(const lattice_t* lat, int32_t vox[3], double off[3], uint16_t* label,
+                      const double u[3], perm_src_t* ps, int* n_enc, int* n_perm, int* n_clamp)
+{
+    uint16_t L = *label;
+    double r[3], p[3];
+    int done[3] = { 0, 0, 0 };
+    int e = 0;
+    for (int k = 0; k < 3; ++k) { r[k] = lat->s[L] * u[k]; p[k] = off[k]; } /* R8: ds of the label at the start */
+
+    for (int it = 0; it < 3; ++it) { /* at most three interactions */
+        int kstar = -1;
+        double tmin = 0.0;
+        for (int k = 0; k < 3; ++k) {
+            if (done[k]) continue;
+            double g = p[k] + r[k];
+            if (g >= 1.0 || g < 0.0) {
+                double t = ((r[k] > 0.0 ? 1.0 : 0.0) - p[k]) / r[k];
+                if (kstar < 0 || t < tmin) { kstar = k; tmin = t; } /* R10: ties -> lowest axis */
+            }
+        }
+        if (kstar < 0) break;
+        int sigma = r[kstar] > 0.0 ? 1 : -1;
+        for (int k = 0; k < 3; ++k) { p[k] += tmin * r[k]; r[k] *= (1.0 - tmin); }
+        p[kstar] = sigma > 0 ? 1.0 : 0.0; /* exactly on the face */
+
+        int32_t nb[3] = { vox[0], vox[1], vox[2] };
+        nb[kstar] += sigma;
+        uint16_t Ln = label_at(lat, nb);
+        int pass;
+        if (Ln == L) {
+            pass = 1; /* face between voxels of one compartment is no membrane */
+        } else {
+            double P = lat->P[(size_t)L * lat->n_labels + Ln];
+            ++*n_enc;
+            pass = (P >= 1.0) || (P > 0.0 && perm_uniform(ps, e) < P); /* permeate with probability P */
+            ++e;
+            if (pass) ++*n_perm;
+        }
+        if (pass) {
+            vox[kstar] += sigma;
+            p[kstar] = sigma > 0 ? 0.0 : 1.0;
+            if (Ln != L) {
+                double scale = lat->s[Ln] / lat->s[L]; /* R7: rest of dt is spent at the new speed */
+                for (int k = 0; k < 3; ++k) r[k] *= scale;
+                L = Ln;
+            }
+        } else {
+            r[kstar] = -r[kstar]; /* elastic collision on the face plane */
+        }
+        done[kstar] = 1;
+    }
+    for (int k = 0; k < 3; ++k) {
+        double f = p[k] + r[k];
+        const double fmax = 1.0 - 1.0 / 9007199254740992.0; /* 1 - 2^-53 */
+        if (f < 0.0) { f = 0.0; ++*n_clamp; }
+        if (f > fmax) { f = fmax; ++*n_clamp; }
+        off[k] = f;
+    }
+    *label = L;
+}
+
+/* Exported single step, for the brute-force pins.  s[n_labels], P[n_labels^2] given directly. */
+int rms_oracle_step(int nx, int ny, int nz, const uint16_t* labels, int n_labels, const double* s, const double* P,
+                    int32_t vox[3], double off[3], uint16_t* label, const double u[3], const double up[3],
+                    int32_t counts[3])
+{
+    lattice_t lat = { nx, ny, nz, labels, n_labels, s, P };
+    int ne = 0, np = 0, nc = 0;
+    perm_src_t ps = { 0, 0, 0, 0, 0, 1, { up[0], up[1], up[2] } };
+    step_core(&lat, vox, off, label, u, &ps, &ne, &np, &nc);
+    counts[0] = ne; counts[1] = np; counts[2] = nc;
+    return ORC_OK;
+}
+
+/* Walker initialisation (P:151 step 1; R13): rejection sampling of a uniform voxel until its label
+ * is allowed, then a uniform in-voxel offset.  Integer arithmetic: v = floor(uni(w) * n). */
+int rms_oracle_init_walker(int nx, int ny, int nz, const uint16_t* labels, const uint8_t* label_allowed,
+                           uint64_t seed, uint64_t walker, int32_t vox[3], double off[3], uint16_t* label)
+{
+    uint32_t w[4];
+    for (uint32_t a = 0; a < ORC_MAX_INIT_ATTEMPTS; ++a) {
+        draw(seed, walker, a, STREAM_INIT, w);
+        int x = (int)(((uint64_t)(w[0] >> 8) * (uint64_t)nx) >> 24);
+        int y = (int)(((uint64_t)(w[1] >> 8) * (uint64_t)ny) >> 24);
+        int z = (int)(((uint64_t)(w[2] >> 8) * (uint64_t)nz) >> 24);
+        uint16_t L = labels[((size_t)z * ny + y) * nx + x];
+        if (label_allowed && !label_allowed[L]) continue;
+        vox[0] = x; vox[1] = y; vox[2] = z;
+        *label = L;
+        draw(seed, walker, 0, STREAM_INIT_OFFSET, w);
+        off[0] = uni(w[0]); off[1] = uni(w[1]); off[2] = uni(w[2]);
+        return ORC_OK;
+    }
+    return ORC_ERR_NO_SPACE;
+}
+
+/* ------------------------------------------------------------------------- */
+/* Whole run: init -> n_steps steps -> sums (Eq.5, Eq.7).           */
+/* ------------------------------------------------------------------------- */
+typedef struct {
+    /* substrate */
+    lattice_t lat;
+    double voxel_um;
+    const double* inv_T2; /* [n_labels], 0 = no relaxation */
+    const uint8_t* label_class;
+    int n_classes;
+    /* walkers */
+    uint64_t n_walkers, first_id, seed;
+    const uint8_t* label_allowed;
+    /* run */
+    double dt;
+    int64_t n_steps;
+    int n_wave; const float* wave;
+    int n_g; const double* gamp;
+    int n_dir; const double* dirs;
+    int n_snap; const int64_t* snap_steps;
+    /* per-walker outputs (optional) */
+    int32_t* final_vox; double* final_off; uint16_t* final_label;
+    int32_t* init_vox; double* init_off; double* phi; double* relax;
+} job_t;
+
+typedef struct {
+    const job_t* job;
+    uint64_t w_begin, w_end; /* indices into [0, n_walkers) */
+    double *sum_alpha, *sig_re, *sig_im, *m2, *m4, *snap_alpha;
+    uint64_t* class_flow;
+    uint64_t counters[4];
+    int status;
+} part_t;
+
+static size_t n_sig(const job_t* j) { return (size_t)j->n_wave * j->n_g * j->n_dir * j->n_classes; }
+static size_t n_mom(const job_t* j) { return (size_t)j->n_snap * j->n_dir * j->n_classes; }
+static size_t n_sal(const job_t* j) { return (size_t)j->n_snap * j->n_classes; }
+static size_t n_flow(const job_t* j) { return (size_t)j->n_snap * j->n_classes * j->n_classes; }
+
+static void* run_part(void* arg)
+{
+    part_t* pt = (part_t*)arg;
+    const job_t* j = pt->job;
+    const lattice_t* lat = &j->lat;
+    double* Phi = (double*)malloc(sizeof(double) * 3 * (size_t)(j->n_wave > 0 ? j->n_wave : 1));
+    if (!Phi) { pt->status = ORC_ERR_OOM; return NULL; }
+
+    for (uint64_t wi = pt->w_begin; wi < pt->w_end; ++wi) {
+        uint64_t id = j->first_id + wi;
+        int32_t v0[3], v[3];
+        double f0[3], f[3];
+        uint16_t L0, L;
+        int st = rms_oracle_init_walker(lat->nx, lat->ny, lat->nz, lat->labels, j->label_allowed, j->seed, id, v0, f0, &L0);
+        if (st != ORC_OK) { pt->status = st; break; }
+        memcpy(v, v0, sizeof v); memcpy(f, f0, sizeof f); L = L0;
+        int c0 = j->label_class ? j->label_class[L0] : 0;
+        double R = 0.0; /* sum_i t_i / T2^(i), Eq.5 */
+        for (int m = 0; m < 3 * j->n_wave; ++m) Phi[m] = 0.0;
+        int snap = 0;
+
+        for (int64_t i = 1; i <= j->n_steps; ++i) {
+            uint32_t wa, wb;
+            double u[3];
+            int ne = 0, np = 0, nc = 0;
+            direction_words(j->seed, id, i, &wa, &wb);
+            rms_oracle_direction(wa, wb, u);
+            perm_src_t ps = { j->seed, id, i, wa, wb, 0, { 0, 0, 0 } };
+            step_core(lat, v, f, &L, u, &ps, &ne, &np, &nc);
+            pt->counters[0] += (uint64_t)ne; pt->counters[1] += (uint64_t)np; pt->counters[2] += (uint64_t)nc;
+            if ((uint64_t)ne > pt->counters[3]) pt->counters[3] = (uint64_t)ne;
+
+            /* displacement in voxel units; the integer part is exact */
+            double dx[3];
+            for (int k = 0; k < 3; ++k) dx[k] = (double)(v[k] - v0[k]) + (f[k] - f0[k]);
+            /* Eq.7 phase, right-endpoint rule (R11): Phi_m += w_m[i] (x_i - x_0) */
+            for (int m = 0; m < j->n_wave; ++m) {
+                double w = (double)j->wave[(size_t)m * j->n_steps + (i - 1)];
+                for (int k = 0; k < 3; ++k) Phi[3 * m + k] += w * dx[k];
+            }
+            /* Eq.5: whole dt to the compartment at the end of the hop (R12) */
+            R += j->dt * j->inv_T2[L];
+
+            while (snap < j->n_snap && j->snap_steps[snap] == i) {
+                double alpha = exp(-R);
+                int cn = j->label_class ? j->label_class[L] : 0;
+                pt->snap_alpha[(size_t)snap * j->n_classes + c0] += alpha;
+                pt->class_flow[((size_t)snap * j->n_classes + c0) * j->n_classes + cn] += 1;
+                for (int d = 0; d < j->n_dir; ++d) {
+                    const double* n = j->dirs + 3 * d;
+                    double X = j->voxel_um * (n[0] * dx[0] + n[1] * dx[1] + n[2] * dx[2]);
+                    size_t o = ((size_t)snap * j->n_dir + d) * j->n_classes + c0;
+                    pt->m2[o] += alpha * X * X;
+                    pt->m4[o] += alpha * X * X * X * X;
+                }
+                ++snap;
+            }
+        }
+        /* signal sums, Eq.7: alpha e^{-i phi} */
+        double alpha = exp(-R);
+        pt->sum_alpha[c0] += alpha;
+        for (int m = 0; m < j->n_wave; ++m)
+            for (int g = 0; g < j->n_g; ++g)
+                for (int d = 0; d < j->n_dir; ++d) {
+                    const double* n = j->dirs + 3 * d;
+                    double proj = n[0] * Phi[3 * m] + n[1] * Phi[3 * m + 1] + n[2] * Phi[3 * m + 2];
+                    double ph = j->gamp[(size_t)m * j->n_g + g] * j->dt * j->voxel_um * proj;
+                    size_t o = (((size_t)m * j->n_g + g) * j->n_dir + d) * j->n_classes + c0;
+                    pt->sig_re[o] += alpha * cos(ph);
+                    pt->sig_im[o] -= alpha * sin(ph);
+                }
+        if (j->final_vox) memcpy(j->final_vox + 3 * wi, v, sizeof v);
+        if (j->final_off) memcpy(j->final_off + 3 * wi, f, sizeof f);
+        if (j->final_label) j->final_label[wi] = L;
+        if (j->init_vox) memcpy(j->init_vox + 3 * wi, v0, sizeof v0);
+        if (j->init_off) memcpy(j->init_off + 3 * wi, f0, sizeof f0);
+        if (j->phi) memcpy(j->phi + 3 * (size_t)j->n_wave * wi, Phi, sizeof(double) * 3 * (size_t)j->n_wave);
+        if (j->relax) j->relax[wi] = R;
+    }
+    free(Phi);
+    return NULL;
+}
+
+int rms_oracle_run(
+    int nx, int ny, int nz, double voxel_um, const uint16_t* labels, int n_labels,
+    const float* D, const float* T2, const float* kappa, const uint8_t* label_class, int n_classes,
+    uint64_t n_walkers, uint64_t first_id, const uint8_t* label_allowed, uint64_t seed,
+    double dt_ms, int64_t n_steps, int n_wave, const float* wave, int n_g, const double* gamp,
+    int n_dir, const double* dirs, int n_snap, const int64_t* snap_steps, int n_threads,
+    double* sum_alpha, double* sig_re, double* sig_im, double* m2, double* m4, double* snap_alpha,
+    uint64_t* class_flow, uint64_t* counters,
+    int32_t* final_vox, double* final_off, uint16_t* final_label,
+    int32_t* init_vox, double* init_off, double* phi, double* relax)
+{
+    if (nx <= 0 || ny <= 0 || nz <= 0 || !labels || n_labels <= 0 || n_classes <= 0 || n_steps < 0 ||
+        n_wave < 0 || n_g < 0 || n_dir < 0 || n_snap < 0 || !sum_alpha || !counters)
+        return ORC_ERR_ARG;
+    size_t nvox = (size_t)nx * ny * nz;
+    for (size_t i = 0; i < nvox; ++i) if (labels[i] >= n_labels) return ORC_ERR_ARG;
+    if (label_class) for (int a = 0; a < n_labels; ++a) if (label_class[a] >= n_classes) return ORC_ERR_ARG;
+    for (int s = 0; s < n_snap; ++s) {
+        if (snap_steps[s] < 1 || snap_steps[s] > n_steps) return ORC_ERR_ARG;
+        if (s > 0 && snap_steps[s] <= snap_steps[s - 1]) return ORC_ERR_ARG;
+    }
+    for (int d = 0; d < n_dir; ++d) {
+        const double* n = dirs + 3 * d;
+        if (fabs(n[0] * n[0] + n[1] * n[1] + n[2] * n[2] - 1.0) > 1e-6) return ORC_ERR_ARG;
+    }
+
+    double* s_tab = (double*)malloc(sizeof(double) * n_labels);
+    double* P_tab = (double*)malloc(sizeof(double) * (size_t)n_labels * n_labels);
+    double* inv_T2 = (double*)malloc(sizeof(double) * n_labels);
+    if (!s_tab || !P_tab || !inv_T2) { free(s_tab); free(P_tab); free(inv_T2); return ORC_ERR_OOM; }
+    int st = rms_oracle_tables(n_labels, D, kappa, voxel_um, dt_ms, s_tab, P_tab);
+    if (st != ORC_OK) { free(s_tab); free(P_tab); free(inv_T2); return st; }
+    for (int a = 0; a < n_labels; ++a) {
+        double t2 = T2 ? (double)T2[a] : 0.0;
+        inv_T2[a] = (t2 > 0.0 && !isinf(t2)) ? 1.0 / t2 : 0.0; /* T2 <= 0 or inf: no relaxation */
+    }
+
+    job_t job;
+    memset(&job, 0, sizeof job);
+    job.lat.nx = nx; job.lat.ny = ny; job.lat.nz = nz; job.lat.labels = labels; job.lat.n_labels = n_labels;
+    job.lat.s = s_tab; job.lat.P = P_tab;
+    job.voxel_um = voxel_um; job.inv_T2 = inv_T2; job.label_class = label_class; job.n_classes = n_classes;
+    job.n_walkers = n_walkers; job.first_id = first_id; job.seed = seed; job.label_allowed = label_allowed;
+    job.dt = dt_ms; job.n_steps = n_steps; job.n_wave = n_wave; job.wave = wave; job.n_g = n_g; job.gamp = gamp;
+    job.n_dir = n_dir; job.dirs = dirs; job.n_snap = n_snap; job.snap_steps = snap_steps;
+    job.final_vox = final_vox; job.final_off = final_off; job.final_label = final_label;
+    job.init_vox = init_vox; job.init_off = init_off; job.phi = phi; job.relax = relax;
+
+    if (n_threads < 1) n_threads = 1;
+    if ((uint64_t)n_threads > n_walkers && n_walkers > 0) n_threads = (int)n_walkers;
+    part_t* parts = (part_t*)calloc((size_t)n_threads, sizeof(part_t));
+    pthread_t* tids = (pthread_t*)calloc((size_t)n_threads, sizeof(pthread_t));
+    int status = ORC_OK;
+    if (!parts || !tids) { status = ORC_ERR_OOM; goto done; }
+    for (int t = 0; t < n_threads; ++t) {
+        part_t* p = &parts[t];
+        p->job = &job;
+        p->w_begin = n_walkers * (uint64_t)t / (uint64_t)n_threads;
+        p->w_end = n_walkers * (uint64_t)(t + 1) / (uint64_t)n_threads;
+        p->sum_alpha = (double*)calloc((size_t)n_classes, sizeof(double));
+        p->sig_re = (double*)calloc(n_sig(&job) + 1, sizeof(double));
+        p->sig_im = (double*)calloc(n_sig(&job) + 1, sizeof(double));
+        p->m2 = (double*)calloc(n_mom(&job) + 1, sizeof(double));
+        p->m4 = (double*)calloc(n_mom(&job) + 1, sizeof(double));
+        p->snap_alpha = (double*)calloc(n_sal(&job) + 1, sizeof(double));
+        p->class_flow = (uint64_t*)calloc(n_flow(&job) + 1, sizeof(uint64_t));
+        if (!p->sum_alpha || !p->sig_re || !p->sig_im || !p->m2 || !p->m4 || !p->snap_alpha || !p->class_flow)
+            status = ORC_ERR_OOM;
+    }
+    if (status == ORC_OK) {
+        /* walker ids are only partitioned over threads; every walker's arithmetic is unchanged */
+        for (int t = 1; t < n_threads; ++t) pthread_create(&tids[t], NULL, run_part, &parts[t]);
+        run_part(&parts[0]);
+        for (int t = 1; t < n_threads; ++t) pthread_join(tids[t], NULL);
+        for (int c = 0; c < n_classes; ++c) sum_alpha[c] = 0.0;
+        if (sig_re) memset(sig_re, 0, sizeof(double) * n_sig(&job));
+        if (sig_im) memset(sig_im, 0, sizeof(double) * n_sig(&job));
+        if (m2) memset(m2, 0, sizeof(double) * n_mom(&job));
+        if (m4) memset(m4, 0, sizeof(double) * n_mom(&job));
+        if (snap_alpha) memset(snap_alpha, 0, sizeof(double) * n_sal(&job));
+        if (class_flow) memset(class_flow, 0, sizeof(uint64_t) * n_flow(&job));
+        memset(counters, 0, sizeof(uint64_t) * 4);
+        for (int t = 0; t < n_threads; ++t) { /* partial sums added in walker order */
+            part_t* p = &parts[t];
+            if (p->status != ORC_OK) status = p->status;
+            for (int c = 0; c < n_classes; ++c) sum_alpha[c] += p->sum_alpha[c];
+            if (sig_re) for (size_t i = 0; i < n_sig(&job); ++i) sig_re[i] += p->sig_re[i];
+            if (sig_im) for (size_t i = 0; i < n_sig(&job); ++i) sig_im[i] += p->sig_im[i];
+            if (m2) for (size_t i = 0; i < n_mom(&job); ++i) m2[i] += p->m2[i];
+            if (m4) for (size_t i = 0; i < n_mom(&job); ++i) m4[i] += p->m4[i];
+            if (snap_alpha) for (size_t i = 0; i < n_sal(&job); ++i) snap_alpha[i] += p->snap_alpha[i];
+            if (class_flow) for (size_t i = 0; i < n_flow(&job); ++i) class_flow[i] += p->class_flow[i];
+            counters[0] += p->counters[0]; counters[1] += p->counters[1]; counters[2] += p->counters[2];
+            if (p->counters[3] > counters[3]) counters[3] = p->counters[3];
+        }
+    }
+done:
+    if (parts) for (int t = 0; t < n_threads; ++t) {
+        free(parts[t].sum_alpha); free(parts[t].sig_re); free(parts[t].sig_im); free(parts[t].m2);
+        free(parts[t].m4); free(parts[t].snap_alpha); free(parts[t].class_flow);
+    }
+    free(parts); free(tids); free(s_tab); free(P_tab); free(inv_T2);
+    return status;
+}

@@ -1,0 +1,191 @@
+"""ctypes wrapper of oracle/rms_oracle.c (TEST INFRASTRUCTURE, not the product).
+
+Marshals numpy arrays into the plain-C oracle and writes out the last line of the method,
+the normalisation of Eq.7 and of the narrow-pulse moments, in numpy fp64.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+import subprocess
+from pathlib import Path
+
+import numpy as np
+
+_HERE = Path(__file__).resolve().parent
+_SRC = _HERE / "rms_oracle.c"
+_LIB = _HERE / "librms_oracle.so"
+_lib = None
+
+_ERRORS = {-1: "bad argument", -2: "step length >= voxel size (PAPER.md lines 62, 189)",
+           -3: "Eq.3 gives P > 1 for a finite kappa (PAPER.md line 624)",
+           -4: "no voxel with an allowed label", -5: "out of memory"}
+
+
+class OracleError(RuntimeError):
+    def __init__(self, code):
+        super().__init__(f"oracle error {code}: {_ERRORS.get(code, '?')}")
+        self.code = code
+
+
+def build(force: bool = False) -> Path:
+    """Compile the oracle with gcc (building the checker is not using it)."""
+    if force or not _LIB.exists() or _LIB.stat().st_mtime < _SRC.stat().st_mtime:
+        cmd = ["gcc", "-O2", "-std=c11", "-Wall", "-Wextra", "-fPIC", "-shared", "-o", str(_LIB), str(_SRC),
+               "-lm", "-lpthread"]
+        subprocess.run(cmd, check=True)
+    return _LIB
+
+
+def _load():
+    global _lib
+    if _lib is None:
+        build()
+        _lib = C.CDLL(str(_LIB))
+        _lib.rms_oracle_run.restype = C.c_int
+        _lib.rms_oracle_step.restype = C.c_int
+        _lib.rms_oracle_tables.restype = C.c_int
+        _lib.rms_oracle_init_walker.restype = C.c_int
+        _lib.rms_oracle_philox4x32_10.restype = None
+        _lib.rms_oracle_direction.restype = None
+    return _lib
+
+
+def _p(a, ctype):
+    return None if a is None else a.ctypes.data_as(C.POINTER(ctype))
+
+
+def philox4x32_10(ctr, key):
+    c = np.asarray(ctr, dtype=np.uint32).copy()
+    k = np.asarray(key, dtype=np.uint32).copy()
+    out = np.zeros(4, np.uint32)
+    _load().rms_oracle_philox4x32_10(_p(c, C.c_uint32), _p(k, C.c_uint32), _p(out, C.c_uint32))
+    return out
+
+
+def direction(wa: int, wb: int):
+    u = np.zeros(3)
+    _load().rms_oracle_direction(C.c_uint32(int(wa)), C.c_uint32(int(wb)), _p(u, C.c_double))
+    return u
+
+
+def tables(D, kappa, voxel_um, dt_ms):
+    """(s[n_labels], P[n_labels, n_labels]) of Eq.1 and Eq.3."""
+    D = np.ascontiguousarray(D, np.float32)
+    n = D.size
+    kappa = None if kappa is None else np.ascontiguousarray(kappa, np.float32).reshape(n, n)
+    s = np.zeros(n)
+    P = np.zeros((n, n))
+    st = _load().rms_oracle_tables(C.c_int(n), _p(D, C.c_float), _p(kappa, C.c_float), C.c_double(voxel_um),
+                                   C.c_double(dt_ms), _p(s, C.c_double), _p(P, C.c_double))
+    if st:
+        raise OracleError(st)
+    return s, P
+
+
+def step(labels, s, P, vox, off, label, u, u_perm=(0.5, 0.5, 0.5)):
+    """One Monte Carlo step with a given unit direction and given permeation uniforms."""
+    labels = np.ascontiguousarray(labels, np.uint16)
+    nz, ny, nx = labels.shape
+    s = np.ascontiguousarray(s, np.float64)
+    P = np.ascontiguousarray(P, np.float64)
+    v = np.asarray(vox, np.int32).copy()
+    f = np.asarray(off, np.float64).copy()
+    L = C.c_uint16(int(label))
+    uu = np.asarray(u, np.float64).copy()
+    up = np.asarray(u_perm, np.float64).copy()
+    cnt = np.zeros(3, np.int32)
+    _load().rms_oracle_step(C.c_int(nx), C.c_int(ny), C.c_int(nz), _p(labels, C.c_uint16), C.c_int(s.size),
+                            _p(s, C.c_double), _p(P, C.c_double), _p(v, C.c_int32), _p(f, C.c_double), C.byref(L),
+                            _p(uu, C.c_double), _p(up, C.c_double), _p(cnt, C.c_int32))
+    return v, f, int(L.value), dict(encounters=int(cnt[0]), permeations=int(cnt[1]), clamps=int(cnt[2]))
+
+
+def init_walker(labels, label_allowed, seed, walker):
+    labels = np.ascontiguousarray(labels, np.uint16)
+    nz, ny, nx = labels.shape
+    allowed = None if label_allowed is None else np.ascontiguousarray(label_allowed, np.uint8)
+    v = np.zeros(3, np.int32)
+    f = np.zeros(3)
+    L = C.c_uint16(0)
+    st = _load().rms_oracle_init_walker(C.c_int(nx), C.c_int(ny), C.c_int(nz), _p(labels, C.c_uint16),
+                                        _p(allowed, C.c_uint8), C.c_uint64(seed), C.c_uint64(walker),
+                                        _p(v, C.c_int32), _p(f, C.c_double), C.byref(L))
+    if st:
+        raise OracleError(st)
+    return v, f, int(L.value)
+
+
+def normalise(raw, dt_ms, snap_steps):
+    """Eq.7 and the narrow-pulse D, K, pooled over classes and per class.
+
+    K is normalised by <alpha> in both moments (R14).
+    """
+    out = dict(raw)
+    sa = raw["sum_alpha"]
+    tot = sa.sum()
+    out["S"] = (raw["sig_re"].sum(-1) + 1j * raw["sig_im"].sum(-1)) / tot
+    with np.errstate(divide="ignore", invalid="ignore"):
+        out["S_class"] = (raw["sig_re"] + 1j * raw["sig_im"]) / sa
+        t = np.asarray(snap_steps, np.float64) * dt_ms
+        a_s = raw["snap_alpha"].sum(-1)                       # [n_snap]
+        m2 = raw["m2"].sum(-1) / a_s[:, None]                 # [n_snap, n_dir]
+        m4 = raw["m4"].sum(-1) / a_s[:, None]
+        out["msd"] = m2
+        out["D"] = m2 / (2.0 * t[:, None])
+        out["K"] = m4 / (m2 * m2) - 3.0
+    return out
+
+
+def run(sub, seq, n_walkers, seed, first_id=0, n_threads=1, per_walker=False):
+    """Whole path on the CPU: init -> steps -> sums.  `sub`, `seq` are rms_inputs.Substrate / Sequence."""
+    lib = _load()
+    labels = np.ascontiguousarray(sub.labels, np.uint16)
+    nz, ny, nx = labels.shape
+    nL, nC = sub.n_labels, int(sub.n_classes)
+    D = np.ascontiguousarray(sub.D, np.float32)
+    T2 = np.ascontiguousarray(sub.T2, np.float32)
+    kappa = np.ascontiguousarray(sub.kappa, np.float32)
+    lclass = np.ascontiguousarray(sub.label_class, np.uint8)
+    allowed = np.ascontiguousarray(sub.label_allowed, np.uint8)
+    wave = np.ascontiguousarray(seq.wave, np.float32)
+    gamp = np.ascontiguousarray(seq.gamp, np.float64)
+    dirs = np.ascontiguousarray(seq.dirs, np.float64)
+    snaps = np.ascontiguousarray(seq.snap_steps, np.int64)
+    n_wave, n_steps = wave.shape if wave.ndim == 2 else (0, int(seq.n_steps))
+    n_g = gamp.shape[1] if gamp.ndim == 2 and n_wave else 0
+    n_dir, n_snap = dirs.shape[0], snaps.size
+    r = dict(
+        sum_alpha=np.zeros(nC), sig_re=np.zeros((n_wave, n_g, n_dir, nC)), sig_im=np.zeros((n_wave, n_g, n_dir, nC)),
+        m2=np.zeros((n_snap, n_dir, nC)), m4=np.zeros((n_snap, n_dir, nC)), snap_alpha=np.zeros((n_snap, nC)),
+        class_flow=np.zeros((n_snap, nC, nC), np.uint64))
+    counters = np.zeros(4, np.uint64)
+    pw = {}
+    if per_walker:
+        pw = dict(final_vox=np.zeros((n_walkers, 3), np.int32), final_off=np.zeros((n_walkers, 3)),
+                  final_label=np.zeros(n_walkers, np.uint16), init_vox=np.zeros((n_walkers, 3), np.int32),
+                  init_off=np.zeros((n_walkers, 3)), phi=np.zeros((n_walkers, max(n_wave, 1), 3)),
+                  relax=np.zeros(n_walkers))
+    st = lib.rms_oracle_run(
+        C.c_int(nx), C.c_int(ny), C.c_int(nz), C.c_double(sub.voxel_um), _p(labels, C.c_uint16), C.c_int(nL),
+        _p(D, C.c_float), _p(T2, C.c_float), _p(kappa, C.c_float), _p(lclass, C.c_uint8), C.c_int(nC),
+        C.c_uint64(n_walkers), C.c_uint64(first_id), _p(allowed, C.c_uint8), C.c_uint64(seed),
+        C.c_double(seq.dt_ms), C.c_int64(n_steps), C.c_int(n_wave), _p(wave, C.c_float), C.c_int(n_g),
+        _p(gamp, C.c_double), C.c_int(n_dir), _p(dirs, C.c_double), C.c_int(n_snap), _p(snaps, C.c_int64),
+        C.c_int(n_threads),
+        _p(r["sum_alpha"], C.c_double), _p(r["sig_re"], C.c_double), _p(r["sig_im"], C.c_double),
+        _p(r["m2"], C.c_double), _p(r["m4"], C.c_double), _p(r["snap_alpha"], C.c_double),
+        _p(r["class_flow"], C.c_uint64), _p(counters, C.c_uint64),
+        _p(pw.get("final_vox"), C.c_int32), _p(pw.get("final_off"), C.c_double), _p(pw.get("final_label"), C.c_uint16),
+        _p(pw.get("init_vox"), C.c_int32), _p(pw.get("init_off"), C.c_double),
+        _p(pw.get("phi") if n_wave else None, C.c_double), _p(pw.get("relax"), C.c_double))
+    if st:
+        raise OracleError(st)
+    r.update(pw)
+    r.update(n_encounters=int(counters[0]), n_permeations=int(counters[1]), n_clamps=int(counters[2]),
+             max_encounters_per_step=int(counters[3]))
+    return normalise(r, seq.dt_ms, snaps)
+
+
+def default_threads() -> int:
+    return len(os.sched_getaffinity(0))

@@ -1,0 +1,257 @@
+"""Pins of the oracle's pieces: Philox, word->real maps, direction, tables, init, single step.
+
+None of these re-types an oracle formula: they check known answers, closed-form moments, the
+paper's printed values / identities, and an independently written brute-force ray march.
+"""
+import math
+
+import numpy as np
+import pytest
+
+import oracle
+import rms_inputs as ri
+
+
+# ------------------------------------------------------------------ Philox (pin K1)
+def test_philox_known_answers(golden_dir):
+    rows = [l.split() for l in (golden_dir / "philox4x32_10_kat.txt").read_text().splitlines()
+            if l.strip() and not l.startswith("#")]
+    assert len(rows) == 3
+    for r in rows:
+        v = [int(x, 16) for x in r]
+        out = oracle.philox4x32_10(v[0:4], v[4:6])
+        assert [int(x) for x in out] == v[6:10]
+
+
+def test_philox_is_a_bijection_of_the_counter_on_a_sample():
+    # distinct counters -> distinct outputs (a dropped round or a wrong shuffle usually collides or repeats words)
+    seen = set()
+    for i in range(2000):
+        out = tuple(int(x) for x in oracle.philox4x32_10([i, 0, i >> 3, 1], [7, 9]))
+        seen.add(out)
+    assert len(seen) == 2000
+    words = np.array(sorted(seen), dtype=np.uint64).ravel()
+    bits = ((words[:, None] >> np.arange(32, dtype=np.uint64)) & 1).mean(0)
+    assert np.all(np.abs(bits - 0.5) < 5 * 0.5 / math.sqrt(words.size))
+
+
+# ------------------------------------------------------------------ direction (pin K2)
+def test_direction_is_unit_and_isotropic():
+    rng = np.random.default_rng(11)
+    w = rng.integers(0, 2 ** 32, size=(60000, 2), dtype=np.uint64)
+    u = np.array([oracle.direction(a, b) for a, b in w])
+    assert np.allclose(np.linalg.norm(u, axis=1), 1.0, atol=1e-12)
+    n = len(u)
+    # closed-form moments of a uniform unit vector: <u_k>=0, <u_k^2>=1/3, <u_k^4>=1/5, <u_x^2 u_y^2>=1/15
+    assert np.all(np.abs(u.mean(0)) < 4 * math.sqrt(1 / 3 / n))
+    assert np.all(np.abs((u ** 2).mean(0) - 1 / 3) < 4 * math.sqrt((1 / 5 - 1 / 9) / n))
+    assert np.all(np.abs((u ** 4).mean(0) - 1 / 5) < 4 * math.sqrt((1 / 9 - 1 / 25) / n))
+    assert abs((u[:, 0] ** 2 * u[:, 1] ** 2).mean() - 1 / 15) < 4 * math.sqrt((1 / 105 - 1 / 225) / n) + 1e-3
+    # azimuth uniform: <cos 2psi> = 0 separately in the upper and lower half
+    for half in (u[:, 2] > 0, u[:, 2] < 0):
+        psi = np.arctan2(u[half, 1], u[half, 0])
+        assert abs(np.cos(2 * psi).mean()) < 4 / math.sqrt(2 * half.sum())
+
+
+def test_direction_word_map_is_exactly_symmetric_and_fp32_exact():
+    # word w and its bitwise complement give exactly opposite z (sym is odd under k -> 2^23-1-k)
+    for w in (0, 1, 0x1FF, 0x200, 0x7FFFFFFF, 0x80000000, 0xFFFFFFFF, 0x12345678):
+        z1 = oracle.direction(w, 0x80000000)[2]
+        z2 = oracle.direction((~w) & 0xFFFFFFFF, 0x80000000)[2]
+        assert z1 == -z2
+        assert z1 != 0.0 and abs(z1) < 1.0
+        assert float(np.float32(z1)) == z1           # representable in fp32: both sides start from the same value
+    # extreme words: |z| = 1 - 2^-23
+    assert oracle.direction(0xFFFFFFFF, 0)[2] == 1.0 - 2.0 ** -23
+    assert oracle.direction(0, 0)[2] == -(1.0 - 2.0 ** -23)
+    # azimuth: wb -> psi = pi*sym(wb); wb = 0x80000000 gives the smallest positive angle pi*2^-23
+    u = oracle.direction(0x80000000, 0x80000000)     # z = 2^-23
+    assert math.isclose(math.atan2(u[1], u[0]), math.pi * 2.0 ** -23, rel_tol=1e-9)
+    # the low 9 bits of either word do not move the direction (they feed the permeation draw, R5)
+    assert np.array_equal(oracle.direction(0xABCDE000, 0x12345600), oracle.direction(0xABCDE1FF, 0x123457FF))
+
+
+# ------------------------------------------------------------------ tables (pin K3)
+def _golden(golden_dir):
+    out = {}
+    for l in (golden_dir / "paper_constants.txt").read_text().splitlines():
+        if l.strip() and not l.startswith("#"):
+            k, v, tol = l.split()[:3]
+            out[k] = (float(v), float(tol))
+    return out
+
+
+def test_step_length_matches_the_value_the_paper_prints(golden_dir):
+    val, tol = _golden(golden_dir)["step_length_um_D2_dt2e-4"]
+    s, _ = oracle.tables([2.0], None, 0.1, 2e-4)
+    assert abs(s[0] * 0.1 - val) < tol
+    assert math.isclose(s[0] * 0.1, math.sqrt(6 * 2.0 * 2e-4), rel_tol=1e-7)   # Eq.1, d = 3
+
+
+def test_permeation_table_identities():
+    D = np.array([2.0, 1.0, 0.5], np.float32)
+    kap = np.array([[0, 0.02, 0.4], [0.02, 0, 0.1], [0.4, 0.1, 0]], np.float32)
+    dt, lp = 2e-4, 0.1
+    s, P = oracle.tables(D, kap, lp, dt)
+    ds = s * lp
+    for a in range(3):
+        assert P[a, a] == 1.0
+        for b in range(3):
+            if a == b:
+                continue
+            k = float(kap[a, b])
+            # Eq.2a for each side, then Eq.3 == Eq.2a / (1 + alpha), alpha = mean of the two Eq.2a values
+            # (Eq.C.8 with kappa_0 -> kappa as in the text below Eq.C.8)
+            p2a_ab = k * ds[a] / D[a] * (2 / 3)
+            p2a_ba = k * ds[b] / D[b] * (2 / 3)
+            assert math.isclose(P[a, b], p2a_ab / (1 + 0.5 * (p2a_ab + p2a_ba)), rel_tol=3e-7)
+            # equilibrium ratio P12/P21 = sqrt(D2)/sqrt(D1) (c1 = c2)
+            assert math.isclose(P[a, b] / P[b, a], math.sqrt(D[b] / D[a]), rel_tol=3e-7)
+            assert P[a, b] < p2a_ab                           # kappa > kappa_0, Eq.C.7
+    # cfg3 numbers quoted in SURVEY.md section 8 (kappa = 0.02, D_in = 2, D_out = 1)
+    _, P3 = oracle.tables([1.0, 2.0], [[0, 0.02], [0.02, 0]], 0.1, 2e-4)
+    assert math.isclose(P3[1, 0], 3.2647e-4, rel_tol=2e-4)
+    assert math.isclose(P3[0, 1], 4.6170e-4, rel_tol=2e-4)
+
+
+def test_table_special_cases_and_errors():
+    inf = float("inf")
+    # kappa = 0: impermeable; kappa = inf: Baxter-Frank Eq.C.15 with c1 = c2: high-flux side -> sqrt(D2/D1)
+    _, P = oracle.tables([2.0, 0.5], [[0, inf], [inf, 0]], 0.1, 2e-4)
+    assert P[0, 1] == np.float32(0.5) and P[1, 0] == 1.0
+    _, P = oracle.tables([2.0, 0.5], [[0, 0], [0, 0]], 0.1, 2e-4)
+    assert P[0, 1] == 0.0 and P[1, 0] == 0.0
+    with pytest.raises(oracle.OracleError) as e:              # ds >= l_p
+        oracle.tables([2.0], None, 0.04, 2e-4)
+    assert e.value.code == -2
+    with pytest.raises(oracle.OracleError) as e:              # Eq.3 > 1 (cf. constraint P:624)
+        oracle.tables([2.0, 0.01], [[0, 5000.0], [5000.0, 0]], 0.1, 2e-4)
+    assert e.value.code == -3
+
+
+# ------------------------------------------------------------------ init
+def test_init_is_uniform_over_allowed_voxels_and_independent_of_batch():
+    sub = ri.random_lattice((6, 5, 4), n_labels=3, seed=5)
+    allowed = np.array([1, 0, 1], np.uint8)
+    n = 30000
+    vox = np.zeros((n, 3), np.int64)
+    off = np.zeros((n, 3))
+    for i in range(n):
+        v, f, L = oracle.init_walker(sub.labels, allowed, seed=9, walker=i)
+        assert allowed[L] == 1 and sub.labels[v[2], v[1], v[0]] == L
+        vox[i], off[i] = v, f
+    assert np.all((off >= 0) & (off < 1))
+    ok = allowed[sub.labels]                                   # (nz, ny, nx)
+    counts = np.zeros_like(sub.labels, dtype=np.int64)
+    np.add.at(counts, (vox[:, 2], vox[:, 1], vox[:, 0]), 1)
+    assert counts[ok == 0].sum() == 0                          # never in dead space
+    exp = n / ok.sum()
+    chi2 = ((counts[ok == 1] - exp) ** 2 / exp).sum()
+    dof = ok.sum() - 1
+    assert abs(chi2 - dof) < 5 * math.sqrt(2 * dof)
+    assert np.all(np.abs(off.mean(0) - 0.5) < 4 * math.sqrt(1 / 12 / n))
+    # a walker's start depends only on (seed, id)
+    r = oracle.run(sub, ri.pgse_sequence(2e-4, 2, 2e-4, 2e-4, [0.0], np.eye(3)), 7, 9, first_id=100, per_walker=True)
+    for j in range(7):
+        v, f, _ = oracle.init_walker(sub.labels, sub.label_allowed, 9, 100 + j)
+        assert np.array_equal(r["init_vox"][j], v) and np.array_equal(r["init_off"][j], f)
+
+
+def test_init_reports_no_space():
+    sub = ri.uniform_lattice((4, 4, 4))
+    with pytest.raises(oracle.OracleError) as e:
+        oracle.init_walker(sub.labels, np.array([0], np.uint8), 1, 0)
+    assert e.value.code == -4
+
+
+# ------------------------------------------------------------------ one step vs brute force (pin K14)
+def _ray_march(labels, s_tab, vox, off, label, u, decisions, n_sub=5000):
+    """Independent brute force: march the hop in tiny time slices; at the first contact with a voxel face
+    look at the label behind it; unlike label -> take the next forced decision (True = permeate)."""
+    nz, ny, nx = labels.shape
+    dims = (nx, ny, nz)
+    pos = np.asarray(vox, float) + np.asarray(off, float)     # unwrapped position in voxel units
+    cell = np.asarray(vox, np.int64).copy()
+    vel = np.asarray(u, float) * s_tab[label]                 # displacement per unit "time"; whole hop = time 1
+    L = label
+    dec = list(decisions)
+    h = 1.0 / n_sub
+    for _ in range(n_sub):
+        for k in range(3):                                    # one axis at a time inside a slice (error O(h))
+            new = pos[k] + vel[k] * h
+            c = math.floor(new)
+            if c == cell[k]:
+                pos[k] = new
+                continue
+            sgn = 1 if c > cell[k] else -1
+            nb = cell.copy(); nb[k] += sgn
+            Ln = labels[nb[2] % dims[2], nb[1] % dims[1], nb[0] % dims[0]]
+            go = True
+            if Ln != L:
+                go = dec.pop(0)
+            if go:
+                pos[k] = new
+                cell[k] = c
+                if Ln != L:
+                    vel = vel * (s_tab[Ln] / s_tab[L])
+                    L = Ln
+            else:
+                plane = cell[k] + (1 if sgn > 0 else 0)
+                pos[k] = 2 * plane - new
+                vel[k] = -vel[k]
+    return pos, cell, L, len(decisions) - len(dec)
+
+
+@pytest.mark.parametrize("seed", [0, 1, 2])
+def test_step_matches_brute_force_ray_march(seed):
+    rng = np.random.default_rng(100 + seed)
+    sub = ri.random_lattice((3 + seed, 3, 4), n_labels=3, seed=seed)
+    s_tab = np.array([0.49, 0.35, 0.8])                      # different hop lengths per label: rescale rule R7
+    nL = 3
+    checked = multi = 0
+    for trial in range(70):
+        vox = rng.integers(-3, 6, size=3)
+        # starts hugging faces / edges / corners half of the time, so 2 and 3 interactions are common
+        off = np.where(rng.random(3) < 0.5, rng.random(3), rng.choice([0.02, 0.97, 0.5], size=3))
+        u = rng.normal(size=3); u /= np.linalg.norm(u)
+        dims = sub.shape_xyz
+        label = int(sub.labels[vox[2] % dims[2], vox[1] % dims[1], vox[0] % dims[0]])
+        for decisions in ([False] * 3, [True] * 3, [True, False, True], [False, True, False]):
+            # forced decisions through the P table: P = 1 (permeate) or 0 (reflect) for every unlike pair is too
+            # coarse, so drive them through the uniforms: P = 0.5 and u_e = 0.25 (pass) / 0.75 (reflect)
+            P = np.full((nL, nL), 0.5); np.fill_diagonal(P, 1.0)
+            up = [0.25 if d else 0.75 for d in decisions]
+            v1, f1, L1, cnt = oracle.step(sub.labels, s_tab, P, vox, off, label, u, up)
+            pos, cell, L2, used = _ray_march(sub.labels, s_tab, vox, off, label, u, decisions)
+            got = v1 + f1
+            assert cnt["encounters"] <= 3
+            # the two can differ by O(1/n_sub) only; skip the voxel comparison when sitting on a face
+            assert np.allclose(got, pos, atol=4e-3), (trial, decisions, got, pos)
+            frac = pos - np.floor(pos)
+            if np.all((frac > 1e-2) & (frac < 1 - 1e-2)):
+                assert np.array_equal(v1, cell) and L1 == L2 and cnt["encounters"] == used
+                checked += 1
+                multi += cnt["encounters"] >= 2
+            assert np.all((f1 >= 0) & (f1 < 1))
+            assert sub.labels[v1[2] % dims[2], v1[1] % dims[1], v1[0] % dims[0]] == L1   # cached label = lattice
+    assert checked > 150 and multi > 15
+
+
+def test_step_without_membranes_is_plain_addition():
+    sub = ri.uniform_lattice((3, 3, 3))
+    rng = np.random.default_rng(3)
+    for _ in range(200):
+        off = rng.random(3); u = rng.normal(size=3); u /= np.linalg.norm(u)
+        v, f, L, cnt = oracle.step(sub.labels, [0.9], [[1.0]], [0, 0, 0], off, 0, u)
+        assert np.allclose(v + f, off + 0.9 * u, atol=1e-14) and cnt["encounters"] == 0   # Eq.6
+
+
+def test_corner_reflector_sends_the_hop_back():
+    # Fig.2: three consecutive reflections in an impermeable corner reverse the direction
+    lab = np.zeros((2, 2, 2), np.uint16); lab[0, 0, 0] = 1      # single voxel of label 1, all faces are membranes
+    s = [0.9, 0.9]; P = [[1, 0], [0, 1]]
+    off = np.array([0.9, 0.8, 0.85]); u = np.ones(3) / math.sqrt(3)
+    v, f, L, cnt = oracle.step(lab, s, P, [0, 0, 0], off, 1, u)
+    assert cnt["encounters"] == 3 and L == 1 and np.array_equal(v, [0, 0, 0])
+    # mirror image: per axis the path length is conserved: f = 2*1 - (off + s u)
+    assert np.allclose(f, 2 - (off + 0.9 * u), atol=1e-14)
