@@ -1,0 +1,283 @@
+#!/usr/bin/env python
+"""bench.py -- walker-steps/s of the whole RMS hot path on B200 (BASELINE.json metric), one JSON line.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl reference]
+    python -m torch.distributed.run --nnodes=1 --nproc-per-node N ... bench.py --gpus N ...
+
+Workload (config.workload): the cfg4 throughput point of BASELINE.json on the synthetic mouse-like axon
+substrate of cfg2 -- 500x500x2000 uint16 lattice, ~300 axons, 1e6 intra-axonal walkers x 10,000 Monte Carlo
+steps, PGSE with 60 directions x 11 b-values, impermeable membranes, D = 2 um^2/ms, dt = 2e-4 ms.
+One bench "step" is one pass of the whole path: rms_substrate_create (face-mask lattice built from labels
+resident in HBM) -> rms_walkers_init -> rms_run (walk, phase/T2 accumulation, moment and signal reductions,
+normalisation).  `value` = walker-steps/s with the labels already in HBM; `e2e` = the same through the C ABI
+from pinned HOST labels (host->device copy and result read-back inside the timed region).
+
+`--impl reference` times the CPU oracle (oracle/, test infrastructure) on a bounded sample of the same workload.
+"""
+from __future__ import annotations
+
+import argparse
+import dataclasses
+import json
+import os
+import statistics
+import subprocess
+import sys
+import threading
+import time
+from pathlib import Path
+
+import numpy as np
+
+ROOT = Path(__file__).resolve().parent
+sys.path.insert(0, str(ROOT))
+
+# Algorithmic thread-instructions per walker-step, frozen in DESIGN.md ("Roofline") before tuning.
+ALGORITHMIC_INSTR_PER_STEP = 80.0
+N_SM, LANES_PER_SM = 148, 128          # B200: 4 schedulers x 32 lanes per SM, one warp instruction per clock each
+# DRAM traffic of the step kernel per launch from the committed ncu capture (profiles/), or None.
+NCU_TRAFFIC_BYTES_PER_LAUNCH = None
+
+
+def parse_args():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--walkers", type=int, default=1_000_000)
+    ap.add_argument("--mc-steps", type=int, default=10_000)
+    ap.add_argument("--dirs", type=int, default=60)
+    ap.add_argument("--lattice", default="facemask", choices=["facemask", "labels"])
+    ap.add_argument("--scale", default="full", choices=["full", "test"])
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--cpu-sample-walkers", type=int, default=40_000)
+    return ap.parse_args()
+
+
+class ClockSampler:
+    """nvidia-smi clocks and throttle reasons DURING the timed region (B200_PROFILING.md recipe)."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.index, self.proc, self.lines = index, None, []
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits", "-lms", "100",
+                                          "-i", str(self.index)], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thread = threading.Thread(target=self._read, daemon=True)
+            self.thread.start()
+        except OSError:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.lines.append(line.strip())
+
+    def stop(self):
+        if not self.proc:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.proc.kill()
+        sm, mx, reasons, power = [], [], set(), []
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for l in self.lines:
+            f = [x.strip() for x in l.split(",")]
+            if len(f) < 7:
+                continue
+            try:
+                sm.append(float(f[0])); mx.append(float(f[1])); power.append(float(f[2]))
+            except ValueError:
+                continue
+            for nm, v in zip(names, f[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(nm)
+        return {"sm_mhz": statistics.median(sm) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "power_w_max": max(power) if power else None, "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def make_workload(args):
+    import rms_inputs as ri
+    cfg = ri.make_config("cfg4", args.scale, n_walkers=args.walkers, n_steps=args.mc_steps, n_dir=args.dirs)
+    return cfg
+
+
+def workload_config(args, cfg, extra=None):
+    nx, ny, nz = cfg.substrate.shape_xyz
+    c = {"workload": "cfg4 point on the cfg2 synthetic axon substrate (BASELINE.json configs[4] on configs[2])",
+         "lattice": f"{nx}x{ny}x{nz} uint16", "n_axons": cfg.substrate.meta.get("n_axons"),
+         "intra_fraction": round(cfg.substrate.meta.get("intra_fraction", 0.0), 4),
+         "walkers_per_gpu": args.walkers, "mc_steps": args.mc_steps, "dt_ms": cfg.sequence.dt_ms,
+         "directions": int(cfg.sequence.dirs.shape[0]), "b_values": int(cfg.sequence.gamp.shape[1]),
+         "lattice_path": args.lattice, "pass": "rms_substrate_create + rms_walkers_init + rms_run",
+         "l2": "inputs larger than L2 (lattice 1.0 GB + 0.5 GB face masks vs 126 MB L2)" if args.scale == "full"
+         else "reduced test lattice (fits L2) -- not a valid bench configuration"}
+    if extra:
+        c.update(extra)
+    return c
+
+
+def run_reference(args):
+    """The CPU oracle as it stands, on the host cores, on a bounded sample of the workload."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    import oracle
+    cfg = make_workload(args)
+    threads = oracle.rms_oracle.default_threads()
+    sample = min(args.cpu_sample_walkers, args.walkers)
+    oracle.build()
+    times = []
+    for it in range(args.warmup + args.steps):
+        t0 = time.perf_counter()
+        oracle.run(cfg.substrate, cfg.sequence, sample, cfg.seed, first_id=0, n_threads=threads)
+        t1 = time.perf_counter()
+        if it >= args.warmup:
+            times.append(t1 - t0)
+    total = sum(times)
+    value = sample * args.mc_steps * len(times) / total
+    line = {"impl": "reference", "metric": "walker_steps_per_s", "value": value, "unit": "walker-steps/s", "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * total / len(times), "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": workload_config(args, cfg, {"sample": f"first {sample} walker ids x {args.mc_steps} steps per step"}),
+            "cpu_baseline": {"value": value, "unit": "walker-steps/s", "cores": threads, "kind": "oracle",
+                             "sample": f"first {sample} walker ids x {args.mc_steps} steps"},
+            "e2e": {"value": value, "unit": "walker-steps/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
+    print(json.dumps(line))
+
+
+def main():
+    args = parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+        return
+    import torch
+    import torch.distributed as dist
+    import paper_2012_06478_b200 as rms
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: there is no CPU fallback")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    rms.load_library()
+
+    cfg = make_workload(args)
+    sub, seq = cfg.substrate, cfg.sequence
+    n_walkers, mc_steps = args.walkers, args.mc_steps
+    first_id = rank * n_walkers                       # weak scaling: every rank owns its own walker-id range
+    flags = rms.RMS_RUN_LABEL_GATHER if args.lattice == "labels" else 0
+    t_ms = np.asarray(seq.snap_steps, np.float64) * seq.dt_ms
+
+    labels_dev = torch.from_numpy(sub.labels.view(np.int16)).cuda()          # resident in HBM before timing
+    labels_pin = torch.from_numpy(sub.labels.view(np.int16)).pin_memory()    # e2e: pinned host buffer
+    labels_pin_np = labels_pin.numpy().view(np.uint16)
+    stream = torch.cuda.current_stream()
+
+    sub_pin = dataclasses.replace(sub, labels=labels_pin_np)   # same substrate, labels in pinned host memory
+
+    def one_pass(device):
+        if device:   # labels already resident in HBM: adopted in place
+            r = rms.simulate(sub, seq, n_walkers, cfg.seed, first_id=first_id, flags=flags, device_labels=labels_dev)
+        else:        # host labels: rms_substrate_create copies them host -> device inside the call
+            r = rms.simulate(sub_pin, seq, n_walkers, cfg.seed, first_id=first_id, flags=flags)
+        if world > 1:
+            r = rms.api.allreduce_result(r, t_ms)
+        return r
+
+    def timed(n_iter, device):
+        kernel_ms, launches = 0.0, 0
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        t0 = time.perf_counter()
+        e0.record(stream)
+        r = None
+        for _ in range(n_iter):
+            r = one_pass(device)
+            kernel_ms += r["kernel_ms"]
+            launches += r["n_launches"] + 2           # + face-mask build + walker init kernels
+        e1.record(stream)
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+        wall = time.perf_counter() - t0
+        dev_ms = e0.elapsed_time(e1)
+        if world > 1:
+            t = torch.tensor([dev_ms, wall * 1e3], device="cuda", dtype=torch.float64)
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            dev_ms, wall = float(t[0]), float(t[1]) / 1e3
+        return dev_ms, wall, kernel_ms, launches, r
+
+    timed(args.warmup, True)
+    sampler = ClockSampler(local)
+    sampler.start()
+    dev_ms, wall, kernel_ms, launches, r = timed(args.steps, True)
+    clocks = sampler.stop()
+    total_steps = float(world) * n_walkers * mc_steps * args.steps
+    value = total_steps / (dev_ms * 1e-3)
+
+    e2e = None
+    if not args.no_e2e:
+        timed(1, False)
+        e_ms, e_wall, _, _, re = timed(args.steps, False)
+        h2d = sub.labels.nbytes + sub.D.nbytes + sub.T2.nbytes + sub.kappa.nbytes + sub.label_class.nbytes + \
+            sub.label_allowed.nbytes + seq.wave.nbytes + seq.gamp.nbytes + seq.dirs.nbytes + seq.snap_steps.nbytes
+        d2h = sum(re[k].nbytes for k in rms.api.RAW_SUMS) + 64
+        e2e = {"value": total_steps / (e_ms * 1e-3), "unit": "walker-steps/s", "h2d_bytes_per_step": int(h2d),
+               "d2h_bytes_per_step": int(d2h), "ms_per_step": e_ms / args.steps, "wall_ms_per_step": 1e3 * e_wall / args.steps}
+
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+
+    # roofline of the dominant kernel (rms_step_kernel): ALU issue bound
+    peaks_file = ROOT / "MEASURED_PEAKS.json"
+    sm_mhz = clocks.get("sm_mhz") or 1965.0
+    peak_ginstr = N_SM * LANES_PER_SM * sm_mhz * 1e6 / 1e9
+    k_ms_per_launch = kernel_ms / args.steps
+    achieved_ginstr = ALGORITHMIC_INSTR_PER_STEP * n_walkers * mc_steps / (k_ms_per_launch * 1e-3) / 1e9
+    roofline = {"bound": "alu", "kernel": "rms_step_kernel", "achieved": achieved_ginstr, "peak": peak_ginstr,
+                "unit": "Ginstr/s (thread-instructions)", "frac": achieved_ginstr / peak_ginstr,
+                "traffic": NCU_TRAFFIC_BYTES_PER_LAUNCH,
+                "algorithmic_instr_per_walker_step": ALGORITHMIC_INSTR_PER_STEP, "kernel_ms_per_launch": k_ms_per_launch,
+                "kernel_share_of_step": kernel_ms / dev_ms,
+                "peak_source": f"148 SM x 128 lanes x SM clock measured during the run ({sm_mhz:.0f} MHz; "
+                               f"MEASURED_PEAKS.json present: {peaks_file.exists()})"}
+
+    cpu_baseline = None
+    if not args.no_cpu_baseline:
+        import oracle
+        threads = oracle.rms_oracle.default_threads()
+        sample = min(args.cpu_sample_walkers, n_walkers)
+        t0 = time.perf_counter()
+        ro = oracle.run(sub, seq, sample, cfg.seed, first_id=0, n_threads=threads)
+        dt = time.perf_counter() - t0
+        cpu_baseline = {"value": sample * mc_steps / dt, "unit": "walker-steps/s", "cores": threads, "kind": "oracle",
+                        "sample": f"first {sample} walker ids x {mc_steps} steps of the same workload ({dt:.1f} s)"}
+
+    line = {"metric": "walker_steps_per_s", "value": value, "unit": "walker-steps/s", "n_gpus": world, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": dev_ms / args.steps, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f32", "data": "synthetic", "config": workload_config(args, cfg),
+            "clocks": clocks, "e2e": e2e, "gpu_launches": launches, "roofline": roofline, "cpu_baseline": cpu_baseline,
+            "wall_ms_per_step": 1e3 * wall / args.steps,
+            "check": {"S_b_max_dir0": float(abs(r["S"][0, -1, 0])), "n_encounters": r["n_encounters"],
+                      "n_membrane_faces": r["substrate_info"]["n_membrane_faces"]}}
+    print(json.dumps(line))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

@@ -1,0 +1,211 @@
+/*
+ * rms.h -- C ABI of the B200-native hot path of the Realistic Microstructure Simulator
+ *          (arXiv 2012.06478): Monte Carlo random walkers in a 3d voxelised label lattice.
+ *
+ * Citations "P:<n>" are line numbers of the paper text with the section / equation they
+ * fall in; "R<n>" are the numbered readings in DESIGN.md (what the paper leaves open).
+ *
+ * Conventions
+ *   - Every function returns 0 (RMS_OK) or a negative rms_status; nothing throws, aborts or prints.
+ *     rms_last_error() returns a thread-local, statically stored message for the last failure.
+ *   - Units: um and ms.  Lattice coordinates are in voxels; the box is periodic (R1).
+ *   - "host" / "device" is stated for every pointer.  The library never keeps a host pointer after
+ *     a call returns.  Handles are owned by the library and freed by the *_destroy calls.
+ *   - `cuda_stream` is a cudaStream_t (e.g. torch.cuda.current_stream().cuda_stream); NULL = the
+ *     legacy default stream.  All work of a call is enqueued on that stream; calls that write host
+ *     outputs (rms_run, rms_walkers_read, ...) synchronise that stream before they return.
+ *   - There is no CPU fallback: without a CUDA device every compute call fails with RMS_ERR_CUDA.
+ */
+#ifndef RMS_H
+#define RMS_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum {
+    RMS_OK = 0,
+    RMS_ERR_ARG = -1,            /* null pointer, label >= n_labels, non-unit direction, unsorted snapshots ...  */
+    RMS_ERR_STEP_TOO_LARGE = -2, /* max_L sqrt(6 D_L dt) >= voxel size: voids the <=3-interaction rule */
+    RMS_ERR_P_RANGE = -3,        /* Eq.3 gives P > 1 for a finite kappa (cf. the constraint at P:624)             */
+    RMS_ERR_NO_SPACE = -4,       /* no voxel carries an allowed label                                     */
+    RMS_ERR_OOM = -5,
+    RMS_ERR_CUDA = -6,           /* no device, launch or runtime failure                                          */
+    RMS_ERR_UNSUPPORTED = -7     /* e.g. n_wave above RMS_MAX_WAVES                                                */
+} rms_status;
+
+#define RMS_MAX_WAVES 4
+
+typedef struct rms_substrate rms_substrate; /* opaque */
+typedef struct rms_walkers rms_walkers;     /* opaque */
+
+/* ------------------------------------------------------------------------------------------------
+ * rms_substrate_create -- upload the cell-label lattice and build what the walk reads (2.1.1:
+ * "the voxelized geometry serves as the lookup table itself").
+ *
+ * labels       [nx*ny*nz] uint16, x fastest: idx = (z*ny + y)*nx + x.  Host pointer unless
+ *              RMS_LABELS_ON_DEVICE.  Copied, unless RMS_ADOPT_DEVICE_PTR (then the caller keeps the
+ *              device buffer alive and unchanged until rms_substrate_destroy).  Every label < n_labels.
+ * D            [n_labels] intrinsic diffusivity, um^2/ms, > 0            (host; Table 1)
+ * T2           [n_labels] ms; +inf or <= 0 means no relaxation; NULL = none (host; Eq.5)
+ * kappa        [n_labels*n_labels] membrane permeability um/ms between label pairs, symmetric, diagonal
+ *              ignored; 0 = impermeable; +inf = no membrane (Eq.C.15 with c1 = c2); NULL = all 0 (host; Eq.3)
+ * label_class  [n_labels] output compartment class of each label, < n_classes; NULL = all 0 (host)
+ * flags        RMS_LABELS_ON_DEVICE | RMS_ADOPT_DEVICE_PTR | RMS_NO_BRICKS
+ *
+ * Derived on the device: the bit-packed face-mask bricks (one 32-byte record per 4x4x4 voxels holding,
+ * for every voxel face of the brick, whether the labels on its two sides differ, i.e. whether the
+ * face is a membrane), unless RMS_NO_BRICKS.
+ * Errors: RMS_ERR_ARG, RMS_ERR_OOM, RMS_ERR_CUDA.
+ */
+#define RMS_LABELS_ON_DEVICE 1u
+#define RMS_ADOPT_DEVICE_PTR 2u
+#define RMS_NO_BRICKS 4u
+
+typedef struct {
+    int32_t nx, ny, nz;
+    double voxel_um;            /* l_p, isotropic */
+    const uint16_t* labels;
+    int32_t n_labels;
+    const float* D;
+    const float* T2;
+    const float* kappa;
+    const uint8_t* label_class;
+    int32_t n_classes;
+    uint32_t flags;
+} rms_substrate_desc;
+
+int rms_substrate_create(const rms_substrate_desc* desc, void* cuda_stream, rms_substrate** out);
+int rms_substrate_destroy(rms_substrate* s);
+
+typedef struct {
+    int32_t nx, ny, nz, n_labels, n_classes;
+    uint64_t n_voxels;
+    uint64_t n_membrane_faces;  /* voxel faces whose two sides carry different labels (each face once) */
+    uint64_t lattice_bytes;     /* uint16 lattice on the device                                          */
+    uint64_t brick_bytes;       /* face-mask bricks on the device (0 with RMS_NO_BRICKS)                 */
+    int32_t has_bricks;
+} rms_substrate_info;
+
+int rms_substrate_get_info(const rms_substrate* s, rms_substrate_info* out /* host */);
+
+/* ------------------------------------------------------------------------------------------------
+ * rms_walkers_init -- place walkers with homogeneous density over the voxels whose label is allowed
+ * (step 1 of 2.2; labels that are not allowed are the paper's "dead space" for placement).
+ * Walker ids are first_walker_id .. first_walker_id + n_walkers - 1; a walker's start and its whole
+ * trajectory depend only on (seed, id), never on the batch or the launch shape (R2, R13).
+ * label_allowed [n_labels] host, 1 = place here; NULL = everywhere.
+ * Errors: RMS_ERR_NO_SPACE (a walker found no allowed voxel in 2^20 proposals), RMS_ERR_ARG/OOM/CUDA.
+ */
+int rms_walkers_init(const rms_substrate* s, uint64_t n_walkers, uint64_t first_walker_id,
+                     const uint8_t* label_allowed, uint64_t seed, void* cuda_stream, rms_walkers** out);
+int rms_walkers_destroy(rms_walkers* w);
+
+/* ------------------------------------------------------------------------------------------------
+ * rms_run -- advance every walker by n_steps Monte Carlo steps (2.2 steps 2-4: fixed-length
+ * hop sqrt(6 D dt) in a random direction; at a voxel face between unlike labels elastic reflection or
+ * permeation with the probability of Eq.3; at most three interactions per step), accumulate the
+ * gradient phase and the T2 weight (Eq.5, Eq.7), and reduce to signals and moments.
+ *
+ * wave        [n_wave*n_steps] unit-less gradient shape w_m[i] for step i = 1..n_steps of THIS call (host)
+ * gamp        [n_wave*n_g] gradient amplitudes, rad/(ms um):  phi = gamp * dt * sum_i w_m[i] n.(x_i - x_0)
+ *             (right-endpoint rule, R11) (host)
+ * dirs        [n_dir*3] unit vectors (host)
+ * snap_steps  [n_snap] ascending step numbers in 1..n_steps of this call at which the displacement
+ *             moments are taken (host)
+ * flags       RMS_RUN_LABEL_GATHER: test faces by gathering the neighbour's uint16 label (the paper's
+ *             lookup table) instead of the face-mask bricks.
+ *
+ * A second rms_run on the same walkers continues the trajectories (the random numbers are keyed on the
+ * absolute step), so long runs may be chunked; phases and T2 weights keep accumulating.
+ *
+ * Outputs (rms_result, all HOST arrays allocated by the caller; any pointer may be NULL):
+ *   sum_alpha  [n_classes]                      sum_w alpha_w at the end of the call, by class of the
+ *                                               walker's INITIAL label
+ *   sig_re/im  [n_wave][n_g][n_dir][n_classes]  sum alpha cos(phi), -sum alpha sin(phi)   (Eq.7 numerator)
+ *   m2, m4     [n_snap][n_dir][n_classes]       sum alpha X^2, sum alpha X^4, X = n.(x - x_0) in um
+ *   snap_alpha [n_snap][n_classes]              sum alpha at the snapshot
+ *   class_flow [n_snap][n_classes][n_classes]   walkers by (initial class, class at the snapshot)
+ *   S_re/im    [n_wave][n_g][n_dir]             Eq.7: S = <alpha e^{-i phi}> / <alpha>, classes pooled
+ *   Dapp, Kapp [n_snap][n_dir]                  D = <alpha X^2>/(2 t <alpha>), K = <alpha X^4><alpha>/<alpha X^2>^2 - 3
+ *                                               with t = (steps since the walkers' start) * dt (R14)
+ *   n_encounters / n_permeations / n_clamps     unlike-label faces met / crossed; offsets clamped to [0,1)
+ * Errors: RMS_ERR_ARG, RMS_ERR_STEP_TOO_LARGE, RMS_ERR_P_RANGE, RMS_ERR_UNSUPPORTED, RMS_ERR_OOM, RMS_ERR_CUDA.
+ */
+#define RMS_RUN_LABEL_GATHER 1u
+
+typedef struct {
+    double dt_ms;               /* Table 1: dt */
+    int64_t n_steps;            /* Table 1: N_step (of this call) */
+    int32_t n_wave;
+    const float* wave;
+    int32_t n_g;
+    const double* gamp;
+    int32_t n_dir;
+    const double* dirs;
+    int32_t n_snap;
+    const int64_t* snap_steps;
+    uint32_t flags;
+} rms_run_desc;
+
+typedef struct {
+    double* sum_alpha;
+    double* sig_re;
+    double* sig_im;
+    double* m2;
+    double* m4;
+    double* snap_alpha;
+    uint64_t* class_flow;
+    double* S_re;
+    double* S_im;
+    double* Dapp;
+    double* Kapp;
+    uint64_t n_encounters, n_permeations, n_clamps; /* written by rms_run */
+    double kernel_ms;           /* device time of the step kernels of this call (CUDA events)          */
+    double total_ms;            /* device time of everything this call enqueued                         */
+    uint32_t n_launches;        /* kernels launched by this call                                        */
+} rms_result;
+
+int rms_run(const rms_substrate* s, rms_walkers* w, const rms_run_desc* desc, void* cuda_stream, rms_result* out);
+
+/* ------------------------------------------------------------------------------------------------
+ * rms_walkers_read -- copy the state of walkers [first, first+count) to the host: the parity hook
+ * (final voxel per walker) and the checkpoint format.
+ */
+typedef struct {
+    int32_t vox[3];   /* current voxel, unwrapped (vox0 + whole-voxel displacement)   */
+    float off[3];     /* in-voxel offset in [0,1)                                      */
+    int32_t vox0[3];  /* initial voxel (inside the box)                                */
+    float off0[3];
+    uint16_t label, label0;
+    float relax;      /* sum_i t_i / T2^(i), Eq.5                                      */
+    double phi[RMS_MAX_WAVES][3]; /* Phi_m = sum_i w_m[i] (x_i - x_0), voxel units     */
+} rms_walker_state;
+
+int rms_walkers_read(const rms_walkers* w, uint64_t first, uint64_t count, rms_walker_state* host_out,
+                     void* cuda_stream);
+int rms_walkers_steps_done(const rms_walkers* w, uint64_t* out /* host */);
+
+/* Tables the run derives from (D, kappa, dt): hop length s_L = sqrt(6 D_L dt)/l_p (Eq.1, d = 3) and the
+ * permeation probabilities P[a][b] of Eq.3, both as the fp32 values the kernels use.  Host outputs,
+ * s_out [n_labels], P_out [n_labels*n_labels] (may be NULL).  Pure host function. */
+int rms_tables(const rms_substrate* s, double dt_ms, float* s_out, float* P_out);
+
+/* H8 on its own: normalise reduced sums (e.g. after adding the sums of several walker-id shards).
+ * Host arrays laid out as in rms_result; t_ms [n_snap] diffusion time of each snapshot.  Pure host function:
+ *   S = (sum_c sig_re + i sum_c sig_im) / sum_c sum_alpha                         (Eq.7)
+ *   D = <alpha X^2> / (2 t <alpha>),  K = <alpha X^4><alpha> / <alpha X^2>^2 - 3   (R14)        */
+int rms_normalise(int n_classes, int n_q, const double* sum_alpha, const double* sig_re, const double* sig_im,
+                  int n_snap, int n_dir, const double* snap_alpha, const double* m2, const double* m4,
+                  const double* t_ms, double* S_re, double* S_im, double* Dapp, double* Kapp);
+
+const char* rms_last_error(void);
+const char* rms_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* RMS_H */

@@ -1,0 +1,189 @@
+// rms_internal.cuh -- shared declarations of the CUDA implementation behind include/rms.h.
+// Product code: shares nothing with oracle/ (the random-number counter scheme is restated here
+// from DESIGN.md "Random numbers", not included from the oracle).
+#pragma once
+
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <stdio.h>
+#include <string>
+#include <vector>
+
+#include "../../include/rms.h"
+
+// ------------------------------------------------------------------------------------------------
+// error plumbing
+// ------------------------------------------------------------------------------------------------
+void rms_set_error(const char* fmt, ...);
+
+#define RMS_CUDA_TRY(expr)                                                                         \
+    do {                                                                                           \
+        cudaError_t _e = (expr);                                                                   \
+        if (_e != cudaSuccess) {                                                                   \
+            rms_set_error("%s failed: %s (%s:%d)", #expr, cudaGetErrorString(_e), __FILE__, __LINE__); \
+            return (_e == cudaErrorMemoryAllocation) ? RMS_ERR_OOM : RMS_ERR_CUDA;                 \
+        }                                                                                          \
+    } while (0)
+
+#define RMS_REQUIRE(cond, code, ...)                                                               \
+    do {                                                                                           \
+        if (!(cond)) {                                                                             \
+            rms_set_error(__VA_ARGS__);                                                            \
+            return (code);                                                                         \
+        }                                                                                          \
+    } while (0)
+
+// ------------------------------------------------------------------------------------------------
+// handles
+// ------------------------------------------------------------------------------------------------
+struct rms_substrate {
+    int nx = 0, ny = 0, nz = 0;
+    double voxel_um = 0;
+    int n_labels = 0, n_classes = 0;
+    uint64_t n_vox = 0;
+    const uint16_t* d_labels = nullptr;  // device, x fastest
+    bool owns_labels = false;
+    // face-mask lattice: one byte per voxel of the lattice padded by a one-voxel periodic ghost shell,
+    // bit (k + 3*neg) = the face of this voxel towards +k (neg = 0) / -k (neg = 1) is a membrane,
+    // bit 6 = ghost voxel.
+    uint8_t* d_faces = nullptr;
+    int NX = 0, NY = 0, NZ = 0;          // padded dims (n + 2)
+    uint64_t n_membrane_faces = 0;
+    std::vector<float> D, T2, kappa;     // host copies of the per-label tables
+    std::vector<uint8_t> label_class;
+    uint8_t* d_label_class = nullptr;
+    bool all_impermeable = true;         // every off-diagonal kappa is 0
+};
+
+// Walker state between launches, structure of arrays (coalesced): during rms_run's step kernel the
+// state lives in registers; it is written back only at launch boundaries (snapshots, end of call).
+struct rms_walker_arrays {
+    int32_t* w[3];     // voxel inside the box
+    int32_t* dI[3];    // whole-voxel displacement since the start (unwrapped - initial)
+    float* f[3];       // in-voxel offset [0,1)
+    int32_t* v0[3];    // initial voxel
+    float* f0[3];      // initial offset
+    uint32_t* lab;     // label | label0 << 16
+    float* relax;      // sum t_i / T2_i (Eq.5)
+    double* phi;       // [n_wave_alloc*3][n]: Phi_m,k, voxel units
+};
+
+struct rms_walkers {
+    const rms_substrate* sub = nullptr;
+    uint64_t n = 0, first_id = 0, seed = 0;
+    uint64_t steps_done = 0;
+    int n_wave_alloc = 0;
+    rms_walker_arrays a{};
+    void* d_block = nullptr;   // one allocation behind all arrays but phi
+    unsigned long long* d_counters = nullptr;  // [8]
+};
+
+// ------------------------------------------------------------------------------------------------
+// random numbers: Philox4x32-10, key = (seed_lo, seed_hi), counter = (walker_lo, walker_hi, index, stream)
+// ------------------------------------------------------------------------------------------------
+enum { RMS_STREAM_INIT = 0, RMS_STREAM_DIR = 1, RMS_STREAM_PERM = 2, RMS_STREAM_INIT_OFFSET = 3 };
+
+#define RMS_PHILOX_M0 0xD2511F53u
+#define RMS_PHILOX_M1 0xCD9E8D57u
+#define RMS_PHILOX_W0 0x9E3779B9u
+#define RMS_PHILOX_W1 0xBB67AE85u
+
+struct rms_philox_keys { uint32_t k[20]; };  // round keys k0 + r*W0, k1 + r*W1, r = 0..9
+
+static inline rms_philox_keys rms_make_keys(uint64_t seed)
+{
+    rms_philox_keys rk;
+    uint32_t k0 = (uint32_t)seed, k1 = (uint32_t)(seed >> 32);
+    for (int r = 0; r < 10; ++r) {
+        rk.k[2 * r] = k0 + (uint32_t)r * RMS_PHILOX_W0;
+        rk.k[2 * r + 1] = k1 + (uint32_t)r * RMS_PHILOX_W1;
+    }
+    return rk;
+}
+
+#ifdef __CUDACC__
+__device__ __forceinline__ void rms_philox(const rms_philox_keys& rk, uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3,
+                                           uint32_t& o0, uint32_t& o1, uint32_t& o2, uint32_t& o3)
+{
+#pragma unroll
+    for (int r = 0; r < 10; ++r) {
+        const unsigned long long p0 = (unsigned long long)RMS_PHILOX_M0 * c0;
+        const unsigned long long p1 = (unsigned long long)RMS_PHILOX_M1 * c2;
+        const uint32_t n0 = (uint32_t)(p1 >> 32) ^ c1 ^ rk.k[2 * r];
+        const uint32_t n2 = (uint32_t)(p0 >> 32) ^ c3 ^ rk.k[2 * r + 1];
+        c1 = (uint32_t)p1;
+        c3 = (uint32_t)p0;
+        c0 = n0;
+        c2 = n2;
+    }
+    o0 = c0; o1 = c1; o2 = c2; o3 = c3;
+}
+
+// words -> reals, exact in fp32: sym(w) = (2 (w>>9) + 1 - 2^23) 2^-23, uni(w) = (w>>8) 2^-24
+__device__ __forceinline__ float rms_sym(uint32_t w)
+{
+    const float m = __uint_as_float((w >> 9) | 0x3F800000u);  // 1 + k 2^-23
+    return fmaf(m - 1.5f, 2.0f, 1.1920928955078125e-07f);     // exact: odd multiple of 2^-23
+}
+__device__ __forceinline__ float rms_uni(uint32_t w) { return (float)(w >> 8) * 5.9604644775390625e-08f; }
+#endif
+
+// ------------------------------------------------------------------------------------------------
+// step kernel parameters
+// ------------------------------------------------------------------------------------------------
+struct rms_segment {          // a run of steps on which every waveform is constant (integer valued)
+    uint32_t n;               // steps in the segment
+    uint32_t flags;           // bit 0: some w != 0 ; bit 1: some remaining weight != 0 inside the segment
+    int32_t w[RMS_MAX_WAVES];
+    int32_t wrem_end[RMS_MAX_WAVES];  // sum of w over the steps of this launch after the segment
+};
+
+enum { RMS_WMODE_CONST = 0, RMS_WMODE_TABLE = 1 };
+enum { RMS_LAT_LABELS = 0, RMS_LAT_FACES = 1 };
+
+struct rms_step_params {
+    int nx, ny, nz;
+    const uint16_t* labels;
+    const uint8_t* faces;
+    int NX, NY;               // padded dims of the face lattice
+    rms_walker_arrays st;
+    uint64_t n, first_id;
+    rms_philox_keys rk;
+    const float* s_tab;       // [n_labels] hop length in voxels
+    const float* P512;        // [n_labels^2] 512 * P(a->b)
+    const float* rate;        // [n_labels] dt / T2
+    int n_labels;
+    uint32_t step0;           // steps done before this launch
+    uint32_t n_steps;         // steps of this launch
+    int n_seg;
+    const rms_segment* segs;  // device (CONST mode)
+    const float* wave;        // device, [n_wave][wave_stride], element 0 = first step of this launch (TABLE mode)
+    const double* wsuf;       // device, same indexing: suffix sum of w from this step to the end of the call
+    int64_t wave_stride;
+    int64_t wsuf_stride;
+    double wsuf_end[RMS_MAX_WAVES];  // suffix sum just after the last step of this launch
+    double wtot[RMS_MAX_WAVES];      // sum of w over the steps of this launch
+    int n_wave;
+    unsigned long long* counters;    // [0] encounters [1] permeations [2] clamps [3] init failures
+};
+
+int rms_launch_step(const rms_step_params& p, int n_wave, int wmode, int lat, bool permeable, cudaStream_t stream);
+
+// reductions (rms_reduce.cu)
+struct rms_reduce_params {
+    rms_walker_arrays st;
+    uint64_t n;
+    const uint8_t* label_class;  // device
+    int n_classes;
+    const float* rate;           // device [n_labels] (unused: relax is final at launch end)
+    int n_dir;
+    const double* dirs;          // device [n_dir*3]
+    double voxel_um;
+};
+int rms_launch_moments(const rms_reduce_params& p, double* d_m2, double* d_m4, double* d_alpha,
+                       unsigned long long* d_flow, cudaStream_t stream);
+// qv: device [nq*3] phase per unit Phi in turns; qwave: device [nq] waveform index
+int rms_launch_signal(const rms_reduce_params& p, int n_wave, int nq, const double* d_qv, const int* d_qwave, double* d_re,
+                      double* d_im, double* d_sum_alpha, cudaStream_t stream, unsigned* n_launches);
+int rms_compute_tables(const rms_substrate* s, double dt, std::vector<float>& s_tab, std::vector<float>& P_tab);
+int rms_walkers_reserve_waves(rms_walkers* w, int n_wave, cudaStream_t stream);

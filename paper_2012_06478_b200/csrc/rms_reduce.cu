@@ -1,0 +1,224 @@
+// rms_reduce.cu -- H6/H7: per-walker epilogue and the reductions to signal and moment sums.
+//
+//   moments: thread = walker; X = l_p n.(x - x0) per direction; warp-shuffle reduction per class, then
+//            shared-memory fp64 accumulators per block, then fp64 atomics (one per block and output).
+//   signal:  thread = one (waveform, gradient amplitude, direction) triple; the block stages a tile of
+//            walkers in shared memory and every thread sums alpha e^{-i phi} over the tile in registers
+//            (the walker is warp-uniform, so class handling never diverges); fp64 throughout the phase
+//            reduction to a fraction of a turn, fp32 sincospi on the fraction.
+#include "rms_internal.cuh"
+
+#define RED_BLOCK 256
+
+__device__ __forceinline__ double warp_sum(double v)
+{
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    return v;
+}
+
+// ------------------------------------------------------------------------------------------------
+// moments at a snapshot
+// ------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(RED_BLOCK) rms_moments_kernel(const rms_reduce_params p, double* __restrict__ g_m2,
+                                                                 double* __restrict__ g_m4, double* __restrict__ g_alpha,
+                                                                 unsigned long long* __restrict__ g_flow, int use_smem)
+{
+    extern __shared__ double sm[];   // [n_dir*n_classes] m2, then m4, then [n_classes] alpha
+    const int nD = p.n_dir, nC = p.n_classes;
+    const int n_acc = 2 * nD * nC + nC;
+    if (use_smem) {
+        for (int t = threadIdx.x; t < n_acc; t += RED_BLOCK) sm[t] = 0.0;
+        __syncthreads();
+    }
+    double* a_m2 = use_smem ? sm : g_m2;
+    double* a_m4 = use_smem ? sm + nD * nC : g_m4;
+    double* a_al = use_smem ? sm + 2 * nD * nC : g_alpha;
+    const int lane = threadIdx.x & 31;
+
+    const uint64_t n_tiles = (p.n + RED_BLOCK - 1) / RED_BLOCK;
+    for (uint64_t tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
+        const uint64_t i = tile * RED_BLOCK + threadIdx.x;
+        const bool valid = i < p.n;
+        double dx = 0, dy = 0, dz = 0, alpha = 0;
+        int c0 = -1, cn = 0;
+        if (valid) {
+            dx = (double)p.st.dI[0][i] + ((double)p.st.f[0][i] - (double)p.st.f0[0][i]);
+            dy = (double)p.st.dI[1][i] + ((double)p.st.f[1][i] - (double)p.st.f0[1][i]);
+            dz = (double)p.st.dI[2][i] + ((double)p.st.f[2][i] - (double)p.st.f0[2][i]);
+            alpha = exp(-(double)p.st.relax[i]);          // Eq.5
+            const uint32_t lab = p.st.lab[i];
+            c0 = p.label_class[lab >> 16];
+            cn = p.label_class[lab & 0xFFFFu];
+        }
+        {   // class_flow: one atomic per distinct (initial class, class now) pair in the warp
+            const int key = valid ? c0 * nC + cn : -1;
+            const unsigned same = __match_any_sync(0xffffffffu, key);
+            if (valid && lane == __ffs(same) - 1) atomicAdd(&g_flow[key], (unsigned long long)__popc(same));
+        }
+        // classes present in this warp, one at a time (2 in the usual intra/extra split)
+        unsigned todo = __ballot_sync(0xffffffffu, valid);
+        while (todo) {
+            const int leader = __ffs(todo) - 1;
+            const int cc = __shfl_sync(0xffffffffu, c0, leader);
+            const bool mine = valid && (c0 == cc);
+            todo &= ~__ballot_sync(0xffffffffu, mine);
+            const double a = mine ? alpha : 0.0;
+            const double sa = warp_sum(a);
+            if (lane == 0) atomicAdd(&a_al[cc], sa);
+            for (int d = 0; d < nD; ++d) {
+                const double X = p.voxel_um * (p.dirs[3 * d] * dx + p.dirs[3 * d + 1] * dy + p.dirs[3 * d + 2] * dz);
+                const double X2 = X * X;
+                const double s2 = warp_sum(a * X2);
+                const double s4 = warp_sum(a * X2 * X2);
+                if (lane == 0) {
+                    atomicAdd(&a_m2[d * nC + cc], s2);
+                    atomicAdd(&a_m4[d * nC + cc], s4);
+                }
+            }
+        }
+    }
+    if (use_smem) {
+        __syncthreads();
+        for (int t = threadIdx.x; t < n_acc; t += RED_BLOCK) {
+            const double v = sm[t];
+            if (v != 0.0) {
+                if (t < nD * nC) atomicAdd(&g_m2[t], v);
+                else if (t < 2 * nD * nC) atomicAdd(&g_m4[t - nD * nC], v);
+                else atomicAdd(&g_alpha[t - 2 * nD * nC], v);
+            }
+        }
+    }
+}
+
+int rms_launch_moments(const rms_reduce_params& p, double* d_m2, double* d_m4, double* d_alpha, unsigned long long* d_flow,
+                       cudaStream_t stream)
+{
+    const size_t n_acc = (size_t)2 * p.n_dir * p.n_classes + p.n_classes;
+    const int use_smem = n_acc * sizeof(double) <= 40 * 1024;
+    const uint64_t n_tiles = (p.n + RED_BLOCK - 1) / RED_BLOCK;
+    const unsigned grid = (unsigned)(n_tiles < 148ull * 4 ? n_tiles : 148ull * 4);
+    rms_moments_kernel<<<grid, RED_BLOCK, use_smem ? n_acc * sizeof(double) : 0, stream>>>(p, d_m2, d_m4, d_alpha, d_flow,
+                                                                                          use_smem);
+    RMS_CUDA_TRY(cudaGetLastError());
+    return RMS_OK;
+}
+
+// ------------------------------------------------------------------------------------------------
+// signal sums at the end of a call
+// ------------------------------------------------------------------------------------------------
+#define SIG_TILE 256
+#define SIG_QPT 4   // q-triples per thread: a launch covers up to RED_BLOCK * SIG_QPT of them
+
+__global__ void __launch_bounds__(RED_BLOCK) rms_signal_kernel(const rms_reduce_params p, int n_wave, int nq_l, int q_begin,
+                                                                const double* __restrict__ qv, const int* __restrict__ qwave,
+                                                                double* __restrict__ g_re, double* __restrict__ g_im,
+                                                                double* __restrict__ g_sum_alpha)
+{
+    extern __shared__ double sm[];
+    const int nC = p.n_classes;
+    double* s_phi = sm;                                             // [n_wave*3][SIG_TILE]
+    double* s_acc = s_phi + (size_t)n_wave * 3 * SIG_TILE;          // [nq_l][nC][2]
+    double* s_alsum = s_acc + (size_t)nq_l * nC * 2;                // [nC]
+    float* s_alpha = (float*)(s_alsum + nC);                        // [SIG_TILE]
+    int* s_cls = (int*)(s_alpha + SIG_TILE);                        // [SIG_TILE]
+
+    for (int t = threadIdx.x; t < nq_l * nC * 2 + nC; t += RED_BLOCK) s_acc[t] = 0.0;
+
+    double qx[SIG_QPT], qy[SIG_QPT], qz[SIG_QPT];
+    int qm[SIG_QPT];
+#pragma unroll
+    for (int c = 0; c < SIG_QPT; ++c) {
+        const int jl = c * RED_BLOCK + threadIdx.x;
+        const bool ok = jl < nq_l;
+        const int j = q_begin + jl;
+        qx[c] = ok ? qv[3 * j] : 0.0; qy[c] = ok ? qv[3 * j + 1] : 0.0; qz[c] = ok ? qv[3 * j + 2] : 0.0;
+        qm[c] = ok ? qwave[j] : -1;
+    }
+
+    const uint64_t n_tiles = (p.n + SIG_TILE - 1) / SIG_TILE;
+    for (uint64_t tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
+        __syncthreads();
+        const uint64_t i = tile * SIG_TILE + threadIdx.x;
+        const int n_in = (int)min((uint64_t)SIG_TILE, p.n - tile * SIG_TILE);
+        if (threadIdx.x < n_in) {
+            for (int k = 0; k < 3 * n_wave; ++k) s_phi[k * SIG_TILE + threadIdx.x] = p.st.phi[(size_t)k * p.n + i];
+            const float al = (float)exp(-(double)p.st.relax[i]);
+            const int c0 = p.label_class[p.st.lab[i] >> 16];
+            s_alpha[threadIdx.x] = al;
+            s_cls[threadIdx.x] = c0;
+            if (q_begin == 0) atomicAdd(&s_alsum[c0], (double)al);
+        }
+        __syncthreads();
+        for (int cc = 0; cc < nC; ++cc) {
+            double are[SIG_QPT], aim[SIG_QPT];
+#pragma unroll
+            for (int c = 0; c < SIG_QPT; ++c) { are[c] = 0.0; aim[c] = 0.0; }
+            bool any = false;
+            for (int w = 0; w < n_in; ++w) {
+                if (s_cls[w] != cc) continue;                    // warp-uniform
+                any = true;
+                const double al = (double)s_alpha[w];
+#pragma unroll
+                for (int c = 0; c < SIG_QPT; ++c) {
+                    if (qm[c] < 0) continue;
+                    const double* ph = s_phi + (size_t)qm[c] * 3 * SIG_TILE + w;
+                    const double turns = qx[c] * ph[0] + qy[c] * ph[SIG_TILE] + qz[c] * ph[2 * SIG_TILE];
+                    const float fr = (float)(2.0 * (turns - rint(turns)));   // phase / pi in [-1, 1]
+                    float sn, cs;
+                    sincospif(fr, &sn, &cs);
+                    are[c] += al * (double)cs;                   // Eq.7: alpha e^{-i phi}
+                    aim[c] -= al * (double)sn;
+                }
+            }
+            if (any) {
+#pragma unroll
+                for (int c = 0; c < SIG_QPT; ++c) {
+                    const int jl = c * RED_BLOCK + threadIdx.x;
+                    if (jl < nq_l) {
+                        s_acc[((size_t)jl * nC + cc) * 2] += are[c];      // (jl, cc) is owned by this thread
+                        s_acc[((size_t)jl * nC + cc) * 2 + 1] += aim[c];
+                    }
+                }
+            }
+        }
+    }
+    __syncthreads();
+    for (int t = threadIdx.x; t < nq_l * nC; t += RED_BLOCK) {
+        const int jl = t / nC, cc = t - jl * nC;
+        const size_t o = (size_t)(q_begin + jl) * nC + cc;
+        atomicAdd(&g_re[o], s_acc[2 * t]);
+        atomicAdd(&g_im[o], s_acc[2 * t + 1]);
+    }
+    if (q_begin == 0)
+        for (int t = threadIdx.x; t < nC; t += RED_BLOCK)
+            if (s_alsum[t] != 0.0) atomicAdd(&g_sum_alpha[t], s_alsum[t]);
+}
+
+int rms_launch_signal(const rms_reduce_params& p, int n_wave, int nq, const double* d_qv, const int* d_qwave, double* d_re,
+                      double* d_im, double* d_sum_alpha, cudaStream_t stream, unsigned* n_launches)
+{
+    const uint64_t n_tiles = (p.n + SIG_TILE - 1) / SIG_TILE;
+    const unsigned grid = (unsigned)(n_tiles < 148ull * 2 ? n_tiles : 148ull * 2);
+    const int nw = n_wave > 0 ? n_wave : 1;
+    const size_t fixed = ((size_t)nw * 3 * SIG_TILE + p.n_classes) * sizeof(double) + SIG_TILE * (sizeof(float) + sizeof(int));
+    const size_t budget = 160 * 1024;
+    const size_t per_q = (size_t)p.n_classes * 2 * sizeof(double);
+    if (fixed + per_q > budget) {
+        rms_set_error("signal reduction: n_classes = %d needs more shared memory than a block has", p.n_classes);
+        return RMS_ERR_UNSUPPORTED;
+    }
+    int q_batch = (int)((budget - fixed) / per_q);
+    if (q_batch > RED_BLOCK * SIG_QPT) q_batch = RED_BLOCK * SIG_QPT;
+    int q_begin = 0;
+    do {   // nq == 0: still one launch, for sum_alpha
+        const int nq_l = nq - q_begin < q_batch ? nq - q_begin : q_batch;
+        const size_t smem = fixed + (size_t)(nq_l > 0 ? nq_l : 0) * per_q;
+        if (smem > 48 * 1024)
+            RMS_CUDA_TRY(cudaFuncSetAttribute(rms_signal_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)budget));
+        rms_signal_kernel<<<grid, RED_BLOCK, smem, stream>>>(p, nw, nq_l, q_begin, d_qv, d_qwave, d_re, d_im, d_sum_alpha);
+        RMS_CUDA_TRY(cudaGetLastError());
+        if (n_launches) ++*n_launches;
+        q_begin += q_batch;
+    } while (q_begin < nq);
+    return RMS_OK;
+}

@@ -1,0 +1,321 @@
+// rms_run.cu -- rms_run: host orchestration of the step launches, the reductions and H8 (normalisation).
+#include <math.h>
+#include <string.h>
+
+#include <algorithm>
+
+#include "rms_internal.cuh"
+
+namespace {
+
+struct DeviceBuf {   // frees on scope exit
+    void* p = nullptr;
+    ~DeviceBuf() { if (p) cudaFree(p); }
+    template <class T> T* as() { return (T*)p; }
+};
+
+struct Events {
+    std::vector<cudaEvent_t> ev;
+    ~Events() { for (auto e : ev) cudaEventDestroy(e); }
+    cudaEvent_t make() { cudaEvent_t e = nullptr; cudaEventCreate(&e); ev.push_back(e); return e; }
+};
+
+// Is every weight an integer small enough for the exact int32 path (piecewise-constant gradients such as PGSE)?
+bool wave_is_integer(const float* wave, size_t count)
+{
+    for (size_t i = 0; i < count; ++i) {
+        const float w = wave[i];
+        if (!(fabsf(w) <= 32767.f) || w != rintf(w)) return false;
+    }
+    return true;
+}
+
+}  // namespace
+
+// H8: Eq.7 S = <alpha e^{-i phi}> / <alpha>, and the narrow-pulse D, K of P:174 with both moments
+// normalised by <alpha> (R14).  Classes are pooled.  Pure host arithmetic on the reduced sums.
+extern "C" int rms_normalise(int n_classes, int n_q, const double* sum_alpha, const double* sig_re, const double* sig_im,
+                             int n_snap, int n_dir, const double* snap_alpha, const double* m2, const double* m4,
+                             const double* t_ms, double* S_re, double* S_im, double* Dapp, double* Kapp)
+{
+    RMS_REQUIRE(n_classes > 0 && n_q >= 0 && n_snap >= 0 && n_dir >= 0, RMS_ERR_ARG, "rms_normalise: bad counts");
+    RMS_REQUIRE(n_q == 0 || (sum_alpha && sig_re && sig_im), RMS_ERR_ARG, "rms_normalise: null signal sums");
+    RMS_REQUIRE(n_snap * n_dir == 0 || (snap_alpha && m2 && m4 && t_ms), RMS_ERR_ARG, "rms_normalise: null moment sums");
+    const int nC = n_classes;
+    double tot_alpha = 0.0;
+    for (int c = 0; c < nC && sum_alpha; ++c) tot_alpha += sum_alpha[c];
+    for (int q = 0; q < n_q; ++q) {
+        double re = 0, im = 0;
+        for (int c = 0; c < nC; ++c) { re += sig_re[(size_t)q * nC + c]; im += sig_im[(size_t)q * nC + c]; }
+        if (S_re) S_re[q] = re / tot_alpha;
+        if (S_im) S_im[q] = im / tot_alpha;
+    }
+    for (int s = 0; s < n_snap; ++s) {
+        double al = 0;
+        for (int c = 0; c < nC; ++c) al += snap_alpha[(size_t)s * nC + c];
+        for (int k = 0; k < n_dir; ++k) {
+            double a2 = 0, a4 = 0;
+            for (int c = 0; c < nC; ++c) {
+                a2 += m2[((size_t)s * n_dir + k) * nC + c];
+                a4 += m4[((size_t)s * n_dir + k) * nC + c];
+            }
+            a2 /= al; a4 /= al;
+            if (Dapp) Dapp[(size_t)s * n_dir + k] = a2 / (2.0 * t_ms[s]);
+            if (Kapp) Kapp[(size_t)s * n_dir + k] = a4 / (a2 * a2) - 3.0;
+        }
+    }
+    return RMS_OK;
+}
+
+extern "C" int rms_run(const rms_substrate* s, rms_walkers* w, const rms_run_desc* d, void* cuda_stream, rms_result* out)
+{
+    RMS_REQUIRE(s && w && d && out, RMS_ERR_ARG, "rms_run: null argument");
+    RMS_REQUIRE(w->sub == s, RMS_ERR_ARG, "rms_run: walkers were initialised on another substrate");
+    RMS_REQUIRE(d->n_steps >= 0, RMS_ERR_ARG, "n_steps is negative");
+    RMS_REQUIRE(d->n_wave >= 0 && d->n_g >= 0 && d->n_dir >= 0 && d->n_snap >= 0, RMS_ERR_ARG, "negative count in rms_run_desc");
+    RMS_REQUIRE(d->n_wave <= RMS_MAX_WAVES, RMS_ERR_UNSUPPORTED, "n_wave = %d is above RMS_MAX_WAVES = %d", d->n_wave,
+                RMS_MAX_WAVES);
+    RMS_REQUIRE(d->n_wave == 0 || (d->wave && (d->n_g == 0 || d->gamp)), RMS_ERR_ARG, "wave / gamp is null");
+    RMS_REQUIRE(d->n_dir == 0 || d->dirs, RMS_ERR_ARG, "dirs is null");
+    RMS_REQUIRE(d->n_snap == 0 || d->snap_steps, RMS_ERR_ARG, "snap_steps is null");
+    RMS_REQUIRE(w->steps_done + (uint64_t)d->n_steps < 0xFFFFFFF0ull, RMS_ERR_UNSUPPORTED, "more than 2^32 steps per walker");
+    for (int i = 0; i < d->n_dir; ++i) {
+        const double* n = d->dirs + 3 * i;
+        RMS_REQUIRE(fabs(n[0] * n[0] + n[1] * n[1] + n[2] * n[2] - 1.0) <= 1e-6, RMS_ERR_ARG, "dirs[%d] is not a unit vector", i);
+    }
+    for (int i = 0; i < d->n_snap; ++i) {
+        RMS_REQUIRE(d->snap_steps[i] >= 1 && d->snap_steps[i] <= d->n_steps, RMS_ERR_ARG, "snap_steps[%d] outside 1..n_steps", i);
+        RMS_REQUIRE(i == 0 || d->snap_steps[i] > d->snap_steps[i - 1], RMS_ERR_ARG, "snap_steps must be strictly ascending");
+    }
+    for (size_t i = 0; i < (size_t)d->n_wave * d->n_steps; ++i)
+        RMS_REQUIRE(isfinite(d->wave[i]), RMS_ERR_ARG, "wave[%zu] is not finite", i);
+
+    cudaStream_t stream = (cudaStream_t)cuda_stream;
+    const int nL = s->n_labels, nC = s->n_classes, nW = d->n_wave, nG = d->n_g, nD = d->n_dir, nS = d->n_snap;
+    const int64_t nT = d->n_steps;
+    const uint64_t n = w->n;
+
+    // ---- H0 (run-time part): tables from (D, kappa, T2, dt) ---------------------------------------
+    std::vector<float> s_tab, P_tab;
+    int rc = rms_compute_tables(s, d->dt_ms, s_tab, P_tab);
+    if (rc != RMS_OK) return rc;
+    std::vector<float> tabs((size_t)nL * 2 + (size_t)nL * nL);
+    float* h_s = tabs.data();
+    float* h_rate = h_s + nL;
+    float* h_P512 = h_rate + nL;
+    bool permeable = false;
+    for (int a = 0; a < nL; ++a) {
+        h_s[a] = s_tab[a];
+        const float t2 = s->T2[a];
+        h_rate[a] = (t2 > 0 && isfinite(t2)) ? (float)(d->dt_ms / (double)t2) : 0.f;
+        for (int b = 0; b < nL; ++b) {
+            h_P512[(size_t)a * nL + b] = 512.f * P_tab[(size_t)a * nL + b];
+            if (a != b && P_tab[(size_t)a * nL + b] > 0.f) permeable = true;
+        }
+    }
+    const bool want_labels = (d->flags & RMS_RUN_LABEL_GATHER) != 0;
+    const int lat = (!permeable && s->d_faces && !want_labels) ? RMS_LAT_FACES : RMS_LAT_LABELS;
+
+    rc = rms_walkers_reserve_waves(w, nW, stream);
+    if (rc != RMS_OK) return rc;
+
+    // ---- waveform analysis ---------------------------------------------------------------------------
+    // suffix sums S[m][j] = sum_{i > j} w_m[i] (j = 0..nT, steps are 1-based), fp64
+    std::vector<double> suf((size_t)std::max(nW, 1) * (nT + 1), 0.0);
+    for (int m = 0; m < nW; ++m) {
+        double acc = 0.0;
+        double* S = &suf[(size_t)m * (nT + 1)];
+        for (int64_t j = nT; j >= 1; --j) { acc += (double)d->wave[(size_t)m * nT + (j - 1)]; S[j - 1] = acc; }
+    }
+    bool const_mode = wave_is_integer(d->wave, (size_t)nW * nT);
+    for (size_t i = 0; const_mode && i < suf.size(); ++i) const_mode = fabs(suf[i]) < 1073741824.0;
+
+    // launch boundaries: snapshots and the end of the call
+    std::vector<int64_t> bounds;
+    for (int i = 0; i < nS; ++i) bounds.push_back(d->snap_steps[i]);
+    if (bounds.empty() || bounds.back() != nT) bounds.push_back(nT);
+
+    std::vector<rms_segment> segs;
+    std::vector<std::pair<size_t, size_t>> seg_range;   // per launch: [first, count)
+    if (const_mode) {
+        int64_t a = 0;
+        for (int64_t b : bounds) {
+            const size_t first = segs.size();
+            int64_t j = a;
+            while (j < b) {
+                int64_t e = j + 1;
+                auto same = [&](int64_t x, int64_t y) {
+                    for (int m = 0; m < nW; ++m)
+                        if (d->wave[(size_t)m * nT + x] != d->wave[(size_t)m * nT + y]) return false;
+                    return true;
+                };
+                while (e < b && same(j, e)) ++e;
+                rms_segment sg;
+                memset(&sg, 0, sizeof sg);
+                sg.n = (uint32_t)(e - j);
+                for (int m = 0; m < nW; ++m) {
+                    sg.w[m] = (int32_t)d->wave[(size_t)m * nT + j];
+                    sg.wrem_end[m] = (int32_t)llrint(suf[(size_t)m * (nT + 1) + e] - suf[(size_t)m * (nT + 1) + b]);
+                    if (sg.w[m] != 0) sg.flags |= 3u;
+                    if (sg.wrem_end[m] != 0) sg.flags |= 2u;
+                }
+                segs.push_back(sg);
+                j = e;
+            }
+            seg_range.push_back({first, segs.size() - first});
+            a = b;
+        }
+        if (segs.size() > (1u << 20)) { const_mode = false; segs.clear(); seg_range.clear(); }
+    }
+    const int wmode = const_mode ? RMS_WMODE_CONST : RMS_WMODE_TABLE;
+
+    // ---- device scratch: tables | segments or wave tables | q vectors | result sums -------------------
+    const int nQ = nW * nG * nD;
+    const size_t n_sig = (size_t)nQ * nC, n_mom = (size_t)nS * nD * nC, n_sal = (size_t)nS * nC, n_flow = (size_t)nS * nC * nC;
+    const size_t n_res_d = 2 * n_sig + 2 * n_mom + n_sal + nC;       // doubles
+    DeviceBuf b_tabs, b_segs, b_wave, b_wsuf, b_q, b_res, b_dirs;
+    RMS_CUDA_TRY(cudaMalloc(&b_tabs.p, tabs.size() * sizeof(float)));
+    RMS_CUDA_TRY(cudaMemcpyAsync(b_tabs.p, tabs.data(), tabs.size() * sizeof(float), cudaMemcpyHostToDevice, stream));
+    if (const_mode) {
+        if (!segs.empty()) {
+            RMS_CUDA_TRY(cudaMalloc(&b_segs.p, segs.size() * sizeof(rms_segment)));
+            RMS_CUDA_TRY(cudaMemcpyAsync(b_segs.p, segs.data(), segs.size() * sizeof(rms_segment), cudaMemcpyHostToDevice, stream));
+        }
+    } else if (nW > 0 && nT > 0) {
+        RMS_CUDA_TRY(cudaMalloc(&b_wave.p, (size_t)nW * nT * sizeof(float)));
+        RMS_CUDA_TRY(cudaMemcpyAsync(b_wave.p, d->wave, (size_t)nW * nT * sizeof(float), cudaMemcpyHostToDevice, stream));
+        RMS_CUDA_TRY(cudaMalloc(&b_wsuf.p, (size_t)nW * (nT + 1) * sizeof(double)));
+        RMS_CUDA_TRY(cudaMemcpyAsync(b_wsuf.p, suf.data(), (size_t)nW * (nT + 1) * sizeof(double), cudaMemcpyHostToDevice, stream));
+    }
+    // phase per unit Phi, in turns: gamp dt l_p n / (2 pi)   (Eq.7 with the right-endpoint rule, R11)
+    std::vector<double> qv((size_t)std::max(nQ, 1) * 3, 0.0);
+    std::vector<int> qwave(std::max(nQ, 1), 0);
+    for (int m = 0; m < nW; ++m)
+        for (int g = 0; g < nG; ++g)
+            for (int k = 0; k < nD; ++k) {
+                const size_t q = ((size_t)m * nG + g) * nD + k;
+                const double c = d->gamp[(size_t)m * nG + g] * d->dt_ms * s->voxel_um / (2.0 * 3.14159265358979323846);
+                for (int x = 0; x < 3; ++x) qv[3 * q + x] = c * d->dirs[3 * k + x];
+                qwave[q] = m;
+            }
+    RMS_CUDA_TRY(cudaMalloc(&b_q.p, qv.size() * sizeof(double) + qwave.size() * sizeof(int)));
+    RMS_CUDA_TRY(cudaMemcpyAsync(b_q.p, qv.data(), qv.size() * sizeof(double), cudaMemcpyHostToDevice, stream));
+    int* d_qwave = (int*)(b_q.as<double>() + qv.size());
+    RMS_CUDA_TRY(cudaMemcpyAsync(d_qwave, qwave.data(), qwave.size() * sizeof(int), cudaMemcpyHostToDevice, stream));
+    RMS_CUDA_TRY(cudaMalloc(&b_dirs.p, std::max(nD, 1) * 3 * sizeof(double)));
+    if (nD) RMS_CUDA_TRY(cudaMemcpyAsync(b_dirs.p, d->dirs, (size_t)nD * 3 * sizeof(double), cudaMemcpyHostToDevice, stream));
+    const size_t res_bytes = n_res_d * sizeof(double) + n_flow * sizeof(unsigned long long);
+    RMS_CUDA_TRY(cudaMalloc(&b_res.p, res_bytes));
+    RMS_CUDA_TRY(cudaMemsetAsync(b_res.p, 0, res_bytes, stream));
+    double* d_re = b_res.as<double>();
+    double* d_im = d_re + n_sig;
+    double* d_m2 = d_im + n_sig;
+    double* d_m4 = d_m2 + n_mom;
+    double* d_sal = d_m4 + n_mom;
+    double* d_sum_alpha = d_sal + n_sal;
+    unsigned long long* d_flow = (unsigned long long*)(d_sum_alpha + nC);
+    RMS_CUDA_TRY(cudaMemsetAsync(w->d_counters, 0, 64, stream));
+
+    // ---- launches ------------------------------------------------------------------------------------
+    Events evs;
+    cudaEvent_t ev_begin = evs.make(), ev_end = evs.make();
+    std::vector<std::pair<cudaEvent_t, cudaEvent_t>> step_ev;
+    RMS_CUDA_TRY(cudaEventRecord(ev_begin, stream));
+    unsigned n_launches = 0;
+
+    rms_step_params sp;
+    memset(&sp, 0, sizeof sp);
+    sp.nx = s->nx; sp.ny = s->ny; sp.nz = s->nz;
+    sp.labels = s->d_labels; sp.faces = s->d_faces; sp.NX = s->NX; sp.NY = s->NY;
+    sp.st = w->a; sp.n = n; sp.first_id = w->first_id; sp.rk = rms_make_keys(w->seed);
+    sp.s_tab = b_tabs.as<float>(); sp.rate = sp.s_tab + nL; sp.P512 = sp.rate + nL; sp.n_labels = nL;
+    sp.counters = w->d_counters; sp.n_wave = nW; sp.wave_stride = nT; sp.wsuf_stride = nT + 1;
+
+    rms_reduce_params rp;
+    memset(&rp, 0, sizeof rp);
+    rp.st = w->a; rp.n = n; rp.label_class = s->d_label_class; rp.n_classes = nC; rp.n_dir = nD;
+    rp.dirs = b_dirs.as<double>(); rp.voxel_um = s->voxel_um;
+
+    int64_t a = 0;
+    int snap = 0;
+    for (size_t li = 0; li < bounds.size(); ++li) {
+        const int64_t b = bounds[li];
+        if (b > a) {
+            sp.step0 = (uint32_t)(w->steps_done + (uint64_t)a);
+            sp.n_steps = (uint32_t)(b - a);
+            for (int m = 0; m < nW; ++m) {
+                const double* S = &suf[(size_t)m * (nT + 1)];
+                sp.wtot[m] = S[a] - S[b];
+                sp.wsuf_end[m] = S[b];
+            }
+            if (const_mode) {
+                sp.n_seg = (int)seg_range[li].second;
+                sp.segs = b_segs.as<rms_segment>() + seg_range[li].first;
+            } else {
+                sp.n_seg = 1;
+                sp.wave = b_wave.as<float>() ? b_wave.as<float>() + a : nullptr;
+                // wsuf element 0 must be the suffix sum that includes the first step of this launch: S[a]
+                sp.wsuf = b_wsuf.as<double>() ? b_wsuf.as<double>() + a : nullptr;
+            }
+            cudaEvent_t e0 = evs.make(), e1 = evs.make();
+            RMS_CUDA_TRY(cudaEventRecord(e0, stream));
+            rc = rms_launch_step(sp, nW, wmode, lat, permeable, stream);
+            if (rc != RMS_OK) return rc;
+            RMS_CUDA_TRY(cudaEventRecord(e1, stream));
+            step_ev.push_back({e0, e1});
+            ++n_launches;
+        }
+        while (snap < nS && d->snap_steps[snap] == b) {
+            rc = rms_launch_moments(rp, d_m2 + (size_t)snap * nD * nC, d_m4 + (size_t)snap * nD * nC, d_sal + (size_t)snap * nC,
+                                    d_flow + (size_t)snap * nC * nC, stream);
+            if (rc != RMS_OK) return rc;
+            ++n_launches;
+            ++snap;
+        }
+        a = b;
+    }
+    rc = rms_launch_signal(rp, nW, nQ, b_q.as<double>(), d_qwave, d_re, d_im, d_sum_alpha, stream, &n_launches);
+    if (rc != RMS_OK) return rc;
+    RMS_CUDA_TRY(cudaEventRecord(ev_end, stream));
+
+    // ---- read back and normalise (H8) -------------------------------------------------------------
+    std::vector<double> h_res(n_res_d);
+    std::vector<unsigned long long> h_flow(std::max<size_t>(n_flow, 1));
+    unsigned long long h_cnt[8] = {0};
+    RMS_CUDA_TRY(cudaMemcpyAsync(h_res.data(), b_res.p, n_res_d * sizeof(double), cudaMemcpyDeviceToHost, stream));
+    if (n_flow) RMS_CUDA_TRY(cudaMemcpyAsync(h_flow.data(), d_flow, n_flow * sizeof(unsigned long long), cudaMemcpyDeviceToHost, stream));
+    RMS_CUDA_TRY(cudaMemcpyAsync(h_cnt, w->d_counters, 64, cudaMemcpyDeviceToHost, stream));
+    RMS_CUDA_TRY(cudaStreamSynchronize(stream));
+    RMS_CUDA_TRY(cudaGetLastError());
+
+    const double* h_re = h_res.data();
+    const double* h_im = h_re + n_sig;
+    const double* h_m2 = h_im + n_sig;
+    const double* h_m4 = h_m2 + n_mom;
+    const double* h_sal = h_m4 + n_mom;
+    const double* h_sum_alpha = h_sal + n_sal;
+    if (out->sum_alpha) memcpy(out->sum_alpha, h_sum_alpha, nC * sizeof(double));
+    if (out->sig_re) memcpy(out->sig_re, h_re, n_sig * sizeof(double));
+    if (out->sig_im) memcpy(out->sig_im, h_im, n_sig * sizeof(double));
+    if (out->m2) memcpy(out->m2, h_m2, n_mom * sizeof(double));
+    if (out->m4) memcpy(out->m4, h_m4, n_mom * sizeof(double));
+    if (out->snap_alpha) memcpy(out->snap_alpha, h_sal, n_sal * sizeof(double));
+    if (out->class_flow && n_flow) memcpy(out->class_flow, h_flow.data(), n_flow * sizeof(uint64_t));
+    {
+        std::vector<double> t_ms(std::max(nS, 1));
+        for (int sidx = 0; sidx < nS; ++sidx) t_ms[sidx] = (double)(w->steps_done + (uint64_t)d->snap_steps[sidx]) * d->dt_ms;
+        rms_normalise(nC, nQ, h_sum_alpha, h_re, h_im, nS, nD, h_sal, h_m2, h_m4, t_ms.data(), out->S_re, out->S_im, out->Dapp,
+                      out->Kapp);
+    }
+    out->n_encounters = h_cnt[0];
+    out->n_permeations = h_cnt[1];
+    out->n_clamps = h_cnt[2];
+    float ms = 0.f, tot = 0.f;
+    for (auto& pr : step_ev) { float t1 = 0.f; cudaEventElapsedTime(&t1, pr.first, pr.second); ms += t1; }
+    cudaEventElapsedTime(&tot, ev_begin, ev_end);
+    out->kernel_ms = ms;
+    out->total_ms = tot;
+    out->n_launches = n_launches;
+    w->steps_done += (uint64_t)nT;
+    return RMS_OK;
+}

@@ -1,0 +1,266 @@
+// rms_substrate.cu -- H0: substrate upload and the derived face-mask lattice (include/rms.h, rms_substrate_create).
+#include <math.h>
+#include <stdarg.h>
+#include <string.h>
+
+#include "rms_internal.cuh"
+
+// ------------------------------------------------------------------------------------------------
+// thread-local error message
+// ------------------------------------------------------------------------------------------------
+static thread_local char g_err[512] = "";
+
+void rms_set_error(const char* fmt, ...)
+{
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(g_err, sizeof g_err, fmt, ap);
+    va_end(ap);
+}
+
+extern "C" const char* rms_last_error(void) { return g_err; }
+extern "C" const char* rms_version(void) { return "rms-b200 0.1 (sm_100a)"; }
+
+// ------------------------------------------------------------------------------------------------
+// Face-mask lattice.  A membrane is a voxel face whose two sides carry different labels; the
+// walk only ever asks "is the face I am about to cross a membrane?", so that one bit per face is
+// precomputed.  Layout: (nx+2)(ny+2)(nz+2) bytes, x fastest; voxel (x,y,z) of the box sits at padded
+// (x+1,y+1,z+1); the shell replicates the periodic images (R1) so that a walker can step over the box
+// edge without any wrap arithmetic and is folded back when it lands on a ghost voxel (bit 6).
+// ------------------------------------------------------------------------------------------------
+__device__ __forceinline__ int rms_wrap1(int a, int n) { return a < 0 ? a + n : (a >= n ? a - n : a); }
+
+__global__ void __launch_bounds__(128) rms_build_faces_kernel(const uint16_t* __restrict__ labels, int nx, int ny, int nz,
+                                                               uint8_t* __restrict__ faces, int n_labels,
+                                                               unsigned long long* __restrict__ stats)
+{
+    const int NX = nx + 2, NY = ny + 2;
+    const int X = blockIdx.x * blockDim.x + threadIdx.x;
+    const int Y = blockIdx.y, Z = blockIdx.z;
+    unsigned n_faces = 0, bad = 0;
+    if (X < NX) {
+        // periodic image of the padded coordinate (n may be 1: wrap twice is not needed since |X-1| <= n)
+        const int x = rms_wrap1(X - 1, nx), y = rms_wrap1(Y - 1, ny), z = rms_wrap1(Z - 1, nz);
+        const size_t row = ((size_t)z * ny + y) * nx;
+        const uint16_t L = labels[row + x];
+        const uint16_t xp = labels[row + rms_wrap1(x + 1, nx)];
+        const uint16_t xm = labels[row + rms_wrap1(x - 1, nx)];
+        const uint16_t yp = labels[((size_t)z * ny + rms_wrap1(y + 1, ny)) * nx + x];
+        const uint16_t ym = labels[((size_t)z * ny + rms_wrap1(y - 1, ny)) * nx + x];
+        const uint16_t zp = labels[((size_t)rms_wrap1(z + 1, nz) * ny + y) * nx + x];
+        const uint16_t zm = labels[((size_t)rms_wrap1(z - 1, nz) * ny + y) * nx + x];
+        unsigned m = (xp != L) | ((yp != L) << 1) | ((zp != L) << 2) | ((xm != L) << 3) | ((ym != L) << 4) | ((zm != L) << 5);
+        const bool ghost = (X == 0) | (X == NX - 1) | (Y == 0) | (Y == NY - 1) | (Z == 0) | (Z == nz + 1);
+        if (ghost) m |= 64u;
+        faces[((size_t)Z * NY + Y) * NX + X] = (uint8_t)m;
+        if (!ghost) {
+            n_faces = __popc(m & 7u);   // each face counted once, from its lower side
+            bad = (L >= n_labels);
+        }
+    }
+    // warp-shuffle reduction, then one atomic per warp
+    for (int o = 16; o > 0; o >>= 1) {
+        n_faces += __shfl_xor_sync(0xffffffffu, n_faces, o);
+        bad += __shfl_xor_sync(0xffffffffu, bad, o);
+    }
+    if ((threadIdx.x & 31) == 0) {
+        if (n_faces) atomicAdd(&stats[0], (unsigned long long)n_faces);
+        if (bad) atomicAdd(&stats[1], (unsigned long long)bad);
+    }
+}
+
+// label check + membrane count without building the face lattice (RMS_NO_BRICKS)
+__global__ void __launch_bounds__(256) rms_check_labels_kernel(const uint16_t* __restrict__ labels, size_t n, int n_labels,
+                                                                unsigned long long* __restrict__ stats)
+{
+    unsigned bad = 0;
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x)
+        bad += labels[i] >= n_labels;
+    for (int o = 16; o > 0; o >>= 1) bad += __shfl_xor_sync(0xffffffffu, bad, o);
+    if ((threadIdx.x & 31) == 0 && bad) atomicAdd(&stats[1], (unsigned long long)bad);
+}
+
+extern "C" int rms_substrate_create(const rms_substrate_desc* d, void* cuda_stream, rms_substrate** out)
+{
+    RMS_REQUIRE(d && out, RMS_ERR_ARG, "rms_substrate_create: null descriptor or output");
+    *out = nullptr;
+    RMS_REQUIRE(d->nx > 0 && d->ny > 0 && d->nz > 0, RMS_ERR_ARG, "lattice dimensions must be positive");
+    RMS_REQUIRE(d->labels, RMS_ERR_ARG, "labels is null");
+    RMS_REQUIRE(d->voxel_um > 0, RMS_ERR_ARG, "voxel_um must be positive");
+    RMS_REQUIRE(d->n_labels > 0 && d->n_labels <= 65536, RMS_ERR_ARG, "n_labels must be in 1..65536");
+    RMS_REQUIRE(d->n_classes > 0 && d->n_classes <= 256, RMS_ERR_ARG, "n_classes must be in 1..256");
+    RMS_REQUIRE(d->D, RMS_ERR_ARG, "D is null");
+    RMS_REQUIRE(!(d->flags & RMS_ADOPT_DEVICE_PTR) || (d->flags & RMS_LABELS_ON_DEVICE), RMS_ERR_ARG,
+                "RMS_ADOPT_DEVICE_PTR needs RMS_LABELS_ON_DEVICE");
+    const uint64_t n_vox = (uint64_t)d->nx * d->ny * d->nz;
+    RMS_REQUIRE((uint64_t)(d->nx + 2) * (d->ny + 2) * (d->nz + 2) < (1ull << 31), RMS_ERR_UNSUPPORTED,
+                "lattice too large: padded voxel count must stay below 2^31");
+    const int nL = d->n_labels;
+    for (int a = 0; a < nL; ++a) {
+        RMS_REQUIRE(d->D[a] > 0 && isfinite(d->D[a]), RMS_ERR_ARG, "D[%d] must be positive and finite", a);
+        if (d->label_class) RMS_REQUIRE(d->label_class[a] < d->n_classes, RMS_ERR_ARG, "label_class[%d] >= n_classes", a);
+    }
+    bool all_imp = true;
+    if (d->kappa) {
+        for (int a = 0; a < nL; ++a)
+            for (int b = 0; b < nL; ++b) {
+                if (a == b) continue;
+                const float k = d->kappa[(size_t)a * nL + b];
+                RMS_REQUIRE(k >= 0 && k == k, RMS_ERR_ARG, "kappa[%d][%d] is negative or NaN", a, b);
+                RMS_REQUIRE(k == d->kappa[(size_t)b * nL + a], RMS_ERR_ARG, "kappa is not symmetric at (%d,%d)", a, b);
+                if (k != 0) all_imp = false;
+            }
+    }
+
+    int dev_count = 0;
+    cudaError_t ce = cudaGetDeviceCount(&dev_count);
+    RMS_REQUIRE(ce == cudaSuccess && dev_count > 0, RMS_ERR_CUDA, "no CUDA device: %s (there is no CPU fallback)",
+                cudaGetErrorString(ce));
+    cudaStream_t stream = (cudaStream_t)cuda_stream;
+
+    rms_substrate* s = new (std::nothrow) rms_substrate();
+    RMS_REQUIRE(s, RMS_ERR_OOM, "out of host memory");
+    s->nx = d->nx; s->ny = d->ny; s->nz = d->nz; s->voxel_um = d->voxel_um;
+    s->n_labels = nL; s->n_classes = d->n_classes; s->n_vox = n_vox;
+    s->D.assign(d->D, d->D + nL);
+    if (d->T2) s->T2.assign(d->T2, d->T2 + nL); else s->T2.assign(nL, INFINITY);
+    if (d->kappa) s->kappa.assign(d->kappa, d->kappa + (size_t)nL * nL); else s->kappa.assign((size_t)nL * nL, 0.f);
+    if (d->label_class) s->label_class.assign(d->label_class, d->label_class + nL); else s->label_class.assign(nL, 0);
+    s->all_impermeable = all_imp;
+
+    int rc = RMS_OK;
+    unsigned long long* d_stats = nullptr;
+    unsigned long long h_stats[2] = {0, 0};
+#define SUB_TRY(expr)                                                                                    \
+    do {                                                                                                 \
+        cudaError_t _e = (expr);                                                                         \
+        if (_e != cudaSuccess) {                                                                         \
+            rms_set_error("%s failed: %s", #expr, cudaGetErrorString(_e));                               \
+            rc = (_e == cudaErrorMemoryAllocation) ? RMS_ERR_OOM : RMS_ERR_CUDA;                         \
+            goto fail;                                                                                   \
+        }                                                                                                \
+    } while (0)
+
+    if (d->flags & RMS_ADOPT_DEVICE_PTR) {
+        s->d_labels = d->labels;
+        s->owns_labels = false;
+    } else {
+        uint16_t* buf = nullptr;
+        SUB_TRY(cudaMalloc(&buf, n_vox * sizeof(uint16_t)));
+        s->d_labels = buf;
+        s->owns_labels = true;
+        SUB_TRY(cudaMemcpyAsync(buf, d->labels, n_vox * sizeof(uint16_t),
+                                (d->flags & RMS_LABELS_ON_DEVICE) ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice, stream));
+    }
+    {
+        uint8_t* lc = nullptr;
+        SUB_TRY(cudaMalloc(&lc, nL));
+        s->d_label_class = lc;
+        SUB_TRY(cudaMemcpyAsync(lc, s->label_class.data(), nL, cudaMemcpyHostToDevice, stream));
+    }
+    SUB_TRY(cudaMalloc(&d_stats, 2 * sizeof(unsigned long long)));
+    SUB_TRY(cudaMemsetAsync(d_stats, 0, 2 * sizeof(unsigned long long), stream));
+    if (!(d->flags & RMS_NO_BRICKS)) {
+        s->NX = s->nx + 2; s->NY = s->ny + 2; s->NZ = s->nz + 2;
+        SUB_TRY(cudaMalloc(&s->d_faces, (size_t)s->NX * s->NY * s->NZ));
+        dim3 grid((s->NX + 127) / 128, s->NY, s->NZ);
+        if (grid.y > 65535u || grid.z > 65535u) {
+            rms_set_error("lattice too large for the face-mask build (ny+2, nz+2 must be <= 65535)");
+            rc = RMS_ERR_UNSUPPORTED;
+            goto fail;
+        }
+        rms_build_faces_kernel<<<grid, 128, 0, stream>>>(s->d_labels, s->nx, s->ny, s->nz, s->d_faces, nL, d_stats);
+        SUB_TRY(cudaGetLastError());
+    } else {
+        rms_check_labels_kernel<<<148 * 8, 256, 0, stream>>>(s->d_labels, (size_t)n_vox, nL, d_stats);
+        SUB_TRY(cudaGetLastError());
+    }
+    SUB_TRY(cudaMemcpyAsync(h_stats, d_stats, sizeof h_stats, cudaMemcpyDeviceToHost, stream));
+    SUB_TRY(cudaStreamSynchronize(stream));
+    cudaFree(d_stats);
+    d_stats = nullptr;
+    if (h_stats[1] != 0) {
+        rms_set_error("%llu voxels carry a label >= n_labels (%d)", h_stats[1], nL);
+        rc = RMS_ERR_ARG;
+        goto fail;
+    }
+    s->n_membrane_faces = h_stats[0];
+    *out = s;
+    return RMS_OK;
+fail:
+    if (d_stats) cudaFree(d_stats);
+    rms_substrate_destroy(s);
+    return rc;
+#undef SUB_TRY
+}
+
+extern "C" int rms_substrate_destroy(rms_substrate* s)
+{
+    if (!s) return RMS_OK;
+    if (s->owns_labels && s->d_labels) cudaFree((void*)s->d_labels);
+    if (s->d_faces) cudaFree(s->d_faces);
+    if (s->d_label_class) cudaFree(s->d_label_class);
+    delete s;
+    return RMS_OK;
+}
+
+extern "C" int rms_substrate_get_info(const rms_substrate* s, rms_substrate_info* out)
+{
+    RMS_REQUIRE(s && out, RMS_ERR_ARG, "rms_substrate_get_info: null argument");
+    out->nx = s->nx; out->ny = s->ny; out->nz = s->nz;
+    out->n_labels = s->n_labels; out->n_classes = s->n_classes;
+    out->n_voxels = s->n_vox;
+    out->n_membrane_faces = s->n_membrane_faces;
+    out->lattice_bytes = s->n_vox * sizeof(uint16_t);
+    out->brick_bytes = s->d_faces ? (uint64_t)s->NX * s->NY * s->NZ : 0;
+    out->has_bricks = s->d_faces != nullptr;
+    return RMS_OK;
+}
+
+// Eq.1 and Eq.3, Eq.C.15 for kappa = inf; fp64 on the host, rounded once to fp32.
+int rms_compute_tables(const rms_substrate* s, double dt, std::vector<float>& s_tab, std::vector<float>& P_tab)
+{
+    const int nL = s->n_labels;
+    const double C3 = 2.0 / 3.0;
+    RMS_REQUIRE(dt > 0 && isfinite(dt), RMS_ERR_ARG, "dt_ms must be positive and finite");
+    s_tab.resize(nL);
+    P_tab.assign((size_t)nL * nL, 0.f);
+    for (int a = 0; a < nL; ++a) {
+        s_tab[a] = (float)(sqrt(6.0 * (double)s->D[a] * dt) / s->voxel_um);
+        RMS_REQUIRE(s_tab[a] < 1.0f, RMS_ERR_STEP_TOO_LARGE,
+                    "hop length sqrt(6 D dt) = %.4g voxels for label %d: must stay below the voxel size (P:62, P:189)",
+                    (double)s_tab[a], a);
+    }
+    for (int a = 0; a < nL; ++a)
+        for (int b = 0; b < nL; ++b) {
+            double P;
+            if (a == b) {
+                P = 1.0;
+            } else {
+                const double k = s->kappa[(size_t)a * nL + b], Da = s->D[a], Db = s->D[b];
+                if (k == 0) {
+                    P = 0;
+                } else if (isinf(k)) {
+                    P = fmin(1.0, sqrt(Db / Da));
+                } else {
+                    const double Aab = k * sqrt(6.0 * dt / Da) * C3, Aba = k * sqrt(6.0 * dt / Db) * C3;
+                    P = Aab / (1.0 + 0.5 * (Aab + Aba));
+                    RMS_REQUIRE(P <= 1.0, RMS_ERR_P_RANGE,
+                                "Eq.3 gives P = %.4g > 1 from label %d into %d: lower kappa or dt (P:624)", P, a, b);
+                }
+            }
+            P_tab[(size_t)a * nL + b] = (float)P;
+        }
+    return RMS_OK;
+}
+
+extern "C" int rms_tables(const rms_substrate* s, double dt_ms, float* s_out, float* P_out)
+{
+    RMS_REQUIRE(s, RMS_ERR_ARG, "rms_tables: null substrate");
+    std::vector<float> st, pt;
+    int rc = rms_compute_tables(s, dt_ms, st, pt);
+    if (rc != RMS_OK) return rc;
+    if (s_out) memcpy(s_out, st.data(), st.size() * sizeof(float));
+    if (P_out) memcpy(P_out, pt.data(), pt.size() * sizeof(float));
+    return RMS_OK;
+}

@@ -1,0 +1,204 @@
+"""GPU parity tests: the CUDA path (through the C ABI) against the oracle, element by element, on the same
+seeded inputs.  Tolerances are north_star's: >= 99.9 % of walkers in the same final voxel, |dS| <= 1e-4 per
+b-value and direction, moments within 1e-4 relative; integer work (placement) bit exact."""
+import math
+
+import numpy as np
+import pytest
+
+import rms_inputs as ri
+from parity_util import compare, gpu_run, oracle_run
+
+pytestmark = pytest.mark.gpu
+
+LABEL_GATHER = 1   # RMS_RUN_LABEL_GATHER
+
+
+@pytest.fixture(scope="module")
+def rms():
+    import torch
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    import paper_2012_06478_b200 as rms
+    rms.load_library()
+    return rms
+
+
+def _both(cfg, n_walkers=None, flags=0, first_id=0):
+    n = cfg.n_walkers if n_walkers is None else n_walkers
+    g = gpu_run(cfg.substrate, cfg.sequence, n, cfg.seed, first_id=first_id, flags=flags)
+    o = oracle_run(cfg.substrate, cfg.sequence, n, cfg.seed, first_id=first_id)
+    return g, o, n
+
+
+@pytest.mark.parametrize("flags", [0, LABEL_GATHER], ids=["facemask", "labels"])
+def test_cfg0_single_cylinder(rms, flags):
+    cfg = ri.make_config("cfg0")
+    g, o, n = _both(cfg, flags=flags)
+    rep = compare(g, o, n)
+    print("cfg0", flags, rep)
+    assert g["n_permeations"] == 0
+    assert np.all(g["walkers"]["label"] == 1)
+    # b = 0: S = 1 exactly
+    assert np.allclose(g["S"][0, 0], 1.0, atol=1e-12)
+    # the straight cylinder is free along z: product-of-sincs closed form for the discrete walk
+    seq = cfg.sequence
+    ds = math.sqrt(6 * 2.0 * seq.dt_ms)
+    W = np.cumsum(seq.wave[0][::-1].astype(float))[::-1]
+    for gi, gamp in enumerate(seq.gamp[0]):
+        exact = np.prod(np.sinc(gamp * seq.dt_ms * ds * W / np.pi))
+        assert abs(g["S"][0, gi, 1].real - exact) < 4 * math.sqrt(0.5 / n)
+
+
+@pytest.mark.parametrize("flags", [0, LABEL_GATHER], ids=["facemask", "labels"])
+def test_cfg1_packed_cylinders_reduced(rms, flags):
+    cfg = ri.make_config("cfg1", "test")
+    g, o, n = _both(cfg, flags=flags)
+    print("cfg1", flags, compare(g, o, n))
+
+
+@pytest.mark.parametrize("flags", [0, LABEL_GATHER], ids=["facemask", "labels"])
+def test_cfg2_axons_reduced_with_snapshots(rms, flags):
+    cfg = ri.make_config("cfg2", "test")
+    g, o, n = _both(cfg, flags=flags)
+    print("cfg2", flags, compare(g, o, n))
+    assert g["m2"].shape == (5, 60, 2)
+
+
+def test_cfg3_permeable_heterogeneous_reduced(rms):
+    cfg = ri.make_config("cfg3", "test")
+    g, o, n = _both(cfg)
+    rep = compare(g, o, n)
+    print("cfg3", rep)
+    assert g["n_permeations"] > 0
+    # T2 weights: per-walker relaxation exponent
+    assert np.allclose(g["walkers"]["relax"], o["relax"], rtol=2e-6, atol=1e-7)
+
+
+def test_strongly_permeable_slabs_with_D_contrast(rms):
+    # P ~ 0.1-0.3 and D contrast: exercises the fine permeation draw, the rescaled remainder (R7) and Eq.C.15
+    for kap in (40.0, float("inf")):
+        sub = ri.slabs(6, 6, (3, 3), 0.1, D_extra=2.0, D_intra=0.5, kappa_membrane=kap, T2_extra=0.05, T2_intra=0.2)
+        seq = ri.pgse_sequence(2e-4, 600, 0.04, 0.06, [0.0, 5.0, 50.0], ri.fibonacci_dirs(7), snap_steps=[101, 600])
+        n = 20000
+        g = gpu_run(sub, seq, n, 7)
+        o = oracle_run(sub, seq, n, 7)
+        rep = compare(g, o, n)
+        print("slabs", kap, rep)
+        assert g["n_permeations"] > 10000
+
+
+def test_chunked_run_continues_the_same_trajectories(rms):
+    cfg = ri.make_config("cfg0")
+    sub, seq = cfg.substrate, cfg.sequence
+    n = 4000
+    o = oracle_run(sub, seq, n, cfg.seed)
+    S = rms.rms_substrate_create(sub.labels, sub.voxel_um, sub.D, sub.T2, sub.kappa, sub.label_class, sub.n_classes)
+    W = rms.rms_walkers_init(S, n, 0, sub.label_allowed, cfg.seed)
+    cuts = [0, 333, 334, 1000]                                  # odd boundary: the Philox pair is split across calls
+    enc = 0
+    for a, b in zip(cuts[:-1], cuts[1:]):
+        r = rms.rms_run(S, W, seq.dt_ms, b - a, seq.wave[:, a:b], seq.gamp, seq.dirs, [b - a])
+        enc += r["n_encounters"]
+    r["n_encounters"] = enc
+    assert W.steps_done() == 1000
+    r["walkers"] = W.read()
+    rep = compare(r, o, n)
+    print("chunked", rep)
+
+
+def test_general_waveform_table_mode_and_two_waves(rms):
+    # non-integer gradient shapes (sine, trapezoid) take the table path; two waveforms share one trajectory set
+    sub = ri.single_cylinder(24, 7.5, 0.1)
+    n_steps = 801
+    t = (np.arange(n_steps) + 1.0) / n_steps
+    wave = np.stack([np.sin(2 * np.pi * t), np.clip(4 * np.minimum(t, 1 - t), 0, 1) * np.sign(0.5 - t)]).astype(np.float32)
+    seq = ri.Sequence(dt_ms=2e-4, n_steps=n_steps, wave=wave, gamp=np.array([[0.0, 40.0, 90.0], [10.0, 60.0, 120.0]]),
+                      dirs=ri.fibonacci_dirs(5), snap_steps=np.array([400, 801]))
+    n = 6000
+    g = gpu_run(sub, seq, n, 5)
+    o = oracle_run(sub, seq, n, 5)
+    print("table", compare(g, o, n))
+    # integer-valued pair of waveforms (const path, NW = 2)
+    wave2 = np.stack([ri.pgse_wave(n_steps, 200, 500), ri.pgse_wave(n_steps, 100, 300)])
+    seq2 = ri.Sequence(dt_ms=2e-4, n_steps=n_steps, wave=wave2, gamp=np.array([[0.0, 30.0], [0.0, 80.0]]),
+                       dirs=ri.fibonacci_dirs(4), snap_steps=np.array([801]))
+    g = gpu_run(sub, seq2, n, 5)
+    o = oracle_run(sub, seq2, n, 5)
+    print("two waves", compare(g, o, n))
+
+
+@pytest.mark.parametrize("dims", [(5, 7, 3), (1, 1, 9), (2, 3, 4)])
+@pytest.mark.parametrize("flags", [0, LABEL_GATHER], ids=["facemask", "labels"])
+def test_ragged_tiny_lattices_with_heavy_wrapping(rms, dims, flags):
+    # random labels per voxel, impermeable: almost every face is a membrane or a periodic wrap
+    sub = ri.random_lattice(dims, n_labels=2, seed=3)
+    seq = ri.pgse_sequence(2e-4, 400, 0.02, 0.04, [0.0, 20.0], np.eye(3), snap_steps=[399, 400])
+    n = 3000
+    g = gpu_run(sub, seq, n, 11, flags=flags)
+    o = oracle_run(sub, seq, n, 11)
+    print("tiny", dims, compare(g, o, n))
+
+
+def test_free_box_wraps_many_times(rms):
+    # no membranes at all, small periodic box: every walker wraps the box repeatedly (ghost-shell folding)
+    sub = ri.uniform_lattice((4, 3, 5))
+    seq = ri.pgse_sequence(2e-4, 2000, 0.1, 0.2, [0.0, 1.0, 3.0], ri.fibonacci_dirs(6), snap_steps=[2000])
+    n = 5000
+    g = gpu_run(sub, seq, n, 13)
+    o = oracle_run(sub, seq, n, 13)
+    rep = compare(g, o, n)
+    print("free", rep)
+    assert g["n_encounters"] == 0
+    assert np.abs(g["walkers"]["vox"]).max() > 8               # really left the box
+
+
+def test_walker_subrange_and_placement_only(rms):
+    cfg = ri.make_config("cfg1", "test")
+    g, o, n = _both(cfg, n_walkers=257, first_id=1000)          # ragged: 2 blocks + 1 walker
+    print("subrange", compare(g, o, n))
+    # zero steps: placement only
+    seq0 = ri.Sequence(dt_ms=2e-4, n_steps=0, wave=np.zeros((1, 0), np.float32), gamp=np.array([[0.0, 1.0]]),
+                       dirs=np.eye(3), snap_steps=np.zeros(0, np.int64))
+    g0 = gpu_run(cfg.substrate, seq0, 1, cfg.seed)
+    assert np.allclose(g0["S"], 1.0) and g0["sum_alpha"].sum() == 1.0
+
+
+def test_error_codes(rms):
+    cfg = ri.make_config("cfg0")
+    sub, seq = cfg.substrate, cfg.sequence
+    with pytest.raises(rms.RmsError) as e:      # label >= n_labels
+        rms.rms_substrate_create(sub.labels, 0.1, sub.D[:1], None, None, None, 1)
+    assert e.value.code == -1
+    S = rms.rms_substrate_create(sub.labels, 0.1, sub.D, sub.T2, sub.kappa, sub.label_class, 2)
+    with pytest.raises(rms.RmsError) as e:
+        rms.rms_walkers_init(S, 10, 0, np.zeros(2, np.uint8), 1)
+    assert e.value.code == -4
+    W = rms.rms_walkers_init(S, 10, 0, sub.label_allowed, 1)
+    with pytest.raises(rms.RmsError) as e:      # hop longer than a voxel
+        rms.rms_run(S, W, 1e-3, 10, seq.wave[:, :10], seq.gamp, seq.dirs, [10])
+    assert e.value.code == -2
+    with pytest.raises(rms.RmsError) as e:      # non-unit direction
+        rms.rms_run(S, W, 2e-4, 10, seq.wave[:, :10], seq.gamp, seq.dirs * 2, [10])
+    assert e.value.code == -1
+    with pytest.raises(rms.RmsError) as e:      # unsorted snapshots
+        rms.rms_run(S, W, 2e-4, 10, seq.wave[:, :10], seq.gamp, seq.dirs, [5, 4])
+    assert e.value.code == -1
+    assert W.steps_done() == 0
+    S2 = rms.rms_substrate_create(sub.labels, 0.1, [2.0, 0.01], None, [[0, 5000.0], [5000.0, 0]], sub.label_class, 2)
+    W2 = rms.rms_walkers_init(S2, 10, 0, None, 1)
+    with pytest.raises(rms.RmsError) as e:      # Eq.3 above 1
+        rms.rms_run(S2, W2, 2e-4, 10, seq.wave[:, :10], seq.gamp, seq.dirs, [10])
+    assert e.value.code == -3
+
+
+def test_tables_match_oracle(rms):
+    import oracle
+    D = np.array([2.0, 1.0, 0.5], np.float32)
+    kap = np.array([[0, 0.02, 0.4], [0.02, 0, np.inf], [0.4, np.inf, 0]], np.float32)
+    lab = np.zeros((2, 2, 3), np.uint16)
+    S = rms.rms_substrate_create(lab, 0.1, D, None, kap, None, 1)
+    s_g, P_g = S.tables(2e-4)
+    s_o, P_o = oracle.tables(D, kap, 0.1, 2e-4)
+    assert np.array_equal(s_g.astype(np.float64), s_o) and np.array_equal(P_g.astype(np.float64), P_o)
+    info = S.info()
+    assert info["n_membrane_faces"] == 0 and info["has_bricks"] == 1
