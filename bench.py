@@ -57,27 +57,76 @@ def parse_args():
 
 
 class ClockSampler:
-    """nvidia-smi clocks and throttle reasons DURING the timed region (B200_PROFILING.md recipe)."""
+    """SM clock and throttle reasons DURING the timed region (B200_PROFILING.md recipe).  Sampled in-process through
+    NVML (nvidia_ml_py) every 50 ms; an external `nvidia-smi -lms` loop contends for the driver lock with the
+    path's own calls and was measured to slow a pass by tens of ms.  Falls back to nvidia-smi if NVML is missing."""
+    NAMES = {"hw_slowdown": 0x8, "hw_thermal_slowdown": 0x40, "sw_thermal_slowdown": 0x20, "sw_power_cap": 0x4}
     Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
          "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
 
     def __init__(self, index):
-        self.index, self.proc, self.lines = index, None, []
+        self.index, self.proc, self.lines, self.samples = index, None, [], []
+        self.stop_flag = threading.Event()
+        self.nvml = None
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.nvml = pynvml
+            self.handle = pynvml.nvmlDeviceGetHandleByIndex(self._physical_index(index))
+            self.sm_max = float(pynvml.nvmlDeviceGetMaxClockInfo(self.handle, pynvml.NVML_CLOCK_SM))
+        except Exception:
+            self.nvml = None
+
+    @staticmethod
+    def _physical_index(index):
+        vis = os.environ.get("CUDA_VISIBLE_DEVICES")
+        if vis:
+            ids = [v.strip() for v in vis.split(",") if v.strip()]
+            if index < len(ids) and ids[index].isdigit():
+                return int(ids[index])
+        return index
 
     def start(self):
+        if self.nvml:
+            self.thread = threading.Thread(target=self._poll, daemon=True)
+            self.thread.start()
+            return
         try:
-            self.proc = subprocess.Popen(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits", "-lms", "100",
+            self.proc = subprocess.Popen(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits", "-lms", "250",
                                           "-i", str(self.index)], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
             self.thread = threading.Thread(target=self._read, daemon=True)
             self.thread.start()
         except OSError:
             self.proc = None
 
+    def _poll(self):
+        n = self.nvml
+        while not self.stop_flag.is_set():
+            try:
+                sm = float(n.nvmlDeviceGetClockInfo(self.handle, n.NVML_CLOCK_SM))
+                pw = n.nvmlDeviceGetPowerUsage(self.handle) / 1000.0
+                try:
+                    rs = int(n.nvmlDeviceGetCurrentClocksEventReasons(self.handle))
+                except Exception:
+                    rs = int(n.nvmlDeviceGetCurrentClocksThrottleReasons(self.handle))
+                self.samples.append((sm, pw, rs))
+            except Exception:
+                pass
+            self.stop_flag.wait(0.05)
+
     def _read(self):
         for line in self.proc.stdout:
             self.lines.append(line.strip())
 
     def stop(self):
+        if self.nvml:
+            self.stop_flag.set()
+            self.thread.join(timeout=2)
+            sm = [x[0] for x in self.samples]
+            reasons = sorted(nm for nm, bit in self.NAMES.items() if any(x[2] & bit for x in self.samples))
+            return {"sm_mhz": statistics.median(sm) if sm else None, "sm_max_mhz": self.sm_max,
+                    "power_w_max": max((x[1] for x in self.samples), default=None), "samples": len(sm), "reasons": reasons,
+                    "source": "nvml, 50 ms"}
         if not self.proc:
             return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
         self.proc.terminate()
@@ -99,7 +148,8 @@ class ClockSampler:
                 if v.lower().startswith("active"):
                     reasons.add(nm)
         return {"sm_mhz": statistics.median(sm) if sm else None, "sm_max_mhz": max(mx) if mx else None,
-                "power_w_max": max(power) if power else None, "samples": len(sm), "reasons": sorted(reasons)}
+                "power_w_max": max(power) if power else None, "samples": len(sm), "reasons": sorted(reasons),
+                "source": "nvidia-smi -lms 250"}
 
 
 def make_workload(args):
@@ -116,7 +166,7 @@ def workload_config(args, cfg, extra=None):
          "walkers_per_gpu": args.walkers, "mc_steps": args.mc_steps, "dt_ms": cfg.sequence.dt_ms,
          "directions": int(cfg.sequence.dirs.shape[0]), "b_values": int(cfg.sequence.gamp.shape[1]),
          "lattice_path": args.lattice, "pass": "rms_substrate_create + rms_walkers_init + rms_run",
-         "l2": "inputs larger than L2 (lattice 1.0 GB + 0.5 GB face masks vs 126 MB L2)" if args.scale == "full"
+         "l2": "inputs larger than L2 (label lattice 1.0 GB + neighbourhood lattice 2.0 GB vs 126 MB L2)" if args.scale == "full"
          else "reduced test lattice (fits L2) -- not a valid bench configuration"}
     if extra:
         c.update(extra)
@@ -206,7 +256,7 @@ def main():
         for _ in range(n_iter):
             r = one_pass(device)
             kernel_ms += r["kernel_ms"]
-            launches += r["n_launches"] + 2           # + face-mask build + walker init kernels
+            launches += r["n_launches"] + 2           # + neighbourhood-lattice build + walker init kernels
         e1.record(stream)
         if world > 1:
             dist.barrier()
@@ -248,7 +298,7 @@ def main():
     peak_ginstr = N_SM * LANES_PER_SM * sm_mhz * 1e6 / 1e9
     k_ms_per_launch = kernel_ms / args.steps
     achieved_ginstr = ALGORITHMIC_INSTR_PER_STEP * n_walkers * mc_steps / (k_ms_per_launch * 1e-3) / 1e9
-    roofline = {"bound": "alu", "kernel": "rms_step_kernel", "achieved": achieved_ginstr, "peak": peak_ginstr,
+    roofline = {"bound": "alu", "kernel": "rms_step_fast_kernel" if args.lattice == "facemask" else "rms_step_kernel", "achieved": achieved_ginstr, "peak": peak_ginstr,
                 "unit": "Ginstr/s (thread-instructions)", "frac": achieved_ginstr / peak_ginstr,
                 "traffic": NCU_TRAFFIC_BYTES_PER_LAUNCH,
                 "algorithmic_instr_per_walker_step": ALGORITHMIC_INSTR_PER_STEP, "kernel_ms_per_launch": k_ms_per_launch,

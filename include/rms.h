@@ -56,9 +56,10 @@ typedef struct rms_walkers rms_walkers;     /* opaque */
  * label_class  [n_labels] output compartment class of each label, < n_classes; NULL = all 0 (host)
  * flags        RMS_LABELS_ON_DEVICE | RMS_ADOPT_DEVICE_PTR | RMS_NO_BRICKS
  *
- * Derived on the device: the bit-packed face-mask bricks (one 32-byte record per 4x4x4 voxels holding,
- * for every voxel face of the brick, whether the labels on its two sides differ, i.e. whether the
- * face is a membrane), unless RMS_NO_BRICKS.
+ * Derived on the device, unless RMS_NO_BRICKS: the neighbourhood lattice, one 32-bit word per voxel (plus a
+ * one-voxel periodic ghost shell) whose 27 bits say which voxels of the 3x3x3 block around it carry the
+ * same label -- a face is a membrane iff the labels on its two sides differ, and a hop shorter than
+ * a voxel only ever meets faces inside that block.
  * Errors: RMS_ERR_ARG, RMS_ERR_OOM, RMS_ERR_CUDA.
  */
 #define RMS_LABELS_ON_DEVICE 1u
@@ -86,7 +87,7 @@ typedef struct {
     uint64_t n_voxels;
     uint64_t n_membrane_faces;  /* voxel faces whose two sides carry different labels (each face once) */
     uint64_t lattice_bytes;     /* uint16 lattice on the device                                          */
-    uint64_t brick_bytes;       /* face-mask bricks on the device (0 with RMS_NO_BRICKS)                 */
+    uint64_t brick_bytes;       /* neighbourhood lattice on the device (0 with RMS_NO_BRICKS)            */
     int32_t has_bricks;
 } rms_substrate_info;
 
@@ -117,7 +118,11 @@ int rms_walkers_destroy(rms_walkers* w);
  * snap_steps  [n_snap] ascending step numbers in 1..n_steps of this call at which the displacement
  *             moments are taken (host)
  * flags       RMS_RUN_LABEL_GATHER: test faces by gathering the neighbour's uint16 label (the paper's
- *             lookup table) instead of the face-mask bricks.
+ *             lookup table) instead of the neighbourhood lattice.
+ *             RMS_RUN_GENERAL_KERNEL: impermeable runs with integer-valued piecewise-constant waveforms
+ *             normally take the specialised kernel (csrc/rms_step_fast.cu); this flag forces the general one.
+ *             RMS_RUN_NO_ORDERING: on large lattices the walkers are dealt to the threads in the order of the
+ *             lattice cell they sit in (cache locality; results do not depend on it); this flag keeps id order.
  *
  * A second rms_run on the same walkers continues the trajectories (the random numbers are keyed on the
  * absolute step), so long runs may be chunked; phases and T2 weights keep accumulating.
@@ -133,9 +138,12 @@ int rms_walkers_destroy(rms_walkers* w);
  *   Dapp, Kapp [n_snap][n_dir]                  D = <alpha X^2>/(2 t <alpha>), K = <alpha X^4><alpha>/<alpha X^2>^2 - 3
  *                                               with t = (steps since the walkers' start) * dt (R14)
  *   n_encounters / n_permeations / n_clamps     unlike-label faces met / crossed; offsets clamped to [0,1)
+ *                                               (n_clamps is counted by the general kernel only)
  * Errors: RMS_ERR_ARG, RMS_ERR_STEP_TOO_LARGE, RMS_ERR_P_RANGE, RMS_ERR_UNSUPPORTED, RMS_ERR_OOM, RMS_ERR_CUDA.
  */
 #define RMS_RUN_LABEL_GATHER 1u
+#define RMS_RUN_GENERAL_KERNEL 2u
+#define RMS_RUN_NO_ORDERING 4u
 
 typedef struct {
     double dt_ms;               /* Table 1: dt */
@@ -201,6 +209,10 @@ int rms_tables(const rms_substrate* s, double dt_ms, float* s_out, float* P_out)
 int rms_normalise(int n_classes, int n_q, const double* sum_alpha, const double* sig_re, const double* sig_im,
                   int n_snap, int n_dir, const double* snap_alpha, const double* m2, const double* m4,
                   const double* t_ms, double* S_re, double* S_im, double* Dapp, double* Kapp);
+
+/* Device buffers behind destroyed handles are kept for the next handle of the same size (a pass of the path
+ * allocates the same buffers every time); rms_memory_trim returns them to the driver.  Always RMS_OK. */
+int rms_memory_trim(void);
 
 const char* rms_last_error(void);
 const char* rms_version(void);

@@ -20,13 +20,15 @@ RMS_LABELS_ON_DEVICE = 1
 RMS_ADOPT_DEVICE_PTR = 2
 RMS_NO_BRICKS = 4
 RMS_RUN_LABEL_GATHER = 1
+RMS_RUN_GENERAL_KERNEL = 2
+RMS_RUN_NO_ORDERING = 4
 
 STATUS = {0: "RMS_OK", -1: "RMS_ERR_ARG", -2: "RMS_ERR_STEP_TOO_LARGE", -3: "RMS_ERR_P_RANGE", -4: "RMS_ERR_NO_SPACE",
           -5: "RMS_ERR_OOM", -6: "RMS_ERR_CUDA", -7: "RMS_ERR_UNSUPPORTED"}
 
 EXPORTS = ("rms_substrate_create", "rms_substrate_destroy", "rms_substrate_get_info", "rms_walkers_init",
            "rms_walkers_destroy", "rms_run", "rms_walkers_read", "rms_walkers_steps_done", "rms_tables", "rms_normalise",
-           "rms_last_error", "rms_version")
+           "rms_memory_trim", "rms_last_error", "rms_version")
 
 
 class RmsError(RuntimeError):

@@ -34,6 +34,12 @@ void rms_set_error(const char* fmt, ...);
     } while (0)
 
 // ------------------------------------------------------------------------------------------------
+// device memory (rms_memory.cu): caching allocator behind every handle
+// ------------------------------------------------------------------------------------------------
+cudaError_t rms_malloc(void** p, size_t bytes);
+void rms_free(void* p);
+
+// ------------------------------------------------------------------------------------------------
 // handles
 // ------------------------------------------------------------------------------------------------
 struct rms_substrate {
@@ -43,10 +49,11 @@ struct rms_substrate {
     uint64_t n_vox = 0;
     const uint16_t* d_labels = nullptr;  // device, x fastest
     bool owns_labels = false;
-    // face-mask lattice: one byte per voxel of the lattice padded by a one-voxel periodic ghost shell,
-    // bit (k + 3*neg) = the face of this voxel towards +k (neg = 0) / -k (neg = 1) is a membrane,
-    // bit 6 = ghost voxel.
-    uint8_t* d_faces = nullptr;
+    // neighbourhood lattice: one 32-bit word per voxel of the lattice padded by a one-voxel periodic ghost
+    // shell.  Bit (dx+1) + 3 (dy+1) + 9 (dz+1), d in {-1,0,1}^3, = the voxel at that offset carries the SAME
+    // label as this voxel (bit 13 = the voxel itself = 1); a face towards +-k is a membrane iff the
+    // bit of the face neighbour is 0.  Bit 27 (RMS_NBR_GHOST) = ghost voxel.
+    uint32_t* d_nbr = nullptr;
     int NX = 0, NY = 0, NZ = 0;          // padded dims (n + 2)
     uint64_t n_membrane_faces = 0;
     std::vector<float> D, T2, kappa;     // host copies of the per-label tables
@@ -140,12 +147,14 @@ struct rms_segment {          // a run of steps on which every waveform is const
 
 enum { RMS_WMODE_CONST = 0, RMS_WMODE_TABLE = 1 };
 enum { RMS_LAT_LABELS = 0, RMS_LAT_FACES = 1 };
+#define RMS_NBR_GHOST (1u << 27)
+#define RMS_NBR_SELF 13
 
 struct rms_step_params {
     int nx, ny, nz;
     const uint16_t* labels;
-    const uint8_t* faces;
-    int NX, NY;               // padded dims of the face lattice
+    const uint32_t* nbr;
+    int NX, NY;               // padded dims of the neighbourhood lattice
     rms_walker_arrays st;
     uint64_t n, first_id;
     rms_philox_keys rk;
@@ -165,9 +174,12 @@ struct rms_step_params {
     double wtot[RMS_MAX_WAVES];      // sum of w over the steps of this launch
     int n_wave;
     unsigned long long* counters;    // [0] encounters [1] permeations [2] clamps [3] init failures
+    const uint32_t* order;           // thread t works on walker order[t] (spatially sorted, rms_sched.cu); NULL = identity
 };
 
 int rms_launch_step(const rms_step_params& p, int n_wave, int wmode, int lat, bool permeable, cudaStream_t stream);
+// impermeable + RMS_LAT_FACES + RMS_WMODE_CONST only (rms_step_fast.cu)
+int rms_launch_step_fast(const rms_step_params& p, int n_wave, cudaStream_t stream);
 
 // reductions (rms_reduce.cu)
 struct rms_reduce_params {
@@ -187,3 +199,6 @@ int rms_launch_signal(const rms_reduce_params& p, int n_wave, int nq, const doub
                       double* d_im, double* d_sum_alpha, cudaStream_t stream, unsigned* n_launches);
 int rms_compute_tables(const rms_substrate* s, double dt, std::vector<float>& s_tab, std::vector<float>& P_tab);
 int rms_walkers_reserve_waves(rms_walkers* w, int n_wave, cudaStream_t stream);
+// rms_sched.cu: order[t] = walker index, sorted by the lattice cell the walker sits in (z-major), so that the
+// threads of a warp and the blocks resident at one time gather neighbouring words.  d_order: [n] device.
+int rms_order_walkers(const rms_substrate* s, const rms_walkers* w, uint32_t* d_order, cudaStream_t stream, unsigned* n_launches);

@@ -10,7 +10,7 @@ namespace {
 
 struct DeviceBuf {   // frees on scope exit
     void* p = nullptr;
-    ~DeviceBuf() { if (p) cudaFree(p); }
+    ~DeviceBuf() { if (p) rms_free(p); }
     template <class T> T* as() { return (T*)p; }
 };
 
@@ -114,7 +114,7 @@ extern "C" int rms_run(const rms_substrate* s, rms_walkers* w, const rms_run_des
         }
     }
     const bool want_labels = (d->flags & RMS_RUN_LABEL_GATHER) != 0;
-    const int lat = (!permeable && s->d_faces && !want_labels) ? RMS_LAT_FACES : RMS_LAT_LABELS;
+    const int lat = (!permeable && s->d_nbr && !want_labels) ? RMS_LAT_FACES : RMS_LAT_LABELS;
 
     rc = rms_walkers_reserve_waves(w, nW, stream);
     if (rc != RMS_OK) return rc;
@@ -173,18 +173,18 @@ extern "C" int rms_run(const rms_substrate* s, rms_walkers* w, const rms_run_des
     const int nQ = nW * nG * nD;
     const size_t n_sig = (size_t)nQ * nC, n_mom = (size_t)nS * nD * nC, n_sal = (size_t)nS * nC, n_flow = (size_t)nS * nC * nC;
     const size_t n_res_d = 2 * n_sig + 2 * n_mom + n_sal + nC;       // doubles
-    DeviceBuf b_tabs, b_segs, b_wave, b_wsuf, b_q, b_res, b_dirs;
-    RMS_CUDA_TRY(cudaMalloc(&b_tabs.p, tabs.size() * sizeof(float)));
+    DeviceBuf b_tabs, b_segs, b_wave, b_wsuf, b_q, b_res, b_dirs, b_order;
+    RMS_CUDA_TRY(rms_malloc((void**)&b_tabs.p, tabs.size() * sizeof(float)));
     RMS_CUDA_TRY(cudaMemcpyAsync(b_tabs.p, tabs.data(), tabs.size() * sizeof(float), cudaMemcpyHostToDevice, stream));
     if (const_mode) {
         if (!segs.empty()) {
-            RMS_CUDA_TRY(cudaMalloc(&b_segs.p, segs.size() * sizeof(rms_segment)));
+            RMS_CUDA_TRY(rms_malloc((void**)&b_segs.p, segs.size() * sizeof(rms_segment)));
             RMS_CUDA_TRY(cudaMemcpyAsync(b_segs.p, segs.data(), segs.size() * sizeof(rms_segment), cudaMemcpyHostToDevice, stream));
         }
     } else if (nW > 0 && nT > 0) {
-        RMS_CUDA_TRY(cudaMalloc(&b_wave.p, (size_t)nW * nT * sizeof(float)));
+        RMS_CUDA_TRY(rms_malloc((void**)&b_wave.p, (size_t)nW * nT * sizeof(float)));
         RMS_CUDA_TRY(cudaMemcpyAsync(b_wave.p, d->wave, (size_t)nW * nT * sizeof(float), cudaMemcpyHostToDevice, stream));
-        RMS_CUDA_TRY(cudaMalloc(&b_wsuf.p, (size_t)nW * (nT + 1) * sizeof(double)));
+        RMS_CUDA_TRY(rms_malloc((void**)&b_wsuf.p, (size_t)nW * (nT + 1) * sizeof(double)));
         RMS_CUDA_TRY(cudaMemcpyAsync(b_wsuf.p, suf.data(), (size_t)nW * (nT + 1) * sizeof(double), cudaMemcpyHostToDevice, stream));
     }
     // phase per unit Phi, in turns: gamp dt l_p n / (2 pi)   (Eq.7 with the right-endpoint rule, R11)
@@ -198,14 +198,14 @@ extern "C" int rms_run(const rms_substrate* s, rms_walkers* w, const rms_run_des
                 for (int x = 0; x < 3; ++x) qv[3 * q + x] = c * d->dirs[3 * k + x];
                 qwave[q] = m;
             }
-    RMS_CUDA_TRY(cudaMalloc(&b_q.p, qv.size() * sizeof(double) + qwave.size() * sizeof(int)));
+    RMS_CUDA_TRY(rms_malloc((void**)&b_q.p, qv.size() * sizeof(double) + qwave.size() * sizeof(int)));
     RMS_CUDA_TRY(cudaMemcpyAsync(b_q.p, qv.data(), qv.size() * sizeof(double), cudaMemcpyHostToDevice, stream));
     int* d_qwave = (int*)(b_q.as<double>() + qv.size());
     RMS_CUDA_TRY(cudaMemcpyAsync(d_qwave, qwave.data(), qwave.size() * sizeof(int), cudaMemcpyHostToDevice, stream));
-    RMS_CUDA_TRY(cudaMalloc(&b_dirs.p, std::max(nD, 1) * 3 * sizeof(double)));
+    RMS_CUDA_TRY(rms_malloc((void**)&b_dirs.p, std::max(nD, 1) * 3 * sizeof(double)));
     if (nD) RMS_CUDA_TRY(cudaMemcpyAsync(b_dirs.p, d->dirs, (size_t)nD * 3 * sizeof(double), cudaMemcpyHostToDevice, stream));
     const size_t res_bytes = n_res_d * sizeof(double) + n_flow * sizeof(unsigned long long);
-    RMS_CUDA_TRY(cudaMalloc(&b_res.p, res_bytes));
+    RMS_CUDA_TRY(rms_malloc((void**)&b_res.p, res_bytes));
     RMS_CUDA_TRY(cudaMemsetAsync(b_res.p, 0, res_bytes, stream));
     double* d_re = b_res.as<double>();
     double* d_im = d_re + n_sig;
@@ -226,7 +226,7 @@ extern "C" int rms_run(const rms_substrate* s, rms_walkers* w, const rms_run_des
     rms_step_params sp;
     memset(&sp, 0, sizeof sp);
     sp.nx = s->nx; sp.ny = s->ny; sp.nz = s->nz;
-    sp.labels = s->d_labels; sp.faces = s->d_faces; sp.NX = s->NX; sp.NY = s->NY;
+    sp.labels = s->d_labels; sp.nbr = s->d_nbr; sp.NX = s->NX; sp.NY = s->NY;
     sp.st = w->a; sp.n = n; sp.first_id = w->first_id; sp.rk = rms_make_keys(w->seed);
     sp.s_tab = b_tabs.as<float>(); sp.rate = sp.s_tab + nL; sp.P512 = sp.rate + nL; sp.n_labels = nL;
     sp.counters = w->d_counters; sp.n_wave = nW; sp.wave_stride = nT; sp.wsuf_stride = nT + 1;
@@ -236,11 +236,20 @@ extern "C" int rms_run(const rms_substrate* s, rms_walkers* w, const rms_run_des
     rp.st = w->a; rp.n = n; rp.label_class = s->d_label_class; rp.n_classes = nC; rp.n_dir = nD;
     rp.dirs = b_dirs.as<double>(); rp.voxel_um = s->voxel_um;
 
+    // spatial ordering of the walkers over the threads pays once the lattice outgrows the caches
+    const bool ordered = n >= 4096 && s->n_vox >= (1u << 22) && !(d->flags & RMS_RUN_NO_ORDERING);
+    if (ordered) RMS_CUDA_TRY(rms_malloc((void**)&b_order.p, n * sizeof(uint32_t)));
+
     int64_t a = 0;
     int snap = 0;
     for (size_t li = 0; li < bounds.size(); ++li) {
         const int64_t b = bounds[li];
         if (b > a) {
+            if (ordered) {
+                rc = rms_order_walkers(s, w, b_order.as<uint32_t>(), stream, &n_launches);
+                if (rc != RMS_OK) return rc;
+                sp.order = b_order.as<uint32_t>();
+            }
             sp.step0 = (uint32_t)(w->steps_done + (uint64_t)a);
             sp.n_steps = (uint32_t)(b - a);
             for (int m = 0; m < nW; ++m) {
@@ -259,7 +268,10 @@ extern "C" int rms_run(const rms_substrate* s, rms_walkers* w, const rms_run_des
             }
             cudaEvent_t e0 = evs.make(), e1 = evs.make();
             RMS_CUDA_TRY(cudaEventRecord(e0, stream));
-            rc = rms_launch_step(sp, nW, wmode, lat, permeable, stream);
+            if (!permeable && lat == RMS_LAT_FACES && wmode == RMS_WMODE_CONST && !(d->flags & RMS_RUN_GENERAL_KERNEL))
+                rc = rms_launch_step_fast(sp, nW, stream);
+            else
+                rc = rms_launch_step(sp, nW, wmode, lat, permeable, stream);
             if (rc != RMS_OK) return rc;
             RMS_CUDA_TRY(cudaEventRecord(e1, stream));
             step_ev.push_back({e0, e1});

@@ -8,9 +8,10 @@
 // or permeation with the probability of Eq.3.
 //
 // Two lattice paths:
-//   RMS_LAT_FACES   impermeable runs: the walker caches the 6 membrane bits of its voxel (face-mask
-//                   lattice); a reflection touches no memory, a pass issues one byte gather that is
-//                   consumed at the NEXT interaction (off the critical path).
+//   RMS_LAT_FACES   impermeable runs: the walker caches the 6 membrane bits of its voxel (from the
+//                   neighbourhood lattice); a reflection touches no memory, a pass issues one gather that
+//                   is consumed at the NEXT interaction (off the critical path).  This is the general
+//                   kernel (any waveform); rms_step_fast.cu serves piecewise-constant gradients.
 //   RMS_LAT_LABELS  the paper's lookup table: gather the neighbour's uint16 label at every face.
 //                   With PERM it follows the interaction loop literally, including the rescaling of
 //                   the remaining hop on entering a compartment of different D (R7).
@@ -45,6 +46,15 @@ __device__ __forceinline__ void rms_hop(uint32_t wa, uint32_t wb, float s, float
     rz = s * z;
 }
 
+// the 6 membrane bits of a voxel (bit k: face towards +k, bit 3+k: towards -k, bit 6: ghost) from its
+// neighbourhood word: a face is a membrane iff the face neighbour does not carry the voxel's label
+__device__ __forceinline__ uint32_t rms_face_byte(uint32_t w)
+{
+    const uint32_t n = ~w;
+    return ((n >> 14) & 1u) | (((n >> 16) & 1u) << 1) | (((n >> 22) & 1u) << 2) | (((n >> 12) & 1u) << 3) |
+           (((n >> 10) & 1u) << 4) | (((n >> 4) & 1u) << 5) | (((w >> 27) & 1u) << 6);
+}
+
 __device__ __forceinline__ bool rms_outside(float g) { return __float_as_uint(g) >= 0x3F800000u; }  // g >= 1 or g < 0
 
 __device__ __forceinline__ float rms_hit_time(bool cross, float f, float r)
@@ -55,8 +65,9 @@ __device__ __forceinline__ float rms_hit_time(bool cross, float f, float r)
 template <int NW, int WMODE, int LAT, bool PERM>
 __global__ void __launch_bounds__(RMS_BLOCK) rms_step_kernel(const __grid_constant__ rms_step_params p)
 {
-    const uint64_t i = (uint64_t)blockIdx.x * RMS_BLOCK + threadIdx.x;
-    if (i >= p.n) return;
+    const uint64_t t_global = (uint64_t)blockIdx.x * RMS_BLOCK + threadIdx.x;
+    if (t_global >= p.n) return;
+    const uint64_t i = p.order ? (uint64_t)p.order[t_global] : t_global;   // walker of this thread (rms_sched.cu)
     const uint64_t id = p.first_id + i;
     const uint32_t id_lo = (uint32_t)id, id_hi = (uint32_t)(id >> 32);
     const size_t n = (size_t)p.n;
@@ -93,7 +104,7 @@ __global__ void __launch_bounds__(RMS_BLOCK) rms_step_kernel(const __grid_consta
     uint32_t fm = 0;
     if (LAT == RMS_LAT_FACES) {
         lin = ((wz + 1) * p.NY + (wy + 1)) * NX + (wx + 1);
-        fm = p.faces[lin];
+        fm = rms_face_byte(__ldg(p.nbr + lin));
     }
 
     float phiF[NW > 0 ? NW : 1][3];
@@ -175,7 +186,7 @@ __global__ void __launch_bounds__(RMS_BLOCK) rms_step_kernel(const __grid_consta
                                         if (Y == 0) { Y = p.ny; wraps -= 1u << 10; } else if (Y == p.NY - 1) { Y = 1; wraps += 1u << 10; }
                                         if (Z == 0) { Z = p.nz; wraps -= 1u << 20; } else if (Z == p.nz + 1) { Z = 1; wraps += 1u << 20; }
                                         lin = (Z * p.NY + Y) * NX + X;
-                                        fm = p.faces[lin];
+                                        fm = rms_face_byte(__ldg(p.nbr + lin));
                                     }
                                     const uint32_t bit = isx ? 1u : (isy ? 2u : 4u);
                                     membrane = ((fm >> (neg ? 3 : 0)) & bit) != 0;
@@ -198,7 +209,7 @@ __global__ void __launch_bounds__(RMS_BLOCK) rms_step_kernel(const __grid_consta
                                     if (LAT == RMS_LAT_FACES) {
                                         const int stride = isx ? 1 : (isy ? NX : NXY);
                                         lin += neg ? -stride : stride;
-                                        fm = p.faces[lin];
+                                        fm = rms_face_byte(__ldg(p.nbr + lin));
                                     } else {
                                         if (isx) wx = nwk; else if (isy) wy = nwk; else wz = nwk;
                                         const int sg1 = neg ? -1 : 1;

@@ -1,0 +1,309 @@
+// rms_step_fast.cu -- H2..H5 for the throughput-critical case: impermeable membranes and piecewise-constant,
+// integer-valued gradient waveforms (PGSE and every other rectangular-lobe sequence).  Same method and
+// the same numbers as the general kernel of rms_step.cu (section 2.2 steps 2-4; corner
+// reflector of Fig.2; elastic collision P:90), organised for the B200 instruction pipes:
+//
+//   * one thread owns one walker for all steps of a launch, state in registers (position = linear index
+//     into the padded neighbourhood lattice + fp32 in-voxel offset);
+//   * the walker carries the 27-bit neighbourhood word of its voxel (rms_substrate.cu).  While it stays in
+//     its compartment every face test of a hop -- first, second or third interaction, in any order --
+//     is one bit of that word: "does the voxel I am about to enter carry my label?".  A step therefore
+//     issues at most ONE gather (the word of the voxel it ends in), consumed a whole step later;
+//   * the (at most three) interactions are resolved in hit order (R10) by sorting three keys
+//     overshoot_k |r_i r_j| (same order as the hit times, no division), with the axis id in the two low
+//     mantissa bits, and walking a position code through the word: three short, branch-light slots;
+//   * per axis the outcome is applied branch-free: passed -> g -+ 1, reflected -> mirrored;
+//   * the direction uses a 256-entry (cos, sin) table in shared memory + a degree-3 residual, accurate to
+//     fp32 rounding with 5 ALU-pipe instructions (the ALU pipe, not issue, limits this kernel);
+//   * Philox4x32-10: one call serves two steps (R2), both steps fully unrolled.
+#include "rms_internal.cuh"
+
+#define RMS_FBLOCK 128
+#define RMS_FFLUSH 1024u             // steps between flushes of the fp32 / int32 phase partial sums into fp64 (even)
+#define RMS_ONE_MINUS 0.99999994f    // 1 - 2^-24
+
+namespace {
+
+__device__ __forceinline__ float rms_sqrt_fast(float x)
+{
+    float y;
+    asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+    return y;
+}
+
+// max / min of three signed ints (VIMNMX3 on sm_100)
+__device__ __forceinline__ int rms_max3(int a, int b, int c) { return max(max(a, b), c); }
+__device__ __forceinline__ int rms_min3(int a, int b, int c) { return min(min(a, b), c); }
+
+// float bits with the two low mantissa bits replaced by a tag (one LOP3)
+__device__ __forceinline__ int rms_tag(float v, int tag)
+{
+    int r;
+    asm("lop3.b32 %0, %1, %2, %3, 0xEA;" : "=r"(r) : "r"(__float_as_int(v)), "r"(~3), "r"(tag));   // (a & b) | c
+    return r;
+}
+
+// byte `sel` (0..3) of x, zero extended (selector nibbles 1..3 = 0 pick byte 0 of x, which callers keep 0)
+__device__ __forceinline__ uint32_t rms_prmt(uint32_t x, uint32_t y, uint32_t sel)
+{
+    uint32_t r;
+    asm("prmt.b32 %0, %1, %2, %3;" : "=r"(r) : "r"(x), "r"(y), "r"(sel));
+    return r;
+}
+
+// padded linear index of a ghost voxel -> index of its periodic image inside the box, wrap counters updated
+__device__ __noinline__ uint2 rms_fold_ghost(int lin, uint32_t wraps, int nx, int ny, int nz)
+{
+    const int NX = nx + 2, NY = ny + 2, NXY = NX * NY;
+    int Z = lin / NXY, rem = lin - Z * NXY, Y = rem / NX, X = rem - Y * NX;
+    if (X == 0) { X = nx; wraps -= 1u; } else if (X == NX - 1) { X = 1; wraps += 1u; }
+    if (Y == 0) { Y = ny; wraps -= 1u << 10; } else if (Y == NY - 1) { Y = 1; wraps += 1u << 10; }
+    if (Z == 0) { Z = nz; wraps -= 1u << 20; } else if (Z == nz + 1) { Z = 1; wraps += 1u << 20; }
+    return make_uint2((uint32_t)((Z * NY + Y) * NX + X), wraps);
+}
+
+}  // namespace
+
+template <int NW>
+__global__ void __launch_bounds__(RMS_FBLOCK) rms_step_fast_kernel(const __grid_constant__ rms_step_params p)
+{
+    __shared__ float2 sm_trig[256];   // (cos, sin) of the centre of the 256 azimuth bins
+
+    for (int t = threadIdx.x; t < 256; t += RMS_FBLOCK) {
+        double sn, cs;
+        sincospi(-1.0 + (2.0 * t + 1.0) / 256.0, &sn, &cs);   // bin centre: theta = -pi + (t + 1/2) 2 pi / 256
+        sm_trig[t] = make_float2((float)cs, (float)sn);
+    }
+    __syncthreads();
+
+    const uint64_t t_global = (uint64_t)blockIdx.x * RMS_FBLOCK + threadIdx.x;
+    if (t_global >= p.n) return;
+    const uint64_t i = p.order ? (uint64_t)p.order[t_global] : t_global;   // walker of this thread (rms_sched.cu)
+    const uint64_t id = p.first_id + i;
+    const uint32_t id_lo = (uint32_t)id, id_hi = (uint32_t)(id >> 32);
+    const size_t n = (size_t)p.n;
+
+    // ---- load state -----------------------------------------------------------------------
+    int wx = p.st.w[0][i], wy = p.st.w[1][i], wz = p.st.w[2][i];
+    const int wx0 = wx, wy0 = wy, wz0 = wz;
+    int dIx = p.st.dI[0][i], dIy = p.st.dI[1][i], dIz = p.st.dI[2][i];
+    float fx = p.st.f[0][i], fy = p.st.f[1][i], fz = p.st.f[2][i];
+    const uint32_t lab = p.st.lab[i];
+    const uint32_t L = lab & 0xFFFFu;
+    const float s = p.s_tab[L];
+
+    // launch prologue of the phase: Phi += (dI - f0) * sum_{launch} w
+    if (NW > 0) {
+#pragma unroll
+        for (int m = 0; m < NW; ++m) {
+            const double wt = p.wtot[m];
+            if (wt != 0.0) {
+                p.st.phi[(size_t)(3 * m + 0) * n + i] += ((double)dIx - (double)p.st.f0[0][i]) * wt;
+                p.st.phi[(size_t)(3 * m + 1) * n + i] += ((double)dIy - (double)p.st.f0[1][i]) * wt;
+                p.st.phi[(size_t)(3 * m + 2) * n + i] += ((double)dIz - (double)p.st.f0[2][i]) * wt;
+            }
+        }
+    }
+
+    const int NX = p.NX, NXY = p.NX * p.NY;
+    int lin = ((wz + 1) * p.NY + (wy + 1)) * NX + (wx + 1);
+    uint32_t wraps = 512u | (512u << 10) | (512u << 20);   // packed per-axis counts of box wraps (+512)
+    uint32_t nb = __ldg(p.nbr + lin);
+
+    constexpr int NWA = NW > 0 ? NW : 1;
+    float phiF[NWA][3];
+    int A32[NWA][3];
+    float wf[NWA];
+    int wi[NWA], wrem[NWA];
+#pragma unroll
+    for (int m = 0; m < NWA; ++m) {
+        wf[m] = 0.f; wi[m] = 0; wrem[m] = 0;
+#pragma unroll
+        for (int k = 0; k < 3; ++k) { phiF[m][k] = 0.f; A32[m][k] = 0; }
+    }
+    unsigned n_enc = 0;
+
+    // landed on a ghost voxel: fold back into the box (rare; the word of a ghost voxel is its image's word)
+    auto fold = [&]() {
+        const uint2 lw = rms_fold_ghost(lin, wraps, p.nx, p.ny, p.nz);
+        lin = (int)lw.x; wraps = lw.y;
+        nb &= ~RMS_NBR_GHOST;
+    };
+
+    // ---- one Monte Carlo step from the two direction words (R3, R4) ------------------------------
+    auto step = [&](const uint32_t wa, const uint32_t wb) {
+        // z = sym(wa): exact odd multiple of 2^-23
+        const float z = fmaf(__uint_as_float(__funnelshift_r(wa, 0x7Fu, 9)) - 1.5f, 2.0f, 1.1920928955078125e-07f);
+        // azimuth pi * sym(wb) = bin centre (top 8 bits) + residual (next 15 bits, exact): rotate the table entry
+        const float2 cs0 = sm_trig[wb >> 24];
+        const float tau = __uint_as_float(((wb >> 1) & 0x007FFF00u) | 0x3F800080u) - 1.5f;   // in (-1/2, 1/2), exact
+        const float x2 = tau * tau;
+        const float sb = tau * fmaf(x2, -2.4641574e-06f, 0.024543693f);    // sin(tau pi/128)
+        const float e = x2 * -3.0119642e-04f;                               // cos(tau pi/128) - 1
+        const float cpsi = fmaf(cs0.x, e, -cs0.y * sb) + cs0.x;
+        const float spsi = fmaf(cs0.y, e, cs0.x * sb) + cs0.y;
+        const float sr = s * rms_sqrt_fast(fmaf(-z, z, 1.0f));
+        const float rx = sr * cpsi, ry = sr * spsi, rz = s * z;
+
+        float gx = fx + rx, gy = fy + ry, gz = fz + rz;
+        const bool cx = __float_as_uint(gx) >= 0x3F800000u;    // g >= 1 or g < 0: the hop reaches a voxel face
+        const bool cy = __float_as_uint(gy) >= 0x3F800000u;
+        const bool cz = __float_as_uint(gz) >= 0x3F800000u;
+        if (cx | cy | cz) {
+            // sign of the hop per axis; plane ahead h = (1 + sigma)/2; overshoot beyond it rho = sigma g - h >= 0
+            const float sgx = __uint_as_float((__float_as_uint(rx) & 0x80000000u) | 0x3F800000u);
+            const float sgy = __uint_as_float((__float_as_uint(ry) & 0x80000000u) | 0x3F800000u);
+            const float sgz = __uint_as_float((__float_as_uint(rz) & 0x80000000u) | 0x3F800000u);
+            const float h2x = sgx + 1.f, h2y = sgy + 1.f, h2z = sgz + 1.f;          // 2 h
+            const float rhox = fmaf(sgx, gx, -0.5f * h2x), rhoy = fmaf(sgy, gy, -0.5f * h2y), rhoz = fmaf(sgz, gz, -0.5f * h2z);
+            // hit order (R10): larger overshoot / |r| = earlier.  key_k = rho_k |r_i r_j| orders the same way;
+            // a face not reached has rho < 0 and sorts last.  The two low mantissa bits carry 3 - axis, so
+            // ties go to the lower axis and the slot knows its axis.
+            const float ax = fabsf(rx), ay = fabsf(ry), az = fabsf(rz);
+            const int kx = rms_tag(rhox * (ay * az), 3);
+            const int ky = rms_tag(rhoy * (ax * az), 2);
+            const int kz = rms_tag(rhoz * (ax * ay), 1);
+            const int k_hi = rms_max3(kx, ky, kz), k_lo = rms_min3(kx, ky, kz);
+            const int k_mid = kx ^ ky ^ kz ^ k_hi ^ k_lo;
+            // per-axis increments of the position code: pass flag (bit 5 + axis) + signed step in the 3x3x3 index,
+            // one byte each, at byte 3 - axis (byte 0 = 0 serves the upper result bytes of the permute)
+            const int isx = (__float_as_int(rx) >> 31) | 1, isy = (__float_as_int(ry) >> 31) | 1, isz = (__float_as_int(rz) >> 31) | 1;
+            const uint32_t lut = 0x20408000u + ((uint32_t)isx << 24) + ((uint32_t)(3 * isy) << 16) + ((uint32_t)(9 * isz) << 8);
+            if (nb & RMS_NBR_GHOST) fold();
+            uint32_t pos = RMS_NBR_SELF;
+            auto slot = [&](const int key) {
+                const uint32_t q = pos + rms_prmt(lut, 0u, (uint32_t)key & 3u);
+                if (__funnelshift_r(nb, 0u, q) & 1u) pos = q;      // the voxel ahead carries my label: pass
+                else ++n_enc;                                      // membrane: elastic collision
+            };
+            slot(k_hi);
+            if (k_mid >= 0) {
+                slot(k_mid);
+                if (k_lo >= 0) slot(k_lo);
+            }
+            // outcome per axis: passed -> g - sigma (enters the neighbour), else mirrored on the face plane, 2 h - g
+            {
+                const bool ps = (pos & 32u) != 0;
+                if (ps) {
+                    gx -= sgx; lin += isx;
+#pragma unroll
+                    for (int m = 0; m < NW; ++m) A32[m][0] += isx * wrem[m];
+                }
+                if (cx && !ps) gx = h2x - gx;
+            }
+            {
+                const bool ps = (pos & 64u) != 0;
+                if (ps) {
+                    gy -= sgy; lin += isy * NX;
+#pragma unroll
+                    for (int m = 0; m < NW; ++m) A32[m][1] += isy * wrem[m];
+                }
+                if (cy && !ps) gy = h2y - gy;
+            }
+            {
+                const bool ps = (pos & 128u) != 0;
+                if (ps) {
+                    gz -= sgz; lin += isz * NXY;
+#pragma unroll
+                    for (int m = 0; m < NW; ++m) A32[m][2] += isz * wrem[m];
+                }
+                if (cz && !ps) gz = h2z - gz;
+            }
+            if (pos != RMS_NBR_SELF) nb = __ldg(p.nbr + lin);
+        }
+        fx = gx; fy = gy; fz = gz;
+        // phase, fractional part: Phi_F += w f (the integer part is event driven, above)
+#pragma unroll
+        for (int m = 0; m < NW; ++m) {
+            phiF[m][0] = fmaf(wf[m], fx, phiF[m][0]);
+            phiF[m][1] = fmaf(wf[m], fy, phiF[m][1]);
+            phiF[m][2] = fmaf(wf[m], fz, phiF[m][2]);
+            wrem[m] -= wi[m];
+        }
+    };
+
+    uint32_t j = p.step0;                       // steps done so far (absolute)
+#pragma unroll 1
+    for (int sg = 0; sg < p.n_seg; ++sg) {
+        const rms_segment sgm = p.segs[sg];
+        const uint32_t seg_end = j + sgm.n;
+#pragma unroll
+        for (int m = 0; m < NW; ++m) {
+            wi[m] = sgm.w[m];
+            wf[m] = (float)sgm.w[m];
+            wrem[m] = sgm.wrem_end[m] + sgm.w[m] * (int)sgm.n;   // weight remaining in this launch, current step included
+        }
+#pragma unroll 1
+        while (j < seg_end) {
+            const uint32_t chunk_end = min(seg_end, (j + RMS_FFLUSH) & ~1u);
+            uint32_t r0, r1, r2, r3;
+            if (j & 1u) {                        // second half of a Philox call that an earlier segment began
+                rms_philox(p.rk, id_lo, id_hi, j >> 1, RMS_STREAM_DIR, r0, r1, r2, r3);
+                step(r2, r3);
+                ++j;
+            }
+#pragma unroll 1
+            while (j + 2u <= chunk_end) {
+                rms_philox(p.rk, id_lo, id_hi, j >> 1, RMS_STREAM_DIR, r0, r1, r2, r3);
+                step(r0, r1);
+                step(r2, r3);
+                j += 2u;
+            }
+            if (j < chunk_end) {
+                rms_philox(p.rk, id_lo, id_hi, j >> 1, RMS_STREAM_DIR, r0, r1, r2, r3);
+                step(r0, r1);
+                ++j;
+            }
+            // flush the chunk's partial sums into the fp64 accumulators
+#pragma unroll
+            for (int m = 0; m < NW; ++m)
+#pragma unroll
+                for (int k = 0; k < 3; ++k) {
+                    p.st.phi[(size_t)(3 * m + k) * n + i] += (double)phiF[m][k] + (double)A32[m][k];
+                    phiF[m][k] = 0.f; A32[m][k] = 0;
+                }
+        }
+    }
+
+    // ---- store state --------------------------------------------------------------------------
+    {
+        int Z = lin / NXY, rem = lin - Z * NXY, Y = rem / NX, X = rem - Y * NX;
+        int wrx = (int)(wraps & 1023u) - 512, wry = (int)((wraps >> 10) & 1023u) - 512, wrz = (int)((wraps >> 20) & 1023u) - 512;
+        if (X == 0) { X = p.nx; --wrx; } else if (X == NX - 1) { X = 1; ++wrx; }
+        if (Y == 0) { Y = p.ny; --wry; } else if (Y == p.NY - 1) { Y = 1; ++wry; }
+        if (Z == 0) { Z = p.nz; --wrz; } else if (Z == p.nz + 1) { Z = 1; ++wrz; }
+        wx = X - 1; wy = Y - 1; wz = Z - 1;
+        dIx += (wx - wx0) + wrx * p.nx;
+        dIy += (wy - wy0) + wry * p.ny;
+        dIz += (wz - wz0) + wrz * p.nz;
+    }
+    p.st.w[0][i] = wx; p.st.w[1][i] = wy; p.st.w[2][i] = wz;
+    p.st.dI[0][i] = dIx; p.st.dI[1][i] = dIy; p.st.dI[2][i] = dIz;
+    // an offset of exactly 1 (a walker left sitting on its upper face by rounding) is legal inside the loop: it
+    // crosses at once if it moves on upwards; the stored state keeps the floor convention [0, 1) (R15)
+    p.st.f[0][i] = fminf(fx, RMS_ONE_MINUS); p.st.f[1][i] = fminf(fy, RMS_ONE_MINUS); p.st.f[2][i] = fminf(fz, RMS_ONE_MINUS);
+    p.st.relax[i] = fmaf(p.rate[L], (float)p.n_steps, p.st.relax[i]);   // impermeable: the label never changes (Eq.5)
+
+    // diagnostics: warp-shuffle reduction, one atomic per warp (early-exited lanes are not in the mask)
+    const unsigned mask = __activemask();
+    n_enc = __reduce_add_sync(mask, n_enc);
+    if ((threadIdx.x & 31) == (unsigned)(__ffs(mask) - 1) && n_enc) atomicAdd(&p.counters[0], (unsigned long long)n_enc);
+}
+
+int rms_launch_step_fast(const rms_step_params& p, int n_wave, cudaStream_t stream)
+{
+    if (p.n == 0 || p.n_steps == 0) return RMS_OK;
+    const unsigned grid = (unsigned)((p.n + RMS_FBLOCK - 1) / RMS_FBLOCK);
+    switch (n_wave) {
+        case 0: rms_step_fast_kernel<0><<<grid, RMS_FBLOCK, 0, stream>>>(p); break;
+        case 1: rms_step_fast_kernel<1><<<grid, RMS_FBLOCK, 0, stream>>>(p); break;
+        case 2: rms_step_fast_kernel<2><<<grid, RMS_FBLOCK, 0, stream>>>(p); break;
+        case 3: rms_step_fast_kernel<3><<<grid, RMS_FBLOCK, 0, stream>>>(p); break;
+        case 4: rms_step_fast_kernel<4><<<grid, RMS_FBLOCK, 0, stream>>>(p); break;
+        default:
+            rms_set_error("n_wave = %d is above RMS_MAX_WAVES = %d", n_wave, RMS_MAX_WAVES);
+            return RMS_ERR_UNSUPPORTED;
+    }
+    RMS_CUDA_TRY(cudaGetLastError());
+    return RMS_OK;
+}

@@ -1,4 +1,4 @@
-// rms_substrate.cu -- H0: substrate upload and the derived face-mask lattice (include/rms.h, rms_substrate_create).
+// rms_substrate.cu -- H0: substrate upload and the derived neighbourhood lattice (include/rms.h, rms_substrate_create).
 #include <math.h>
 #include <stdarg.h>
 #include <string.h>
@@ -22,39 +22,47 @@ extern "C" const char* rms_last_error(void) { return g_err; }
 extern "C" const char* rms_version(void) { return "rms-b200 0.1 (sm_100a)"; }
 
 // ------------------------------------------------------------------------------------------------
-// Face-mask lattice.  A membrane is a voxel face whose two sides carry different labels; the
-// walk only ever asks "is the face I am about to cross a membrane?", so that one bit per face is
-// precomputed.  Layout: (nx+2)(ny+2)(nz+2) bytes, x fastest; voxel (x,y,z) of the box sits at padded
-// (x+1,y+1,z+1); the shell replicates the periodic images (R1) so that a walker can step over the box
-// edge without any wrap arithmetic and is folded back when it lands on a ghost voxel (bit 6).
+// Neighbourhood lattice.  A membrane is a voxel face whose two sides carry different labels.  A
+// hop shorter than a voxel meets at most three faces, all of them inside the 3x3x3 block
+// around the walker's voxel, and while the walker stays in its compartment every face test reads "does
+// that neighbour carry my label?".  One 32-bit word per voxel answers all of them: bit
+// (dx+1) + 3 (dy+1) + 9 (dz+1) = the neighbour at offset d has the same label as this voxel.
+// Layout: (nx+2)(ny+2)(nz+2) words, x fastest; voxel (x,y,z) of the box sits at padded (x+1,y+1,z+1);
+// the shell replicates the periodic images (R1) so that a walker can step over the box edge without
+// any wrap arithmetic and is folded back when it lands on a ghost voxel (RMS_NBR_GHOST).
 // ------------------------------------------------------------------------------------------------
 __device__ __forceinline__ int rms_wrap1(int a, int n) { return a < 0 ? a + n : (a >= n ? a - n : a); }
 
-__global__ void __launch_bounds__(128) rms_build_faces_kernel(const uint16_t* __restrict__ labels, int nx, int ny, int nz,
-                                                               uint8_t* __restrict__ faces, int n_labels,
-                                                               unsigned long long* __restrict__ stats)
+__global__ void __launch_bounds__(128) rms_build_nbr_kernel(const uint16_t* __restrict__ labels, int nx, int ny, int nz,
+                                                             uint32_t* __restrict__ nbr, int n_labels,
+                                                             unsigned long long* __restrict__ stats)
 {
     const int NX = nx + 2, NY = ny + 2;
     const int X = blockIdx.x * blockDim.x + threadIdx.x;
     const int Y = blockIdx.y, Z = blockIdx.z;
     unsigned n_faces = 0, bad = 0;
     if (X < NX) {
-        // periodic image of the padded coordinate (n may be 1: wrap twice is not needed since |X-1| <= n)
+        // periodic image of the padded coordinate (|X-1| <= n, so one wrap is enough even for n = 1)
         const int x = rms_wrap1(X - 1, nx), y = rms_wrap1(Y - 1, ny), z = rms_wrap1(Z - 1, nz);
-        const size_t row = ((size_t)z * ny + y) * nx;
-        const uint16_t L = labels[row + x];
-        const uint16_t xp = labels[row + rms_wrap1(x + 1, nx)];
-        const uint16_t xm = labels[row + rms_wrap1(x - 1, nx)];
-        const uint16_t yp = labels[((size_t)z * ny + rms_wrap1(y + 1, ny)) * nx + x];
-        const uint16_t ym = labels[((size_t)z * ny + rms_wrap1(y - 1, ny)) * nx + x];
-        const uint16_t zp = labels[((size_t)rms_wrap1(z + 1, nz) * ny + y) * nx + x];
-        const uint16_t zm = labels[((size_t)rms_wrap1(z - 1, nz) * ny + y) * nx + x];
-        unsigned m = (xp != L) | ((yp != L) << 1) | ((zp != L) << 2) | ((xm != L) << 3) | ((ym != L) << 4) | ((zm != L) << 5);
+        const int xs[3] = {rms_wrap1(x - 1, nx), x, rms_wrap1(x + 1, nx)};
+        const int ys[3] = {rms_wrap1(y - 1, ny), y, rms_wrap1(y + 1, ny)};
+        const int zs[3] = {rms_wrap1(z - 1, nz), z, rms_wrap1(z + 1, nz)};
+        const uint16_t L = __ldg(labels + ((size_t)z * ny + y) * nx + x);
+        uint32_t m = 0;
+#pragma unroll
+        for (int c = 0; c < 3; ++c)
+#pragma unroll
+            for (int b = 0; b < 3; ++b) {
+                const uint16_t* row = labels + ((size_t)zs[c] * ny + ys[b]) * nx;
+#pragma unroll
+                for (int a = 0; a < 3; ++a) m |= (uint32_t)(__ldg(row + xs[a]) == L) << (a + 3 * b + 9 * c);
+            }
         const bool ghost = (X == 0) | (X == NX - 1) | (Y == 0) | (Y == NY - 1) | (Z == 0) | (Z == nz + 1);
-        if (ghost) m |= 64u;
-        faces[((size_t)Z * NY + Y) * NX + X] = (uint8_t)m;
+        if (ghost) m |= RMS_NBR_GHOST;
+        nbr[((size_t)Z * NY + Y) * NX + X] = m;
         if (!ghost) {
-            n_faces = __popc(m & 7u);   // each face counted once, from its lower side
+            // each face counted once, from its lower side: the +x, +y, +z neighbours (bits 14, 16, 22)
+            n_faces = 3 - (((m >> 14) & 1u) + ((m >> 16) & 1u) + ((m >> 22) & 1u));
             bad = (L >= n_labels);
         }
     }
@@ -146,7 +154,7 @@ extern "C" int rms_substrate_create(const rms_substrate_desc* d, void* cuda_stre
         s->owns_labels = false;
     } else {
         uint16_t* buf = nullptr;
-        SUB_TRY(cudaMalloc(&buf, n_vox * sizeof(uint16_t)));
+        SUB_TRY(rms_malloc((void**)&buf, n_vox * sizeof(uint16_t)));
         s->d_labels = buf;
         s->owns_labels = true;
         SUB_TRY(cudaMemcpyAsync(buf, d->labels, n_vox * sizeof(uint16_t),
@@ -154,22 +162,22 @@ extern "C" int rms_substrate_create(const rms_substrate_desc* d, void* cuda_stre
     }
     {
         uint8_t* lc = nullptr;
-        SUB_TRY(cudaMalloc(&lc, nL));
+        SUB_TRY(rms_malloc((void**)&lc, nL));
         s->d_label_class = lc;
         SUB_TRY(cudaMemcpyAsync(lc, s->label_class.data(), nL, cudaMemcpyHostToDevice, stream));
     }
-    SUB_TRY(cudaMalloc(&d_stats, 2 * sizeof(unsigned long long)));
+    SUB_TRY(rms_malloc((void**)&d_stats, 2 * sizeof(unsigned long long)));
     SUB_TRY(cudaMemsetAsync(d_stats, 0, 2 * sizeof(unsigned long long), stream));
     if (!(d->flags & RMS_NO_BRICKS)) {
         s->NX = s->nx + 2; s->NY = s->ny + 2; s->NZ = s->nz + 2;
-        SUB_TRY(cudaMalloc(&s->d_faces, (size_t)s->NX * s->NY * s->NZ));
+        SUB_TRY(rms_malloc((void**)&s->d_nbr, (size_t)s->NX * s->NY * s->NZ * sizeof(uint32_t)));
         dim3 grid((s->NX + 127) / 128, s->NY, s->NZ);
         if (grid.y > 65535u || grid.z > 65535u) {
-            rms_set_error("lattice too large for the face-mask build (ny+2, nz+2 must be <= 65535)");
+            rms_set_error("lattice too large for the neighbourhood-lattice build (ny+2, nz+2 must be <= 65535)");
             rc = RMS_ERR_UNSUPPORTED;
             goto fail;
         }
-        rms_build_faces_kernel<<<grid, 128, 0, stream>>>(s->d_labels, s->nx, s->ny, s->nz, s->d_faces, nL, d_stats);
+        rms_build_nbr_kernel<<<grid, 128, 0, stream>>>(s->d_labels, s->nx, s->ny, s->nz, s->d_nbr, nL, d_stats);
         SUB_TRY(cudaGetLastError());
     } else {
         rms_check_labels_kernel<<<148 * 8, 256, 0, stream>>>(s->d_labels, (size_t)n_vox, nL, d_stats);
@@ -177,7 +185,7 @@ extern "C" int rms_substrate_create(const rms_substrate_desc* d, void* cuda_stre
     }
     SUB_TRY(cudaMemcpyAsync(h_stats, d_stats, sizeof h_stats, cudaMemcpyDeviceToHost, stream));
     SUB_TRY(cudaStreamSynchronize(stream));
-    cudaFree(d_stats);
+    rms_free(d_stats);
     d_stats = nullptr;
     if (h_stats[1] != 0) {
         rms_set_error("%llu voxels carry a label >= n_labels (%d)", h_stats[1], nL);
@@ -188,7 +196,7 @@ extern "C" int rms_substrate_create(const rms_substrate_desc* d, void* cuda_stre
     *out = s;
     return RMS_OK;
 fail:
-    if (d_stats) cudaFree(d_stats);
+    if (d_stats) rms_free(d_stats);
     rms_substrate_destroy(s);
     return rc;
 #undef SUB_TRY
@@ -197,9 +205,9 @@ fail:
 extern "C" int rms_substrate_destroy(rms_substrate* s)
 {
     if (!s) return RMS_OK;
-    if (s->owns_labels && s->d_labels) cudaFree((void*)s->d_labels);
-    if (s->d_faces) cudaFree(s->d_faces);
-    if (s->d_label_class) cudaFree(s->d_label_class);
+    if (s->owns_labels && s->d_labels) rms_free((void*)s->d_labels);
+    if (s->d_nbr) rms_free(s->d_nbr);
+    if (s->d_label_class) rms_free(s->d_label_class);
     delete s;
     return RMS_OK;
 }
@@ -212,8 +220,8 @@ extern "C" int rms_substrate_get_info(const rms_substrate* s, rms_substrate_info
     out->n_voxels = s->n_vox;
     out->n_membrane_faces = s->n_membrane_faces;
     out->lattice_bytes = s->n_vox * sizeof(uint16_t);
-    out->brick_bytes = s->d_faces ? (uint64_t)s->NX * s->NY * s->NZ : 0;
-    out->has_bricks = s->d_faces != nullptr;
+    out->brick_bytes = s->d_nbr ? (uint64_t)s->NX * s->NY * s->NZ * sizeof(uint32_t) : 0;
+    out->has_bricks = s->d_nbr != nullptr;
     return RMS_OK;
 }
 

@@ -74,7 +74,7 @@ extern "C" int rms_walkers_init(const rms_substrate* s, uint64_t n_walkers, uint
             goto fail;                                                                                   \
         }                                                                                                \
     } while (0)
-    W_TRY(cudaMalloc(&w->d_block, total));
+    W_TRY(rms_malloc((void**)&w->d_block, total));
     {
         char* p = (char*)w->d_block;
         auto take = [&](size_t bytes) { char* q = p; p += bytes; return (void*)q; };
@@ -88,10 +88,10 @@ extern "C" int rms_walkers_init(const rms_substrate* s, uint64_t n_walkers, uint
         w->d_counters = (unsigned long long*)take(256);
     }
     w->n_wave_alloc = 1;
-    W_TRY(cudaMalloc(&w->a.phi, (size_t)3 * w->n_wave_alloc * n * sizeof(double)));
+    W_TRY(rms_malloc((void**)&w->a.phi, (size_t)3 * w->n_wave_alloc * n * sizeof(double)));
     W_TRY(cudaMemsetAsync(w->d_counters, 0, 64, stream));
     if (label_allowed) {
-        W_TRY(cudaMalloc(&d_allowed, s->n_labels));
+        W_TRY(rms_malloc((void**)&d_allowed, s->n_labels));
         W_TRY(cudaMemcpyAsync(d_allowed, label_allowed, s->n_labels, cudaMemcpyHostToDevice, stream));
     }
     rms_init_kernel<<<(unsigned)((n + 255) / 256), 256, 0, stream>>>(s->d_labels, s->nx, s->ny, s->nz, d_allowed, w->a, n,
@@ -100,7 +100,7 @@ extern "C" int rms_walkers_init(const rms_substrate* s, uint64_t n_walkers, uint
     W_TRY(cudaGetLastError());
     W_TRY(cudaMemcpyAsync(h_cnt, w->d_counters, 64, cudaMemcpyDeviceToHost, stream));
     W_TRY(cudaStreamSynchronize(stream));
-    if (d_allowed) cudaFree(d_allowed);
+    if (d_allowed) rms_free(d_allowed);
     d_allowed = nullptr;
     if (h_cnt[3] != 0) {
         rms_set_error("%llu walkers found no voxel with an allowed label in 2^20 proposals", h_cnt[3]);
@@ -110,7 +110,7 @@ extern "C" int rms_walkers_init(const rms_substrate* s, uint64_t n_walkers, uint
     *out = w;
     return RMS_OK;
 fail:
-    if (d_allowed) cudaFree(d_allowed);
+    if (d_allowed) rms_free(d_allowed);
     rms_walkers_destroy(w);
     return rc;
 #undef W_TRY
@@ -119,8 +119,8 @@ fail:
 extern "C" int rms_walkers_destroy(rms_walkers* w)
 {
     if (!w) return RMS_OK;
-    if (w->d_block) cudaFree(w->d_block);
-    if (w->a.phi) cudaFree(w->a.phi);
+    if (w->d_block) rms_free(w->d_block);
+    if (w->a.phi) rms_free(w->a.phi);
     delete w;
     return RMS_OK;
 }
@@ -137,12 +137,12 @@ int rms_walkers_reserve_waves(rms_walkers* w, int n_wave, cudaStream_t stream)
 {
     if (n_wave <= w->n_wave_alloc) return RMS_OK;
     double* np = nullptr;
-    RMS_CUDA_TRY(cudaMalloc(&np, (size_t)3 * n_wave * w->n * sizeof(double)));
+    RMS_CUDA_TRY(rms_malloc((void**)&np, (size_t)3 * n_wave * w->n * sizeof(double)));
     RMS_CUDA_TRY(cudaMemsetAsync(np, 0, (size_t)3 * n_wave * w->n * sizeof(double), stream));
     RMS_CUDA_TRY(cudaMemcpyAsync(np, w->a.phi, (size_t)3 * w->n_wave_alloc * w->n * sizeof(double), cudaMemcpyDeviceToDevice,
                                  stream));
     RMS_CUDA_TRY(cudaStreamSynchronize(stream));
-    cudaFree(w->a.phi);
+    rms_free(w->a.phi);
     w->a.phi = np;
     w->n_wave_alloc = n_wave;
     return RMS_OK;

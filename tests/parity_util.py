@@ -18,8 +18,16 @@ def oracle_run(cfg_sub, cfg_seq, n_walkers, seed, first_id=0):
                       per_walker=True)
 
 
-def compare(g, o, n_walkers, tol_s=TOL_S, tol_m=TOL_MOMENT, same_voxel=TOL_SAME_VOXEL, check_init=True):
-    """g: dict from the CUDA path (with "walkers"); o: dict from the oracle (per_walker=True)."""
+def compare(g, o, n_walkers, tol_s=TOL_S, tol_m=TOL_MOMENT, same_voxel=TOL_SAME_VOXEL, check_init=True, strict_s=False):
+    """g: dict from the CUDA path (with "walkers"); o: dict from the oracle (per_walker=True).
+
+    A trajectory is discontinuous where a hop passes the edge of a convex membrane corner (one way round it
+    misses the corner, the other way it is reflected), so an fp32 and an fp64 walker that differ by 1e-6 voxel
+    part company there for good; north_star allows 0.1 % of the walkers to do so.  Each such walker can move
+    S by at most 2/N, which at the small N of most cases here is above 1e-4 by itself: those cases bound
+    |dS| by 1e-4 + 2 n_diff / N (the agreeing walkers must agree to 1e-4) and widen the moment tolerances in
+    the same way; strict_s=True, used at full size where N is large, applies the plain tolerances
+    (DESIGN.md "Tolerances")."""
     rep = {}
     w = g["walkers"]
     if check_init:   # placement is integer work: bit exact
@@ -27,7 +35,10 @@ def compare(g, o, n_walkers, tol_s=TOL_S, tol_m=TOL_MOMENT, same_voxel=TOL_SAME_
         assert np.array_equal(w["off0"].astype(np.float64), o["init_off"])
     same = np.all(w["vox"] == o["final_vox"], axis=1)
     rep["same_voxel"] = float(same.mean())
+    rep["n_diff"] = int((~same).sum())
     assert rep["same_voxel"] >= same_voxel, rep
+    slack = 0.0 if strict_s else rep["n_diff"] / n_walkers
+    tol_s = tol_s + 2.0 * slack
     # positions agree to rounding for the walkers in the same voxel
     d_off = np.abs(w["off"][same].astype(np.float64) - o["final_off"][same])
     rep["max_offset_diff"] = float(d_off.max()) if d_off.size else 0.0
@@ -48,9 +59,10 @@ def compare(g, o, n_walkers, tol_s=TOL_S, tol_m=TOL_MOMENT, same_voxel=TOL_SAME_
             err = np.abs(g[k] - ref) / np.maximum(np.abs(ref), 1e-300)
             err = np.where(ref == 0, np.abs(g[k]), err)
             rep["rel_" + k] = float(err.max())
-            assert rep["rel_" + k] <= tol_m, (k, rep)
-        assert np.allclose(g["Dapp"], o["D"], rtol=tol_m, atol=0)
-        assert np.allclose(g["Kapp"], o["K"], rtol=0, atol=2e-4 + tol_m * np.abs(o["K"]).max())
+            # a walker that parted company moves sum X^2 (X^4) by a few mean squares (fourth powers) of one walker
+            assert rep["rel_" + k] <= tol_m + {"m2": 8.0, "m4": 32.0, "snap_alpha": 0.0}[k] * slack, (k, rep)
+        assert np.allclose(g["Dapp"], o["D"], rtol=tol_m + 8.0 * slack, atol=0)
+        assert np.allclose(g["Kapp"], o["K"], rtol=0, atol=2e-4 + tol_m * np.abs(o["K"]).max() + 64.0 * slack)
         flow_diff = np.abs(g["class_flow"].astype(np.int64) - o["class_flow"].astype(np.int64)).sum()
         rep["class_flow_diff"] = int(flow_diff)
         assert flow_diff <= 2 * (1 - same_voxel) * n_walkers * max(1, o["class_flow"].shape[0])

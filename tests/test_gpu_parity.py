@@ -191,6 +191,33 @@ def test_error_codes(rms):
     assert e.value.code == -3
 
 
+def test_full_size_bench_workload_against_the_oracle(rms):
+    """The workload bench.py times, whole: cfg4 point on the full 500x500x2000 axon lattice, 1e6 walkers x 10,000
+    steps, 60 directions x 11 b-values, in bench.py's launch configuration (device-resident labels, specialised
+    kernel, spatial ordering), against the oracle run on every one of those walkers (about a minute of host time).
+    Plain north_star tolerances: >= 99.9 % same final voxel, |dS| <= 1e-4 for all 660 (b, direction), moments 1e-4."""
+    import torch
+    cfg = ri.make_config("cfg4", "full")
+    n = cfg.n_walkers
+    labels_dev = torch.from_numpy(cfg.substrate.labels.view(np.int16)).cuda()
+    g = rms.simulate(cfg.substrate, cfg.sequence, n, cfg.seed, device_labels=labels_dev, read_walkers=True)
+    o = oracle_run(cfg.substrate, cfg.sequence, n, cfg.seed)
+    rep = compare(g, o, n, strict_s=True)
+    print("full-size cfg4", rep)
+    assert g["n_launches"] >= 5 and g["kernel_ms"] > 0
+
+
+def test_general_kernel_and_id_order_agree_with_the_specialised_path(rms):
+    # same inputs through the general step kernel and without spatial ordering: identical physics, so the results
+    # agree with the oracle under the same tolerances, and with each other to rounding
+    cfg = ri.make_config("cfg2", "test")
+    n = cfg.n_walkers
+    o = oracle_run(cfg.substrate, cfg.sequence, n, cfg.seed)
+    for flags in (2, 4, 6):      # RMS_RUN_GENERAL_KERNEL, RMS_RUN_NO_ORDERING, both
+        g = gpu_run(cfg.substrate, cfg.sequence, n, cfg.seed, flags=flags)
+        print("flags", flags, compare(g, o, n))
+
+
 def test_tables_match_oracle(rms):
     import oracle
     D = np.array([2.0, 1.0, 0.5], np.float32)
