@@ -59,4 +59,5 @@ def build(force: bool = False, extra_flags=(), verbose: bool = False) -> Path:
 
 if __name__ == "__main__":
     flags = ["-DRMS_FAST_TRIG"] if "--fast-trig" in sys.argv else []
+    flags += [a for a in sys.argv[1:] if a.startswith("-D")]
     print(build(force="--force" in sys.argv, extra_flags=flags, verbose="-v" in sys.argv))

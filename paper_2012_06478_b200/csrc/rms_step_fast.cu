@@ -19,6 +19,9 @@
 #include "rms_internal.cuh"
 
 #define RMS_FBLOCK 128
+#ifndef RMS_FMINB
+#define RMS_FMINB 8                  // resident blocks per SM the register allocation is held to
+#endif
 #define RMS_FFLUSH 1024u             // steps between flushes of the fp32 / int32 phase partial sums into fp64 (even)
 #define RMS_ONE_MINUS 0.99999994f    // 1 - 2^-24
 
@@ -35,13 +38,15 @@ __device__ __forceinline__ float rms_sqrt_fast(float x)
 __device__ __forceinline__ int rms_max3(int a, int b, int c) { return max(max(a, b), c); }
 __device__ __forceinline__ int rms_min3(int a, int b, int c) { return min(min(a, b), c); }
 
-// float bits with the two low mantissa bits replaced by a tag (one LOP3)
-__device__ __forceinline__ int rms_tag(float v, int tag)
+// (a & b) | c in one LOP3
+__device__ __forceinline__ int rms_and_or(int a, int b, int c)
 {
     int r;
-    asm("lop3.b32 %0, %1, %2, %3, 0xEA;" : "=r"(r) : "r"(__float_as_int(v)), "r"(~3), "r"(tag));   // (a & b) | c
+    asm("lop3.b32 %0, %1, %2, %3, 0xEA;" : "=r"(r) : "r"(a), "r"(b), "r"(c));
     return r;
 }
+// float bits with the two low mantissa bits replaced by a tag
+__device__ __forceinline__ int rms_tag(float v, int tag) { return rms_and_or(__float_as_int(v), ~3, tag); }
 
 // byte `sel` (0..3) of x, zero extended (selector nibbles 1..3 = 0 pick byte 0 of x, which callers keep 0)
 __device__ __forceinline__ uint32_t rms_prmt(uint32_t x, uint32_t y, uint32_t sel)
@@ -65,7 +70,7 @@ __device__ __noinline__ uint2 rms_fold_ghost(int lin, uint32_t wraps, int nx, in
 }  // namespace
 
 template <int NW>
-__global__ void __launch_bounds__(RMS_FBLOCK) rms_step_fast_kernel(const __grid_constant__ rms_step_params p)
+__global__ void __launch_bounds__(RMS_FBLOCK, RMS_FMINB) rms_step_fast_kernel(const __grid_constant__ rms_step_params p)
 {
     __shared__ float2 sm_trig[256];   // (cos, sin) of the centre of the 256 azimuth bins
 
@@ -136,7 +141,7 @@ __global__ void __launch_bounds__(RMS_FBLOCK) rms_step_fast_kernel(const __grid_
         const float z = fmaf(__uint_as_float(__funnelshift_r(wa, 0x7Fu, 9)) - 1.5f, 2.0f, 1.1920928955078125e-07f);
         // azimuth pi * sym(wb) = bin centre (top 8 bits) + residual (next 15 bits, exact): rotate the table entry
         const float2 cs0 = sm_trig[wb >> 24];
-        const float tau = __uint_as_float(((wb >> 1) & 0x007FFF00u) | 0x3F800080u) - 1.5f;   // in (-1/2, 1/2), exact
+        const float tau = __int_as_float(rms_and_or((int)(wb >> 1), 0x007FFF00, 0x3F800080)) - 1.5f;   // in (-1/2, 1/2), exact
         const float x2 = tau * tau;
         const float sb = tau * fmaf(x2, -2.4641574e-06f, 0.024543693f);    // sin(tau pi/128)
         const float e = x2 * -3.0119642e-04f;                               // cos(tau pi/128) - 1
@@ -166,50 +171,55 @@ __global__ void __launch_bounds__(RMS_FBLOCK) rms_step_fast_kernel(const __grid_
             const int k_hi = rms_max3(kx, ky, kz), k_lo = rms_min3(kx, ky, kz);
             const int k_mid = kx ^ ky ^ kz ^ k_hi ^ k_lo;
             // per-axis increments of the position code: pass flag (bit 5 + axis) + signed step in the 3x3x3 index,
-            // one byte each, at byte 3 - axis (byte 0 = 0 serves the upper result bytes of the permute)
-            const int isx = (__float_as_int(rx) >> 31) | 1, isy = (__float_as_int(ry) >> 31) | 1, isz = (__float_as_int(rz) >> 31) | 1;
-            const uint32_t lut = 0x20408000u + ((uint32_t)isx << 24) + ((uint32_t)(3 * isy) << 16) + ((uint32_t)(9 * isz) << 8);
+            // one byte each at byte 3 - axis (byte 0 = 0 serves the upper result bytes of the permute):
+            // x: 32 +- 1, y: 64 +- 3, z: 128 +- 9, switched by the sign masks of the hop
+            const int mx = __float_as_int(rx) >> 31, my = __float_as_int(ry) >> 31, mz = __float_as_int(rz) >> 31;
+            // (integer multiply-adds: they run on the FMA pipe, the ALU pipe is the busy one)
+            const int isx = 2 * mx + 1, isy = 2 * my + 1, isz = 2 * mz + 1;
+            const uint32_t lut = 0x21438900u + (uint32_t)(mx * 0x02000000 + my * 0x00060000 + mz * 0x00001200);
             if (nb & RMS_NBR_GHOST) fold();
             uint32_t pos = RMS_NBR_SELF;
             auto slot = [&](const int key) {
                 const uint32_t q = pos + rms_prmt(lut, 0u, (uint32_t)key & 3u);
-                if (__funnelshift_r(nb, 0u, q) & 1u) pos = q;      // the voxel ahead carries my label: pass
-                else ++n_enc;                                      // membrane: elastic collision
+                // the voxel ahead carries my label: pass; else a membrane: count the collision in bits 8..9
+                pos = (nb & __funnelshift_l(0u, 1u, q)) ? q : pos + 0x100u;
             };
             slot(k_hi);
             if (k_mid >= 0) {
                 slot(k_mid);
                 if (k_lo >= 0) slot(k_lo);
             }
-            // outcome per axis: passed -> g - sigma (enters the neighbour), else mirrored on the face plane, 2 h - g
+            // outcome per axis: passed -> g - sigma (enters the neighbour); membrane -> elastic collision,
+            // mirrored on the face plane: 2 h - g
             {
-                const bool ps = (pos & 32u) != 0;
+                const bool ps = (pos & 32u) != 0, rf = cx && !ps;
                 if (ps) {
                     gx -= sgx; lin += isx;
 #pragma unroll
                     for (int m = 0; m < NW; ++m) A32[m][0] += isx * wrem[m];
                 }
-                if (cx && !ps) gx = h2x - gx;
+                if (rf) gx = h2x - gx;
             }
             {
-                const bool ps = (pos & 64u) != 0;
+                const bool ps = (pos & 64u) != 0, rf = cy && !ps;
                 if (ps) {
                     gy -= sgy; lin += isy * NX;
 #pragma unroll
                     for (int m = 0; m < NW; ++m) A32[m][1] += isy * wrem[m];
                 }
-                if (cy && !ps) gy = h2y - gy;
+                if (rf) gy = h2y - gy;
             }
             {
-                const bool ps = (pos & 128u) != 0;
+                const bool ps = (pos & 128u) != 0, rf = cz && !ps;
                 if (ps) {
                     gz -= sgz; lin += isz * NXY;
 #pragma unroll
                     for (int m = 0; m < NW; ++m) A32[m][2] += isz * wrem[m];
                 }
-                if (cz && !ps) gz = h2z - gz;
+                if (rf) gz = h2z - gz;
             }
-            if (pos != RMS_NBR_SELF) nb = __ldg(p.nbr + lin);
+            n_enc += pos >> 8;
+            if (pos & 0xE0u) nb = __ldg(p.nbr + lin);
         }
         fx = gx; fy = gy; fz = gz;
         // phase, fractional part: Phi_F += w f (the integer part is event driven, above)
