@@ -7,7 +7,7 @@
 Workload (config.workload): the cfg4 throughput point of BASELINE.json on the synthetic mouse-like axon
 substrate of cfg2 -- 500x500x2000 uint16 lattice, ~300 axons, 1e6 intra-axonal walkers x 10,000 Monte Carlo
 steps, PGSE with 60 directions x 11 b-values, impermeable membranes, D = 2 um^2/ms, dt = 2e-4 ms.
-One bench "step" is one pass of the whole path: rms_substrate_create (face-mask lattice built from labels
+One bench "step" is one pass of the whole path: rms_substrate_create (neighbourhood lattice built from labels
 resident in HBM) -> rms_walkers_init -> rms_run (walk, phase/T2 accumulation, moment and signal reductions,
 normalisation).  `value` = walker-steps/s with the labels already in HBM; `e2e` = the same through the C ABI
 from pinned HOST labels (host->device copy and result read-back inside the timed region).
@@ -36,7 +36,7 @@ sys.path.insert(0, str(ROOT))
 ALGORITHMIC_INSTR_PER_STEP = 80.0
 N_SM, LANES_PER_SM = 148, 128          # B200: 4 schedulers x 32 lanes per SM, one warp instruction per clock each
 # DRAM traffic of the step kernel per launch from the committed ncu capture (profiles/), or None.
-NCU_TRAFFIC_BYTES_PER_LAUNCH = None
+NCU_TRAFFIC_BYTES_PER_LAUNCH = 48.19e9   # profiles/r1b_step_fast_ncu.md: 46.96 GB read + 1.23 GB written
 
 
 def parse_args():
