@@ -24,24 +24,42 @@ __global__ void __launch_bounds__(256) rms_cell_hist_kernel(rms_walker_arrays st
     if (i < n) atomicAdd(&count[rms_cell_of(st.w[0][i], st.w[1][i], st.w[2][i], cx, cy)], 1u);
 }
 
-// exclusive prefix sum over n_cells counters, in place, one block
-__global__ void __launch_bounds__(1024) rms_cell_scan_kernel(uint32_t* count, uint32_t n_cells)
+// exclusive prefix sum over the counters, in place, one block: tiles of 4096 counters (one uint4 per thread, coalesced;
+// the array is padded to a multiple of 4096), scan inside the thread, warp-shuffle scan over the lanes, a second one
+// over the 32 warp totals, running carry between tiles
+__global__ void __launch_bounds__(1024) rms_cell_scan_kernel(uint4* count4, uint32_t n_tiles)
 {
-    __shared__ uint32_t part[1024];
-    const uint32_t per = (n_cells + 1023u) / 1024u;
-    const uint32_t a = min(n_cells, threadIdx.x * per), b = min(n_cells, a + per);
-    uint32_t sum = 0;
-    for (uint32_t c = a; c < b; ++c) sum += count[c];
-    part[threadIdx.x] = sum;
-    __syncthreads();
-    for (uint32_t o = 1; o < 1024u; o <<= 1) {   // Hillis-Steele inclusive scan of the per-thread sums
-        const uint32_t v = threadIdx.x >= o ? part[threadIdx.x - o] : 0u;
+    __shared__ uint32_t wsum[32];
+    const uint32_t lane = threadIdx.x & 31u, warp = threadIdx.x >> 5;
+    uint32_t carry = 0;
+    uint4 v = count4[threadIdx.x];
+    for (uint32_t tile = 0; tile < n_tiles; ++tile) {
+        const uint4 cur = v;
+        if (tile + 1 < n_tiles) v = count4[(size_t)(tile + 1) * 1024u + threadIdx.x];   // prefetch the next tile
+        const uint32_t s1 = cur.x, s2 = s1 + cur.y, s3 = s2 + cur.z, s4 = s3 + cur.w;
+        uint32_t x = s4;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const uint32_t y = __shfl_up_sync(0xffffffffu, x, o);
+            if (lane >= (uint32_t)o) x += y;
+        }
+        if (lane == 31u) wsum[warp] = x;
         __syncthreads();
-        part[threadIdx.x] += v;
+        if (warp == 0) {
+            uint32_t t = wsum[lane];
+#pragma unroll
+            for (int o = 1; o < 32; o <<= 1) {
+                const uint32_t y = __shfl_up_sync(0xffffffffu, t, o);
+                if (lane >= (uint32_t)o) t += y;
+            }
+            wsum[lane] = t;
+        }
+        __syncthreads();
+        const uint32_t base = carry + (warp ? wsum[warp - 1] : 0u) + x - s4;
+        count4[(size_t)tile * 1024u + threadIdx.x] = make_uint4(base, base + s1, base + s2, base + s3);
+        carry += wsum[31];
         __syncthreads();
     }
-    uint32_t run = part[threadIdx.x] - sum;
-    for (uint32_t c = a; c < b; ++c) { const uint32_t v = count[c]; count[c] = run; run += v; }
 }
 
 __global__ void __launch_bounds__(256) rms_cell_scatter_kernel(rms_walker_arrays st, uint64_t n, int cx, int cy, uint32_t* cursor,
@@ -60,12 +78,13 @@ int rms_order_walkers(const rms_substrate* s, const rms_walkers* w, uint32_t* d_
     const uint64_t n_cells = (uint64_t)cx * cy * cz;
     RMS_REQUIRE(n_cells < (1ull << 31) && w->n < (1ull << 32), RMS_ERR_UNSUPPORTED, "too many cells or walkers to order");
     uint32_t* d_count = nullptr;
-    RMS_CUDA_TRY(rms_malloc((void**)&d_count, n_cells * sizeof(uint32_t)));
-    cudaError_t e = cudaMemsetAsync(d_count, 0, n_cells * sizeof(uint32_t), stream);
+    const uint64_t n_tiles = (n_cells + 4095) / 4096;
+    RMS_CUDA_TRY(rms_malloc((void**)&d_count, n_tiles * 4096 * sizeof(uint32_t)));
+    cudaError_t e = cudaMemsetAsync(d_count, 0, n_tiles * 4096 * sizeof(uint32_t), stream);
     if (e == cudaSuccess) {
         const unsigned grid = (unsigned)((w->n + 255) / 256);
         rms_cell_hist_kernel<<<grid, 256, 0, stream>>>(w->a, w->n, cx, cy, d_count);
-        rms_cell_scan_kernel<<<1, 1024, 0, stream>>>(d_count, (uint32_t)n_cells);
+        rms_cell_scan_kernel<<<1, 1024, 0, stream>>>((uint4*)d_count, (uint32_t)n_tiles);
         rms_cell_scatter_kernel<<<grid, 256, 0, stream>>>(w->a, w->n, cx, cy, d_count, d_order);
         e = cudaGetLastError();
         if (n_launches) *n_launches += 3;

@@ -33,38 +33,67 @@ extern "C" const char* rms_version(void) { return "rms-b200 0.1 (sm_100a)"; }
 // ------------------------------------------------------------------------------------------------
 __device__ __forceinline__ int rms_wrap1(int a, int n) { return a < 0 ? a + n : (a >= n ? a - n : a); }
 
+// One thread owns a column of RMS_NBR_ZCHUNK padded voxels along z at fixed (X, Y): it keeps the 3 x 3 labels of the
+// planes z-1, z, z+1 in registers and reads 9 new labels per voxel instead of 27 (consecutive threads = consecutive
+// x: coalesced rows, the +-1 neighbours come out of L1).
+#define RMS_NBR_ZCHUNK 128
+
 __global__ void __launch_bounds__(128) rms_build_nbr_kernel(const uint16_t* __restrict__ labels, int nx, int ny, int nz,
                                                              uint32_t* __restrict__ nbr, int n_labels,
                                                              unsigned long long* __restrict__ stats)
 {
-    const int NX = nx + 2, NY = ny + 2;
+    const int NX = nx + 2, NY = ny + 2, NZ = nz + 2;
     const int X = blockIdx.x * blockDim.x + threadIdx.x;
-    const int Y = blockIdx.y, Z = blockIdx.z;
+    const int Y = blockIdx.y;
+    const int Z0 = blockIdx.z * RMS_NBR_ZCHUNK, Z1 = min(NZ, Z0 + RMS_NBR_ZCHUNK);
     unsigned n_faces = 0, bad = 0;
     if (X < NX) {
         // periodic image of the padded coordinate (|X-1| <= n, so one wrap is enough even for n = 1)
-        const int x = rms_wrap1(X - 1, nx), y = rms_wrap1(Y - 1, ny), z = rms_wrap1(Z - 1, nz);
-        const int xs[3] = {rms_wrap1(x - 1, nx), x, rms_wrap1(x + 1, nx)};
-        const int ys[3] = {rms_wrap1(y - 1, ny), y, rms_wrap1(y + 1, ny)};
-        const int zs[3] = {rms_wrap1(z - 1, nz), z, rms_wrap1(z + 1, nz)};
-        const uint16_t L = __ldg(labels + ((size_t)z * ny + y) * nx + x);
-        uint32_t m = 0;
+        const int x = rms_wrap1(X - 1, nx), y = rms_wrap1(Y - 1, ny);
+        uint32_t off[9];                              // offsets of the 3 x 3 (dx, dy) neighbours inside a z-plane
 #pragma unroll
-        for (int c = 0; c < 3; ++c)
+        for (int b = 0; b < 3; ++b)
 #pragma unroll
-            for (int b = 0; b < 3; ++b) {
-                const uint16_t* row = labels + ((size_t)zs[c] * ny + ys[b]) * nx;
+            for (int a = 0; a < 3; ++a) off[a + 3 * b] = (uint32_t)(rms_wrap1(y + b - 1, ny) * nx + rms_wrap1(x + a - 1, nx));
+        const uint32_t plane = (uint32_t)nx * (uint32_t)ny;   // voxel indices fit 31 bits (checked by the caller)
+        const bool ghost_xy = (X == 0) | (X == NX - 1) | (Y == 0) | (Y == NY - 1);
+        uint32_t pa[9], pb[9], pc[9];                  // labels of the planes z-1, z, z+1 (rotating roles)
+        int z = rms_wrap1(Z0 - 1, nz);                // box z of the padded plane Z0
+        {
+            const uint32_t bl = (uint32_t)rms_wrap1(z - 1, nz) * plane, bm = (uint32_t)z * plane;
 #pragma unroll
-                for (int a = 0; a < 3; ++a) m |= (uint32_t)(__ldg(row + xs[a]) == L) << (a + 3 * b + 9 * c);
-            }
-        const bool ghost = (X == 0) | (X == NX - 1) | (Y == 0) | (Y == NY - 1) | (Z == 0) | (Z == nz + 1);
-        if (ghost) m |= RMS_NBR_GHOST;
-        nbr[((size_t)Z * NY + Y) * NX + X] = m;
-        if (!ghost) {
-            // each face counted once, from its lower side: the +x, +y, +z neighbours (bits 14, 16, 22)
-            n_faces = 3 - (((m >> 14) & 1u) + ((m >> 16) & 1u) + ((m >> 22) & 1u));
-            bad = (L >= n_labels);
+            for (int k = 0; k < 9; ++k) { pa[k] = __ldg(labels + (bl + off[k])); pb[k] = __ldg(labels + (bm + off[k])); }
         }
+        uint32_t* out = nbr + ((size_t)Z0 * NY + Y) * NX + X;
+        const size_t out_stride = (size_t)NY * NX;
+        int Z = Z0;
+        // one voxel: read plane z+1 into HI, compare the 27 labels with the centre of MID, write the word
+#define RMS_NBR_ONE(LO, MID, HI)                                                                              \
+        if (Z < Z1) {                                                                                         \
+            z = (z + 1 == nz) ? 0 : z + 1;                                                                    \
+            const uint32_t bh = (uint32_t)z * plane;                                                          \
+            _Pragma("unroll") for (int k = 0; k < 9; ++k) HI[k] = __ldg(labels + (bh + off[k]));             \
+            const uint32_t L = MID[4];                                                                        \
+            uint32_t m = 0;                                                                                   \
+            _Pragma("unroll") for (int k = 0; k < 9; ++k)                                                    \
+                m += ((LO[k] == L) ? (1u << k) : 0u) + ((MID[k] == L) ? (1u << (k + 9)) : 0u) +                \
+                     ((HI[k] == L) ? (1u << (k + 18)) : 0u);                                                  \
+            const bool ghost = ghost_xy | (Z == 0) | (Z == NZ - 1);                                           \
+            if (ghost) m |= RMS_NBR_GHOST;                                                                    \
+            *out = m;                                                                                         \
+            out += out_stride;                                                                                \
+            if (!ghost) {                                                                                     \
+                n_faces += 3 - (((m >> 14) & 1u) + ((m >> 16) & 1u) + ((m >> 22) & 1u));                      \
+                bad += (L >= (uint32_t)n_labels);                                                             \
+            }                                                                                                 \
+            ++Z;                                                                                              \
+        }
+        while (Z < Z1) {
+            RMS_NBR_ONE(pa, pb, pc)
+            RMS_NBR_ONE(pb, pc, pa)
+            RMS_NBR_ONE(pc, pa, pb)
+        }
+#undef RMS_NBR_ONE
     }
     // warp-shuffle reduction, then one atomic per warp
     for (int o = 16; o > 0; o >>= 1) {
@@ -171,7 +200,7 @@ extern "C" int rms_substrate_create(const rms_substrate_desc* d, void* cuda_stre
     if (!(d->flags & RMS_NO_BRICKS)) {
         s->NX = s->nx + 2; s->NY = s->ny + 2; s->NZ = s->nz + 2;
         SUB_TRY(rms_malloc((void**)&s->d_nbr, (size_t)s->NX * s->NY * s->NZ * sizeof(uint32_t)));
-        dim3 grid((s->NX + 127) / 128, s->NY, s->NZ);
+        dim3 grid((s->NX + 127) / 128, s->NY, (s->NZ + RMS_NBR_ZCHUNK - 1) / RMS_NBR_ZCHUNK);
         if (grid.y > 65535u || grid.z > 65535u) {
             rms_set_error("lattice too large for the neighbourhood-lattice build (ny+2, nz+2 must be <= 65535)");
             rc = RMS_ERR_UNSUPPORTED;
