@@ -53,6 +53,10 @@ def parse_args():
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--cpu-sample-walkers", type=int, default=40_000)
+    ap.add_argument("--sweep", action="store_true",
+                    help="BASELINE.json configs[4]: walkers 1e5..1e8 x {1, 60} directions x {neighbourhood lattice, label "
+                         "gather}, one JSON line per point (not part of the driver contract)")
+    ap.add_argument("--sweep-max-walkers", type=int, default=100_000_000)
     return ap.parse_args()
 
 
@@ -202,10 +206,56 @@ def run_reference(args):
     print(json.dumps(line))
 
 
+def run_sweep(args):
+    """Throughput sweep of BASELINE.json configs[4] on one GPU: device-timed passes of the whole path."""
+    import torch
+    import paper_2012_06478_b200 as rms
+    import rms_inputs as ri
+    torch.cuda.set_device(0)
+    rms.load_library()
+    base = ri.make_config("cfg4", args.scale, n_walkers=1000, n_steps=args.mc_steps, n_dir=60)
+    sub = base.substrate
+    labels_dev = torch.from_numpy(sub.labels.view(np.int16)).cuda()
+    stream = torch.cuda.current_stream()
+    for n_dir in (1, 60):
+        dirs = ri.fibonacci_dirs(n_dir) if n_dir > 1 else np.array([[0.0, 0.0, 1.0]])
+        b = np.linspace(0.0, 25.0, 11) if n_dir > 1 else np.array([1.0])
+        dt = base.sequence.dt_ms
+        seq = ri.pgse_sequence(dt, args.mc_steps, 0.4 * args.mc_steps * dt, 0.6 * args.mc_steps * dt, b, dirs,
+                               snap_steps=[args.mc_steps])
+        for lattice, flags in (("facemask", 0), ("labels", rms.RMS_RUN_LABEL_GATHER)):
+            for n_w in (100_000, 1_000_000, 10_000_000, 100_000_000):
+                if n_w > args.sweep_max_walkers:
+                    continue
+                reps = 3 if n_w <= 1_000_000 else 1
+                rms.simulate(sub, seq, min(n_w, 1_000_000), base.seed, flags=flags, device_labels=labels_dev)   # warm-up
+                e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                torch.cuda.synchronize()
+                e0.record(stream)
+                k_ms = 0.0
+                for _ in range(reps):
+                    r = rms.simulate(sub, seq, n_w, base.seed, flags=flags, device_labels=labels_dev)
+                    k_ms += r["kernel_ms"]
+                e1.record(stream)
+                torch.cuda.synchronize()
+                ms = e0.elapsed_time(e1) / reps
+                steps = float(n_w) * args.mc_steps
+                print(json.dumps({"sweep": "cfg4", "walkers": n_w, "mc_steps": args.mc_steps, "directions": n_dir,
+                                  "b_values": int(seq.gamp.shape[1]), "lattice_path": lattice, "pass_ms": ms,
+                                  "step_kernel_ms": k_ms / reps, "walker_steps_per_s": steps / (ms * 1e-3),
+                                  "step_kernel_walker_steps_per_s": steps / (k_ms / reps * 1e-3),
+                                  "issue_roofline_frac": ALGORITHMIC_INSTR_PER_STEP * steps / (k_ms / reps * 1e-3) /
+                                  (N_SM * LANES_PER_SM * 1.965e9)}), flush=True)
+                rms.load_library().rms_memory_trim()
+
+
 def main():
     args = parse_args()
     if args.impl == "reference":
         run_reference(args)
+        return
+    if args.sweep:
+        run_sweep(args)
         return
     import torch
     import torch.distributed as dist

@@ -127,6 +127,35 @@ def test_general_waveform_table_mode_and_two_waves(rms):
     print("two waves", compare(g, o, n))
 
 
+def test_four_integer_waveforms_odd_boundaries_and_chunks(rms):
+    # specialised kernel at its widest: 4 piecewise-constant waveforms with amplitudes other than +-1, lobes that start
+    # and end on odd steps (the second half of a Philox call opens a segment), snapshots on odd steps (launch boundaries
+    # inside a Philox pair) and the run continued by a second call from an odd step count
+    sub = ri.single_cylinder(20, 6.5, 0.1)
+    n1, n2 = 333, 268
+    nT = n1 + n2
+    wave = np.zeros((4, nT), np.float32)
+    wave[0] = ri.pgse_wave(nT, 151, 301)
+    wave[1, 3:120] = 2.0; wave[1, 333:450] = -2.0
+    wave[2, 0:77] = -3.0; wave[2, 77:154] = 3.0; wave[2, 401:478] = 1.0; wave[2, 478:555] = -1.0
+    wave[3, 5:6] = 7.0; wave[3, 599:600] = -7.0
+    gamp = np.array([[0.0, 60.0], [5.0, 45.0], [0.0, 30.0], [10.0, 400.0]])
+    dirs = ri.fibonacci_dirs(7)
+    n = 8000
+    full = ri.Sequence(dt_ms=2e-4, n_steps=nT, wave=wave, gamp=gamp, dirs=dirs, snap_steps=np.array([1, 77, 333, 600, 601]))
+    o = oracle_run(sub, full, n, 21)
+    g = gpu_run(sub, full, n, 21)
+    print("four waves", compare(g, o, n))
+    # same run in two calls: 333 steps, then 268 more (phases keep accumulating, R11: the waveform is per call)
+    keep = {}
+    s1 = ri.Sequence(dt_ms=2e-4, n_steps=n1, wave=wave[:, :n1].copy(), gamp=gamp, dirs=dirs, snap_steps=np.array([n1]))
+    s2 = ri.Sequence(dt_ms=2e-4, n_steps=n2, wave=wave[:, n1:].copy(), gamp=gamp, dirs=dirs, snap_steps=np.array([n2]))
+    rms.simulate(sub, s1, n, 21, keep=keep)
+    r2 = rms.binding.rms_run(keep["substrate"], keep["walkers"], s2.dt_ms, s2.n_steps, s2.wave, s2.gamp, s2.dirs, s2.snap_steps)
+    assert np.abs(r2["S"] - g["S"]).max() < 1e-9           # identical trajectories and phases, only the summation order differs
+    keep["walkers"].destroy(); keep["substrate"].destroy()
+
+
 @pytest.mark.parametrize("dims", [(5, 7, 3), (1, 1, 9), (2, 3, 4)])
 @pytest.mark.parametrize("flags", [0, LABEL_GATHER], ids=["facemask", "labels"])
 def test_ragged_tiny_lattices_with_heavy_wrapping(rms, dims, flags):
