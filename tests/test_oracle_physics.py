@@ -291,3 +291,37 @@ def test_imaginary_part_has_the_sign_of_exp_minus_i_phi():
     assert S.imag < -0.05
     # the phase the oracle accumulated is q X (one-hot wave), in the oracle's units gamp*dt*l_p*Phi
     assert np.allclose(q / DT * DT * LP * r["phi"][:, 0, 0], q * X, atol=1e-12)
+
+
+# ------------------------------------------------------------------ short-time Mitra S/V law in a cylinder (pin K9)
+def test_short_time_mitra_law_in_a_voxelised_cylinder():
+    """D_xx(t) = D0 [1 - 4/(3 sqrt(pi)) (S_x/V) sqrt(D0 t)] (Mitra et al. 1992), S_x/V = (1/V) oint (n.x)^2 dS.
+
+    The lattice cylinder has a staircase surface, so the law is taken where it is exact for it: diffusion length
+    sqrt(D0 t) = 0.32 voxel, every wall face flat on that scale, and S_x/V counted from the lattice itself (faces with
+    normal +-x between label 1 and label 0, per voxel of label 1).  The hop is 0.05 voxel, 240 hops; the fixed-step walk
+    carries an O(ds / sqrt(D0 t)) ~ 1/sqrt(N) correction to the coefficient and the stair corners an O(D0 t / l_p^2) one,
+    both allowed for (20 % of the deficit) on top of 3 standard errors.  Along the axis the walk is free: no deficit.
+    A walk that stuck to, absorbed at, or ignored the membrane would miss by far more."""
+    r_vox, n = 12.0, 28
+    sub = ri.single_cylinder(n, r_vox, LP, nz=2, D_intra=2.0, D_extra=2.0)
+    lab = sub.labels[0]
+    n_in = int((lab == 1).sum())
+    faces_x = int(np.count_nonzero(lab != np.roll(lab, 1, axis=1)))        # membrane faces with normal +-x in one z-slice
+    SxV = faces_x / (n_in * LP)                                             # 1/um
+    assert abs(SxV - 4 / (math.pi * r_vox * LP)) < 0.05 * SxV               # staircase circle: 4/(pi r), not 1/r
+    D0, s = 2.0, 0.05
+    dt = (s * LP) ** 2 / (6 * D0)
+    n_steps, n_w = 240, 300_000
+    seq = ri.Sequence(dt_ms=dt, n_steps=n_steps, wave=ri.one_hot_wave(n_steps, n_steps)[None], gamp=np.array([[0.0]]),
+                      dirs=np.eye(3), snap_steps=np.array([n_steps], np.int64))
+    r = oracle.run(sub, seq, n_w, seed=31, n_threads=THREADS)
+    t = n_steps * dt
+    deficit = 4 / (3 * math.sqrt(math.pi)) * SxV * math.sqrt(D0 * t)
+    assert 0.02 < deficit < 0.03
+    se = math.sqrt(2.0 / n_w)                                               # relative standard error of <X^2>
+    Dx, Dy, Dz = r["D"][0] / D0
+    for Dk in (Dx, Dy):
+        assert abs((1 - Dk) - deficit) < 0.2 * deficit + 3 * se, (Dk, deficit)
+    assert abs(Dz - 1) < 3 * se, Dz                                         # free along the axis
+    assert r["n_encounters"] > 0 and r["n_permeations"] == 0
