@@ -81,6 +81,13 @@ __global__ void __launch_bounds__(RMS_FBLOCK, RMS_FMINB) rms_step_fast_kernel(co
     }
     __syncthreads();
 
+    // 32-bit shared-window address of the table, held in a register so that the hot loop does not rebuild the
+    // window base every step
+    // (the "memory" clobber also tells the compiler that the table above is read later: its only readers are the
+    // ld.shared of the hot loop, written in PTX)
+    int trig_base;
+    asm volatile("mov.b32 %0, %1;" : "=r"(trig_base) : "r"((int)__cvta_generic_to_shared(sm_trig)) : "memory");
+
     const uint64_t t_global = (uint64_t)blockIdx.x * RMS_FBLOCK + threadIdx.x;
     if (t_global >= p.n) return;
     const uint64_t i = p.order ? (uint64_t)p.order[t_global] : t_global;   // walker of this thread (rms_sched.cu)
@@ -140,7 +147,8 @@ __global__ void __launch_bounds__(RMS_FBLOCK, RMS_FMINB) rms_step_fast_kernel(co
         // z = sym(wa): exact odd multiple of 2^-23
         const float z = fmaf(__uint_as_float(__funnelshift_r(wa, 0x7Fu, 9)) - 1.5f, 2.0f, 1.1920928955078125e-07f);
         // azimuth pi * sym(wb) = bin centre (top 8 bits) + residual (next 15 bits, exact): rotate the table entry
-        const float2 cs0 = sm_trig[wb >> 24];
+        float2 cs0;                                              // sm_trig[wb >> 24]
+        asm("ld.shared.v2.f32 {%0, %1}, [%2];" : "=f"(cs0.x), "=f"(cs0.y) : "r"((int)(wb >> 24) * 8 + trig_base));
         const float tau = __int_as_float(rms_and_or((int)(wb >> 1), 0x007FFF00, 0x3F800080)) - 1.5f;   // in (-1/2, 1/2), exact
         const float x2 = tau * tau;
         const float sb = tau * fmaf(x2, -2.4641574e-06f, 0.024543693f);    // sin(tau pi/128)
@@ -177,7 +185,7 @@ __global__ void __launch_bounds__(RMS_FBLOCK, RMS_FMINB) rms_step_fast_kernel(co
             // (integer multiply-adds: they run on the FMA pipe, the ALU pipe is the busy one)
             const int isx = 2 * mx + 1, isy = 2 * my + 1, isz = 2 * mz + 1;
             const uint32_t lut = 0x21438900u + (uint32_t)(mx * 0x02000000 + my * 0x00060000 + mz * 0x00001200);
-            if (nb & RMS_NBR_GHOST) fold();
+            int dl = 0;                                             // lattice-index change of this hop
             uint32_t pos = RMS_NBR_SELF;
             auto slot = [&](const int key) {
                 const uint32_t q = pos + rms_prmt(lut, 0u, (uint32_t)key & 3u);
@@ -194,7 +202,7 @@ __global__ void __launch_bounds__(RMS_FBLOCK, RMS_FMINB) rms_step_fast_kernel(co
             {
                 const bool ps = (pos & 32u) != 0, rf = cx && !ps;
                 if (ps) {
-                    gx -= sgx; lin += isx;
+                    gx -= sgx; dl = isx;
 #pragma unroll
                     for (int m = 0; m < NW; ++m) A32[m][0] += isx * wrem[m];
                 }
@@ -203,7 +211,7 @@ __global__ void __launch_bounds__(RMS_FBLOCK, RMS_FMINB) rms_step_fast_kernel(co
             {
                 const bool ps = (pos & 64u) != 0, rf = cy && !ps;
                 if (ps) {
-                    gy -= sgy; lin += isy * NX;
+                    gy -= sgy; dl += isy * NX;
 #pragma unroll
                     for (int m = 0; m < NW; ++m) A32[m][1] += isy * wrem[m];
                 }
@@ -212,14 +220,21 @@ __global__ void __launch_bounds__(RMS_FBLOCK, RMS_FMINB) rms_step_fast_kernel(co
             {
                 const bool ps = (pos & 128u) != 0, rf = cz && !ps;
                 if (ps) {
-                    gz -= sgz; lin += isz * NXY;
+                    gz -= sgz; dl += isz * NXY;
 #pragma unroll
                     for (int m = 0; m < NW; ++m) A32[m][2] += isz * wrem[m];
                 }
                 if (rf) gz = h2z - gz;
             }
             n_enc += pos >> 8;
-            if (pos & 0xE0u) nb = __ldg(p.nbr + lin);
+            if (pos & 0xE0u) {
+                // the walker changes voxel.  If it sat on a ghost voxel (it stepped over the box edge earlier; the word of a
+                // ghost voxel is its image's, so the tests above were right) fold it back into the box first.  The test
+                // sits here, after the slots, so that the gather issued a step ago is not waited for any earlier.
+                if (nb & RMS_NBR_GHOST) fold();
+                lin += dl;
+                nb = __ldg(p.nbr + lin);
+            }
         }
         fx = gx; fy = gy; fz = gz;
         // phase, fractional part: Phi_F += w f (the integer part is event driven, above)
