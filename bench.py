@@ -50,6 +50,7 @@ def parse_args():
     ap.add_argument("--dirs", type=int, default=60)
     ap.add_argument("--lattice", default="facemask", choices=["facemask", "labels"])
     ap.add_argument("--scale", default="full", choices=["full", "test"])
+    ap.add_argument("--layout", default="x", choices=["auto", "x", "z"], help="memory order of the neighbourhood lattice")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--cpu-sample-walkers", type=int, default=40_000)
@@ -169,7 +170,7 @@ def workload_config(args, cfg, extra=None):
          "intra_fraction": round(cfg.substrate.meta.get("intra_fraction", 0.0), 4),
          "walkers_per_gpu": args.walkers, "mc_steps": args.mc_steps, "dt_ms": cfg.sequence.dt_ms,
          "directions": int(cfg.sequence.dirs.shape[0]), "b_values": int(cfg.sequence.gamp.shape[1]),
-         "lattice_path": args.lattice, "pass": "rms_substrate_create + rms_walkers_init + rms_run",
+         "lattice_path": args.lattice, "layout": args.layout, "pass": "rms_substrate_create + rms_walkers_init + rms_run",
          "l2": "inputs larger than L2 (label lattice 1.0 GB + neighbourhood lattice 2.0 GB vs 126 MB L2)" if args.scale == "full"
          else "reduced test lattice (fits L2) -- not a valid bench configuration"}
     if extra:
@@ -276,6 +277,7 @@ def main():
     n_walkers, mc_steps = args.walkers, args.mc_steps
     first_id = rank * n_walkers                       # weak scaling: every rank owns its own walker-id range
     flags = rms.RMS_RUN_LABEL_GATHER if args.lattice == "labels" else 0
+    sflags = {"auto": rms.binding.RMS_LAYOUT_AUTO, "x": rms.binding.RMS_LAYOUT_X_FASTEST, "z": rms.binding.RMS_LAYOUT_Z_FASTEST}[args.layout]
     t_ms = np.asarray(seq.snap_steps, np.float64) * seq.dt_ms
 
     labels_dev = torch.from_numpy(sub.labels.view(np.int16)).cuda()          # resident in HBM before timing
@@ -287,9 +289,10 @@ def main():
 
     def one_pass(device):
         if device:   # labels already resident in HBM: adopted in place
-            r = rms.simulate(sub, seq, n_walkers, cfg.seed, first_id=first_id, flags=flags, device_labels=labels_dev)
+            r = rms.simulate(sub, seq, n_walkers, cfg.seed, first_id=first_id, flags=flags, substrate_flags=sflags,
+                             device_labels=labels_dev)
         else:        # host labels: rms_substrate_create copies them host -> device inside the call
-            r = rms.simulate(sub_pin, seq, n_walkers, cfg.seed, first_id=first_id, flags=flags)
+            r = rms.simulate(sub_pin, seq, n_walkers, cfg.seed, first_id=first_id, flags=flags, substrate_flags=sflags)
         if world > 1:
             r = rms.api.allreduce_result(r, t_ms)
         return r

@@ -54,7 +54,7 @@ typedef struct rms_walkers rms_walkers;     /* opaque */
  * kappa        [n_labels*n_labels] membrane permeability um/ms between label pairs, symmetric, diagonal
  *              ignored; 0 = impermeable; +inf = no membrane (Eq.C.15 with c1 = c2); NULL = all 0 (host; Eq.3)
  * label_class  [n_labels] output compartment class of each label, < n_classes; NULL = all 0 (host)
- * flags        RMS_LABELS_ON_DEVICE | RMS_ADOPT_DEVICE_PTR | RMS_NO_BRICKS
+ * flags        RMS_LABELS_ON_DEVICE | RMS_ADOPT_DEVICE_PTR | RMS_NO_BRICKS | RMS_LAYOUT_X_FASTEST | RMS_LAYOUT_Z_FASTEST | RMS_LAYOUT_AUTO
  *
  * Derived on the device, unless RMS_NO_BRICKS: the neighbourhood lattice, one 32-bit word per voxel (plus a
  * one-voxel periodic ghost shell) whose 27 bits say which voxels of the 3x3x3 block around it carry the
@@ -65,6 +65,9 @@ typedef struct rms_walkers rms_walkers;     /* opaque */
 #define RMS_LABELS_ON_DEVICE 1u
 #define RMS_ADOPT_DEVICE_PTR 2u
 #define RMS_NO_BRICKS 4u
+#define RMS_LAYOUT_X_FASTEST 8u   /* memory order of the neighbourhood lattice: x fastest (the default)                  */
+#define RMS_LAYOUT_Z_FASTEST 16u  /* z fastest: the 8 words of a 32-byte sector lie along z (cells elongated along z)    */
+#define RMS_LAYOUT_AUTO 24u       /* x or z, whichever axis has fewer membrane faces normal to it (sampled)              */
 
 typedef struct {
     int32_t nx, ny, nz;

@@ -19,6 +19,9 @@ RMS_MAX_WAVES = 4
 RMS_LABELS_ON_DEVICE = 1
 RMS_ADOPT_DEVICE_PTR = 2
 RMS_NO_BRICKS = 4
+RMS_LAYOUT_X_FASTEST = 8
+RMS_LAYOUT_Z_FASTEST = 16
+RMS_LAYOUT_AUTO = 24
 RMS_RUN_LABEL_GATHER = 1
 RMS_RUN_GENERAL_KERNEL = 2
 RMS_RUN_NO_ORDERING = 4

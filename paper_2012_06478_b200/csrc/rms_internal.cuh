@@ -54,6 +54,11 @@ struct rms_substrate {
     // label as this voxel (bit 13 = the voxel itself = 1); a face towards +-k is a membrane iff the
     // bit of the face neighbour is 0.  Bit 27 (RMS_NBR_GHOST) = ghost voxel.
     uint32_t* d_nbr = nullptr;
+    // memory order of the neighbourhood lattice: index = X SX + Y SY + Z SZ over the padded coordinates.  The axis with
+    // the fewest membrane faces normal to it (the direction the cells run along) is made the fastest one, so that
+    // the 8 words of a 32-byte sector belong to one compartment; x fastest (1, NX, NX NY) or z fastest (NY NZ, NZ, 1).
+    int SX = 0, SY = 0, SZ = 0;
+    uint64_t faces_axis[3] = {0, 0, 0};  // membrane faces with normal x, y, z
     int NX = 0, NY = 0, NZ = 0;          // padded dims (n + 2)
     uint64_t n_membrane_faces = 0;
     std::vector<float> D, T2, kappa;     // host copies of the per-label tables
@@ -109,6 +114,13 @@ static inline rms_philox_keys rms_make_keys(uint64_t seed)
 }
 
 #ifdef __CUDACC__
+// padded coordinates of an index of the neighbourhood lattice (x fastest: SX == 1, else z fastest)
+__device__ __forceinline__ void rms_lattice_coords(int lin, int SX, int SY, int SZ, int& X, int& Y, int& Z)
+{
+    if (SX == 1) { Z = lin / SZ; const int rem = lin - Z * SZ; Y = rem / SY; X = rem - Y * SY; }
+    else         { X = lin / SX; const int rem = lin - X * SX; Y = rem / SY; Z = rem - Y * SY; }
+}
+
 __device__ __forceinline__ void rms_philox(const rms_philox_keys& rk, uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3,
                                            uint32_t& o0, uint32_t& o1, uint32_t& o2, uint32_t& o3)
 {
@@ -155,6 +167,7 @@ struct rms_step_params {
     const uint16_t* labels;
     const uint32_t* nbr;
     int NX, NY;               // padded dims of the neighbourhood lattice
+    int SX, SY, SZ;           // its strides: index = X SX + Y SY + Z SZ; SX == 1 (x fastest) or SZ == 1 (z fastest)
     rms_walker_arrays st;
     uint64_t n, first_id;
     rms_philox_keys rk;

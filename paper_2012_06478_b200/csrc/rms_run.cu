@@ -226,7 +226,7 @@ extern "C" int rms_run(const rms_substrate* s, rms_walkers* w, const rms_run_des
     rms_step_params sp;
     memset(&sp, 0, sizeof sp);
     sp.nx = s->nx; sp.ny = s->ny; sp.nz = s->nz;
-    sp.labels = s->d_labels; sp.nbr = s->d_nbr; sp.NX = s->NX; sp.NY = s->NY;
+    sp.labels = s->d_labels; sp.nbr = s->d_nbr; sp.NX = s->NX; sp.NY = s->NY; sp.SX = s->SX; sp.SY = s->SY; sp.SZ = s->SZ;
     sp.st = w->a; sp.n = n; sp.first_id = w->first_id; sp.rk = rms_make_keys(w->seed);
     sp.s_tab = b_tabs.as<float>(); sp.rate = sp.s_tab + nL; sp.P512 = sp.rate + nL; sp.n_labels = nL;
     sp.counters = w->d_counters; sp.n_wave = nW; sp.wave_stride = nT; sp.wsuf_stride = nT + 1;

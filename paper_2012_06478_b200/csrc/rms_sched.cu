@@ -13,15 +13,18 @@
 
 namespace {
 
-__device__ __forceinline__ uint32_t rms_cell_of(int x, int y, int z, int cx, int cy)
+// cells are numbered in the memory order of the neighbourhood lattice: its fastest axis (x or z) runs fastest
+__device__ __forceinline__ uint32_t rms_cell_of(int x, int y, int z, int cx, int cy, int cz, bool zfast)
 {
-    return ((uint32_t)(z / RMS_CELL_Z) * cy + (uint32_t)(y / RMS_CELL_XY)) * cx + (uint32_t)(x / RMS_CELL_XY);
+    const uint32_t a = (uint32_t)(x / RMS_CELL_XY), b = (uint32_t)(y / RMS_CELL_XY), c = (uint32_t)(z / RMS_CELL_Z);
+    return zfast ? (a * cy + b) * cz + c : (c * cy + b) * cx + a;
 }
 
-__global__ void __launch_bounds__(256) rms_cell_hist_kernel(rms_walker_arrays st, uint64_t n, int cx, int cy, uint32_t* count)
+__global__ void __launch_bounds__(256) rms_cell_hist_kernel(rms_walker_arrays st, uint64_t n, int cx, int cy, int cz, bool zfast,
+                                                             uint32_t* count)
 {
     const uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (i < n) atomicAdd(&count[rms_cell_of(st.w[0][i], st.w[1][i], st.w[2][i], cx, cy)], 1u);
+    if (i < n) atomicAdd(&count[rms_cell_of(st.w[0][i], st.w[1][i], st.w[2][i], cx, cy, cz, zfast)], 1u);
 }
 
 // exclusive prefix sum over the counters, in place, one block: tiles of 4096 counters (one uint4 per thread, coalesced;
@@ -62,11 +65,11 @@ __global__ void __launch_bounds__(1024) rms_cell_scan_kernel(uint4* count4, uint
     }
 }
 
-__global__ void __launch_bounds__(256) rms_cell_scatter_kernel(rms_walker_arrays st, uint64_t n, int cx, int cy, uint32_t* cursor,
-                                                                uint32_t* order)
+__global__ void __launch_bounds__(256) rms_cell_scatter_kernel(rms_walker_arrays st, uint64_t n, int cx, int cy, int cz, bool zfast,
+                                                                uint32_t* cursor, uint32_t* order)
 {
     const uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (i < n) order[atomicAdd(&cursor[rms_cell_of(st.w[0][i], st.w[1][i], st.w[2][i], cx, cy)], 1u)] = (uint32_t)i;
+    if (i < n) order[atomicAdd(&cursor[rms_cell_of(st.w[0][i], st.w[1][i], st.w[2][i], cx, cy, cz, zfast)], 1u)] = (uint32_t)i;
 }
 
 }  // namespace
@@ -83,9 +86,10 @@ int rms_order_walkers(const rms_substrate* s, const rms_walkers* w, uint32_t* d_
     cudaError_t e = cudaMemsetAsync(d_count, 0, n_tiles * 4096 * sizeof(uint32_t), stream);
     if (e == cudaSuccess) {
         const unsigned grid = (unsigned)((w->n + 255) / 256);
-        rms_cell_hist_kernel<<<grid, 256, 0, stream>>>(w->a, w->n, cx, cy, d_count);
+        const bool zfast = s->SZ == 1 && s->SX != 1;
+        rms_cell_hist_kernel<<<grid, 256, 0, stream>>>(w->a, w->n, cx, cy, cz, zfast, d_count);
         rms_cell_scan_kernel<<<1, 1024, 0, stream>>>((uint4*)d_count, (uint32_t)n_tiles);
-        rms_cell_scatter_kernel<<<grid, 256, 0, stream>>>(w->a, w->n, cx, cy, d_count, d_order);
+        rms_cell_scatter_kernel<<<grid, 256, 0, stream>>>(w->a, w->n, cx, cy, cz, zfast, d_count, d_order);
         e = cudaGetLastError();
         if (n_launches) *n_launches += 3;
     }

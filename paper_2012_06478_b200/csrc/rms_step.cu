@@ -98,12 +98,12 @@ __global__ void __launch_bounds__(RMS_BLOCK) rms_step_kernel(const __grid_consta
     }
 
     // FACES path: padded linear index + packed wrap counters instead of coordinates
-    const int NX = p.NX, NXY = p.NX * p.NY;
+    const int SX = p.SX, SY = p.SY, SZ = p.SZ;
     int lin = 0;
     uint32_t wraps = 512u | (512u << 10) | (512u << 20);
     uint32_t fm = 0;
     if (LAT == RMS_LAT_FACES) {
-        lin = ((wz + 1) * p.NY + (wy + 1)) * NX + (wx + 1);
+        lin = (wx + 1) * SX + (wy + 1) * SY + (wz + 1) * SZ;
         fm = rms_face_byte(__ldg(p.nbr + lin));
     }
 
@@ -181,11 +181,12 @@ __global__ void __launch_bounds__(RMS_BLOCK) rms_step_kernel(const __grid_consta
                                 if (LAT == RMS_LAT_FACES) {
                                     if (fm & 64u) {
                                         // landed on a ghost voxel earlier: fold back into the box (rare)
-                                        int Z = lin / NXY, rem = lin - Z * NXY, Y = rem / NX, X = rem - Y * NX;
-                                        if (X == 0) { X = p.nx; wraps -= 1u; } else if (X == NX - 1) { X = 1; wraps += 1u; }
-                                        if (Y == 0) { Y = p.ny; wraps -= 1u << 10; } else if (Y == p.NY - 1) { Y = 1; wraps += 1u << 10; }
+                                        int X, Y, Z;
+                                        rms_lattice_coords(lin, SX, SY, SZ, X, Y, Z);
+                                        if (X == 0) { X = p.nx; wraps -= 1u; } else if (X == p.nx + 1) { X = 1; wraps += 1u; }
+                                        if (Y == 0) { Y = p.ny; wraps -= 1u << 10; } else if (Y == p.ny + 1) { Y = 1; wraps += 1u << 10; }
                                         if (Z == 0) { Z = p.nz; wraps -= 1u << 20; } else if (Z == p.nz + 1) { Z = 1; wraps += 1u << 20; }
-                                        lin = (Z * p.NY + Y) * NX + X;
+                                        lin = X * SX + Y * SY + Z * SZ;
                                         fm = rms_face_byte(__ldg(p.nbr + lin));
                                     }
                                     const uint32_t bit = isx ? 1u : (isy ? 2u : 4u);
@@ -207,7 +208,7 @@ __global__ void __launch_bounds__(RMS_BLOCK) rms_step_kernel(const __grid_consta
                                 } else {
                                     gnew = gk + (1.f - base);       // same compartment: the face does not exist
                                     if (LAT == RMS_LAT_FACES) {
-                                        const int stride = isx ? 1 : (isy ? NX : NXY);
+                                        const int stride = isx ? SX : (isy ? SY : SZ);
                                         lin += neg ? -stride : stride;
                                         fm = rms_face_byte(__ldg(p.nbr + lin));
                                     } else {
@@ -376,10 +377,11 @@ __global__ void __launch_bounds__(RMS_BLOCK) rms_step_kernel(const __grid_consta
 
     // ---- store state --------------------------------------------------------------------------
     if (LAT == RMS_LAT_FACES) {
-        int Z = lin / NXY, rem = lin - Z * NXY, Y = rem / NX, X = rem - Y * NX;
+        int X, Y, Z;
+        rms_lattice_coords(lin, SX, SY, SZ, X, Y, Z);
         int wrx = (int)(wraps & 1023u) - 512, wry = (int)((wraps >> 10) & 1023u) - 512, wrz = (int)((wraps >> 20) & 1023u) - 512;
-        if (X == 0) { X = p.nx; --wrx; } else if (X == NX - 1) { X = 1; ++wrx; }
-        if (Y == 0) { Y = p.ny; --wry; } else if (Y == p.NY - 1) { Y = 1; ++wry; }
+        if (X == 0) { X = p.nx; --wrx; } else if (X == p.nx + 1) { X = 1; ++wrx; }
+        if (Y == 0) { Y = p.ny; --wry; } else if (Y == p.ny + 1) { Y = 1; ++wry; }
         if (Z == 0) { Z = p.nz; --wrz; } else if (Z == p.nz + 1) { Z = 1; ++wrz; }
         wx = X - 1; wy = Y - 1; wz = Z - 1;
         dIx += (wx - wx0) + wrx * p.nx;

@@ -57,14 +57,14 @@ __device__ __forceinline__ uint32_t rms_prmt(uint32_t x, uint32_t y, uint32_t se
 }
 
 // padded linear index of a ghost voxel -> index of its periodic image inside the box, wrap counters updated
-__device__ __noinline__ uint2 rms_fold_ghost(int lin, uint32_t wraps, int nx, int ny, int nz)
+__device__ __noinline__ uint2 rms_fold_ghost(int lin, uint32_t wraps, int nx, int ny, int nz, int SX, int SY, int SZ)
 {
-    const int NX = nx + 2, NY = ny + 2, NXY = NX * NY;
-    int Z = lin / NXY, rem = lin - Z * NXY, Y = rem / NX, X = rem - Y * NX;
-    if (X == 0) { X = nx; wraps -= 1u; } else if (X == NX - 1) { X = 1; wraps += 1u; }
-    if (Y == 0) { Y = ny; wraps -= 1u << 10; } else if (Y == NY - 1) { Y = 1; wraps += 1u << 10; }
+    int X, Y, Z;
+    rms_lattice_coords(lin, SX, SY, SZ, X, Y, Z);
+    if (X == 0) { X = nx; wraps -= 1u; } else if (X == nx + 1) { X = 1; wraps += 1u; }
+    if (Y == 0) { Y = ny; wraps -= 1u << 10; } else if (Y == ny + 1) { Y = 1; wraps += 1u << 10; }
     if (Z == 0) { Z = nz; wraps -= 1u << 20; } else if (Z == nz + 1) { Z = 1; wraps += 1u << 20; }
-    return make_uint2((uint32_t)((Z * NY + Y) * NX + X), wraps);
+    return make_uint2((uint32_t)(X * SX + Y * SY + Z * SZ), wraps);
 }
 
 }  // namespace
@@ -117,8 +117,8 @@ __global__ void __launch_bounds__(RMS_FBLOCK, RMS_FMINB) rms_step_fast_kernel(co
         }
     }
 
-    const int NX = p.NX, NXY = p.NX * p.NY;
-    int lin = ((wz + 1) * p.NY + (wy + 1)) * NX + (wx + 1);
+    const int SX = p.SX, SY = p.SY, SZ = p.SZ;
+    int lin = (wx + 1) * SX + (wy + 1) * SY + (wz + 1) * SZ;
     uint32_t wraps = 512u | (512u << 10) | (512u << 20);   // packed per-axis counts of box wraps (+512)
     uint32_t nb = __ldg(p.nbr + lin);
 
@@ -137,7 +137,7 @@ __global__ void __launch_bounds__(RMS_FBLOCK, RMS_FMINB) rms_step_fast_kernel(co
 
     // landed on a ghost voxel: fold back into the box (rare; the word of a ghost voxel is its image's word)
     auto fold = [&]() {
-        const uint2 lw = rms_fold_ghost(lin, wraps, p.nx, p.ny, p.nz);
+        const uint2 lw = rms_fold_ghost(lin, wraps, p.nx, p.ny, p.nz, SX, SY, SZ);
         lin = (int)lw.x; wraps = lw.y;
         nb &= ~RMS_NBR_GHOST;
     };
@@ -202,7 +202,7 @@ __global__ void __launch_bounds__(RMS_FBLOCK, RMS_FMINB) rms_step_fast_kernel(co
             {
                 const bool ps = (pos & 32u) != 0, rf = cx && !ps;
                 if (ps) {
-                    gx -= sgx; dl = isx;
+                    gx -= sgx; dl = isx * SX;
 #pragma unroll
                     for (int m = 0; m < NW; ++m) A32[m][0] += isx * wrem[m];
                 }
@@ -211,7 +211,7 @@ __global__ void __launch_bounds__(RMS_FBLOCK, RMS_FMINB) rms_step_fast_kernel(co
             {
                 const bool ps = (pos & 64u) != 0, rf = cy && !ps;
                 if (ps) {
-                    gy -= sgy; dl += isy * NX;
+                    gy -= sgy; dl += isy * SY;
 #pragma unroll
                     for (int m = 0; m < NW; ++m) A32[m][1] += isy * wrem[m];
                 }
@@ -220,7 +220,7 @@ __global__ void __launch_bounds__(RMS_FBLOCK, RMS_FMINB) rms_step_fast_kernel(co
             {
                 const bool ps = (pos & 128u) != 0, rf = cz && !ps;
                 if (ps) {
-                    gz -= sgz; dl += isz * NXY;
+                    gz -= sgz; dl += isz * SZ;
 #pragma unroll
                     for (int m = 0; m < NW; ++m) A32[m][2] += isz * wrem[m];
                 }
@@ -292,10 +292,11 @@ __global__ void __launch_bounds__(RMS_FBLOCK, RMS_FMINB) rms_step_fast_kernel(co
 
     // ---- store state --------------------------------------------------------------------------
     {
-        int Z = lin / NXY, rem = lin - Z * NXY, Y = rem / NX, X = rem - Y * NX;
+        int X, Y, Z;
+        rms_lattice_coords(lin, SX, SY, SZ, X, Y, Z);
         int wrx = (int)(wraps & 1023u) - 512, wry = (int)((wraps >> 10) & 1023u) - 512, wrz = (int)((wraps >> 20) & 1023u) - 512;
-        if (X == 0) { X = p.nx; --wrx; } else if (X == NX - 1) { X = 1; ++wrx; }
-        if (Y == 0) { Y = p.ny; --wry; } else if (Y == p.NY - 1) { Y = 1; ++wry; }
+        if (X == 0) { X = p.nx; --wrx; } else if (X == p.nx + 1) { X = 1; ++wrx; }
+        if (Y == 0) { Y = p.ny; --wry; } else if (Y == p.ny + 1) { Y = 1; ++wry; }
         if (Z == 0) { Z = p.nz; --wrz; } else if (Z == p.nz + 1) { Z = 1; ++wrz; }
         wx = X - 1; wy = Y - 1; wz = Z - 1;
         dIx += (wx - wx0) + wrx * p.nx;

@@ -33,21 +33,57 @@ extern "C" const char* rms_version(void) { return "rms-b200 0.1 (sm_100a)"; }
 // ------------------------------------------------------------------------------------------------
 __device__ __forceinline__ int rms_wrap1(int a, int n) { return a < 0 ? a + n : (a >= n ? a - n : a); }
 
+// Membrane faces with normal x, y, z on a sample of the lattice (every `sy`-th row of every `sz`-th plane): decides
+// the memory order of the neighbourhood lattice (rms_substrate::SX..SZ).
+__global__ void __launch_bounds__(256) rms_sample_faces_kernel(const uint16_t* __restrict__ labels, int nx, int ny, int nz,
+                                                                int sy, int sz, unsigned long long* __restrict__ counts)
+{
+    const int rows_y = (ny + sy - 1) / sy, rows_z = (nz + sz - 1) / sz;
+    const size_t total = (size_t)rows_z * rows_y * nx;
+    unsigned cx = 0, cy = 0, cz = 0;
+    for (size_t t = (size_t)blockIdx.x * blockDim.x + threadIdx.x; t < total; t += (size_t)gridDim.x * blockDim.x) {
+        const int x = (int)(t % nx);
+        const size_t r = t / nx;
+        const int y = (int)(r % rows_y) * sy, z = (int)(r / rows_y) * sz;
+        const size_t row = ((size_t)z * ny + y) * nx;
+        const uint16_t L = __ldg(labels + row + x);
+        cx += __ldg(labels + row + rms_wrap1(x + 1, nx)) != L;
+        cy += __ldg(labels + ((size_t)z * ny + rms_wrap1(y + 1, ny)) * nx + x) != L;
+        cz += __ldg(labels + ((size_t)rms_wrap1(z + 1, nz) * ny + y) * nx + x) != L;
+    }
+    for (int o = 16; o > 0; o >>= 1) {
+        cx += __shfl_xor_sync(0xffffffffu, cx, o);
+        cy += __shfl_xor_sync(0xffffffffu, cy, o);
+        cz += __shfl_xor_sync(0xffffffffu, cz, o);
+    }
+    if ((threadIdx.x & 31) == 0) {
+        atomicAdd(&counts[0], (unsigned long long)cx);
+        atomicAdd(&counts[1], (unsigned long long)cy);
+        atomicAdd(&counts[2], (unsigned long long)cz);
+    }
+}
+
 // One thread owns a column of RMS_NBR_ZCHUNK padded voxels along z at fixed (X, Y): it keeps the 3 x 3 labels of the
 // planes z-1, z, z+1 in registers and reads 9 new labels per voxel instead of 27 (consecutive threads = consecutive
-// x: coalesced rows, the +-1 neighbours come out of L1).
+// x: coalesced rows, the +-1 neighbours come out of L1).  ZFAST: the words are written z fastest; a warp stages its
+// 32 (x) x 32 (z) tile in shared memory and writes it transposed, 128 contiguous bytes per x.
 #define RMS_NBR_ZCHUNK 128
 
+template <bool ZFAST>
 __global__ void __launch_bounds__(128) rms_build_nbr_kernel(const uint16_t* __restrict__ labels, int nx, int ny, int nz,
-                                                             uint32_t* __restrict__ nbr, int n_labels,
+                                                             uint32_t* __restrict__ nbr, int SX, int SY, int SZ, int n_labels,
                                                              unsigned long long* __restrict__ stats)
 {
+    __shared__ uint32_t tile[ZFAST ? 4 : 1][ZFAST ? 32 : 1][ZFAST ? 33 : 1];
     const int NX = nx + 2, NY = ny + 2, NZ = nz + 2;
-    const int X = blockIdx.x * blockDim.x + threadIdx.x;
+    const int Xt = blockIdx.x * blockDim.x + threadIdx.x;
+    const bool active = Xt < NX;
+    const int X = active ? Xt : NX - 1;               // idle lanes of the last block shadow the last column (ZFAST needs whole warps)
     const int Y = blockIdx.y;
     const int Z0 = blockIdx.z * RMS_NBR_ZCHUNK, Z1 = min(NZ, Z0 + RMS_NBR_ZCHUNK);
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     unsigned n_faces = 0, bad = 0;
-    if (X < NX) {
+    if (ZFAST || active) {
         // periodic image of the padded coordinate (|X-1| <= n, so one wrap is enough even for n = 1)
         const int x = rms_wrap1(X - 1, nx), y = rms_wrap1(Y - 1, ny);
         uint32_t off[9];                              // offsets of the 3 x 3 (dx, dy) neighbours inside a z-plane
@@ -64,9 +100,8 @@ __global__ void __launch_bounds__(128) rms_build_nbr_kernel(const uint16_t* __re
 #pragma unroll
             for (int k = 0; k < 9; ++k) { pa[k] = __ldg(labels + (bl + off[k])); pb[k] = __ldg(labels + (bm + off[k])); }
         }
-        uint32_t* out = nbr + ((size_t)Z0 * NY + Y) * NX + X;
-        const size_t out_stride = (size_t)NY * NX;
-        int Z = Z0;
+        uint32_t* out = nbr + ((size_t)X * SX + (size_t)Y * SY + (size_t)Z0 * SZ);
+        int Z = Z0, zi = 0, zbase = Z0;
         // one voxel: read plane z+1 into HI, compare the 27 labels with the centre of MID, write the word
 #define RMS_NBR_ONE(LO, MID, HI)                                                                              \
         if (Z < Z1) {                                                                                         \
@@ -80,9 +115,21 @@ __global__ void __launch_bounds__(128) rms_build_nbr_kernel(const uint16_t* __re
                      ((HI[k] == L) ? (1u << (k + 18)) : 0u);                                                  \
             const bool ghost = ghost_xy | (Z == 0) | (Z == NZ - 1);                                           \
             if (ghost) m |= RMS_NBR_GHOST;                                                                    \
-            *out = m;                                                                                         \
-            out += out_stride;                                                                                \
-            if (!ghost) {                                                                                     \
+            if (ZFAST) {                                                                                      \
+                tile[warp][zi][lane] = m;                                                                     \
+                if (++zi == 32 || Z == Z1 - 1) {       /* warp-uniform: flush the staged tile, transposed */  \
+                    __syncwarp();                                                                             \
+                    const int Xw = Xt - lane;                                                                 \
+                    for (int xx = 0; xx < 32 && Xw + xx < NX; ++xx)                                           \
+                        if (lane < zi) nbr[(size_t)(Xw + xx) * SX + (size_t)Y * SY + (size_t)(zbase + lane)] = tile[warp][lane][xx]; \
+                    __syncwarp();                                                                             \
+                    zbase += zi; zi = 0;                                                                      \
+                }                                                                                             \
+            } else {                                                                                          \
+                *out = m;                                                                                     \
+                out += SZ;                                                                                    \
+            }                                                                                                 \
+            if (!ghost && active) {                                                                           \
                 n_faces += 3 - (((m >> 14) & 1u) + ((m >> 16) & 1u) + ((m >> 22) & 1u));                      \
                 bad += (L >= (uint32_t)n_labels);                                                             \
             }                                                                                                 \
@@ -167,7 +214,7 @@ extern "C" int rms_substrate_create(const rms_substrate_desc* d, void* cuda_stre
 
     int rc = RMS_OK;
     unsigned long long* d_stats = nullptr;
-    unsigned long long h_stats[2] = {0, 0};
+    unsigned long long h_stats[5] = {0, 0, 0, 0, 0};   // membrane faces, bad labels, sampled faces with normal x, y, z
 #define SUB_TRY(expr)                                                                                    \
     do {                                                                                                 \
         cudaError_t _e = (expr);                                                                         \
@@ -195,8 +242,8 @@ extern "C" int rms_substrate_create(const rms_substrate_desc* d, void* cuda_stre
         s->d_label_class = lc;
         SUB_TRY(cudaMemcpyAsync(lc, s->label_class.data(), nL, cudaMemcpyHostToDevice, stream));
     }
-    SUB_TRY(rms_malloc((void**)&d_stats, 2 * sizeof(unsigned long long)));
-    SUB_TRY(cudaMemsetAsync(d_stats, 0, 2 * sizeof(unsigned long long), stream));
+    SUB_TRY(rms_malloc((void**)&d_stats, 5 * sizeof(unsigned long long)));
+    SUB_TRY(cudaMemsetAsync(d_stats, 0, 5 * sizeof(unsigned long long), stream));
     if (!(d->flags & RMS_NO_BRICKS)) {
         s->NX = s->nx + 2; s->NY = s->ny + 2; s->NZ = s->nz + 2;
         SUB_TRY(rms_malloc((void**)&s->d_nbr, (size_t)s->NX * s->NY * s->NZ * sizeof(uint32_t)));
@@ -206,13 +253,30 @@ extern "C" int rms_substrate_create(const rms_substrate_desc* d, void* cuda_stre
             rc = RMS_ERR_UNSUPPORTED;
             goto fail;
         }
-        rms_build_nbr_kernel<<<grid, 128, 0, stream>>>(s->d_labels, s->nx, s->ny, s->nz, s->d_nbr, nL, d_stats);
+        // memory order: x fastest unless asked otherwise.  RMS_LAYOUT_AUTO: the axis (x or z) with fewer membrane faces
+        // normal to it runs fastest, so that the words of a sector belong to one compartment (cells elongated along
+        // z, such as axons, give z); a sample of the lattice decides
+        bool zfast = (d->flags & RMS_LAYOUT_AUTO) == RMS_LAYOUT_Z_FASTEST;
+        if ((d->flags & RMS_LAYOUT_AUTO) == RMS_LAYOUT_AUTO) {
+            const int sy = s->ny >= 64 ? 4 : 1, sz = s->nz >= 64 ? 4 : 1;
+            rms_sample_faces_kernel<<<148 * 4, 256, 0, stream>>>(s->d_labels, s->nx, s->ny, s->nz, sy, sz, d_stats + 2);
+            SUB_TRY(cudaGetLastError());
+            SUB_TRY(cudaMemcpyAsync(h_stats + 2, d_stats + 2, 3 * sizeof(unsigned long long), cudaMemcpyDeviceToHost, stream));
+            SUB_TRY(cudaStreamSynchronize(stream));
+            zfast = h_stats[4] < h_stats[2];
+        }
+        if (zfast) { s->SZ = 1; s->SY = s->NZ; s->SX = s->NY * s->NZ; }
+        else       { s->SX = 1; s->SY = s->NX; s->SZ = s->NX * s->NY; }
+        if (zfast)
+            rms_build_nbr_kernel<true><<<grid, 128, 0, stream>>>(s->d_labels, s->nx, s->ny, s->nz, s->d_nbr, s->SX, s->SY, s->SZ, nL, d_stats);
+        else
+            rms_build_nbr_kernel<false><<<grid, 128, 0, stream>>>(s->d_labels, s->nx, s->ny, s->nz, s->d_nbr, s->SX, s->SY, s->SZ, nL, d_stats);
         SUB_TRY(cudaGetLastError());
     } else {
         rms_check_labels_kernel<<<148 * 8, 256, 0, stream>>>(s->d_labels, (size_t)n_vox, nL, d_stats);
         SUB_TRY(cudaGetLastError());
     }
-    SUB_TRY(cudaMemcpyAsync(h_stats, d_stats, sizeof h_stats, cudaMemcpyDeviceToHost, stream));
+    SUB_TRY(cudaMemcpyAsync(h_stats, d_stats, 2 * sizeof(unsigned long long), cudaMemcpyDeviceToHost, stream));
     SUB_TRY(cudaStreamSynchronize(stream));
     rms_free(d_stats);
     d_stats = nullptr;

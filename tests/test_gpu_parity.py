@@ -168,6 +168,25 @@ def test_ragged_tiny_lattices_with_heavy_wrapping(rms, dims, flags):
     print("tiny", dims, compare(g, o, n))
 
 
+@pytest.mark.parametrize("layout", [8, 16, 24], ids=["x_fastest", "z_fastest", "auto"])
+def test_both_memory_orders_of_the_neighbourhood_lattice(rms, layout):
+    # RMS_LAYOUT_X_FASTEST (the default) / RMS_LAYOUT_Z_FASTEST / RMS_LAYOUT_AUTO (picked from a sample of the lattice):
+    # ragged box with heavy wrapping through both step kernels, and the reduced axon substrate
+    sub = ri.random_lattice((37, 5, 70), n_labels=2, seed=4)
+    seq = ri.pgse_sequence(2e-4, 300, 0.02, 0.03, [0.0, 20.0], np.eye(3), snap_steps=[299, 300])
+    n = 3000
+    o = oracle_run(sub, seq, n, 12)
+    for flags in (0, 2):                       # specialised and general kernel
+        g = rms.simulate(sub, seq, n, 12, flags=flags, substrate_flags=layout, read_walkers=True)
+        print("layout", layout, flags, compare(g, o, n))
+    cfg = ri.make_config("cfg2", "test")
+    g = rms.simulate(cfg.substrate, cfg.sequence, cfg.n_walkers, cfg.seed, substrate_flags=layout, read_walkers=True)
+    o = oracle_run(cfg.substrate, cfg.sequence, cfg.n_walkers, cfg.seed)
+    print("layout cfg2", layout, compare(g, o, cfg.n_walkers))
+    assert g["substrate_info"]["n_membrane_faces"] == sum(
+        int(np.count_nonzero(cfg.substrate.labels != np.roll(cfg.substrate.labels, 1, axis=ax))) for ax in range(3))
+
+
 def test_free_box_wraps_many_times(rms):
     # no membranes at all, small periodic box: every walker wraps the box repeatedly (ghost-shell folding)
     sub = ri.uniform_lattice((4, 3, 5))
