@@ -51,6 +51,7 @@ def parse_args():
     ap.add_argument("--lattice", default="facemask", choices=["facemask", "labels"])
     ap.add_argument("--scale", default="full", choices=["full", "test"])
     ap.add_argument("--layout", default="x", choices=["auto", "x", "z"], help="memory order of the neighbourhood lattice")
+    ap.add_argument("--fp64", action="store_true", help="RMS_RUN_FP64: the step kernel in fp64 arithmetic (not the headline)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--cpu-sample-walkers", type=int, default=40_000)
@@ -277,6 +278,8 @@ def main():
     n_walkers, mc_steps = args.walkers, args.mc_steps
     first_id = rank * n_walkers                       # weak scaling: every rank owns its own walker-id range
     flags = rms.RMS_RUN_LABEL_GATHER if args.lattice == "labels" else 0
+    if args.fp64:
+        flags |= rms.binding.RMS_RUN_FP64
     sflags = {"auto": rms.binding.RMS_LAYOUT_AUTO, "x": rms.binding.RMS_LAYOUT_X_FASTEST, "z": rms.binding.RMS_LAYOUT_Z_FASTEST}[args.layout]
     t_ms = np.asarray(seq.snap_steps, np.float64) * seq.dt_ms
 
@@ -351,7 +354,7 @@ def main():
     peak_ginstr = N_SM * LANES_PER_SM * sm_mhz * 1e6 / 1e9
     k_ms_per_launch = kernel_ms / args.steps
     achieved_ginstr = ALGORITHMIC_INSTR_PER_STEP * n_walkers * mc_steps / (k_ms_per_launch * 1e-3) / 1e9
-    roofline = {"bound": "alu", "kernel": "rms_step_fast_kernel" if args.lattice == "facemask" else "rms_step_kernel", "achieved": achieved_ginstr, "peak": peak_ginstr,
+    roofline = {"bound": "alu", "kernel": ("rms_step_precise_kernel" if args.fp64 else "rms_step_fast_kernel") if args.lattice == "facemask" else "rms_step_kernel", "achieved": achieved_ginstr, "peak": peak_ginstr,
                 "unit": "Ginstr/s (thread-instructions)", "frac": achieved_ginstr / peak_ginstr,
                 "traffic": NCU_TRAFFIC_BYTES_PER_LAUNCH,
                 "algorithmic_instr_per_walker_step": ALGORITHMIC_INSTR_PER_STEP, "kernel_ms_per_launch": k_ms_per_launch,
@@ -372,7 +375,7 @@ def main():
 
     line = {"metric": "walker_steps_per_s", "value": value, "unit": "walker-steps/s", "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": dev_ms / args.steps, "higher_is_better": True, "scaling": "weak",
-            "vs_baseline": None, "dtype": "f32", "data": "synthetic", "config": workload_config(args, cfg),
+            "vs_baseline": None, "dtype": "f64" if args.fp64 else "f32", "data": "synthetic", "config": workload_config(args, cfg),
             "clocks": clocks, "e2e": e2e, "gpu_launches": launches, "roofline": roofline, "cpu_baseline": cpu_baseline,
             "wall_ms_per_step": 1e3 * wall / args.steps,
             "check": {"S_b_max_dir0": float(abs(r["S"][0, -1, 0])), "n_encounters": r["n_encounters"],

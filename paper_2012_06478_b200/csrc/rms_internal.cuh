@@ -73,6 +73,7 @@ struct rms_walker_arrays {
     int32_t* w[3];     // voxel inside the box
     int32_t* dI[3];    // whole-voxel displacement since the start (unwrapped - initial)
     float* f[3];       // in-voxel offset [0,1)
+    float* f_lo[3];    // fp64 runs (rms_step_precise.cu): offset = f + f_lo to 2^-48; 0 after an fp32 launch
     int32_t* v0[3];    // initial voxel
     float* f0[3];      // initial offset
     uint32_t* lab;     // label | label0 << 16
@@ -193,6 +194,8 @@ struct rms_step_params {
 int rms_launch_step(const rms_step_params& p, int n_wave, int wmode, int lat, bool permeable, cudaStream_t stream);
 // impermeable + RMS_LAT_FACES + RMS_WMODE_CONST only (rms_step_fast.cu)
 int rms_launch_step_fast(const rms_step_params& p, int n_wave, cudaStream_t stream);
+// the same in fp64 arithmetic (rms_step_precise.cu, RMS_RUN_FP64)
+int rms_launch_step_precise(const rms_step_params& p, int n_wave, cudaStream_t stream);
 
 // reductions (rms_reduce.cu)
 struct rms_reduce_params {

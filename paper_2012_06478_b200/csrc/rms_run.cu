@@ -128,7 +128,7 @@ extern "C" int rms_run(const rms_substrate* s, rms_walkers* w, const rms_run_des
         for (int64_t j = nT; j >= 1; --j) { acc += (double)d->wave[(size_t)m * nT + (j - 1)]; S[j - 1] = acc; }
     }
     bool const_mode = wave_is_integer(d->wave, (size_t)nW * nT);
-    for (size_t i = 0; const_mode && i < suf.size(); ++i) const_mode = fabs(suf[i]) < 1073741824.0;
+    for (size_t i = 0; const_mode && i < suf.size(); ++i) const_mode = fabs(suf[i]) < 1048576.0;   // int32 event sums: <= 1024 steps x 2^20 between flushes
 
     // launch boundaries: snapshots and the end of the call
     std::vector<int64_t> bounds;
@@ -268,7 +268,13 @@ extern "C" int rms_run(const rms_substrate* s, rms_walkers* w, const rms_run_des
             }
             cudaEvent_t e0 = evs.make(), e1 = evs.make();
             RMS_CUDA_TRY(cudaEventRecord(e0, stream));
-            if (!permeable && lat == RMS_LAT_FACES && wmode == RMS_WMODE_CONST && !(d->flags & RMS_RUN_GENERAL_KERNEL))
+            const bool special = !permeable && lat == RMS_LAT_FACES && wmode == RMS_WMODE_CONST;
+            if (d->flags & RMS_RUN_FP64) {
+                RMS_REQUIRE(special, RMS_ERR_UNSUPPORTED,
+                            "RMS_RUN_FP64 serves impermeable substrates with integer-valued piecewise-constant waveforms on the "
+                            "neighbourhood lattice");
+                rc = rms_launch_step_precise(sp, nW, stream);
+            } else if (special && !(d->flags & RMS_RUN_GENERAL_KERNEL))
                 rc = rms_launch_step_fast(sp, nW, stream);
             else
                 rc = rms_launch_step(sp, nW, wmode, lat, permeable, stream);

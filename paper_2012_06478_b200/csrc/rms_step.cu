@@ -392,6 +392,7 @@ __global__ void __launch_bounds__(RMS_BLOCK) rms_step_kernel(const __grid_consta
     p.st.w[0][i] = wx; p.st.w[1][i] = wy; p.st.w[2][i] = wz;
     p.st.dI[0][i] = dIx; p.st.dI[1][i] = dIy; p.st.dI[2][i] = dIz;
     p.st.f[0][i] = fx; p.st.f[1][i] = fy; p.st.f[2][i] = fz;
+    p.st.f_lo[0][i] = 0.f; p.st.f_lo[1][i] = 0.f; p.st.f_lo[2][i] = 0.f;
     p.st.lab[i] = (lab & 0xFFFF0000u) | L;
     p.st.relax[i] = relax;
 

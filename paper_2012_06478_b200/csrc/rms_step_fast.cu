@@ -308,6 +308,7 @@ __global__ void __launch_bounds__(RMS_FBLOCK, RMS_FMINB) rms_step_fast_kernel(co
     // an offset of exactly 1 (a walker left sitting on its upper face by rounding) is legal inside the loop: it
     // crosses at once if it moves on upwards; the stored state keeps the floor convention [0, 1) (R15)
     p.st.f[0][i] = fminf(fx, RMS_ONE_MINUS); p.st.f[1][i] = fminf(fy, RMS_ONE_MINUS); p.st.f[2][i] = fminf(fz, RMS_ONE_MINUS);
+    p.st.f_lo[0][i] = 0.f; p.st.f_lo[1][i] = 0.f; p.st.f_lo[2][i] = 0.f;
     p.st.relax[i] = fmaf(p.rate[L], (float)p.n_steps, p.st.relax[i]);   // impermeable: the label never changes (Eq.5)
 
     // diagnostics: warp-shuffle reduction, one atomic per warp (early-exited lanes are not in the mask)

@@ -38,6 +38,7 @@ __global__ void __launch_bounds__(256) rms_init_kernel(const uint16_t* __restric
     st.f0[0][i] = fx; st.f0[1][i] = fy; st.f0[2][i] = fz;
     st.lab[i] = L | (L << 16);
     st.relax[i] = 0.f;
+    st.f_lo[0][i] = 0.f; st.f_lo[1][i] = 0.f; st.f_lo[2][i] = 0.f;
     for (int k = 0; k < n_phi; ++k) st.phi[(size_t)k * n + i] = 0.0;
 }
 
@@ -59,9 +60,9 @@ extern "C" int rms_walkers_init(const rms_substrate* s, uint64_t n_walkers, uint
     RMS_REQUIRE(w, RMS_ERR_OOM, "out of host memory");
     w->sub = s; w->n = n_walkers; w->first_id = first_walker_id; w->seed = seed;
     const uint64_t n = n_walkers;
-    // 17 arrays of 4 bytes + counters, each 256-byte aligned inside one block
+    // 20 arrays of 4 bytes + counters, each 256-byte aligned inside one block
     const size_t a4 = align_up(n * 4, 256);
-    const size_t total = 17 * a4 + 256;
+    const size_t total = 20 * a4 + 256;
     uint8_t* d_allowed = nullptr;
     int rc = RMS_OK;
     unsigned long long h_cnt[8] = {0};
@@ -81,6 +82,7 @@ extern "C" int rms_walkers_init(const rms_substrate* s, uint64_t n_walkers, uint
         for (int k = 0; k < 3; ++k) w->a.w[k] = (int32_t*)take(a4);
         for (int k = 0; k < 3; ++k) w->a.dI[k] = (int32_t*)take(a4);
         for (int k = 0; k < 3; ++k) w->a.f[k] = (float*)take(a4);
+        for (int k = 0; k < 3; ++k) w->a.f_lo[k] = (float*)take(a4);
         for (int k = 0; k < 3; ++k) w->a.v0[k] = (int32_t*)take(a4);
         for (int k = 0; k < 3; ++k) w->a.f0[k] = (float*)take(a4);
         w->a.lab = (uint32_t*)take(a4);

@@ -266,6 +266,31 @@ def test_general_kernel_and_id_order_agree_with_the_specialised_path(rms):
         print("flags", flags, compare(g, o, n))
 
 
+def test_fp64_mode_stays_on_the_oracle_trajectories_over_a_long_run(rms):
+    """RMS_RUN_FP64 on the reduced axon substrate for 200,000 steps (40 ms of diffusion, the length scale of
+    BASELINE.json's configs 1-3): fp32 positions lose walkers at every convex membrane corner they pass within
+    ~1e-6 voxel of and fall below 99.9 % same-voxel long before this; fp64 positions differ
+    from the oracle's by ~1e-13 and must hold the plain tolerances."""
+    cfg = ri.make_config("cfg2", "test")
+    n, n_steps = 2000, 200_000
+    seq = ri.pgse_sequence(cfg.sequence.dt_ms, n_steps, 10.0, 25.0, np.linspace(0.0, 10.0, 5), ri.fibonacci_dirs(12),
+                           snap_steps=[50_001, 100_000, n_steps])
+    o = oracle_run(cfg.substrate, seq, n, cfg.seed)
+    g64 = gpu_run(cfg.substrate, seq, n, cfg.seed, flags=8)
+    rep = compare(g64, o, n, strict_s=True)
+    print("fp64 200k steps", rep)
+    assert rep["n_diff"] <= 1 and rep["max_offset_diff"] < 1e-6          # offsets are read back as fp32
+    g32 = gpu_run(cfg.substrate, seq, n, cfg.seed)
+    same32 = float(np.all(g32["walkers"]["vox"] == o["final_vox"], axis=1).mean())
+    print("fp32 same-voxel fraction at 200k steps:", same32)
+    assert rep["same_voxel"] >= same32
+    # unsupported combinations are refused, not silently run in fp32
+    c3 = ri.make_config("cfg3", "test")
+    with pytest.raises(rms.RmsError) as e:
+        gpu_run(c3.substrate, c3.sequence, 100, 1, flags=8)
+    assert e.value.code == -7
+
+
 def test_tables_match_oracle(rms):
     import oracle
     D = np.array([2.0, 1.0, 0.5], np.float32)
