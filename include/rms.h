@@ -124,10 +124,10 @@ int rms_walkers_destroy(rms_walkers* w);
  *             lookup table) instead of the neighbourhood lattice.
  *             RMS_RUN_GENERAL_KERNEL: impermeable runs with integer-valued piecewise-constant waveforms
  *             normally take the specialised kernel (csrc/rms_step_fast.cu); this flag forces the general one.
- *             RMS_RUN_FP64: direction, hop, in-voxel offsets, hit order and phase in fp64 instead of fp32 (impermeable
- *             substrates, integer-valued piecewise-constant waveforms; RMS_ERR_UNSUPPORTED otherwise).  About
- *             half the speed; for runs of more than a few 1e4 steps whose trajectories must stay on those of an
- *             fp64 reference (csrc/rms_step_precise.cu says why fp32 cannot).
+ *             RMS_RUN_FP64: direction, hop, in-voxel offsets, hit order and phase in fp64 instead of fp32, for runs
+ *             of more than a few 1e4 steps whose trajectories must stay on those of an fp64 reference
+ *             (csrc/rms_step_precise.cu says why fp32 cannot).  Two thirds of the fp32 speed for impermeable
+ *             substrates with integer-valued piecewise-constant waveforms; a plain, slower kernel otherwise.
  *             RMS_RUN_NO_ORDERING: on large lattices the walkers are dealt to the threads in the order of the
  *             lattice cell they sit in (cache locality; results do not depend on it); this flag keeps id order.
  *

@@ -196,6 +196,8 @@ int rms_launch_step(const rms_step_params& p, int n_wave, int wmode, int lat, bo
 int rms_launch_step_fast(const rms_step_params& p, int n_wave, cudaStream_t stream);
 // the same in fp64 arithmetic (rms_step_precise.cu, RMS_RUN_FP64)
 int rms_launch_step_precise(const rms_step_params& p, int n_wave, cudaStream_t stream);
+// fp64, everything else: permeable / variable D / any waveform, RMS_WMODE_TABLE data, label gathers (rms_step_precise_general.cu)
+int rms_launch_step_precise_general(const rms_step_params& p, int n_wave, cudaStream_t stream);
 
 // reductions (rms_reduce.cu)
 struct rms_reduce_params {

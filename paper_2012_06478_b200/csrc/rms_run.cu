@@ -127,7 +127,10 @@ extern "C" int rms_run(const rms_substrate* s, rms_walkers* w, const rms_run_des
         double* S = &suf[(size_t)m * (nT + 1)];
         for (int64_t j = nT; j >= 1; --j) { acc += (double)d->wave[(size_t)m * nT + (j - 1)]; S[j - 1] = acc; }
     }
-    bool const_mode = wave_is_integer(d->wave, (size_t)nW * nT);
+    // RMS_RUN_FP64: the specialised fp64 kernel serves the impermeable / neighbourhood-lattice / integer-waveform case,
+    // the general fp64 kernel (table-driven waveforms, label gathers) everything else
+    const bool fp64 = (d->flags & RMS_RUN_FP64) != 0;
+    bool const_mode = wave_is_integer(d->wave, (size_t)nW * nT) && !(fp64 && (permeable || lat != RMS_LAT_FACES));
     for (size_t i = 0; const_mode && i < suf.size(); ++i) const_mode = fabs(suf[i]) < 1048576.0;   // int32 event sums: <= 1024 steps x 2^20 between flushes
 
     // launch boundaries: snapshots and the end of the call
@@ -269,12 +272,9 @@ extern "C" int rms_run(const rms_substrate* s, rms_walkers* w, const rms_run_des
             cudaEvent_t e0 = evs.make(), e1 = evs.make();
             RMS_CUDA_TRY(cudaEventRecord(e0, stream));
             const bool special = !permeable && lat == RMS_LAT_FACES && wmode == RMS_WMODE_CONST;
-            if (d->flags & RMS_RUN_FP64) {
-                RMS_REQUIRE(special, RMS_ERR_UNSUPPORTED,
-                            "RMS_RUN_FP64 serves impermeable substrates with integer-valued piecewise-constant waveforms on the "
-                            "neighbourhood lattice");
-                rc = rms_launch_step_precise(sp, nW, stream);
-            } else if (special && !(d->flags & RMS_RUN_GENERAL_KERNEL))
+            if (fp64)
+                rc = special ? rms_launch_step_precise(sp, nW, stream) : rms_launch_step_precise_general(sp, nW, stream);
+            else if (special && !(d->flags & RMS_RUN_GENERAL_KERNEL))
                 rc = rms_launch_step_fast(sp, nW, stream);
             else
                 rc = rms_launch_step(sp, nW, wmode, lat, permeable, stream);

@@ -284,11 +284,42 @@ def test_fp64_mode_stays_on_the_oracle_trajectories_over_a_long_run(rms):
     same32 = float(np.all(g32["walkers"]["vox"] == o["final_vox"], axis=1).mean())
     print("fp32 same-voxel fraction at 200k steps:", same32)
     assert rep["same_voxel"] >= same32
-    # unsupported combinations are refused, not silently run in fp32
+
+
+def test_fp64_mode_general_kernel_permeable_and_table_waveforms(rms):
+    # RMS_RUN_FP64 outside the specialised case: permeable + D contrast + T2 (cfg3 reduced), and a non-integer waveform
     c3 = ri.make_config("cfg3", "test")
-    with pytest.raises(rms.RmsError) as e:
-        gpu_run(c3.substrate, c3.sequence, 100, 1, flags=8)
-    assert e.value.code == -7
+    g = gpu_run(c3.substrate, c3.sequence, c3.n_walkers, c3.seed, flags=8)
+    o = oracle_run(c3.substrate, c3.sequence, c3.n_walkers, c3.seed)
+    rep = compare(g, o, c3.n_walkers, strict_s=True)
+    print("fp64 cfg3 reduced", rep)
+    assert rep["n_diff"] == 0 and rep["perm_diff"] == 0 and g["n_permeations"] > 0
+    sub = ri.single_cylinder(24, 7.5, 0.1)
+    n_steps = 801
+    t = (np.arange(n_steps) + 1.0) / n_steps
+    wave = np.stack([np.sin(2 * np.pi * t), np.clip(4 * np.minimum(t, 1 - t), 0, 1) * np.sign(0.5 - t)]).astype(np.float32)
+    seq = ri.Sequence(dt_ms=2e-4, n_steps=n_steps, wave=wave, gamp=np.array([[0.0, 40.0, 90.0], [10.0, 60.0, 120.0]]),
+                      dirs=ri.fibonacci_dirs(5), snap_steps=np.array([400, 801]))
+    g = gpu_run(sub, seq, 6000, 5, flags=8)
+    o = oracle_run(sub, seq, 6000, 5)
+    rep = compare(g, o, 6000, strict_s=True)
+    print("fp64 table waveforms", rep)
+    assert rep["n_diff"] == 0
+
+
+@pytest.mark.parametrize("name,n_ids", [("cfg1", 20_000), ("cfg2", 2_000), ("cfg3", 4_000)])
+def test_full_length_configs_in_fp64_on_a_sample_of_walker_ids(rms, name, n_ids):
+    """BASELINE.json configs 1-3 at their full lattice size and full number of steps (85,000 / 500,000 / 50,000), on
+    the first n_ids walker ids (what the oracle finishes in seconds; trajectories depend on (seed, id) only, so
+    the sample is exactly the corresponding slice of the full job), in RMS_RUN_FP64: plain tolerances."""
+    import torch
+    cfg = ri.make_config(name, "full")
+    labels_dev = torch.from_numpy(cfg.substrate.labels.view(np.int16)).cuda()
+    g = rms.simulate(cfg.substrate, cfg.sequence, n_ids, cfg.seed, flags=8, device_labels=labels_dev, read_walkers=True)
+    o = oracle_run(cfg.substrate, cfg.sequence, n_ids, cfg.seed)
+    rep = compare(g, o, n_ids, strict_s=True)
+    print("full length", name, cfg.sequence.n_steps, "steps", rep, "kernel_ms", g["kernel_ms"])
+    assert rep["n_diff"] <= max(1, n_ids // 5000)
 
 
 def test_tables_match_oracle(rms):
