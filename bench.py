@@ -54,7 +54,7 @@ def parse_args():
     ap.add_argument("--fp64", action="store_true", help="RMS_RUN_FP64: the step kernel in fp64 arithmetic (not the headline)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--cpu-sample-walkers", type=int, default=40_000)
+    ap.add_argument("--cpu-sample-walkers", type=int, default=250_000)
     ap.add_argument("--sweep", action="store_true",
                     help="BASELINE.json configs[4]: walkers 1e5..1e8 x {1, 60} directions x {neighbourhood lattice, label "
                          "gather}, one JSON line per point (not part of the driver contract)")

@@ -69,7 +69,7 @@ __device__ __noinline__ uint2 rms_fold_ghost(int lin, uint32_t wraps, int nx, in
 
 }  // namespace
 
-template <int NW>
+template <int NW, bool XFAST>
 __global__ void __launch_bounds__(RMS_FBLOCK, RMS_FMINB) rms_step_fast_kernel(const __grid_constant__ rms_step_params p)
 {
     __shared__ float2 sm_trig[256];   // (cos, sin) of the centre of the 256 azimuth bins
@@ -117,7 +117,7 @@ __global__ void __launch_bounds__(RMS_FBLOCK, RMS_FMINB) rms_step_fast_kernel(co
         }
     }
 
-    const int SX = p.SX, SY = p.SY, SZ = p.SZ;
+    const int SX = XFAST ? 1 : p.SX, SY = p.SY, SZ = p.SZ;      // x fastest (the default order): unit stride known at compile time
     int lin = (wx + 1) * SX + (wy + 1) * SY + (wz + 1) * SZ;
     uint32_t wraps = 512u | (512u << 10) | (512u << 20);   // packed per-axis counts of box wraps (+512)
     uint32_t nb = __ldg(p.nbr + lin);
@@ -321,16 +321,19 @@ int rms_launch_step_fast(const rms_step_params& p, int n_wave, cudaStream_t stre
 {
     if (p.n == 0 || p.n_steps == 0) return RMS_OK;
     const unsigned grid = (unsigned)((p.n + RMS_FBLOCK - 1) / RMS_FBLOCK);
+    const bool xf = p.SX == 1;
+#define RMS_FAST_CASE(NWV)                                                                      \
+    case NWV:                                                                                   \
+        if (xf) rms_step_fast_kernel<NWV, true><<<grid, RMS_FBLOCK, 0, stream>>>(p);            \
+        else rms_step_fast_kernel<NWV, false><<<grid, RMS_FBLOCK, 0, stream>>>(p);              \
+        break;
     switch (n_wave) {
-        case 0: rms_step_fast_kernel<0><<<grid, RMS_FBLOCK, 0, stream>>>(p); break;
-        case 1: rms_step_fast_kernel<1><<<grid, RMS_FBLOCK, 0, stream>>>(p); break;
-        case 2: rms_step_fast_kernel<2><<<grid, RMS_FBLOCK, 0, stream>>>(p); break;
-        case 3: rms_step_fast_kernel<3><<<grid, RMS_FBLOCK, 0, stream>>>(p); break;
-        case 4: rms_step_fast_kernel<4><<<grid, RMS_FBLOCK, 0, stream>>>(p); break;
+        RMS_FAST_CASE(0) RMS_FAST_CASE(1) RMS_FAST_CASE(2) RMS_FAST_CASE(3) RMS_FAST_CASE(4)
         default:
             rms_set_error("n_wave = %d is above RMS_MAX_WAVES = %d", n_wave, RMS_MAX_WAVES);
             return RMS_ERR_UNSUPPORTED;
     }
+#undef RMS_FAST_CASE
     RMS_CUDA_TRY(cudaGetLastError());
     return RMS_OK;
 }
