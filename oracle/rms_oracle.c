@@ -27,6 +27,9 @@
  *   run, equilibrium     uniform density kept with D contrast and permeable walls
  *                        (P:78), exchange between slabs vs. the eigen-series
  *   run, T2              alpha = exp(-t/T2) exactly for a single compartment (Eq.5)
+ *   run, cylinder        short-time Mitra law D(t)/D0 = 1 - 4/(3 sqrt(pi)) (S_x/V) sqrt(D0 t)
+ *                        with S_x/V counted on the staircase surface of the lattice cylinder
+ *   run, encounters      membrane encounters per step = surface * step / 4
  * Parity unpinned: wide-pulse signals inside voxelised cylinders / axons have
  *   no closed form; they are pinned only through the pieces above.
  */
