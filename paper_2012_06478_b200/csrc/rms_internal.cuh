@@ -176,6 +176,7 @@ struct rms_step_params {
     const float* P512;        // [n_labels^2] 512 * P(a->b)
     const float* rate;        // [n_labels] dt / T2
     int n_labels;
+    uint32_t t_ceil;          // ceil(512 max P(a->b)) over the membranes: coarse random bits at or above it cannot permeate
     uint32_t step0;           // steps done before this launch
     uint32_t n_steps;         // steps of this launch
     int n_seg;
@@ -192,8 +193,8 @@ struct rms_step_params {
 };
 
 int rms_launch_step(const rms_step_params& p, int n_wave, int wmode, int lat, bool permeable, cudaStream_t stream);
-// impermeable + RMS_LAT_FACES + RMS_WMODE_CONST only (rms_step_fast.cu)
-int rms_launch_step_fast(const rms_step_params& p, int n_wave, cudaStream_t stream);
+// RMS_LAT_FACES + RMS_WMODE_CONST only; permeable: P(a->b) << 1 expected (rms_step_fast.cu)
+int rms_launch_step_fast(const rms_step_params& p, int n_wave, bool permeable, cudaStream_t stream);
 // the same in fp64 arithmetic (rms_step_precise.cu, RMS_RUN_FP64)
 int rms_launch_step_precise(const rms_step_params& p, int n_wave, cudaStream_t stream);
 // fp64, everything else: permeable / variable D / any waveform, RMS_WMODE_TABLE data, label gathers (rms_step_precise_general.cu)

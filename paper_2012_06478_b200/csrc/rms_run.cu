@@ -115,6 +115,14 @@ extern "C" int rms_run(const rms_substrate* s, rms_walkers* w, const rms_run_des
     }
     const bool want_labels = (d->flags & RMS_RUN_LABEL_GATHER) != 0;
     const int lat = (!permeable && s->d_nbr && !want_labels) ? RMS_LAT_FACES : RMS_LAT_LABELS;
+    // permeable runs with P << 1 also take the specialised kernel: ceil(512 P_max) bounds the coarse random
+    // bits that can permeate at all (rms_step_fast.cu)
+    float t_max = 0.f;
+    for (int a = 0; a < nL; ++a)
+        for (int b = 0; b < nL; ++b)
+            if (a != b) t_max = std::max(t_max, h_P512[(size_t)a * nL + b]);
+    const uint32_t t_ceil = (uint32_t)ceilf(t_max);
+    const bool fast_permeable = permeable && s->d_nbr && !want_labels && t_ceil <= 64u;
 
     rc = rms_walkers_reserve_waves(w, nW, stream);
     if (rc != RMS_OK) return rc;
@@ -232,6 +240,7 @@ extern "C" int rms_run(const rms_substrate* s, rms_walkers* w, const rms_run_des
     sp.labels = s->d_labels; sp.nbr = s->d_nbr; sp.NX = s->NX; sp.NY = s->NY; sp.SX = s->SX; sp.SY = s->SY; sp.SZ = s->SZ;
     sp.st = w->a; sp.n = n; sp.first_id = w->first_id; sp.rk = rms_make_keys(w->seed);
     sp.s_tab = b_tabs.as<float>(); sp.rate = sp.s_tab + nL; sp.P512 = sp.rate + nL; sp.n_labels = nL;
+    sp.t_ceil = t_ceil;
     sp.counters = w->d_counters; sp.n_wave = nW; sp.wave_stride = nT; sp.wsuf_stride = nT + 1;
 
     rms_reduce_params rp;
@@ -272,10 +281,11 @@ extern "C" int rms_run(const rms_substrate* s, rms_walkers* w, const rms_run_des
             cudaEvent_t e0 = evs.make(), e1 = evs.make();
             RMS_CUDA_TRY(cudaEventRecord(e0, stream));
             const bool special = !permeable && lat == RMS_LAT_FACES && wmode == RMS_WMODE_CONST;
+            const bool special_perm = fast_permeable && wmode == RMS_WMODE_CONST;
             if (fp64)
                 rc = special ? rms_launch_step_precise(sp, nW, stream) : rms_launch_step_precise_general(sp, nW, stream);
-            else if (special && !(d->flags & RMS_RUN_GENERAL_KERNEL))
-                rc = rms_launch_step_fast(sp, nW, stream);
+            else if ((special || special_perm) && !(d->flags & RMS_RUN_GENERAL_KERNEL))
+                rc = rms_launch_step_fast(sp, nW, permeable, stream);
             else
                 rc = rms_launch_step(sp, nW, wmode, lat, permeable, stream);
             if (rc != RMS_OK) return rc;

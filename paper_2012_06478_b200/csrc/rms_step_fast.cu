@@ -67,9 +67,108 @@ __device__ __noinline__ uint2 rms_fold_ghost(int lin, uint32_t wraps, int nx, in
     return make_uint2((uint32_t)(X * SX + Y * SY + Z * SZ), wraps);
 }
 
+// ------------------------------------------------------------------------------------------------------------------
+// Permeable substrates.  An unlike-label face is crossed with the probability of Eq.3, decided by the 33-bit
+// uniform of R5 whose 9 coarse bits are the spare low bits of the step's direction words: u_e < P needs coarse bits
+// below ceil(512 P_max).  For P << 1 (the paper's regime) that is 1 encounter in several hundred, so the kernel
+// below treats every unlike-label face as a wall unless those bits allow a permeation; if they do, the WHOLE step is
+// redone here by the interaction loop written out (the same arithmetic as rms_step.cu: labels gathered from the
+// uint16 lattice, hop rescaled on entering a compartment of different D, R7).  Rare, so out of line.
+//   st  = { fx, fy, fz, s }           in: offsets before the hop, hop length;  out: offsets after it, new hop length
+//   ist = { lin, wraps, L, dAx, dAy, dAz, n_enc, n_perm }   in: lin, wraps, L;  out: all (dA = net voxel move per axis)
+// ------------------------------------------------------------------------------------------------------------------
+__device__ __noinline__ void rms_permeable_step(const rms_step_params* pp, uint32_t id_lo, uint32_t id_hi, uint32_t j,
+                                                uint32_t wa, uint32_t wb, float rx, float ry, float rz, float* st, int* ist)
+{
+    const rms_step_params& p = *pp;
+    const float INF = __int_as_float(0x7f800000);
+    int X, Y, Z;
+    rms_lattice_coords(ist[0], p.SX, p.SY, p.SZ, X, Y, Z);
+    int wr[3] = {0, 0, 0};
+    if (X == 0) { X = p.nx; --wr[0]; } else if (X == p.nx + 1) { X = 1; ++wr[0]; }     // sitting on a ghost voxel: fold
+    if (Y == 0) { Y = p.ny; --wr[1]; } else if (Y == p.ny + 1) { Y = 1; ++wr[1]; }
+    if (Z == 0) { Z = p.nz; --wr[2]; } else if (Z == p.nz + 1) { Z = 1; ++wr[2]; }
+    int w[3] = {X - 1, Y - 1, Z - 1};
+    const int nk3[3] = {p.nx, p.ny, p.nz};
+    const int str3[3] = {1, p.nx, p.nx * p.ny};
+    float pk3[3] = {st[0], st[1], st[2]};
+    float r3[3] = {rx, ry, rz};
+    float s = st[3];
+    uint32_t L = (uint32_t)ist[2];
+    bool done[3] = {false, false, false};
+    int dA[3] = {0, 0, 0};
+    int e = 0, n_enc = 0, n_perm = 0;
+    uint32_t v0 = 0, v1 = 0, v2 = 0, v3 = 0;
+    bool have_v = false;
+    for (int it = 0; it < 3; ++it) {
+        float t3[3];
+        bool any = false;
+        for (int k = 0; k < 3; ++k) {
+            const float g = pk3[k] + r3[k];
+            const bool c = !done[k] && __float_as_uint(g) >= 0x3F800000u;
+            t3[k] = c ? __fdividef((r3[k] > 0.f ? 1.f : 0.f) - pk3[k], r3[k]) : INF;
+            any |= c;
+        }
+        if (!any) break;
+        const float tm = fminf(t3[0], fminf(t3[1], t3[2]));
+        const int k = (t3[0] == tm) ? 0 : ((t3[1] == tm) ? 1 : 2);           // ties: lowest axis first (R10)
+        const bool neg = r3[k] < 0.f;
+        for (int q = 0; q < 3; ++q) pk3[q] = fmaf(tm, r3[q], pk3[q]);
+        const float rest = 1.f - tm;
+        for (int q = 0; q < 3; ++q) r3[q] *= rest;
+        int nwk = w[k] + (neg ? -1 : 1), dwrap = 0;
+        if (nwk < 0) { nwk = nk3[k] - 1; dwrap = -1; } else if (nwk == nk3[k]) { nwk = 0; dwrap = 1; }
+        const uint32_t Ln = __ldg(p.labels + ((w[2] * p.ny + w[1]) * p.nx + w[0] + (nwk - w[k]) * str3[k]));
+        bool pass = true;
+        if (Ln != L) {
+            ++n_enc;
+            const float T = __ldg(p.P512 + (size_t)L * p.n_labels + Ln);     // 512 P(L -> Ln), Eq.3
+            if (T >= 512.f) pass = true;
+            else if (T <= 0.f) pass = false;
+            else {
+                if (e >= 2 && !have_v) { rms_philox(p.rk, id_lo, id_hi, j + 1u, RMS_STREAM_PERM, v0, v1, v2, v3); have_v = true; }
+                const float cf = (float)((e == 0 ? wa : (e == 1 ? wb : v3)) & 511u);
+                if (cf + 1.f <= T) pass = true;
+                else if (cf >= T) pass = false;
+                else {
+                    if (!have_v) { rms_philox(p.rk, id_lo, id_hi, j + 1u, RMS_STREAM_PERM, v0, v1, v2, v3); have_v = true; }
+                    pass = rms_uni(e == 0 ? v0 : (e == 1 ? v1 : v2)) < (T - cf);
+                }
+            }
+            ++e;
+            n_perm += pass;
+        }
+        const float plane = neg ? 0.f : 1.f;
+        if (pass) {
+            pk3[k] = 1.f - plane;
+            w[k] = nwk;
+            wr[k] += dwrap;
+            dA[k] += neg ? -1 : 1;
+            if (Ln != L) {                   // rest of the hop at the new compartment's speed (R7)
+                const float s_new = __ldg(p.s_tab + Ln);
+                const float sc = __fdividef(s_new, s);
+                for (int q = 0; q < 3; ++q) r3[q] *= sc;
+                s = s_new;
+                L = Ln;
+            }
+        } else {
+            pk3[k] = plane;
+            r3[k] = -r3[k];                  // elastic collision
+        }
+        done[k] = true;
+    }
+    for (int k = 0; k < 3; ++k) st[k] = fminf(fmaxf(pk3[k] + r3[k], 0.f), RMS_ONE_MINUS);
+    st[3] = s;
+    ist[0] = (w[0] + 1) * p.SX + (w[1] + 1) * p.SY + (w[2] + 1) * p.SZ;
+    ist[1] = (int)((uint32_t)ist[1] + (uint32_t)wr[0] + ((uint32_t)wr[1] << 10) + ((uint32_t)wr[2] << 20));
+    ist[2] = (int)L;
+    ist[3] = dA[0]; ist[4] = dA[1]; ist[5] = dA[2];
+    ist[6] = n_enc; ist[7] = n_perm;
+}
+
 }  // namespace
 
-template <int NW, bool XFAST>
+template <int NW, bool XFAST, bool PERM>
 __global__ void __launch_bounds__(RMS_FBLOCK, RMS_FMINB) rms_step_fast_kernel(const __grid_constant__ rms_step_params p)
 {
     __shared__ float2 sm_trig[256];   // (cos, sin) of the centre of the 256 azimuth bins
@@ -101,8 +200,12 @@ __global__ void __launch_bounds__(RMS_FBLOCK, RMS_FMINB) rms_step_fast_kernel(co
     int dIx = p.st.dI[0][i], dIy = p.st.dI[1][i], dIz = p.st.dI[2][i];
     float fx = p.st.f[0][i], fy = p.st.f[1][i], fz = p.st.f[2][i];
     const uint32_t lab = p.st.lab[i];
-    const uint32_t L = lab & 0xFFFFu;
-    const float s = p.s_tab[L];
+    uint32_t L = lab & 0xFFFFu;                 // changes only on a permeation (PERM)
+    float s = p.s_tab[L];
+    float rate = p.rate[L], relax = p.st.relax[i];
+    uint32_t j_rate = p.step0;                  // steps up to here are already in `relax`
+    unsigned n_perm = 0;
+    const uint32_t t_ceil = PERM ? p.t_ceil : 0u;   // permeation needs coarse bits below ceil(512 P_max)
 
     // launch prologue of the phase: Phi += (dI - f0) * sum_{launch} w
     if (NW > 0) {
@@ -143,7 +246,7 @@ __global__ void __launch_bounds__(RMS_FBLOCK, RMS_FMINB) rms_step_fast_kernel(co
     };
 
     // ---- one Monte Carlo step from the two direction words (R3, R4) ------------------------------
-    auto step = [&](const uint32_t wa, const uint32_t wb) {
+    auto step = [&](const uint32_t wa, const uint32_t wb, const uint32_t jj) {
         // z = sym(wa): exact odd multiple of 2^-23
         const float z = fmaf(__uint_as_float(__funnelshift_r(wa, 0x7Fu, 9)) - 1.5f, 2.0f, 1.1920928955078125e-07f);
         // azimuth pi * sym(wb) = bin centre (top 8 bits) + residual (next 15 bits, exact): rotate the table entry
@@ -187,16 +290,41 @@ __global__ void __launch_bounds__(RMS_FBLOCK, RMS_FMINB) rms_step_fast_kernel(co
             const uint32_t lut = 0x21438900u + (uint32_t)(mx * 0x02000000 + my * 0x00060000 + mz * 0x00001200);
             int dl = 0;                                             // lattice-index change of this hop
             uint32_t pos = RMS_NBR_SELF;
+            // PERM: bit e set = the e-th membrane met in this step may be crossed (its coarse random bits are below
+            // ceil(512 P_max); the third draw's bits are not at hand, so it always may)
+            const uint32_t pm = PERM ? ((uint32_t)((wa & 511u) < t_ceil) | ((uint32_t)((wb & 511u) < t_ceil) << 1) | 4u) : 0u;
+            uint32_t redo = 0;
             auto slot = [&](const int key) {
                 const uint32_t q = pos + rms_prmt(lut, 0u, (uint32_t)key & 3u);
                 // the voxel ahead carries my label: pass; else a membrane: count the collision in bits 8..9
-                pos = (nb & __funnelshift_l(0u, 1u, q)) ? q : pos + 0x100u;
+                if (nb & __funnelshift_l(0u, 1u, q)) pos = q;
+                else { if (PERM) redo |= pm >> (pos >> 8); pos += 0x100u; }
             };
             slot(k_hi);
             if (k_mid >= 0) {
                 slot(k_mid);
                 if (k_lo >= 0) slot(k_lo);
             }
+            if (PERM && (redo & 1u)) {
+                // a membrane of this step may be permeated: redo the step by the written-out interaction loop
+                float st[4] = {fx, fy, fz, s};
+                int ist[8] = {lin, (int)wraps, (int)L, 0, 0, 0, 0, 0};
+                rms_permeable_step(&p, id_lo, id_hi, jj, wa, wb, rx, ry, rz, st, ist);
+                gx = st[0]; gy = st[1]; gz = st[2];
+                lin = ist[0]; wraps = (uint32_t)ist[1];
+#pragma unroll
+                for (int m = 0; m < NW; ++m) {
+                    A32[m][0] += ist[3] * wrem[m]; A32[m][1] += ist[4] * wrem[m]; A32[m][2] += ist[5] * wrem[m];
+                }
+                n_enc += (unsigned)ist[6]; n_perm += (unsigned)ist[7];
+                if ((uint32_t)ist[2] != L) {
+                    // Eq.5: the whole dt of this step goes to the compartment at the end of the hop (R12)
+                    relax = fmaf(rate, (float)(jj - j_rate), relax);
+                    j_rate = jj;
+                    L = (uint32_t)ist[2]; s = st[3]; rate = __ldg(p.rate + L);
+                }
+                nb = __ldg(p.nbr + lin);
+            } else {
             // outcome per axis: passed -> g - sigma (enters the neighbour); membrane -> elastic collision,
             // mirrored on the face plane: 2 h - g
             {
@@ -235,6 +363,7 @@ __global__ void __launch_bounds__(RMS_FBLOCK, RMS_FMINB) rms_step_fast_kernel(co
                 lin += dl;
                 nb = __ldg(p.nbr + lin);
             }
+            }
         }
         fx = gx; fy = gy; fz = gz;
         // phase, fractional part: Phi_F += w f (the integer part is event driven, above)
@@ -264,19 +393,19 @@ __global__ void __launch_bounds__(RMS_FBLOCK, RMS_FMINB) rms_step_fast_kernel(co
             uint32_t r0, r1, r2, r3;
             if (j & 1u) {                        // second half of a Philox call that an earlier segment began
                 rms_philox(p.rk, id_lo, id_hi, j >> 1, RMS_STREAM_DIR, r0, r1, r2, r3);
-                step(r2, r3);
+                step(r2, r3, j);
                 ++j;
             }
 #pragma unroll 1
             while (j + 2u <= chunk_end) {
                 rms_philox(p.rk, id_lo, id_hi, j >> 1, RMS_STREAM_DIR, r0, r1, r2, r3);
-                step(r0, r1);
-                step(r2, r3);
+                step(r0, r1, j);
+                step(r2, r3, j + 1u);
                 j += 2u;
             }
             if (j < chunk_end) {
                 rms_philox(p.rk, id_lo, id_hi, j >> 1, RMS_STREAM_DIR, r0, r1, r2, r3);
-                step(r0, r1);
+                step(r0, r1, j);
                 ++j;
             }
             // flush the chunk's partial sums into the fp64 accumulators
@@ -309,23 +438,33 @@ __global__ void __launch_bounds__(RMS_FBLOCK, RMS_FMINB) rms_step_fast_kernel(co
     // crosses at once if it moves on upwards; the stored state keeps the floor convention [0, 1) (R15)
     p.st.f[0][i] = fminf(fx, RMS_ONE_MINUS); p.st.f[1][i] = fminf(fy, RMS_ONE_MINUS); p.st.f[2][i] = fminf(fz, RMS_ONE_MINUS);
     p.st.f_lo[0][i] = 0.f; p.st.f_lo[1][i] = 0.f; p.st.f_lo[2][i] = 0.f;
-    p.st.relax[i] = fmaf(p.rate[L], (float)p.n_steps, p.st.relax[i]);   // impermeable: the label never changes (Eq.5)
+    p.st.relax[i] = fmaf(rate, (float)(p.step0 + p.n_steps - j_rate), relax);   // Eq.5; the label changes only on a permeation
+    if (PERM) p.st.lab[i] = (lab & 0xFFFF0000u) | L;
 
     // diagnostics: warp-shuffle reduction, one atomic per warp (early-exited lanes are not in the mask)
     const unsigned mask = __activemask();
     n_enc = __reduce_add_sync(mask, n_enc);
-    if ((threadIdx.x & 31) == (unsigned)(__ffs(mask) - 1) && n_enc) atomicAdd(&p.counters[0], (unsigned long long)n_enc);
+    if (PERM) n_perm = __reduce_add_sync(mask, n_perm);
+    if ((threadIdx.x & 31) == (unsigned)(__ffs(mask) - 1)) {
+        if (n_enc) atomicAdd(&p.counters[0], (unsigned long long)n_enc);
+        if (PERM && n_perm) atomicAdd(&p.counters[1], (unsigned long long)n_perm);
+    }
 }
 
-int rms_launch_step_fast(const rms_step_params& p, int n_wave, cudaStream_t stream)
+int rms_launch_step_fast(const rms_step_params& p, int n_wave, bool permeable, cudaStream_t stream)
 {
     if (p.n == 0 || p.n_steps == 0) return RMS_OK;
     const unsigned grid = (unsigned)((p.n + RMS_FBLOCK - 1) / RMS_FBLOCK);
     const bool xf = p.SX == 1;
 #define RMS_FAST_CASE(NWV)                                                                      \
     case NWV:                                                                                   \
-        if (xf) rms_step_fast_kernel<NWV, true><<<grid, RMS_FBLOCK, 0, stream>>>(p);            \
-        else rms_step_fast_kernel<NWV, false><<<grid, RMS_FBLOCK, 0, stream>>>(p);              \
+        if (permeable) {                                                                        \
+            if (xf) rms_step_fast_kernel<NWV, true, true><<<grid, RMS_FBLOCK, 0, stream>>>(p);   \
+            else rms_step_fast_kernel<NWV, false, true><<<grid, RMS_FBLOCK, 0, stream>>>(p);     \
+        } else {                                                                                \
+            if (xf) rms_step_fast_kernel<NWV, true, false><<<grid, RMS_FBLOCK, 0, stream>>>(p);  \
+            else rms_step_fast_kernel<NWV, false, false><<<grid, RMS_FBLOCK, 0, stream>>>(p);    \
+        }                                                                                       \
         break;
     switch (n_wave) {
         RMS_FAST_CASE(0) RMS_FAST_CASE(1) RMS_FAST_CASE(2) RMS_FAST_CASE(3) RMS_FAST_CASE(4)
