@@ -87,6 +87,29 @@ def test_strongly_permeable_slabs_with_D_contrast(rms):
         assert g["n_permeations"] > 10000
 
 
+def test_weakly_permeable_runs_take_the_specialised_kernel_and_its_redo_path(rms):
+    # kappa such that 512 P is ~20-45 (below the 64 that keeps the run on the specialised kernel): about one membrane
+    # encounter in 15 has coarse bits that allow a permeation and is redone by the written-out loop, with D contrast
+    # (hop rescaled, R7), T2 contrast (Eq.5 by compartment), heavy periodic wrapping, snapshots on odd steps, 2 waveforms
+    import oracle
+    sub = ri.slabs(5, 4, (3, 2), 0.1, D_extra=2.0, D_intra=1.0, kappa_membrane=4.0, T2_extra=0.05, T2_intra=0.2)
+    _, P = oracle.rms_oracle.tables(sub.D, sub.kappa, sub.voxel_um, 2e-4)
+    assert 15.0 < 512 * np.max(P[~np.eye(2, dtype=bool)]) < 64.0
+    n_steps = 701
+    wave = np.stack([ri.pgse_wave(n_steps, 201, 350), ri.pgse_wave(n_steps, 100, 500)])
+    seq = ri.Sequence(dt_ms=2e-4, n_steps=n_steps, wave=wave, gamp=np.array([[0.0, 30.0], [0.0, 80.0]]),
+                      dirs=ri.fibonacci_dirs(5), snap_steps=np.array([99, 350, 701]))
+    n = 20000
+    o = oracle_run(sub, seq, n, 9)
+    g = gpu_run(sub, seq, n, 9)
+    rep = compare(g, o, n)
+    print("weakly permeable, specialised kernel", rep)
+    assert 1000 < g["n_permeations"] < 0.2 * g["n_encounters"]
+    g2 = gpu_run(sub, seq, n, 9, flags=2)                       # RMS_RUN_GENERAL_KERNEL: same physics, other kernel
+    print("weakly permeable, general kernel", compare(g2, o, n))
+    assert abs(g["n_permeations"] - g2["n_permeations"]) <= 3 and np.abs(g["S"] - g2["S"]).max() < 2e-4
+
+
 def test_chunked_run_continues_the_same_trajectories(rms):
     cfg = ri.make_config("cfg0")
     sub, seq = cfg.substrate, cfg.sequence
