@@ -19,7 +19,9 @@
 //   * Philox4x32-10: one call serves two steps (R2), both steps fully unrolled.
 #include "rms_internal.cuh"
 
+#ifndef RMS_FBLOCK
 #define RMS_FBLOCK 128
+#endif
 #ifndef RMS_FMINB
 #define RMS_FMINB 8                  // resident blocks per SM the register allocation is held to
 #endif
