@@ -51,6 +51,8 @@ def parse_args():
     ap.add_argument("--lattice", default="facemask", choices=["facemask", "labels"])
     ap.add_argument("--scale", default="full", choices=["full", "test"])
     ap.add_argument("--layout", default="x", choices=["auto", "x", "z"], help="memory order of the neighbourhood lattice")
+    ap.add_argument("--waves", type=int, default=1,
+                    help="number of PGSE waveforms evaluated on the same trajectories (sequence sweep, not the headline)")
     ap.add_argument("--fp64", action="store_true", help="RMS_RUN_FP64: the step kernel in fp64 arithmetic (not the headline)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -161,6 +163,12 @@ class ClockSampler:
 def make_workload(args):
     import rms_inputs as ri
     cfg = ri.make_config("cfg4", args.scale, n_walkers=args.walkers, n_steps=args.mc_steps, n_dir=args.dirs)
+    if args.waves > 1:      # sequence sweep: waveform m has delta = Delta / (m + 1) ... all on one set of trajectories
+        seq = cfg.sequence
+        n = seq.n_steps
+        waves = np.stack([ri.pgse_wave(n, max(1, int(0.4 * n / (m + 1))), int(0.6 * n)) for m in range(args.waves)])
+        gamp = np.repeat(seq.gamp, args.waves, axis=0)
+        cfg.sequence = dataclasses.replace(seq, wave=waves.astype(np.float32), gamp=gamp)
     return cfg
 
 

@@ -37,7 +37,7 @@ typedef enum {
     RMS_ERR_UNSUPPORTED = -7     /* e.g. n_wave above RMS_MAX_WAVES                                                */
 } rms_status;
 
-#define RMS_MAX_WAVES 4
+#define RMS_MAX_WAVES 16   /* gradient waveforms evaluated on one set of trajectories in one rms_run (sequence sweep) */
 
 typedef struct rms_substrate rms_substrate; /* opaque */
 typedef struct rms_walkers rms_walkers;     /* opaque */

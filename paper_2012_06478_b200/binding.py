@@ -14,7 +14,7 @@ import numpy as np
 
 _PKG = Path(__file__).resolve().parent
 LIB_PATH = _PKG / "librms_b200.so"
-RMS_MAX_WAVES = 4
+RMS_MAX_WAVES = 16
 
 RMS_LABELS_ON_DEVICE = 1
 RMS_ADOPT_DEVICE_PTR = 2

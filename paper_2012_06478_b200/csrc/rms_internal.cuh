@@ -159,6 +159,8 @@ struct rms_segment {          // a run of steps on which every waveform is const
 };
 
 enum { RMS_WMODE_CONST = 0, RMS_WMODE_TABLE = 1 };
+// the step kernels are compiled for 0..4, 8 and 16 waveforms; a run with 5..7 or 9..15 is padded with zero-weight waveforms
+static inline int rms_kernel_waves(int n_wave) { return n_wave <= 4 ? n_wave : (n_wave <= 8 ? 8 : 16); }
 enum { RMS_LAT_LABELS = 0, RMS_LAT_FACES = 1 };
 #define RMS_NBR_GHOST (1u << 27)
 #define RMS_NBR_SELF 13

@@ -124,12 +124,13 @@ extern "C" int rms_run(const rms_substrate* s, rms_walkers* w, const rms_run_des
     const uint32_t t_ceil = (uint32_t)ceilf(t_max);
     const bool fast_permeable = permeable && s->d_nbr && !want_labels && t_ceil <= 64u;
 
-    rc = rms_walkers_reserve_waves(w, nW, stream);
+    const int nWk = rms_kernel_waves(nW);        // waveforms the step kernel is compiled for; the extra ones carry zero weight
+    rc = rms_walkers_reserve_waves(w, nWk, stream);
     if (rc != RMS_OK) return rc;
 
     // ---- waveform analysis ---------------------------------------------------------------------------
     // suffix sums S[m][j] = sum_{i > j} w_m[i] (j = 0..nT, steps are 1-based), fp64
-    std::vector<double> suf((size_t)std::max(nW, 1) * (nT + 1), 0.0);
+    std::vector<double> suf((size_t)std::max(nWk, 1) * (nT + 1), 0.0);
     for (int m = 0; m < nW; ++m) {
         double acc = 0.0;
         double* S = &suf[(size_t)m * (nT + 1)];
@@ -193,10 +194,11 @@ extern "C" int rms_run(const rms_substrate* s, rms_walkers* w, const rms_run_des
             RMS_CUDA_TRY(cudaMemcpyAsync(b_segs.p, segs.data(), segs.size() * sizeof(rms_segment), cudaMemcpyHostToDevice, stream));
         }
     } else if (nW > 0 && nT > 0) {
-        RMS_CUDA_TRY(rms_malloc((void**)&b_wave.p, (size_t)nW * nT * sizeof(float)));
+        RMS_CUDA_TRY(rms_malloc((void**)&b_wave.p, (size_t)nWk * nT * sizeof(float)));
+        if (nWk > nW) RMS_CUDA_TRY(cudaMemsetAsync(b_wave.p, 0, (size_t)nWk * nT * sizeof(float), stream));
         RMS_CUDA_TRY(cudaMemcpyAsync(b_wave.p, d->wave, (size_t)nW * nT * sizeof(float), cudaMemcpyHostToDevice, stream));
-        RMS_CUDA_TRY(rms_malloc((void**)&b_wsuf.p, (size_t)nW * (nT + 1) * sizeof(double)));
-        RMS_CUDA_TRY(cudaMemcpyAsync(b_wsuf.p, suf.data(), (size_t)nW * (nT + 1) * sizeof(double), cudaMemcpyHostToDevice, stream));
+        RMS_CUDA_TRY(rms_malloc((void**)&b_wsuf.p, (size_t)nWk * (nT + 1) * sizeof(double)));
+        RMS_CUDA_TRY(cudaMemcpyAsync(b_wsuf.p, suf.data(), (size_t)nWk * (nT + 1) * sizeof(double), cudaMemcpyHostToDevice, stream));
     }
     // phase per unit Phi, in turns: gamp dt l_p n / (2 pi)   (Eq.7 with the right-endpoint rule, R11)
     std::vector<double> qv((size_t)std::max(nQ, 1) * 3, 0.0);
@@ -283,11 +285,11 @@ extern "C" int rms_run(const rms_substrate* s, rms_walkers* w, const rms_run_des
             const bool special = !permeable && lat == RMS_LAT_FACES && wmode == RMS_WMODE_CONST;
             const bool special_perm = fast_permeable && wmode == RMS_WMODE_CONST;
             if (fp64)
-                rc = special ? rms_launch_step_precise(sp, nW, stream) : rms_launch_step_precise_general(sp, nW, stream);
+                rc = special ? rms_launch_step_precise(sp, nWk, stream) : rms_launch_step_precise_general(sp, nWk, stream);
             else if ((special || special_perm) && !(d->flags & RMS_RUN_GENERAL_KERNEL))
-                rc = rms_launch_step_fast(sp, nW, permeable, stream);
+                rc = rms_launch_step_fast(sp, nWk, permeable, stream);
             else
-                rc = rms_launch_step(sp, nW, wmode, lat, permeable, stream);
+                rc = rms_launch_step(sp, nWk, wmode, lat, permeable, stream);
             if (rc != RMS_OK) return rc;
             RMS_CUDA_TRY(cudaEventRecord(e1, stream));
             step_ev.push_back({e0, e1});

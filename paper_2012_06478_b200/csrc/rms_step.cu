@@ -431,6 +431,8 @@ static int launch_wm(const rms_step_params& p, int n_wave, int lat, bool permeab
         case 2: return launch_nw<2, WMODE>(p, lat, permeable, stream);
         case 3: return launch_nw<3, WMODE>(p, lat, permeable, stream);
         case 4: return launch_nw<4, WMODE>(p, lat, permeable, stream);
+        case 8: return launch_nw<8, WMODE>(p, lat, permeable, stream);
+        case 16: return launch_nw<16, WMODE>(p, lat, permeable, stream);
     }
     rms_set_error("n_wave = %d is above RMS_MAX_WAVES = %d", n_wave, RMS_MAX_WAVES);
     return RMS_ERR_UNSUPPORTED;

@@ -172,7 +172,7 @@ __device__ __noinline__ void rms_permeable_step(const rms_step_params* pp, uint3
 }  // namespace
 
 template <int NW, bool XFAST, bool PERM>
-__global__ void __launch_bounds__(RMS_FBLOCK, RMS_FMINB) rms_step_fast_kernel(const __grid_constant__ rms_step_params p)
+__global__ void __launch_bounds__(RMS_FBLOCK, (NW <= 4 ? RMS_FMINB : (NW <= 8 ? 4 : 2))) rms_step_fast_kernel(const __grid_constant__ rms_step_params p)
 {
     __shared__ float2 sm_trig[256];   // (cos, sin) of the centre of the 256 azimuth bins
 
@@ -470,7 +470,7 @@ int rms_launch_step_fast(const rms_step_params& p, int n_wave, bool permeable, c
         }                                                                                       \
         break;
     switch (n_wave) {
-        RMS_FAST_CASE(0) RMS_FAST_CASE(1) RMS_FAST_CASE(2) RMS_FAST_CASE(3) RMS_FAST_CASE(4)
+        RMS_FAST_CASE(0) RMS_FAST_CASE(1) RMS_FAST_CASE(2) RMS_FAST_CASE(3) RMS_FAST_CASE(4) RMS_FAST_CASE(8) RMS_FAST_CASE(16)
         default:
             rms_set_error("n_wave = %d is above RMS_MAX_WAVES = %d", n_wave, RMS_MAX_WAVES);
             return RMS_ERR_UNSUPPORTED;

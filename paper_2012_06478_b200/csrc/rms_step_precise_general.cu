@@ -188,6 +188,8 @@ int rms_launch_step_precise_general(const rms_step_params& p, int n_wave, cudaSt
         case 2: rms_step_precise_general_kernel<2><<<grid, RMS_GBLOCK, 0, stream>>>(p); break;
         case 3: rms_step_precise_general_kernel<3><<<grid, RMS_GBLOCK, 0, stream>>>(p); break;
         case 4: rms_step_precise_general_kernel<4><<<grid, RMS_GBLOCK, 0, stream>>>(p); break;
+        case 8: rms_step_precise_general_kernel<8><<<grid, RMS_GBLOCK, 0, stream>>>(p); break;
+        case 16: rms_step_precise_general_kernel<16><<<grid, RMS_GBLOCK, 0, stream>>>(p); break;
         default:
             rms_set_error("n_wave = %d is above RMS_MAX_WAVES = %d", n_wave, RMS_MAX_WAVES);
             return RMS_ERR_UNSUPPORTED;

@@ -179,6 +179,36 @@ def test_four_integer_waveforms_odd_boundaries_and_chunks(rms):
     keep["walkers"].destroy(); keep["substrate"].destroy()
 
 
+@pytest.mark.parametrize("n_wave", [6, 16])
+def test_sequence_sweep_many_waveforms_on_one_set_of_trajectories(rms, n_wave):
+    # S: section 8(f) N1 -- a sweep of PGSE timings (the paper's Delta = delta series) evaluated on the same
+    # trajectories in one run: 6 waveforms run on the 8-waveform kernel padded with zero weights, 16 on the 16-waveform one;
+    # specialised fp32 kernel, general kernel (one extra non-integer waveform -> table mode) and fp64
+    sub = ri.single_cylinder(20, 6.5, 0.1)
+    nT = 640
+    wave = np.zeros((n_wave, nT), np.float32)
+    for m in range(n_wave):
+        n_delta = 20 + 18 * m
+        wave[m] = ri.pgse_wave(nT, n_delta, n_delta + (m % 3) * 7)
+    gamp = np.stack([np.array([0.0, 40.0 / (1 + m)]) for m in range(n_wave)])
+    seq = ri.Sequence(dt_ms=2e-4, n_steps=nT, wave=wave, gamp=gamp, dirs=ri.fibonacci_dirs(4), snap_steps=np.array([321, nT]))
+    n = 6000
+    o = oracle_run(sub, seq, n, 17)
+    for flags in (0, 8):
+        g = gpu_run(sub, seq, n, 17, flags=flags)
+        rep = compare(g, o, n)
+        print("waves", n_wave, "flags", flags, rep)
+        assert g["S"].shape == (n_wave, 2, 4)
+        if flags == 8:
+            assert rep["n_diff"] == 0
+    wave2 = wave.copy()
+    wave2[n_wave - 1] *= 0.5                                     # non-integer -> table mode, general kernels
+    seq2 = ri.Sequence(dt_ms=2e-4, n_steps=nT, wave=wave2, gamp=gamp, dirs=ri.fibonacci_dirs(4), snap_steps=np.array([nT]))
+    o2 = oracle_run(sub, seq2, n, 17)
+    for flags in (0, 8):
+        print("waves", n_wave, "table mode, flags", flags, compare(gpu_run(sub, seq2, n, 17, flags=flags), o2, n))
+
+
 @pytest.mark.parametrize("dims", [(5, 7, 3), (1, 1, 9), (2, 3, 4)])
 @pytest.mark.parametrize("flags", [0, LABEL_GATHER], ids=["facemask", "labels"])
 def test_ragged_tiny_lattices_with_heavy_wrapping(rms, dims, flags):
