@@ -370,6 +370,20 @@ def main():
                 "peak_source": f"148 SM x 128 lanes x SM clock measured during the run ({sm_mhz:.0f} MHz; "
                                f"MEASURED_PEAKS.json present: {peaks_file.exists()})"}
 
+    # second roofline candidate: random-gather ceilings measured on this GPU, against the gather rate of the
+    # step kernel (0.68 voxel changes per walker-step, one 4-byte word each)
+    try:
+        g_l2 = rms.binding.rms_gather_probe(48 << 20, 4, 2048)
+        g_hbm = rms.binding.rms_gather_probe(2 << 30, 4, 512)
+        k_rate = 0.68 * n_walkers * mc_steps / (k_ms_per_launch * 1e-3)
+        k_dram = (NCU_TRAFFIC_BYTES_PER_LAUNCH / 32.0) / (k_ms_per_launch * 1e-3) if NCU_TRAFFIC_BYTES_PER_LAUNCH else None
+        roofline["gather"] = {"kernel_gathers_per_s": k_rate, "kernel_dram_sectors_per_s": k_dram,
+                              "ceiling_l2_resident_48MB": g_l2, "ceiling_hbm_2GB": g_hbm,
+                              "dram_sectors_frac_of_hbm_ceiling": (k_dram / g_hbm) if k_dram else None,
+                              "unit": "random 4-byte gathers/s (one 32-byte sector each); kernel_dram_sectors from the ncu capture"}
+    except Exception as ex:      # the probe is a report, never a reason to lose the bench line
+        roofline["gather"] = {"error": str(ex)}
+
     cpu_baseline = None
     if not args.no_cpu_baseline:
         import oracle

@@ -218,6 +218,12 @@ int rms_normalise(int n_classes, int n_q, const double* sum_alpha, const double*
                   int n_snap, int n_dir, const double* snap_alpha, const double* m2, const double* m4,
                   const double* t_ms, double* S_re, double* S_im, double* Dapp, double* Kapp);
 
+/* Measured ceiling for the label / neighbourhood gathers of the walk (the second roofline candidate): random
+ * gathers of elem_bytes (2 or 4) from a zero-filled device table of table_bytes (48 MB sits in the L2, 1 GB does not),
+ * loads_per_thread each on 148 x 2048 threads; *gathers_per_s (host) = gathers, i.e. 32-byte sectors, per second.
+ * Errors: RMS_ERR_ARG, RMS_ERR_OOM, RMS_ERR_CUDA. */
+int rms_gather_probe(uint64_t table_bytes, int elem_bytes, uint32_t loads_per_thread, void* cuda_stream, double* gathers_per_s);
+
 /* Device buffers behind destroyed handles are kept for the next handle of the same size (a pass of the path
  * allocates the same buffers every time); rms_memory_trim returns them to the driver.  Always RMS_OK. */
 int rms_memory_trim(void);

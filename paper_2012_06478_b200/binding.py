@@ -32,7 +32,7 @@ STATUS = {0: "RMS_OK", -1: "RMS_ERR_ARG", -2: "RMS_ERR_STEP_TOO_LARGE", -3: "RMS
 
 EXPORTS = ("rms_substrate_create", "rms_substrate_destroy", "rms_substrate_get_info", "rms_walkers_init",
            "rms_walkers_destroy", "rms_run", "rms_walkers_read", "rms_walkers_steps_done", "rms_tables", "rms_normalise",
-           "rms_memory_trim", "rms_last_error", "rms_version")
+           "rms_memory_trim", "rms_gather_probe", "rms_last_error", "rms_version")
 
 
 class RmsError(RuntimeError):
@@ -246,6 +246,14 @@ def rms_run(substrate: Substrate, walkers: Walkers, dt_ms, n_steps, wave=None, g
              kernel_ms=float(res.kernel_ms), total_ms=float(res.total_ms), n_launches=int(res.n_launches))
     r["S"] = r["S_re"] + 1j * r["S_im"]
     return r
+
+
+def rms_gather_probe(table_bytes, elem_bytes=4, loads_per_thread=1024, stream=None) -> float:
+    """Random gathers per second from a device table of table_bytes (include/rms.h)."""
+    out = C.c_double()
+    _check(load_library().rms_gather_probe(C.c_uint64(int(table_bytes)), C.c_int(int(elem_bytes)), C.c_uint32(int(loads_per_thread)),
+                                           _stream_ptr(stream), C.byref(out)))
+    return out.value
 
 
 def rms_normalise(r: dict, t_ms) -> dict:

@@ -375,6 +375,15 @@ def test_full_length_configs_in_fp64_on_a_sample_of_walker_ids(rms, name, n_ids)
     assert rep["n_diff"] <= max(1, n_ids // 5000)
 
 
+def test_gather_probe_reports_sane_ceilings(rms):
+    l2 = rms.binding.rms_gather_probe(32 << 20, 4, 256)
+    hbm = rms.binding.rms_gather_probe(1 << 30, 2, 128)
+    print("gather ceilings: L2-resident %.3g /s, HBM %.3g /s" % (l2, hbm))
+    assert l2 > hbm > 1e9
+    with pytest.raises(rms.RmsError):
+        rms.binding.rms_gather_probe(1 << 20, 3, 128)
+
+
 def test_tables_match_oracle(rms):
     import oracle
     D = np.array([2.0, 1.0, 0.5], np.float32)
