@@ -53,7 +53,8 @@ typedef struct rms_walkers rms_walkers;     /* opaque */
  * T2           [n_labels] ms; +inf or <= 0 means no relaxation; NULL = none (host; Eq.5)
  * kappa        [n_labels*n_labels] membrane permeability um/ms between label pairs, symmetric, diagonal
  *              ignored; 0 = impermeable; +inf = no membrane (Eq.C.15 with c1 = c2); NULL = all 0 (host; Eq.3)
- * label_class  [n_labels] output compartment class of each label, < n_classes; NULL = all 0 (host)
+ * label_class  [n_labels] uint16 output compartment class of each label, < n_classes <= 65535; NULL = all 0 (host).
+ *              Two classes (extra / intra-cellular) are the usual choice; class = label gives per-cell outputs.
  * flags        RMS_LABELS_ON_DEVICE | RMS_ADOPT_DEVICE_PTR | RMS_NO_BRICKS | RMS_LAYOUT_X_FASTEST | RMS_LAYOUT_Z_FASTEST | RMS_LAYOUT_AUTO
  *
  * Derived on the device, unless RMS_NO_BRICKS: the neighbourhood lattice, one 32-bit word per voxel (plus a
@@ -77,7 +78,7 @@ typedef struct {
     const float* D;
     const float* T2;
     const float* kappa;
-    const uint8_t* label_class;
+    const uint16_t* label_class;
     int32_t n_classes;
     uint32_t flags;
 } rms_substrate_desc;

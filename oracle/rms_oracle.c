@@ -302,7 +302,7 @@ typedef struct {
     lattice_t lat;
     double voxel_um;
     const double* inv_T2; /* [n_labels], 0 = no relaxation */
-    const uint8_t* label_class;
+    const uint16_t* label_class;
     int n_classes;
     /* walkers */
     uint64_t n_walkers, first_id, seed;
@@ -418,7 +418,7 @@ static void* run_part(void* arg)
 
 int rms_oracle_run(
     int nx, int ny, int nz, double voxel_um, const uint16_t* labels, int n_labels,
-    const float* D, const float* T2, const float* kappa, const uint8_t* label_class, int n_classes,
+    const float* D, const float* T2, const float* kappa, const uint16_t* label_class, int n_classes,
     uint64_t n_walkers, uint64_t first_id, const uint8_t* label_allowed, uint64_t seed,
     double dt_ms, int64_t n_steps, int n_wave, const float* wave, int n_g, const double* gamp,
     int n_dir, const double* dirs, int n_snap, const int64_t* snap_steps, int n_threads,

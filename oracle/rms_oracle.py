@@ -146,7 +146,7 @@ def run(sub, seq, n_walkers, seed, first_id=0, n_threads=1, per_walker=False):
     D = np.ascontiguousarray(sub.D, np.float32)
     T2 = np.ascontiguousarray(sub.T2, np.float32)
     kappa = np.ascontiguousarray(sub.kappa, np.float32)
-    lclass = np.ascontiguousarray(sub.label_class, np.uint8)
+    lclass = np.ascontiguousarray(sub.label_class, np.uint16)
     allowed = np.ascontiguousarray(sub.label_allowed, np.uint8)
     wave = np.ascontiguousarray(seq.wave, np.float32)
     gamp = np.ascontiguousarray(seq.gamp, np.float64)
@@ -168,7 +168,7 @@ def run(sub, seq, n_walkers, seed, first_id=0, n_threads=1, per_walker=False):
                   relax=np.zeros(n_walkers))
     st = lib.rms_oracle_run(
         C.c_int(nx), C.c_int(ny), C.c_int(nz), C.c_double(sub.voxel_um), _p(labels, C.c_uint16), C.c_int(nL),
-        _p(D, C.c_float), _p(T2, C.c_float), _p(kappa, C.c_float), _p(lclass, C.c_uint8), C.c_int(nC),
+        _p(D, C.c_float), _p(T2, C.c_float), _p(kappa, C.c_float), _p(lclass, C.c_uint16), C.c_int(nC),
         C.c_uint64(n_walkers), C.c_uint64(first_id), _p(allowed, C.c_uint8), C.c_uint64(seed),
         C.c_double(seq.dt_ms), C.c_int64(n_steps), C.c_int(n_wave), _p(wave, C.c_float), C.c_int(n_g),
         _p(gamp, C.c_double), C.c_int(n_dir), _p(dirs, C.c_double), C.c_int(n_snap), _p(snaps, C.c_int64),

@@ -170,7 +170,7 @@ def rms_substrate_create(labels, voxel_um, D, T2=None, kappa=None, label_class=N
     D = _host(D, np.float32)
     T2 = _host(T2, np.float32)
     kappa = _host(kappa, np.float32)
-    label_class = _host(label_class, np.uint8)
+    label_class = _host(label_class, np.uint16)
     d = SubstrateDesc(nx, ny, nz, float(voxel_um), lab_ptr, int(D.size), _ptr(D), _ptr(T2), _ptr(kappa), _ptr(label_class),
                       int(n_classes), int(flags))
     h = C.c_void_p()

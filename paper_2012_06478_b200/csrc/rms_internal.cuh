@@ -62,8 +62,8 @@ struct rms_substrate {
     int NX = 0, NY = 0, NZ = 0;          // padded dims (n + 2)
     uint64_t n_membrane_faces = 0;
     std::vector<float> D, T2, kappa;     // host copies of the per-label tables
-    std::vector<uint8_t> label_class;
-    uint8_t* d_label_class = nullptr;
+    std::vector<uint16_t> label_class;
+    uint16_t* d_label_class = nullptr;
     bool all_impermeable = true;         // every off-diagonal kappa is 0
 };
 
@@ -206,7 +206,7 @@ int rms_launch_step_precise_general(const rms_step_params& p, int n_wave, cudaSt
 struct rms_reduce_params {
     rms_walker_arrays st;
     uint64_t n;
-    const uint8_t* label_class;  // device
+    const uint16_t* label_class;  // device
     int n_classes;
     const float* rate;           // device [n_labels] (unused: relax is final at launch end)
     int n_dir;
@@ -216,10 +216,14 @@ struct rms_reduce_params {
 int rms_launch_moments(const rms_reduce_params& p, double* d_m2, double* d_m4, double* d_alpha,
                        unsigned long long* d_flow, cudaStream_t stream);
 // qv: device [nq*3] phase per unit Phi in turns; qwave: device [nq] waveform index
+// order_by_class: device [n], needed (and used) only when n_classes > RMS_SIG_SMALL_CLASSES
+#define RMS_SIG_SMALL_CLASSES 8
 int rms_launch_signal(const rms_reduce_params& p, int n_wave, int nq, const double* d_qv, const int* d_qwave, double* d_re,
-                      double* d_im, double* d_sum_alpha, cudaStream_t stream, unsigned* n_launches);
+                      double* d_im, double* d_sum_alpha, const uint32_t* order_by_class, cudaStream_t stream, unsigned* n_launches);
 int rms_compute_tables(const rms_substrate* s, double dt, std::vector<float>& s_tab, std::vector<float>& P_tab);
 int rms_walkers_reserve_waves(rms_walkers* w, int n_wave, cudaStream_t stream);
 // rms_sched.cu: order[t] = walker index, sorted by the lattice cell the walker sits in (z-major), so that the
 // threads of a warp and the blocks resident at one time gather neighbouring words.  d_order: [n] device.
 int rms_order_walkers(const rms_substrate* s, const rms_walkers* w, uint32_t* d_order, cudaStream_t stream, unsigned* n_launches);
+// order[t] = walker index, sorted by the output class of the walker's initial label (per-cell outputs: hundreds of classes)
+int rms_order_by_class(const rms_substrate* s, const rms_walkers* w, uint32_t* d_order, cudaStream_t stream, unsigned* n_launches);

@@ -196,12 +196,107 @@ __global__ void __launch_bounds__(RED_BLOCK) rms_signal_kernel(const rms_reduce_
             if (s_alsum[t] != 0.0) atomicAdd(&g_sum_alpha[t], s_alsum[t]);
 }
 
+// ------------------------------------------------------------------------------------------------
+// signal sums with many output classes (per-cell outputs: class = label, hundreds of classes).  Per-block accumulators
+// for every (q, class) no longer fit anywhere, so the walkers are visited in the order of their class (rms_sched.cu):
+// a tile of 256 consecutive walkers is one run of a class, occasionally two or three.  Thread = up to SIG_QPT
+// (waveform, b, direction) triples; sums in registers over a run; fp64 atomics into the output at the end of each run.
+// ------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(RED_BLOCK) rms_signal_runs_kernel(const rms_reduce_params p, int n_wave, int nq_l, int q_begin,
+                                                                     const double* __restrict__ qv, const int* __restrict__ qwave,
+                                                                     const uint32_t* __restrict__ order, double* __restrict__ g_re,
+                                                                     double* __restrict__ g_im, double* __restrict__ g_sum_alpha)
+{
+    extern __shared__ double sm[];
+    const int nC = p.n_classes;
+    double* s_phi = sm;                                             // [n_wave*3][SIG_TILE]
+    float* s_alpha = (float*)(s_phi + (size_t)n_wave * 3 * SIG_TILE);   // [SIG_TILE]
+    int* s_cls = (int*)(s_alpha + SIG_TILE);                        // [SIG_TILE]
+
+    double qx[SIG_QPT], qy[SIG_QPT], qz[SIG_QPT];
+    int qm[SIG_QPT];
+#pragma unroll
+    for (int c = 0; c < SIG_QPT; ++c) {
+        const int jl = c * RED_BLOCK + threadIdx.x;
+        const bool ok = jl < nq_l;
+        const int j = q_begin + jl;
+        qx[c] = ok ? qv[3 * j] : 0.0; qy[c] = ok ? qv[3 * j + 1] : 0.0; qz[c] = ok ? qv[3 * j + 2] : 0.0;
+        qm[c] = ok ? qwave[j] : -1;
+    }
+
+    const uint64_t n_tiles = (p.n + SIG_TILE - 1) / SIG_TILE;
+    for (uint64_t tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
+        __syncthreads();
+        const int n_in = (int)min((uint64_t)SIG_TILE, p.n - tile * SIG_TILE);
+        if (threadIdx.x < n_in) {
+            const uint64_t i = order[tile * SIG_TILE + threadIdx.x];
+            for (int k = 0; k < 3 * n_wave; ++k) s_phi[k * SIG_TILE + threadIdx.x] = p.st.phi[(size_t)k * p.n + i];
+            s_alpha[threadIdx.x] = (float)exp(-(double)p.st.relax[i]);
+            s_cls[threadIdx.x] = p.label_class[p.st.lab[i] >> 16];
+        }
+        __syncthreads();
+        double are[SIG_QPT], aim[SIG_QPT], asum = 0.0;
+#pragma unroll
+        for (int c = 0; c < SIG_QPT; ++c) { are[c] = 0.0; aim[c] = 0.0; }
+        int cur = s_cls[0];
+        for (int w = 0; w <= n_in; ++w) {
+            const int cc = w < n_in ? s_cls[w] : -1;                 // warp-uniform
+            if (cc != cur) {                                        // end of a run: flush
+#pragma unroll
+                for (int c = 0; c < SIG_QPT; ++c) {
+                    const int jl = c * RED_BLOCK + threadIdx.x;
+                    if (jl < nq_l) {
+                        const size_t o = (size_t)(q_begin + jl) * nC + cur;
+                        atomicAdd(&g_re[o], are[c]);
+                        atomicAdd(&g_im[o], aim[c]);
+                    }
+                    are[c] = 0.0; aim[c] = 0.0;
+                }
+                if (q_begin == 0 && threadIdx.x == 0) atomicAdd(&g_sum_alpha[cur], asum);
+                asum = 0.0;
+                cur = cc;
+                if (w == n_in) break;
+            }
+            const double al = (double)s_alpha[w];
+            asum += al;
+#pragma unroll
+            for (int c = 0; c < SIG_QPT; ++c) {
+                if (qm[c] < 0) continue;
+                const double* ph = s_phi + (size_t)qm[c] * 3 * SIG_TILE + w;
+                const double turns = qx[c] * ph[0] + qy[c] * ph[SIG_TILE] + qz[c] * ph[2 * SIG_TILE];
+                const float ph32 = (float)(6.283185307179586 * (turns - rint(turns)));
+                float sn, cs;
+                __sincosf(ph32, &sn, &cs);
+                are[c] += al * (double)cs;                       // Eq.7: alpha e^{-i phi}
+                aim[c] -= al * (double)sn;
+            }
+        }
+    }
+}
+
 int rms_launch_signal(const rms_reduce_params& p, int n_wave, int nq, const double* d_qv, const int* d_qwave, double* d_re,
-                      double* d_im, double* d_sum_alpha, cudaStream_t stream, unsigned* n_launches)
+                      double* d_im, double* d_sum_alpha, const uint32_t* order_by_class, cudaStream_t stream, unsigned* n_launches)
 {
     const uint64_t n_tiles = (p.n + SIG_TILE - 1) / SIG_TILE;
     const unsigned grid = (unsigned)(n_tiles < 148ull * 2 ? n_tiles : 148ull * 2);
     const int nw = n_wave > 0 ? n_wave : 1;
+    if (p.n_classes > RMS_SIG_SMALL_CLASSES) {
+        RMS_REQUIRE(order_by_class, RMS_ERR_ARG, "signal reduction with many classes needs the class ordering");
+        const size_t smem = (size_t)nw * 3 * SIG_TILE * sizeof(double) + SIG_TILE * (sizeof(float) + sizeof(int));
+        if (smem > 48 * 1024)
+            RMS_CUDA_TRY(cudaFuncSetAttribute(rms_signal_runs_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        const int q_batch = RED_BLOCK * SIG_QPT;
+        int q_begin = 0;
+        do {
+            const int nq_l = nq - q_begin < q_batch ? nq - q_begin : q_batch;
+            rms_signal_runs_kernel<<<grid, RED_BLOCK, smem, stream>>>(p, nw, nq_l > 0 ? nq_l : 0, q_begin, d_qv, d_qwave, order_by_class,
+                                                                      d_re, d_im, d_sum_alpha);
+            RMS_CUDA_TRY(cudaGetLastError());
+            if (n_launches) ++*n_launches;
+            q_begin += q_batch;
+        } while (q_begin < nq);
+        return RMS_OK;
+    }
     const size_t fixed = ((size_t)nw * 3 * SIG_TILE + p.n_classes) * sizeof(double) + SIG_TILE * (sizeof(float) + sizeof(int));
     const size_t budget = 160 * 1024;
     const size_t per_q = (size_t)p.n_classes * 2 * sizeof(double);

@@ -185,6 +185,8 @@ extern "C" int rms_run(const rms_substrate* s, rms_walkers* w, const rms_run_des
     const int nQ = nW * nG * nD;
     const size_t n_sig = (size_t)nQ * nC, n_mom = (size_t)nS * nD * nC, n_sal = (size_t)nS * nC, n_flow = (size_t)nS * nC * nC;
     const size_t n_res_d = 2 * n_sig + 2 * n_mom + n_sal + nC;       // doubles
+    RMS_REQUIRE(n_flow <= ((size_t)1 << 27) && n_res_d <= ((size_t)1 << 28), RMS_ERR_UNSUPPORTED,
+                "n_classes = %d with %d snapshots, %d signals: the result arrays would exceed 1-2 GB", nC, nS, nQ);
     DeviceBuf b_tabs, b_segs, b_wave, b_wsuf, b_q, b_res, b_dirs, b_order;
     RMS_CUDA_TRY(rms_malloc((void**)&b_tabs.p, tabs.size() * sizeof(float)));
     RMS_CUDA_TRY(cudaMemcpyAsync(b_tabs.p, tabs.data(), tabs.size() * sizeof(float), cudaMemcpyHostToDevice, stream));
@@ -304,7 +306,13 @@ extern "C" int rms_run(const rms_substrate* s, rms_walkers* w, const rms_run_des
         }
         a = b;
     }
-    rc = rms_launch_signal(rp, nW, nQ, b_q.as<double>(), d_qwave, d_re, d_im, d_sum_alpha, stream, &n_launches);
+    if (nC > RMS_SIG_SMALL_CLASSES) {     // many classes (per-cell outputs): the signal reduction visits the walkers class by class
+        if (!b_order.p) RMS_CUDA_TRY(rms_malloc((void**)&b_order.p, std::max<uint64_t>(n, 1) * sizeof(uint32_t)));
+        rc = rms_order_by_class(s, w, b_order.as<uint32_t>(), stream, &n_launches);
+        if (rc != RMS_OK) return rc;
+    }
+    rc = rms_launch_signal(rp, nW, nQ, b_q.as<double>(), d_qwave, d_re, d_im, d_sum_alpha, b_order.as<uint32_t>(), stream,
+                           &n_launches);
     if (rc != RMS_OK) return rc;
     RMS_CUDA_TRY(cudaEventRecord(ev_end, stream));
 

@@ -72,7 +72,42 @@ __global__ void __launch_bounds__(256) rms_cell_scatter_kernel(rms_walker_arrays
     if (i < n) order[atomicAdd(&cursor[rms_cell_of(st.w[0][i], st.w[1][i], st.w[2][i], cx, cy, cz, zfast)], 1u)] = (uint32_t)i;
 }
 
+// the same counting sort keyed on the output class of the walker's initial label (many-class signal reduction)
+__global__ void __launch_bounds__(256) rms_class_hist_kernel(rms_walker_arrays st, uint64_t n, const uint16_t* __restrict__ label_class,
+                                                              uint32_t* count)
+{
+    const uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n) atomicAdd(&count[label_class[st.lab[i] >> 16]], 1u);
+}
+
+__global__ void __launch_bounds__(256) rms_class_scatter_kernel(rms_walker_arrays st, uint64_t n, const uint16_t* __restrict__ label_class,
+                                                                 uint32_t* cursor, uint32_t* order)
+{
+    const uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n) order[atomicAdd(&cursor[label_class[st.lab[i] >> 16]], 1u)] = (uint32_t)i;
+}
+
 }  // namespace
+
+int rms_order_by_class(const rms_substrate* s, const rms_walkers* w, uint32_t* d_order, cudaStream_t stream, unsigned* n_launches)
+{
+    RMS_REQUIRE(w->n < (1ull << 32), RMS_ERR_UNSUPPORTED, "too many walkers to order");
+    uint32_t* d_count = nullptr;
+    const uint64_t n_tiles = ((uint64_t)s->n_classes + 4095) / 4096;
+    RMS_CUDA_TRY(rms_malloc((void**)&d_count, n_tiles * 4096 * sizeof(uint32_t)));
+    cudaError_t e = cudaMemsetAsync(d_count, 0, n_tiles * 4096 * sizeof(uint32_t), stream);
+    if (e == cudaSuccess) {
+        const unsigned grid = (unsigned)((w->n + 255) / 256);
+        rms_class_hist_kernel<<<grid, 256, 0, stream>>>(w->a, w->n, s->d_label_class, d_count);
+        rms_cell_scan_kernel<<<1, 1024, 0, stream>>>((uint4*)d_count, (uint32_t)n_tiles);
+        rms_class_scatter_kernel<<<grid, 256, 0, stream>>>(w->a, w->n, s->d_label_class, d_count, d_order);
+        e = cudaGetLastError();
+        if (n_launches) *n_launches += 3;
+    }
+    rms_free(d_count);
+    RMS_CUDA_TRY(e);
+    return RMS_OK;
+}
 
 int rms_order_walkers(const rms_substrate* s, const rms_walkers* w, uint32_t* d_order, cudaStream_t stream, unsigned* n_launches)
 {

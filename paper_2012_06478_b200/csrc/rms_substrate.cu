@@ -172,7 +172,7 @@ extern "C" int rms_substrate_create(const rms_substrate_desc* d, void* cuda_stre
     RMS_REQUIRE(d->labels, RMS_ERR_ARG, "labels is null");
     RMS_REQUIRE(d->voxel_um > 0, RMS_ERR_ARG, "voxel_um must be positive");
     RMS_REQUIRE(d->n_labels > 0 && d->n_labels <= 65536, RMS_ERR_ARG, "n_labels must be in 1..65536");
-    RMS_REQUIRE(d->n_classes > 0 && d->n_classes <= 256, RMS_ERR_ARG, "n_classes must be in 1..256");
+    RMS_REQUIRE(d->n_classes > 0 && d->n_classes <= 65535, RMS_ERR_ARG, "n_classes must be in 1..65535");
     RMS_REQUIRE(d->D, RMS_ERR_ARG, "D is null");
     RMS_REQUIRE(!(d->flags & RMS_ADOPT_DEVICE_PTR) || (d->flags & RMS_LABELS_ON_DEVICE), RMS_ERR_ARG,
                 "RMS_ADOPT_DEVICE_PTR needs RMS_LABELS_ON_DEVICE");
@@ -237,10 +237,10 @@ extern "C" int rms_substrate_create(const rms_substrate_desc* d, void* cuda_stre
                                 (d->flags & RMS_LABELS_ON_DEVICE) ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice, stream));
     }
     {
-        uint8_t* lc = nullptr;
-        SUB_TRY(rms_malloc((void**)&lc, nL));
+        uint16_t* lc = nullptr;
+        SUB_TRY(rms_malloc((void**)&lc, nL * sizeof(uint16_t)));
         s->d_label_class = lc;
-        SUB_TRY(cudaMemcpyAsync(lc, s->label_class.data(), nL, cudaMemcpyHostToDevice, stream));
+        SUB_TRY(cudaMemcpyAsync(lc, s->label_class.data(), nL * sizeof(uint16_t), cudaMemcpyHostToDevice, stream));
     }
     SUB_TRY(rms_malloc((void**)&d_stats, 5 * sizeof(unsigned long long)));
     SUB_TRY(cudaMemsetAsync(d_stats, 0, 5 * sizeof(unsigned long long), stream));

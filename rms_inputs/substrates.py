@@ -17,7 +17,7 @@ class Substrate:
     D: np.ndarray                      # [n_labels] float32, um^2/ms
     T2: np.ndarray                     # [n_labels] float32, ms (inf = no relaxation)
     kappa: np.ndarray                  # [n_labels, n_labels] float32, um/ms
-    label_class: np.ndarray            # [n_labels] uint8
+    label_class: np.ndarray            # [n_labels] uint16
     n_classes: int
     label_allowed: np.ndarray          # [n_labels] uint8: 1 = walkers are placed here
     meta: dict = field(default_factory=dict)
@@ -41,7 +41,7 @@ def _tables(n_labels, D_extra, D_intra, T2_extra, T2_intra, kappa_membrane, plac
     if kappa_membrane:
         kappa[0, 1:] = kappa_membrane
         kappa[1:, 0] = kappa_membrane
-    label_class = np.ones(n_labels, dtype=np.uint8)
+    label_class = np.ones(n_labels, dtype=np.uint16)
     label_class[0] = 0
     allowed = np.ones(n_labels, dtype=np.uint8)
     if place == "intra":

@@ -375,6 +375,36 @@ def test_full_length_configs_in_fp64_on_a_sample_of_walker_ids(rms, name, n_ids)
     assert rep["n_diff"] <= max(1, n_ids // 5000)
 
 
+def test_per_cell_outputs_class_equals_label(rms):
+    """S: section 8(f) N2 -- the paper reports its results per axon: class = label, so that signals and moments
+    come out per cell.  13 classes on the reduced axon substrate, 300 on a lattice of random labels; more than 8
+    classes take the class-ordered signal reduction."""
+    import dataclasses
+    cfg = ri.make_config("cfg2", "test")
+    sub = cfg.substrate
+    nL = len(sub.D)
+    per_cell = dataclasses.replace(sub, label_class=np.arange(nL, dtype=np.uint16), n_classes=nL)
+    n = cfg.n_walkers
+    g = gpu_run(per_cell, cfg.sequence, n, cfg.seed)
+    o = oracle_run(per_cell, cfg.sequence, n, cfg.seed)
+    rep = compare(g, o, n)
+    print("per-axon classes", nL, rep)
+    assert g["sig_re"].shape[-1] == nL and g["sum_alpha"][0] == 0 and np.count_nonzero(g["sum_alpha"]) >= nL - 2
+    # pooled over the classes it is the two-class run
+    g2 = gpu_run(sub, cfg.sequence, n, cfg.seed)
+    assert np.abs(g["S"] - g2["S"]).max() < 1e-9 and np.allclose(g["sig_re"].sum(-1), g2["sig_re"].sum(-1), atol=1e-6)
+    # 300 classes, walkers everywhere, two waveforms, a snapshot on the way
+    sub3 = ri.random_lattice((12, 11, 10), n_labels=300, seed=8)
+    sub3 = dataclasses.replace(sub3, label_class=np.arange(300, dtype=np.uint16), n_classes=300)
+    wave = np.stack([ri.pgse_wave(300, 100, 150), ri.pgse_wave(300, 40, 200)])
+    seq = ri.Sequence(dt_ms=2e-4, n_steps=300, wave=wave, gamp=np.array([[0.0, 25.0], [5.0, 60.0]]), dirs=ri.fibonacci_dirs(3),
+                      snap_steps=np.array([150, 300]))
+    g = gpu_run(sub3, seq, 20000, 3)
+    o = oracle_run(sub3, seq, 20000, 3)
+    print("300 classes", compare(g, o, 20000))
+    assert g["class_flow"].shape == (2, 300, 300) and g["class_flow"].sum() == 2 * 20000
+
+
 def test_gather_probe_reports_sane_ceilings(rms):
     l2 = rms.binding.rms_gather_probe(32 << 20, 4, 256)
     hbm = rms.binding.rms_gather_probe(1 << 30, 2, 128)
