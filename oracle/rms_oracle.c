@@ -73,7 +73,7 @@ void rms_oracle_philox4x32_10(const uint32_t ctr[4], const uint32_t key[2], uint
 }
 
 /* Counter layout (R2): key = (seed_lo, seed_hi); ctr = (walker_lo, walker_hi, index, stream). */
-enum { STREAM_INIT = 0, STREAM_DIR = 1, STREAM_PERM = 2, STREAM_INIT_OFFSET = 3 };
+enum { STREAM_INIT = 0, STREAM_DIR = 1, STREAM_PERM = 2, STREAM_INIT_OFFSET = 3, STREAM_MT = 4 };
 
 static void draw(uint64_t seed, uint64_t walker, uint32_t index, uint32_t stream, uint32_t out[4])
 {
@@ -120,6 +120,36 @@ static void permeation_uniforms(uint64_t seed, uint64_t walker, int64_t step, ui
     u[0] = ((double)(wa & 511u) + uni(v[0])) / 512.0;
     u[1] = ((double)(wb & 511u) + uni(v[1])) / 512.0;
     u[2] = ((double)(v[3] & 511u) + uni(v[2])) / 512.0;
+}
+
+/* Saturation (magnetisation transfer) uniforms of step i (R20): u_e = uni(m_e) for the e-th
+ * unlike-label encounter of the step, m_0..m_3 = Philox(walker, index = step, stream MT). */
+static void saturation_uniforms(uint64_t seed, uint64_t walker, int64_t step, double u[3])
+{
+    uint32_t m[4];
+    draw(seed, walker, (uint32_t)step, STREAM_MT, m);
+    u[0] = uni(m[0]); u[1] = uni(m[1]); u[2] = uni(m[2]);
+}
+
+/* Absorbing membranes / surface relaxation (Eq.4): a walker in label a that meets a
+ * membrane towards label b is saturated with probability P_MT = rho_ab ds_a / D_a C_d, the
+ * same C_d as in Eq.2a.  Rounded once to an fp32-representable value (R6). */
+int rms_oracle_mt_table(int n_labels, const float* D, const float* rho, double dt_ms, double* Q_out)
+{
+    const double C3 = 2.0 / 3.0;
+    if (n_labels <= 0 || !D || !rho || !(dt_ms > 0)) return ORC_ERR_ARG;
+    for (int a = 0; a < n_labels; ++a)
+        for (int b = 0; b < n_labels; ++b) {
+            double q = 0.0;
+            if (a != b) {
+                double r = (double)rho[a * n_labels + b];
+                if (r < 0 || r != r) return ORC_ERR_ARG;
+                q = r * sqrt(6.0 * dt_ms / (double)D[a]) * C3;
+                if (q > 1.0) return ORC_ERR_P_RANGE;
+            }
+            Q_out[a * n_labels + b] = (double)(float)q;
+        }
+    return ORC_OK;
 }
 
 /* ------------------------------------------------------------------------- */
@@ -179,6 +209,7 @@ typedef struct {
     int n_labels;
     const double* s; /* [n_labels] */
     const double* P; /* [n_labels^2] */
+    const double* Q; /* [n_labels^2] saturation probability P_MT, or NULL (no absorbing membranes) */
 } lattice_t;
 
 static int wrap(int64_t a, int n) { int64_t m = a % n; return (int)(m < 0 ? m + n : m); }
@@ -198,8 +229,18 @@ static double perm_uniform(perm_src_t* ps, int e)
     return ps->u[e < 3 ? e : 2];
 }
 
+/* saturation uniforms, drawn only when an absorbing membrane (P_MT > 0) is met */
+typedef struct { uint64_t seed, walker; int64_t step; int have; double u[3]; } mt_src_t;
+
+static double mt_uniform(mt_src_t* ms, int e)
+{
+    if (!ms->have) { saturation_uniforms(ms->seed, ms->walker, ms->step, ms->u); ms->have = 1; }
+    return ms->u[e < 3 ? e : 2];
+}
+
 static void step_core(const lattice_t* lat, int32_t vox[3], double off[3], uint16_t* label,
-                      const double u[3], perm_src_t* ps, int* n_enc, int* n_perm, int* n_clamp)
+                      const double u[3], perm_src_t* ps, mt_src_t* ms, int* saturated,
+                      int* n_enc, int* n_perm, int* n_clamp)
 {
     uint16_t L = *label;
     double r[3], p[3];
@@ -232,6 +273,10 @@ static void step_core(const lattice_t* lat, int32_t vox[3], double off[3], uint1
         } else {
             double P = lat->P[(size_t)L * lat->n_labels + Ln];
             ++*n_enc;
+            if (lat->Q && ms) { /* Eq.4: the encounter saturates the walker with probability P_MT; its walk goes on */
+                double Q = lat->Q[(size_t)L * lat->n_labels + Ln];
+                if (Q > 0.0 && mt_uniform(ms, e) < Q) *saturated = 1;
+            }
             pass = (P >= 1.0) || (P > 0.0 && perm_uniform(ps, e) < P); /* permeate with probability P */
             ++e;
             if (pass) ++*n_perm;
@@ -264,10 +309,10 @@ int rms_oracle_step(int nx, int ny, int nz, const uint16_t* labels, int n_labels
                     int32_t vox[3], double off[3], uint16_t* label, const double u[3], const double up[3],
                     int32_t counts[3])
 {
-    lattice_t lat = { nx, ny, nz, labels, n_labels, s, P };
+    lattice_t lat = { nx, ny, nz, labels, n_labels, s, P, NULL };
     int ne = 0, np = 0, nc = 0;
     perm_src_t ps = { 0, 0, 0, 0, 0, 1, { up[0], up[1], up[2] } };
-    step_core(&lat, vox, off, label, u, &ps, &ne, &np, &nc);
+    step_core(&lat, vox, off, label, u, &ps, NULL, NULL, &ne, &np, &nc);
     counts[0] = ne; counts[1] = np; counts[2] = nc;
     return ORC_OK;
 }
@@ -324,7 +369,7 @@ typedef struct {
     uint64_t w_begin, w_end; /* indices into [0, n_walkers) */
     double *sum_alpha, *sig_re, *sig_im, *m2, *m4, *snap_alpha;
     uint64_t* class_flow;
-    uint64_t counters[4];
+    uint64_t counters[5];
     int status;
 } part_t;
 
@@ -361,7 +406,10 @@ static void* run_part(void* arg)
             direction_words(j->seed, id, i, &wa, &wb);
             rms_oracle_direction(wa, wb, u);
             perm_src_t ps = { j->seed, id, i, wa, wb, 0, { 0, 0, 0 } };
-            step_core(lat, v, f, &L, u, &ps, &ne, &np, &nc);
+            mt_src_t ms = { j->seed, id, i, 0, { 0, 0, 0 } };
+            int sat = 0;
+            step_core(lat, v, f, &L, u, &ps, &ms, &sat, &ne, &np, &nc);
+            if (sat && !isinf(R)) { R = INFINITY; pt->counters[4] += 1; } /* Eq.4: alpha_rho = 0 from here on */
             pt->counters[0] += (uint64_t)ne; pt->counters[1] += (uint64_t)np; pt->counters[2] += (uint64_t)nc;
             if ((uint64_t)ne > pt->counters[3]) pt->counters[3] = (uint64_t)ne;
 
@@ -374,7 +422,7 @@ static void* run_part(void* arg)
                 for (int k = 0; k < 3; ++k) Phi[3 * m + k] += w * dx[k];
             }
             /* Eq.5: whole dt to the compartment at the end of the hop (R12) */
-            R += j->dt * j->inv_T2[L];
+            R += j->dt * j->inv_T2[L]; /* (stays +inf once saturated) */
 
             while (snap < j->n_snap && j->snap_steps[snap] == i) {
                 double alpha = exp(-R);
@@ -418,7 +466,7 @@ static void* run_part(void* arg)
 
 int rms_oracle_run(
     int nx, int ny, int nz, double voxel_um, const uint16_t* labels, int n_labels,
-    const float* D, const float* T2, const float* kappa, const uint16_t* label_class, int n_classes,
+    const float* D, const float* T2, const float* kappa, const float* rho, const uint16_t* label_class, int n_classes,
     uint64_t n_walkers, uint64_t first_id, const uint8_t* label_allowed, uint64_t seed,
     double dt_ms, int64_t n_steps, int n_wave, const float* wave, int n_g, const double* gamp,
     int n_dir, const double* dirs, int n_snap, const int64_t* snap_steps, int n_threads,
@@ -445,9 +493,11 @@ int rms_oracle_run(
     double* s_tab = (double*)malloc(sizeof(double) * n_labels);
     double* P_tab = (double*)malloc(sizeof(double) * (size_t)n_labels * n_labels);
     double* inv_T2 = (double*)malloc(sizeof(double) * n_labels);
-    if (!s_tab || !P_tab || !inv_T2) { free(s_tab); free(P_tab); free(inv_T2); return ORC_ERR_OOM; }
+    double* Q_tab = rho ? (double*)malloc(sizeof(double) * (size_t)n_labels * n_labels) : NULL;
+    if (!s_tab || !P_tab || !inv_T2 || (rho && !Q_tab)) { free(s_tab); free(P_tab); free(inv_T2); free(Q_tab); return ORC_ERR_OOM; }
     int st = rms_oracle_tables(n_labels, D, kappa, voxel_um, dt_ms, s_tab, P_tab);
-    if (st != ORC_OK) { free(s_tab); free(P_tab); free(inv_T2); return st; }
+    if (st == ORC_OK && rho) st = rms_oracle_mt_table(n_labels, D, rho, dt_ms, Q_tab);
+    if (st != ORC_OK) { free(s_tab); free(P_tab); free(inv_T2); free(Q_tab); return st; }
     for (int a = 0; a < n_labels; ++a) {
         double t2 = T2 ? (double)T2[a] : 0.0;
         inv_T2[a] = (t2 > 0.0 && !isinf(t2)) ? 1.0 / t2 : 0.0; /* T2 <= 0 or inf: no relaxation */
@@ -456,7 +506,7 @@ int rms_oracle_run(
     job_t job;
     memset(&job, 0, sizeof job);
     job.lat.nx = nx; job.lat.ny = ny; job.lat.nz = nz; job.lat.labels = labels; job.lat.n_labels = n_labels;
-    job.lat.s = s_tab; job.lat.P = P_tab;
+    job.lat.s = s_tab; job.lat.P = P_tab; job.lat.Q = Q_tab;
     job.voxel_um = voxel_um; job.inv_T2 = inv_T2; job.label_class = label_class; job.n_classes = n_classes;
     job.n_walkers = n_walkers; job.first_id = first_id; job.seed = seed; job.label_allowed = label_allowed;
     job.dt = dt_ms; job.n_steps = n_steps; job.n_wave = n_wave; job.wave = wave; job.n_g = n_g; job.gamp = gamp;
@@ -497,7 +547,7 @@ int rms_oracle_run(
         if (m4) memset(m4, 0, sizeof(double) * n_mom(&job));
         if (snap_alpha) memset(snap_alpha, 0, sizeof(double) * n_sal(&job));
         if (class_flow) memset(class_flow, 0, sizeof(uint64_t) * n_flow(&job));
-        memset(counters, 0, sizeof(uint64_t) * 4);
+        memset(counters, 0, sizeof(uint64_t) * 5);
         for (int t = 0; t < n_threads; ++t) { /* partial sums added in walker order */
             part_t* p = &parts[t];
             if (p->status != ORC_OK) status = p->status;
@@ -510,6 +560,7 @@ int rms_oracle_run(
             if (class_flow) for (size_t i = 0; i < n_flow(&job); ++i) class_flow[i] += p->class_flow[i];
             counters[0] += p->counters[0]; counters[1] += p->counters[1]; counters[2] += p->counters[2];
             if (p->counters[3] > counters[3]) counters[3] = p->counters[3];
+            counters[4] += p->counters[4];
         }
     }
 done:
@@ -517,6 +568,6 @@ done:
         free(parts[t].sum_alpha); free(parts[t].sig_re); free(parts[t].sig_im); free(parts[t].m2);
         free(parts[t].m4); free(parts[t].snap_alpha); free(parts[t].class_flow);
     }
-    free(parts); free(tids); free(s_tab); free(P_tab); free(inv_T2);
+    free(parts); free(tids); free(s_tab); free(P_tab); free(inv_T2); free(Q_tab);
     return status;
 }

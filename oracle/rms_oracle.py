@@ -146,6 +146,8 @@ def run(sub, seq, n_walkers, seed, first_id=0, n_threads=1, per_walker=False):
     D = np.ascontiguousarray(sub.D, np.float32)
     T2 = np.ascontiguousarray(sub.T2, np.float32)
     kappa = np.ascontiguousarray(sub.kappa, np.float32)
+    rho = getattr(sub, "rho", None)
+    rho = None if rho is None else np.ascontiguousarray(rho, np.float32)
     lclass = np.ascontiguousarray(sub.label_class, np.uint16)
     allowed = np.ascontiguousarray(sub.label_allowed, np.uint8)
     wave = np.ascontiguousarray(seq.wave, np.float32)
@@ -159,7 +161,7 @@ def run(sub, seq, n_walkers, seed, first_id=0, n_threads=1, per_walker=False):
         sum_alpha=np.zeros(nC), sig_re=np.zeros((n_wave, n_g, n_dir, nC)), sig_im=np.zeros((n_wave, n_g, n_dir, nC)),
         m2=np.zeros((n_snap, n_dir, nC)), m4=np.zeros((n_snap, n_dir, nC)), snap_alpha=np.zeros((n_snap, nC)),
         class_flow=np.zeros((n_snap, nC, nC), np.uint64))
-    counters = np.zeros(4, np.uint64)
+    counters = np.zeros(8, np.uint64)
     pw = {}
     if per_walker:
         pw = dict(final_vox=np.zeros((n_walkers, 3), np.int32), final_off=np.zeros((n_walkers, 3)),
@@ -168,7 +170,7 @@ def run(sub, seq, n_walkers, seed, first_id=0, n_threads=1, per_walker=False):
                   relax=np.zeros(n_walkers))
     st = lib.rms_oracle_run(
         C.c_int(nx), C.c_int(ny), C.c_int(nz), C.c_double(sub.voxel_um), _p(labels, C.c_uint16), C.c_int(nL),
-        _p(D, C.c_float), _p(T2, C.c_float), _p(kappa, C.c_float), _p(lclass, C.c_uint16), C.c_int(nC),
+        _p(D, C.c_float), _p(T2, C.c_float), _p(kappa, C.c_float), _p(rho, C.c_float), _p(lclass, C.c_uint16), C.c_int(nC),
         C.c_uint64(n_walkers), C.c_uint64(first_id), _p(allowed, C.c_uint8), C.c_uint64(seed),
         C.c_double(seq.dt_ms), C.c_int64(n_steps), C.c_int(n_wave), _p(wave, C.c_float), C.c_int(n_g),
         _p(gamp, C.c_double), C.c_int(n_dir), _p(dirs, C.c_double), C.c_int(n_snap), _p(snaps, C.c_int64),
@@ -183,7 +185,7 @@ def run(sub, seq, n_walkers, seed, first_id=0, n_threads=1, per_walker=False):
         raise OracleError(st)
     r.update(pw)
     r.update(n_encounters=int(counters[0]), n_permeations=int(counters[1]), n_clamps=int(counters[2]),
-             max_encounters_per_step=int(counters[3]))
+             max_encounters_per_step=int(counters[3]), n_saturations=int(counters[4]))
     return normalise(r, seq.dt_ms, snaps)
 
 

@@ -21,6 +21,7 @@ class Substrate:
     n_classes: int
     label_allowed: np.ndarray          # [n_labels] uint8: 1 = walkers are placed here
     meta: dict = field(default_factory=dict)
+    rho: np.ndarray | None = None      # [n_labels, n_labels] float32, um/ms: surface relaxivity (absorbing membranes), or None
 
     @property
     def n_labels(self) -> int:
