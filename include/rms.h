@@ -53,6 +53,9 @@ typedef struct rms_walkers rms_walkers;     /* opaque */
  * T2           [n_labels] ms; +inf or <= 0 means no relaxation; NULL = none (host; Eq.5)
  * kappa        [n_labels*n_labels] membrane permeability um/ms between label pairs, symmetric, diagonal
  *              ignored; 0 = impermeable; +inf = no membrane (Eq.C.15 with c1 = c2); NULL = all 0 (host; Eq.3)
+ * rho          [n_labels*n_labels] surface relaxivity um/ms of the membrane met by a walker in label a towards label b
+ *              (absorbing membrane / magnetisation transfer): the encounter saturates the walker
+ *              (alpha_rho = 0, Eq.4) with probability rho_ab ds_a / D_a C_d; NULL = none (host)
  * label_class  [n_labels] uint16 output compartment class of each label, < n_classes <= 65535; NULL = all 0 (host).
  *              Two classes (extra / intra-cellular) are the usual choice; class = label gives per-cell outputs.
  * flags        RMS_LABELS_ON_DEVICE | RMS_ADOPT_DEVICE_PTR | RMS_NO_BRICKS | RMS_LAYOUT_X_FASTEST | RMS_LAYOUT_Z_FASTEST | RMS_LAYOUT_AUTO
@@ -78,6 +81,7 @@ typedef struct {
     const float* D;
     const float* T2;
     const float* kappa;
+    const float* rho;
     const uint16_t* label_class;
     int32_t n_classes;
     uint32_t flags;
@@ -181,6 +185,7 @@ typedef struct {
     double* Dapp;
     double* Kapp;
     uint64_t n_encounters, n_permeations, n_clamps; /* written by rms_run */
+    uint64_t n_saturations;     /* walkers saturated at absorbing membranes during this call (Eq.4)   */
     double kernel_ms;           /* device time of the step kernels of this call (CUDA events)          */
     double total_ms;            /* device time of everything this call enqueued                         */
     uint32_t n_launches;        /* kernels launched by this call                                        */

@@ -11,7 +11,7 @@ import numpy as np
 from . import binding as B
 
 RAW_SUMS = ("sum_alpha", "sig_re", "sig_im", "m2", "m4", "snap_alpha", "class_flow")
-COUNTERS = ("n_encounters", "n_permeations", "n_clamps")
+COUNTERS = ("n_encounters", "n_permeations", "n_clamps", "n_saturations")
 
 
 def shard_range(rank: int, world: int, n_walkers: int):
@@ -30,7 +30,7 @@ def simulate(sub, seq, n_walkers, seed, first_id=0, flags=0, substrate_flags=0, 
     """
     labels = device_labels if device_labels is not None else sub.labels
     S = B.rms_substrate_create(labels, sub.voxel_um, sub.D, sub.T2, sub.kappa, sub.label_class, sub.n_classes,
-                               flags=substrate_flags, stream=stream)
+                               flags=substrate_flags, stream=stream, rho=getattr(sub, "rho", None))
     W = None
     try:
         W = B.rms_walkers_init(S, n_walkers, first_id, sub.label_allowed, seed, stream=stream)

@@ -44,7 +44,7 @@ class RmsError(RuntimeError):
 class SubstrateDesc(C.Structure):
     _fields_ = [("nx", C.c_int32), ("ny", C.c_int32), ("nz", C.c_int32), ("voxel_um", C.c_double),
                 ("labels", C.c_void_p), ("n_labels", C.c_int32), ("D", C.c_void_p), ("T2", C.c_void_p),
-                ("kappa", C.c_void_p), ("label_class", C.c_void_p), ("n_classes", C.c_int32), ("flags", C.c_uint32)]
+                ("kappa", C.c_void_p), ("rho", C.c_void_p), ("label_class", C.c_void_p), ("n_classes", C.c_int32), ("flags", C.c_uint32)]
 
 
 class SubstrateInfo(C.Structure):
@@ -63,7 +63,7 @@ class Result(C.Structure):
     _fields_ = [("sum_alpha", C.c_void_p), ("sig_re", C.c_void_p), ("sig_im", C.c_void_p), ("m2", C.c_void_p),
                 ("m4", C.c_void_p), ("snap_alpha", C.c_void_p), ("class_flow", C.c_void_p), ("S_re", C.c_void_p),
                 ("S_im", C.c_void_p), ("Dapp", C.c_void_p), ("Kapp", C.c_void_p), ("n_encounters", C.c_uint64),
-                ("n_permeations", C.c_uint64), ("n_clamps", C.c_uint64), ("kernel_ms", C.c_double),
+                ("n_permeations", C.c_uint64), ("n_clamps", C.c_uint64), ("n_saturations", C.c_uint64), ("kernel_ms", C.c_double),
                 ("total_ms", C.c_double), ("n_launches", C.c_uint32)]
 
 
@@ -150,7 +150,7 @@ class Substrate:
 
 
 def rms_substrate_create(labels, voxel_um, D, T2=None, kappa=None, label_class=None, n_classes=1, flags=0,
-                         stream=None) -> Substrate:
+                         stream=None, rho=None) -> Substrate:
     """labels: numpy uint16 (nz, ny, nx) on the host, or a torch.uint16/int16 CUDA tensor of that shape
     (then the lattice is adopted in place, no copy)."""
     lib = load_library()
@@ -171,7 +171,8 @@ def rms_substrate_create(labels, voxel_um, D, T2=None, kappa=None, label_class=N
     T2 = _host(T2, np.float32)
     kappa = _host(kappa, np.float32)
     label_class = _host(label_class, np.uint16)
-    d = SubstrateDesc(nx, ny, nz, float(voxel_um), lab_ptr, int(D.size), _ptr(D), _ptr(T2), _ptr(kappa), _ptr(label_class),
+    rho = _host(rho, np.float32)
+    d = SubstrateDesc(nx, ny, nz, float(voxel_um), lab_ptr, int(D.size), _ptr(D), _ptr(T2), _ptr(kappa), _ptr(rho), _ptr(label_class),
                       int(n_classes), int(flags))
     h = C.c_void_p()
     _check(lib.rms_substrate_create(C.byref(d), _stream_ptr(stream), C.byref(h)))
@@ -243,6 +244,7 @@ def rms_run(substrate: Substrate, walkers: Walkers, dt_ms, n_steps, wave=None, g
         setattr(res, k, r[k].ctypes.data)
     _check(load_library().rms_run(substrate.handle, walkers.handle, C.byref(d), _stream_ptr(stream), C.byref(res)))
     r.update(n_encounters=int(res.n_encounters), n_permeations=int(res.n_permeations), n_clamps=int(res.n_clamps),
+             n_saturations=int(res.n_saturations),
              kernel_ms=float(res.kernel_ms), total_ms=float(res.total_ms), n_launches=int(res.n_launches))
     r["S"] = r["S_re"] + 1j * r["S_im"]
     return r

@@ -62,6 +62,7 @@ struct rms_substrate {
     int NX = 0, NY = 0, NZ = 0;          // padded dims (n + 2)
     uint64_t n_membrane_faces = 0;
     std::vector<float> D, T2, kappa;     // host copies of the per-label tables
+    std::vector<float> rho;              // surface relaxivity per label pair (absorbing membranes, Eq.4); empty = none
     std::vector<uint16_t> label_class;
     uint16_t* d_label_class = nullptr;
     bool all_impermeable = true;         // every off-diagonal kappa is 0
@@ -94,7 +95,7 @@ struct rms_walkers {
 // ------------------------------------------------------------------------------------------------
 // random numbers: Philox4x32-10, key = (seed_lo, seed_hi), counter = (walker_lo, walker_hi, index, stream)
 // ------------------------------------------------------------------------------------------------
-enum { RMS_STREAM_INIT = 0, RMS_STREAM_DIR = 1, RMS_STREAM_PERM = 2, RMS_STREAM_INIT_OFFSET = 3 };
+enum { RMS_STREAM_INIT = 0, RMS_STREAM_DIR = 1, RMS_STREAM_PERM = 2, RMS_STREAM_INIT_OFFSET = 3, RMS_STREAM_MT = 4 };
 
 #define RMS_PHILOX_M0 0xD2511F53u
 #define RMS_PHILOX_M1 0xCD9E8D57u
@@ -176,6 +177,7 @@ struct rms_step_params {
     rms_philox_keys rk;
     const float* s_tab;       // [n_labels] hop length in voxels
     const float* P512;        // [n_labels^2] 512 * P(a->b)
+    const float* PMT;         // [n_labels^2] saturation probability at an encounter a -> b (Eq.4, R20), or NULL
     const float* rate;        // [n_labels] dt / T2
     int n_labels;
     uint32_t t_ceil;          // ceil(512 max P(a->b)) over the membranes: coarse random bits at or above it cannot permeate
@@ -190,7 +192,7 @@ struct rms_step_params {
     double wsuf_end[RMS_MAX_WAVES];  // suffix sum just after the last step of this launch
     double wtot[RMS_MAX_WAVES];      // sum of w over the steps of this launch
     int n_wave;
-    unsigned long long* counters;    // [0] encounters [1] permeations [2] clamps [3] init failures
+    unsigned long long* counters;    // [0] encounters [1] permeations [2] clamps [3] init failures [4] saturations
     const uint32_t* order;           // thread t works on walker order[t] (spatially sorted, rms_sched.cu); NULL = identity
 };
 

@@ -99,10 +99,19 @@ extern "C" int rms_run(const rms_substrate* s, rms_walkers* w, const rms_run_des
     std::vector<float> s_tab, P_tab;
     int rc = rms_compute_tables(s, d->dt_ms, s_tab, P_tab);
     if (rc != RMS_OK) return rc;
-    std::vector<float> tabs((size_t)nL * 2 + (size_t)nL * nL);
+    const bool mt = !s->rho.empty();             // absorbing membranes (Eq.4)
+    std::vector<float> tabs((size_t)nL * 2 + (size_t)nL * nL * (mt ? 2 : 1));
     float* h_s = tabs.data();
     float* h_rate = h_s + nL;
     float* h_P512 = h_rate + nL;
+    float* h_PMT = h_P512 + (size_t)nL * nL;
+    if (mt)       // P_MT(a->b) = rho_ab ds_a / D_a C_d, C_3 = 2/3 (R20), fp64 then rounded once to fp32 (R6)
+        for (int a = 0; a < nL; ++a)
+            for (int b = 0; b < nL; ++b) {
+                const double q = a == b ? 0.0 : (double)s->rho[(size_t)a * nL + b] * sqrt(6.0 * d->dt_ms / (double)s->D[a]) * (2.0 / 3.0);
+                RMS_REQUIRE(q <= 1.0, RMS_ERR_P_RANGE, "P_MT = %.4g > 1 from label %d towards %d: lower rho or dt", q, a, b);
+                h_PMT[(size_t)a * nL + b] = (float)q;
+            }
     bool permeable = false;
     for (int a = 0; a < nL; ++a) {
         h_s[a] = s_tab[a];
@@ -114,6 +123,7 @@ extern "C" int rms_run(const rms_substrate* s, rms_walkers* w, const rms_run_des
         }
     }
     const bool want_labels = (d->flags & RMS_RUN_LABEL_GATHER) != 0;
+    if (mt) permeable = true;                    // absorbing membranes are handled where labels are read: the general kernels
     const int lat = (!permeable && s->d_nbr && !want_labels) ? RMS_LAT_FACES : RMS_LAT_LABELS;
     // permeable runs with P << 1 also take the specialised kernel: ceil(512 P_max) bounds the coarse random
     // bits that can permeate at all (rms_step_fast.cu)
@@ -122,7 +132,7 @@ extern "C" int rms_run(const rms_substrate* s, rms_walkers* w, const rms_run_des
         for (int b = 0; b < nL; ++b)
             if (a != b) t_max = std::max(t_max, h_P512[(size_t)a * nL + b]);
     const uint32_t t_ceil = (uint32_t)ceilf(t_max);
-    const bool fast_permeable = permeable && s->d_nbr && !want_labels && t_ceil <= 64u;
+    const bool fast_permeable = permeable && !mt && s->d_nbr && !want_labels && t_ceil <= 64u;
 
     const int nWk = rms_kernel_waves(nW);        // waveforms the step kernel is compiled for; the extra ones carry zero weight
     rc = rms_walkers_reserve_waves(w, nWk, stream);
@@ -244,6 +254,7 @@ extern "C" int rms_run(const rms_substrate* s, rms_walkers* w, const rms_run_des
     sp.labels = s->d_labels; sp.nbr = s->d_nbr; sp.NX = s->NX; sp.NY = s->NY; sp.SX = s->SX; sp.SY = s->SY; sp.SZ = s->SZ;
     sp.st = w->a; sp.n = n; sp.first_id = w->first_id; sp.rk = rms_make_keys(w->seed);
     sp.s_tab = b_tabs.as<float>(); sp.rate = sp.s_tab + nL; sp.P512 = sp.rate + nL; sp.n_labels = nL;
+    sp.PMT = mt ? sp.P512 + (size_t)nL * nL : nullptr;
     sp.t_ceil = t_ceil;
     sp.counters = w->d_counters; sp.n_wave = nW; sp.wave_stride = nT; sp.wsuf_stride = nT + 1;
 
@@ -348,6 +359,7 @@ extern "C" int rms_run(const rms_substrate* s, rms_walkers* w, const rms_run_des
     out->n_encounters = h_cnt[0];
     out->n_permeations = h_cnt[1];
     out->n_clamps = h_cnt[2];
+    out->n_saturations = h_cnt[4];
     float ms = 0.f, tot = 0.f;
     for (auto& pr : step_ev) { float t1 = 0.f; cudaEventElapsedTime(&t1, pr.first, pr.second); ms += t1; }
     cudaEventElapsedTime(&tot, ev_begin, ev_end);

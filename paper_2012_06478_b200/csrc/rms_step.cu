@@ -115,7 +115,7 @@ __global__ void __launch_bounds__(RMS_BLOCK) rms_step_kernel(const __grid_consta
 #pragma unroll
         for (int k = 0; k < 3; ++k) { phiF[m][k] = 0.f; A32[m][k] = 0; Ad[m][k] = 0.0; }
 
-    unsigned n_enc = 0, n_perm = 0, n_clamp = 0;
+    unsigned n_enc = 0, n_perm = 0, n_clamp = 0, n_sat = 0;
 
     uint32_t j = p.step0;                       // steps done so far (absolute)
     const uint32_t j_launch_end = p.step0 + p.n_steps;
@@ -242,10 +242,12 @@ __global__ void __launch_bounds__(RMS_BLOCK) rms_step_kernel(const __grid_consta
                     } else {
                         // ---------------- permeable / variable D: the interaction loop written out (LABELS only) ----
                         float px = fx, py = fy, pz = fz;
-                        bool dx = false, dy = false, dz = false;
+                        bool dx = false, dy = false, dz = false, saturated = false;
                         int e = 0;
                         uint32_t v0 = 0, v1 = 0, v2 = 0, v3 = 0;
                         bool have_v = false;
+                        uint32_t m0 = 0, m1 = 0, m2 = 0, m3 = 0;
+                        bool have_m = false;
 #pragma unroll 1
                         for (int it = 0; it < 3; ++it) {
                             const float gx = px + rx, gy = py + ry, gz = pz + rz;
@@ -270,6 +272,16 @@ __global__ void __launch_bounds__(RMS_BLOCK) rms_step_kernel(const __grid_consta
                             bool pass = true;
                             if (Ln != L) {
                                 ++n_enc;
+                                if (p.PMT) {   // absorbing membrane (Eq.4, R20): the encounter saturates the walker with P_MT
+                                    const float Q = __ldg(p.PMT + (size_t)L * p.n_labels + Ln);
+                                    if (Q > 0.f) {
+                                        if (!have_m) {
+                                            rms_philox(p.rk, id_lo, id_hi, j + 1u, RMS_STREAM_MT, m0, m1, m2, m3);
+                                            have_m = true;
+                                        }
+                                        if (rms_uni(e == 0 ? m0 : (e == 1 ? m1 : m2)) < Q) saturated = true;
+                                    }
+                                }
                                 const float T = __ldg(p.P512 + (size_t)L * p.n_labels + Ln);   // 512 P
                                 if (T >= 512.f) {
                                     pass = true;
@@ -344,6 +356,10 @@ __global__ void __launch_bounds__(RMS_BLOCK) rms_step_kernel(const __grid_consta
                         fy = fminf(fmaxf(gy, 0.f), RMS_ONE_MINUS);
                         fz = fminf(fmaxf(gz, 0.f), RMS_ONE_MINUS);
                         n_clamp += (fx != gx) + (fy != gy) + (fz != gz);
+                        if (saturated && relax != RMS_INF) {   // alpha_rho = 0 from here on (Eq.4); the walk goes on
+                            relax = RMS_INF;
+                            ++n_sat;
+                        }
                     }
 
                     // ---------------- phase: fractional part, Phi_F += w f (the integer part is event driven) ----
@@ -401,10 +417,12 @@ __global__ void __launch_bounds__(RMS_BLOCK) rms_step_kernel(const __grid_consta
     n_enc = __reduce_add_sync(mask, n_enc);
     n_perm = __reduce_add_sync(mask, n_perm);
     n_clamp = __reduce_add_sync(mask, n_clamp);
+    n_sat = __reduce_add_sync(mask, n_sat);
     if ((threadIdx.x & 31) == (unsigned)(__ffs(mask) - 1)) {
         if (n_enc) atomicAdd(&p.counters[0], (unsigned long long)n_enc);
         if (n_perm) atomicAdd(&p.counters[1], (unsigned long long)n_perm);
         if (n_clamp) atomicAdd(&p.counters[2], (unsigned long long)n_clamp);
+        if (n_sat) atomicAdd(&p.counters[4], (unsigned long long)n_sat);
     }
 }
 

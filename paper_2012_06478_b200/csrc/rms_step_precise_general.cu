@@ -31,6 +31,7 @@ __global__ void __launch_bounds__(RMS_GBLOCK) rms_step_precise_general_kernel(co
     double s = (double)p.s_tab[L];
     double rate = (double)p.rate[L];
     double relax = 0.0;                      // added to the stored fp32 exponent at the end
+    bool dead = isinf(p.st.relax[i]);        // saturated in an earlier launch (Eq.4)
 
     if (NW > 0) {
 #pragma unroll
@@ -49,7 +50,7 @@ __global__ void __launch_bounds__(RMS_GBLOCK) rms_step_precise_general_kernel(co
     for (int m = 0; m < NWA; ++m)
 #pragma unroll
         for (int k = 0; k < 3; ++k) { phiD[m][k] = 0.0; Ad[m][k] = 0.0; }
-    unsigned n_enc = 0, n_perm = 0, n_clamp = 0;
+    unsigned n_enc = 0, n_perm = 0, n_clamp = 0, n_sat = 0;
     const double PI = 3.14159265358979323846;
 
 #pragma unroll 1
@@ -73,6 +74,8 @@ __global__ void __launch_bounds__(RMS_GBLOCK) rms_step_precise_general_kernel(co
         int e = 0;
         uint32_t v0 = 0, v1 = 0, v2 = 0, v3 = 0;
         bool have_v = false;
+        uint32_t m0 = 0, m1 = 0, m2 = 0, m3 = 0;
+        bool have_m = false, saturated = false;
 #pragma unroll 1
         for (int it = 0; it < 3; ++it) {
             const double gx = px + rx, gy = py + ry, gz = pz + rz;
@@ -98,6 +101,13 @@ __global__ void __launch_bounds__(RMS_GBLOCK) rms_step_precise_general_kernel(co
             bool pass = true;
             if (Ln != L) {                                                     // a membrane
                 ++n_enc;
+                if (p.PMT) {   // absorbing membrane (Eq.4, R20): the encounter saturates the walker with probability P_MT
+                    const float Q = __ldg(p.PMT + (size_t)L * p.n_labels + Ln);
+                    if (Q > 0.f) {
+                        if (!have_m) { rms_philox(p.rk, id_lo, id_hi, j + 1u, RMS_STREAM_MT, m0, m1, m2, m3); have_m = true; }
+                        if (rms_uni(e == 0 ? m0 : (e == 1 ? m1 : m2)) < Q) saturated = true;
+                    }
+                }
                 const float T = __ldg(p.P512 + (size_t)L * p.n_labels + Ln);   // 512 P(L -> Ln), Eq.3
                 if (T >= 512.f) pass = true;
                 else if (T <= 0.f) pass = false;
@@ -145,6 +155,11 @@ __global__ void __launch_bounds__(RMS_GBLOCK) rms_step_precise_general_kernel(co
         fx = fmin(fmax(gx, 0.0), one_minus); fy = fmin(fmax(gy, 0.0), one_minus); fz = fmin(fmax(gz, 0.0), one_minus);
         n_clamp += (fx != gx) + (fy != gy) + (fz != gz);
         relax += rate;                                                        // whole dt to the label at the end of the hop (R12)
+        if (saturated && !dead) {                                             // alpha_rho = 0 from here on (Eq.4); the walk goes on
+            relax = __longlong_as_double(0x7ff0000000000000ll);
+            dead = true;
+            ++n_sat;
+        }
 #pragma unroll
         for (int m = 0; m < NW; ++m) {
             phiD[m][0] = fma(w_now[m], fx, phiD[m][0]);
@@ -171,10 +186,12 @@ __global__ void __launch_bounds__(RMS_GBLOCK) rms_step_precise_general_kernel(co
     n_enc = __reduce_add_sync(mask, n_enc);
     n_perm = __reduce_add_sync(mask, n_perm);
     n_clamp = __reduce_add_sync(mask, n_clamp);
+    n_sat = __reduce_add_sync(mask, n_sat);
     if ((threadIdx.x & 31) == (unsigned)(__ffs(mask) - 1)) {
         if (n_enc) atomicAdd(&p.counters[0], (unsigned long long)n_enc);
         if (n_perm) atomicAdd(&p.counters[1], (unsigned long long)n_perm);
         if (n_clamp) atomicAdd(&p.counters[2], (unsigned long long)n_clamp);
+        if (n_sat) atomicAdd(&p.counters[4], (unsigned long long)n_sat);
     }
 }
 

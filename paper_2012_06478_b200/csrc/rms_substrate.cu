@@ -196,6 +196,13 @@ extern "C" int rms_substrate_create(const rms_substrate_desc* d, void* cuda_stre
             }
     }
 
+    bool any_rho = false;
+    if (d->rho)
+        for (size_t i = 0; i < (size_t)nL * nL; ++i) {
+            RMS_REQUIRE(d->rho[i] >= 0 && d->rho[i] == d->rho[i], RMS_ERR_ARG, "rho[%zu] is negative or NaN", i);
+            any_rho |= (i / nL != i % nL) && d->rho[i] > 0;
+        }
+
     int dev_count = 0;
     cudaError_t ce = cudaGetDeviceCount(&dev_count);
     RMS_REQUIRE(ce == cudaSuccess && dev_count > 0, RMS_ERR_CUDA, "no CUDA device: %s (there is no CPU fallback)",
@@ -210,6 +217,7 @@ extern "C" int rms_substrate_create(const rms_substrate_desc* d, void* cuda_stre
     if (d->T2) s->T2.assign(d->T2, d->T2 + nL); else s->T2.assign(nL, INFINITY);
     if (d->kappa) s->kappa.assign(d->kappa, d->kappa + (size_t)nL * nL); else s->kappa.assign((size_t)nL * nL, 0.f);
     if (d->label_class) s->label_class.assign(d->label_class, d->label_class + nL); else s->label_class.assign(nL, 0);
+    if (any_rho) s->rho.assign(d->rho, d->rho + (size_t)nL * nL);
     s->all_impermeable = all_imp;
 
     int rc = RMS_OK;

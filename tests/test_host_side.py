@@ -88,7 +88,7 @@ def _fake_result(rank, nC=2, nW=1, nG=3, nD=4, nS=2):
     return dict(sum_alpha=rng.uniform(5, 6, nC), sig_re=rng.normal(size=(nW, nG, nD, nC)), sig_im=rng.normal(size=(nW, nG, nD, nC)),
                 m2=rng.uniform(1, 2, (nS, nD, nC)), m4=rng.uniform(3, 9, (nS, nD, nC)), snap_alpha=rng.uniform(5, 6, (nS, nC)),
                 class_flow=rng.integers(0, 1000, (nS, nC, nC)).astype(np.uint64), n_encounters=10 + rank, n_permeations=rank,
-                n_clamps=0)
+                n_clamps=0, n_saturations=3 * rank)
 
 
 def _worker(rank, world, port, out_dir):
@@ -117,4 +117,4 @@ def test_allreduce_of_two_shards_over_gloo_equals_the_merged_job(rms, tmp_path):
         for k in ("sum_alpha", "sig_re", "sig_im", "m2", "m4", "snap_alpha", "S", "Dapp", "Kapp"):
             assert np.allclose(got[k], ref[k], rtol=1e-13), k
         assert np.array_equal(got["class_flow"], ref["class_flow"])
-        assert int(got["n_encounters"]) == 21 and int(got["n_permeations"]) == 1
+        assert int(got["n_encounters"]) == 21 and int(got["n_permeations"]) == 1 and int(got["n_saturations"]) == 3
