@@ -438,6 +438,38 @@ def test_absorbing_membranes_magnetisation_transfer(rms):
     assert e.value.code == -3          # RMS_ERR_P_RANGE: P_MT > 1
 
 
+def test_degenerate_and_ragged_cases(rms):
+    # one walker; 1, 2, 3 steps with a snapshot on every step; no waveform / no directions; hop of 0.99 voxel (three
+    # interactions in most steps); a single-voxel pore (every face a membrane: the corner reflector of Fig.2)
+    sub = ri.single_cylinder(16, 5.5, 0.1)
+    for n_steps in (1, 2, 3):
+        seq = ri.Sequence(dt_ms=2e-4, n_steps=n_steps, wave=np.ones((1, n_steps), np.float32), gamp=np.array([[0.0, 300.0]]),
+                          dirs=np.eye(3), snap_steps=np.arange(1, n_steps + 1))
+        for n in (1, 129):
+            print("steps", n_steps, "walkers", n, compare(gpu_run(sub, seq, n, 3), oracle_run(sub, seq, n, 3), n))
+    seq0 = ri.Sequence(dt_ms=2e-4, n_steps=200, wave=np.zeros((0, 200), np.float32), gamp=np.zeros((0, 0)), dirs=np.eye(3),
+                       snap_steps=np.array([100, 200]))
+    g, o = gpu_run(sub, seq0, 3000, 4), oracle_run(sub, seq0, 3000, 4)
+    print("no waveform", compare(g, o, 3000))
+    assert g["S"].size == 0 and g["m2"].shape == (2, 3, 2)
+    seq1 = ri.Sequence(dt_ms=2e-4, n_steps=200, wave=ri.pgse_wave(200, 50, 100)[None], gamp=np.array([[0.0, 50.0]]),
+                       dirs=np.zeros((0, 3)), snap_steps=np.zeros(0, np.int64))
+    g, o = gpu_run(sub, seq1, 3000, 4), oracle_run(sub, seq1, 3000, 4)
+    print("no directions", compare(g, o, 3000))
+    # hop length 0.99 voxel: D = 0.99^2 l_p^2 / (6 dt)
+    big = ri.random_lattice((6, 5, 7), n_labels=2, seed=5, D_extra=0.99 ** 2 * 0.01 / (6 * 2e-4), D_intra=0.99 ** 2 * 0.01 / (6 * 2e-4))
+    seq = ri.pgse_sequence(2e-4, 300, 0.02, 0.03, [0.0, 20.0], np.eye(3), snap_steps=[300])
+    for flags in (0, 2, 8):
+        print("hop 0.99 voxel, flags", flags, compare(gpu_run(big, seq, 4000, 6, flags=flags), oracle_run(big, seq, 4000, 6), 4000))
+    lab = np.zeros((3, 3, 3), np.uint16); lab[1, 1, 1] = 1
+    pore = ri.Substrate(labels=lab, voxel_um=0.1, D=np.array([2.0, 2.0], np.float32), T2=np.array([np.inf, np.inf], np.float32),
+                        kappa=np.zeros((2, 2), np.float32), label_class=np.array([0, 1], np.uint16), n_classes=2,
+                        label_allowed=np.array([0, 1], np.uint8))
+    g, o = gpu_run(pore, seq, 2000, 8), oracle_run(pore, seq, 2000, 8)
+    print("single-voxel pore", compare(g, o, 2000))
+    assert np.all(g["walkers"]["vox"] == 1) and g["n_encounters"] > 2000 * 300 * 0.5
+
+
 def test_gather_probe_reports_sane_ceilings(rms):
     l2 = rms.binding.rms_gather_probe(32 << 20, 4, 256)
     hbm = rms.binding.rms_gather_probe(1 << 30, 2, 128)
