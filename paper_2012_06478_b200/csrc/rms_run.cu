@@ -298,9 +298,9 @@ extern "C" int rms_run(const rms_substrate* s, rms_walkers* w, const rms_run_des
             const bool special = !permeable && lat == RMS_LAT_FACES && wmode == RMS_WMODE_CONST;
             const bool special_perm = fast_permeable && wmode == RMS_WMODE_CONST;
             if (fp64)
-                rc = special ? rms_launch_step_precise(sp, nWk, stream) : rms_launch_step_precise_general(sp, nWk, stream);
+                rc = special ? rms_launch_step_precise(sp, nW, stream) : rms_launch_step_precise_general(sp, nWk, stream);
             else if ((special || special_perm) && !(d->flags & RMS_RUN_GENERAL_KERNEL))
-                rc = rms_launch_step_fast(sp, nWk, permeable, stream);
+                rc = rms_launch_step_fast(sp, nW, permeable, stream);
             else
                 rc = rms_launch_step(sp, nWk, wmode, lat, permeable, stream);
             if (rc != RMS_OK) return rc;

@@ -25,7 +25,7 @@
 #ifndef RMS_FMINB
 #define RMS_FMINB 8                  // resident blocks per SM the register allocation is held to
 #endif
-#define RMS_FFLUSH 1024u             // steps between flushes of the fp32 / int32 phase partial sums into fp64 (even)
+#define RMS_FCHUNK 512u              // steps per chunk of the phase sums (even; 512 keeps the packed event sums inside int32)
 #define RMS_ONE_MINUS 0.99999994f    // 1 - 2^-24
 
 namespace {
@@ -171,8 +171,8 @@ __device__ __noinline__ void rms_permeable_step(const rms_step_params* pp, uint3
 
 }  // namespace
 
-template <int NW, bool XFAST, bool PERM>
-__global__ void __launch_bounds__(RMS_FBLOCK, (NW <= 4 ? RMS_FMINB : (NW <= 8 ? 4 : 2))) rms_step_fast_kernel(const __grid_constant__ rms_step_params p)
+template <bool XFAST, bool PERM>
+__global__ void __launch_bounds__(RMS_FBLOCK, RMS_FMINB) rms_step_fast_kernel(const __grid_constant__ rms_step_params p)
 {
     __shared__ float2 sm_trig[256];   // (cos, sin) of the centre of the 256 azimuth bins
 
@@ -210,35 +210,23 @@ __global__ void __launch_bounds__(RMS_FBLOCK, (NW <= 4 ? RMS_FMINB : (NW <= 8 ? 
     unsigned n_perm = 0;
     const uint32_t t_ceil = PERM ? p.t_ceil : 0u;   // permeation needs coarse bits below ceil(512 P_max)
 
-    // launch prologue of the phase: Phi += (dI - f0) * sum_{launch} w
-    if (NW > 0) {
-#pragma unroll
-        for (int m = 0; m < NW; ++m) {
-            const double wt = p.wtot[m];
-            if (wt != 0.0) {
-                p.st.phi[(size_t)(3 * m + 0) * n + i] += ((double)dIx - (double)p.st.f0[0][i]) * wt;
-                p.st.phi[(size_t)(3 * m + 1) * n + i] += ((double)dIy - (double)p.st.f0[1][i]) * wt;
-                p.st.phi[(size_t)(3 * m + 2) * n + i] += ((double)dIz - (double)p.st.f0[2][i]) * wt;
-            }
-        }
-    }
-
     const int SX = XFAST ? 1 : p.SX, SY = p.SY, SZ = p.SZ;      // x fastest (the default order): unit stride known at compile time
     int lin = (wx + 1) * SX + (wy + 1) * SY + (wz + 1) * SZ;
     uint32_t wraps = 512u | (512u << 10) | (512u << 20);   // packed per-axis counts of box wraps (+512)
     uint32_t nb = __ldg(p.nbr + lin);
 
-    constexpr int NWA = NW > 0 ? NW : 1;
-    float phiF[NWA][3];
-    int A32[NWA][3];
-    float wf[NWA];
-    int wi[NWA], wrem[NWA];
-#pragma unroll
-    for (int m = 0; m < NWA; ++m) {
-        wf[m] = 0.f; wi[m] = 0; wrem[m] = 0;
-#pragma unroll
-        for (int k = 0; k < 3; ++k) { phiF[m][k] = 0.f; A32[m][k] = 0; }
-    }
+    // Phase (Eq.7, R11): Phi_m = sum_i w_m[i] (x_i - x_0).  Inside a segment every waveform is constant, so all of them
+    // need the same sum  sum_i (x_i - x_0)  over the segment, taken in chunks of <= RMS_FCHUNK steps:
+    //   sum_i f_i              -> SF (fp32, flushed to fp64 per chunk)
+    //   sum_i (voxel index)    -> event driven: a face passage at a step adds +-1 to every later x_i of the chunk, i.e.
+    //                             +-(steps left in the chunk); A collects that in its low 21 bits and, 2^21 apart, the
+    //                             net number of passages, which moves the chunk's starting voxel Dst along
+    //   Phi_m += w_m (SF + A_low + (Dst - f_0) len)   at the end of the chunk, for every waveform.
+    // The cost per step does not depend on the number of waveforms.
+    float SFx = 0.f, SFy = 0.f, SFz = 0.f;
+    int Ax = 0, Ay = 0, Az = 0;
+    int Dstx = dIx, Dsty = dIy, Dstz = dIz;
+    int remK = 0;                               // steps left in the chunk (this one included) + 2^21
     unsigned n_enc = 0;
 
     // landed on a ghost voxel: fold back into the box (rare; the word of a ghost voxel is its image's word)
@@ -315,10 +303,7 @@ __global__ void __launch_bounds__(RMS_FBLOCK, (NW <= 4 ? RMS_FMINB : (NW <= 8 ? 
                 rms_permeable_step(&p, id_lo, id_hi, jj, wa, wb, rx, ry, rz, st, ist);
                 gx = st[0]; gy = st[1]; gz = st[2];
                 lin = ist[0]; wraps = (uint32_t)ist[1];
-#pragma unroll
-                for (int m = 0; m < NW; ++m) {
-                    A32[m][0] += ist[3] * wrem[m]; A32[m][1] += ist[4] * wrem[m]; A32[m][2] += ist[5] * wrem[m];
-                }
+                Ax += ist[3] * remK; Ay += ist[4] * remK; Az += ist[5] * remK;
                 n_enc += (unsigned)ist[6]; n_perm += (unsigned)ist[7];
                 if ((uint32_t)ist[2] != L) {
                     // Eq.5: the whole dt of this step goes to the compartment at the end of the hop (R12)
@@ -334,8 +319,7 @@ __global__ void __launch_bounds__(RMS_FBLOCK, (NW <= 4 ? RMS_FMINB : (NW <= 8 ? 
                 const bool ps = (pos & 32u) != 0, rf = cx && !ps;
                 if (ps) {
                     gx -= sgx; dl = isx * SX;
-#pragma unroll
-                    for (int m = 0; m < NW; ++m) A32[m][0] += isx * wrem[m];
+                    Ax += isx * remK;
                 }
                 if (rf) gx = h2x - gx;
             }
@@ -343,8 +327,7 @@ __global__ void __launch_bounds__(RMS_FBLOCK, (NW <= 4 ? RMS_FMINB : (NW <= 8 ? 
                 const bool ps = (pos & 64u) != 0, rf = cy && !ps;
                 if (ps) {
                     gy -= sgy; dl += isy * SY;
-#pragma unroll
-                    for (int m = 0; m < NW; ++m) A32[m][1] += isy * wrem[m];
+                    Ay += isy * remK;
                 }
                 if (rf) gy = h2y - gy;
             }
@@ -352,8 +335,7 @@ __global__ void __launch_bounds__(RMS_FBLOCK, (NW <= 4 ? RMS_FMINB : (NW <= 8 ? 
                 const bool ps = (pos & 128u) != 0, rf = cz && !ps;
                 if (ps) {
                     gz -= sgz; dl += isz * SZ;
-#pragma unroll
-                    for (int m = 0; m < NW; ++m) A32[m][2] += isz * wrem[m];
+                    Az += isz * remK;
                 }
                 if (rf) gz = h2z - gz;
             }
@@ -369,30 +351,20 @@ __global__ void __launch_bounds__(RMS_FBLOCK, (NW <= 4 ? RMS_FMINB : (NW <= 8 ? 
             }
         }
         fx = gx; fy = gy; fz = gz;
-        // phase, fractional part: Phi_F += w f (the integer part is event driven, above)
-#pragma unroll
-        for (int m = 0; m < NW; ++m) {
-            phiF[m][0] = fmaf(wf[m], fx, phiF[m][0]);
-            phiF[m][1] = fmaf(wf[m], fy, phiF[m][1]);
-            phiF[m][2] = fmaf(wf[m], fz, phiF[m][2]);
-            wrem[m] -= wi[m];
-        }
+        // phase: sum of the in-voxel offsets (the voxel part is event driven, above)
+        SFx += fx; SFy += fy; SFz += fz;
+        --remK;
     };
 
     uint32_t j = p.step0;                       // steps done so far (absolute)
 #pragma unroll 1
     for (int sg = 0; sg < p.n_seg; ++sg) {
-        const rms_segment sgm = p.segs[sg];
-        const uint32_t seg_end = j + sgm.n;
-#pragma unroll
-        for (int m = 0; m < NW; ++m) {
-            wi[m] = sgm.w[m];
-            wf[m] = (float)sgm.w[m];
-            wrem[m] = sgm.wrem_end[m] + sgm.w[m] * (int)sgm.n;   // weight remaining in this launch, current step included
-        }
+        const uint32_t seg_end = j + p.segs[sg].n;
+        const bool seg_weighted = (p.segs[sg].flags & 1u) != 0;          // some waveform is non-zero on this segment
 #pragma unroll 1
         while (j < seg_end) {
-            const uint32_t chunk_end = min(seg_end, (j + RMS_FFLUSH) & ~1u);
+            const uint32_t chunk_end = min(seg_end, (j + RMS_FCHUNK) & ~1u), chunk_begin = j;
+            remK = (int)(chunk_end - j) + (1 << 21);
             uint32_t r0, r1, r2, r3;
             if (j & 1u) {                        // second half of a Philox call that an earlier segment began
                 rms_philox(p.rk, id_lo, id_hi, j >> 1, RMS_STREAM_DIR, r0, r1, r2, r3);
@@ -411,14 +383,25 @@ __global__ void __launch_bounds__(RMS_FBLOCK, (NW <= 4 ? RMS_FMINB : (NW <= 8 ? 
                 step(r0, r1, j);
                 ++j;
             }
-            // flush the chunk's partial sums into the fp64 accumulators
-#pragma unroll
-            for (int m = 0; m < NW; ++m)
-#pragma unroll
-                for (int k = 0; k < 3; ++k) {
-                    p.st.phi[(size_t)(3 * m + k) * n + i] += (double)phiF[m][k] + (double)A32[m][k];
-                    phiF[m][k] = 0.f; A32[m][k] = 0;
-                }
+            // end of the chunk: its sum of (x_i - x_0) per axis, in fp64, times the weight of every waveform
+            {
+                const int netx = (Ax + (1 << 20)) >> 21, nety = (Ay + (1 << 20)) >> 21, netz = (Az + (1 << 20)) >> 21;
+                const double len = (double)(chunk_end - chunk_begin);
+                const double cx = (double)SFx + (double)(Ax - (netx << 21)) + ((double)Dstx - (double)p.st.f0[0][i]) * len;
+                const double cy = (double)SFy + (double)(Ay - (nety << 21)) + ((double)Dsty - (double)p.st.f0[1][i]) * len;
+                const double cz = (double)SFz + (double)(Az - (netz << 21)) + ((double)Dstz - (double)p.st.f0[2][i]) * len;
+                Dstx += netx; Dsty += nety; Dstz += netz;
+                SFx = SFy = SFz = 0.f; Ax = Ay = Az = 0;
+                if (seg_weighted)
+                    for (int m = 0; m < p.n_wave; ++m) {
+                        const double wm = (double)__ldg(&p.segs[sg].w[m]);
+                        if (wm != 0.0) {
+                            p.st.phi[(size_t)(3 * m + 0) * n + i] += wm * cx;
+                            p.st.phi[(size_t)(3 * m + 1) * n + i] += wm * cy;
+                            p.st.phi[(size_t)(3 * m + 2) * n + i] += wm * cz;
+                        }
+                    }
+            }
         }
     }
 
@@ -458,24 +441,16 @@ int rms_launch_step_fast(const rms_step_params& p, int n_wave, bool permeable, c
 {
     if (p.n == 0 || p.n_steps == 0) return RMS_OK;
     const unsigned grid = (unsigned)((p.n + RMS_FBLOCK - 1) / RMS_FBLOCK);
+    RMS_REQUIRE(n_wave >= 0 && n_wave <= RMS_MAX_WAVES, RMS_ERR_UNSUPPORTED, "n_wave = %d is above RMS_MAX_WAVES = %d", n_wave,
+                RMS_MAX_WAVES);
     const bool xf = p.SX == 1;
-#define RMS_FAST_CASE(NWV)                                                                      \
-    case NWV:                                                                                   \
-        if (permeable) {                                                                        \
-            if (xf) rms_step_fast_kernel<NWV, true, true><<<grid, RMS_FBLOCK, 0, stream>>>(p);   \
-            else rms_step_fast_kernel<NWV, false, true><<<grid, RMS_FBLOCK, 0, stream>>>(p);     \
-        } else {                                                                                \
-            if (xf) rms_step_fast_kernel<NWV, true, false><<<grid, RMS_FBLOCK, 0, stream>>>(p);  \
-            else rms_step_fast_kernel<NWV, false, false><<<grid, RMS_FBLOCK, 0, stream>>>(p);    \
-        }                                                                                       \
-        break;
-    switch (n_wave) {
-        RMS_FAST_CASE(0) RMS_FAST_CASE(1) RMS_FAST_CASE(2) RMS_FAST_CASE(3) RMS_FAST_CASE(4) RMS_FAST_CASE(8) RMS_FAST_CASE(16)
-        default:
-            rms_set_error("n_wave = %d is above RMS_MAX_WAVES = %d", n_wave, RMS_MAX_WAVES);
-            return RMS_ERR_UNSUPPORTED;
+    if (permeable) {
+        if (xf) rms_step_fast_kernel<true, true><<<grid, RMS_FBLOCK, 0, stream>>>(p);
+        else rms_step_fast_kernel<false, true><<<grid, RMS_FBLOCK, 0, stream>>>(p);
+    } else {
+        if (xf) rms_step_fast_kernel<true, false><<<grid, RMS_FBLOCK, 0, stream>>>(p);
+        else rms_step_fast_kernel<false, false><<<grid, RMS_FBLOCK, 0, stream>>>(p);
     }
-#undef RMS_FAST_CASE
     RMS_CUDA_TRY(cudaGetLastError());
     return RMS_OK;
 }

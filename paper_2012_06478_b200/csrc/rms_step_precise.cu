@@ -39,7 +39,6 @@ __device__ __forceinline__ long long rms_tag_d(double v, int tag) { return (__do
 
 }  // namespace
 
-template <int NW>
 __global__ void __launch_bounds__(RMS_PBLOCK) rms_step_precise_kernel(const __grid_constant__ rms_step_params p)
 {
     __shared__ double2 sm_trig[256];   // (cos, sin) of the centre of the 256 azimuth bins
@@ -68,34 +67,19 @@ __global__ void __launch_bounds__(RMS_PBLOCK) rms_step_precise_kernel(const __gr
     const uint32_t L = p.st.lab[i] & 0xFFFFu;
     const double s = (double)p.s_tab[L];        // the fp32 table value, as on the oracle's side (R6)
 
-    if (NW > 0) {
-#pragma unroll
-        for (int m = 0; m < NW; ++m) {
-            const double wt = p.wtot[m];
-            if (wt != 0.0) {
-                p.st.phi[(size_t)(3 * m + 0) * n + i] += ((double)dIx - (double)p.st.f0[0][i]) * wt;
-                p.st.phi[(size_t)(3 * m + 1) * n + i] += ((double)dIy - (double)p.st.f0[1][i]) * wt;
-                p.st.phi[(size_t)(3 * m + 2) * n + i] += ((double)dIz - (double)p.st.f0[2][i]) * wt;
-            }
-        }
-    }
-
     const int SX = p.SX, SY = p.SY, SZ = p.SZ;
     int lin = (wx + 1) * SX + (wy + 1) * SY + (wz + 1) * SZ;
     uint32_t wraps = 512u | (512u << 10) | (512u << 20);
     uint32_t nb = __ldg(p.nbr + lin);
 
-    constexpr int NWA = NW > 0 ? NW : 1;
-    double phiD[NWA][3];            // sum_i w_i f_i
-    long long A64[NWA][3];          // event-driven integer part: +-(weight remaining) per face passage
-    double wd[NWA];
-    int wi[NWA], wrem[NWA];
-#pragma unroll
-    for (int m = 0; m < NWA; ++m) {
-        wd[m] = 0.0; wi[m] = 0; wrem[m] = 0;
-#pragma unroll
-        for (int k = 0; k < 3; ++k) { phiD[m][k] = 0.0; A64[m][k] = 0; }
-    }
+    // Phase (Eq.7, R11), as in rms_step_fast.cu: inside a segment all waveforms are constant and share the sum of
+    // (x_i - x_0) over the segment = sum f_i (SF) + event-driven voxel part (A: +-(steps left) per face passage) +
+    // (Dst - f_0) x length, Dst = whole-voxel displacement at the start of the segment, moved along by the net passages
+    double SFx = 0.0, SFy = 0.0, SFz = 0.0;
+    long long Ax = 0, Ay = 0, Az = 0;
+    int netx = 0, nety = 0, netz = 0;
+    int Dstx = dIx, Dsty = dIy, Dstz = dIz;
+    long long rem = 0;                          // steps left in the segment, this one included
     unsigned n_enc = 0;
 
     auto step = [&](const uint32_t wa, const uint32_t wb) {
@@ -142,8 +126,7 @@ __global__ void __launch_bounds__(RMS_PBLOCK) rms_step_precise_kernel(const __gr
                 const bool ps = (pos & 32u) != 0, rf = cx && !ps;
                 if (ps) {
                     gx -= sgx; dl = isx * SX;
-#pragma unroll
-                    for (int m = 0; m < NW; ++m) A64[m][0] += isx * wrem[m];
+                    Ax += isx * rem; netx += isx;
                 }
                 if (rf) gx = h2x - gx;
             }
@@ -151,8 +134,7 @@ __global__ void __launch_bounds__(RMS_PBLOCK) rms_step_precise_kernel(const __gr
                 const bool ps = (pos & 64u) != 0, rf = cy && !ps;
                 if (ps) {
                     gy -= sgy; dl += isy * SY;
-#pragma unroll
-                    for (int m = 0; m < NW; ++m) A64[m][1] += isy * wrem[m];
+                    Ay += isy * rem; nety += isy;
                 }
                 if (rf) gy = h2y - gy;
             }
@@ -160,8 +142,7 @@ __global__ void __launch_bounds__(RMS_PBLOCK) rms_step_precise_kernel(const __gr
                 const bool ps = (pos & 128u) != 0, rf = cz && !ps;
                 if (ps) {
                     gz -= sgz; dl += isz * SZ;
-#pragma unroll
-                    for (int m = 0; m < NW; ++m) A64[m][2] += isz * wrem[m];
+                    Az += isz * rem; netz += isz;
                 }
                 if (rf) gz = h2z - gz;
             }
@@ -176,26 +157,15 @@ __global__ void __launch_bounds__(RMS_PBLOCK) rms_step_precise_kernel(const __gr
             }
         }
         fx = gx; fy = gy; fz = gz;
-#pragma unroll
-        for (int m = 0; m < NW; ++m) {
-            phiD[m][0] = fma(wd[m], fx, phiD[m][0]);
-            phiD[m][1] = fma(wd[m], fy, phiD[m][1]);
-            phiD[m][2] = fma(wd[m], fz, phiD[m][2]);
-            wrem[m] -= wi[m];
-        }
+        SFx += fx; SFy += fy; SFz += fz;
+        --rem;
     };
 
     uint32_t j = p.step0;
 #pragma unroll 1
     for (int sg = 0; sg < p.n_seg; ++sg) {
-        const rms_segment sgm = p.segs[sg];
-        const uint32_t seg_end = j + sgm.n;
-#pragma unroll
-        for (int m = 0; m < NW; ++m) {
-            wi[m] = sgm.w[m];
-            wd[m] = (double)sgm.w[m];
-            wrem[m] = sgm.wrem_end[m] + sgm.w[m] * (int)sgm.n;
-        }
+        const uint32_t seg_n = p.segs[sg].n, seg_end = j + seg_n;
+        rem = (long long)seg_n;
         uint32_t r0, r1, r2, r3;
         if ((j & 1u) && j < seg_end) {
             rms_philox(p.rk, id_lo, id_hi, j >> 1, RMS_STREAM_DIR, r0, r1, r2, r3);
@@ -214,11 +184,25 @@ __global__ void __launch_bounds__(RMS_PBLOCK) rms_step_precise_kernel(const __gr
             step(r0, r1);
             ++j;
         }
+        // end of the segment: its sum of (x_i - x_0) per axis times the weight of every waveform
+        {
+            const double len = (double)seg_n;
+            const double cx = SFx + (double)Ax + ((double)Dstx - (double)p.st.f0[0][i]) * len;
+            const double cy = SFy + (double)Ay + ((double)Dsty - (double)p.st.f0[1][i]) * len;
+            const double cz = SFz + (double)Az + ((double)Dstz - (double)p.st.f0[2][i]) * len;
+            Dstx += netx; Dsty += nety; Dstz += netz;
+            SFx = SFy = SFz = 0.0; Ax = Ay = Az = 0; netx = nety = netz = 0;
+            if (p.segs[sg].flags & 1u)
+                for (int m = 0; m < p.n_wave; ++m) {
+                    const double wm = (double)__ldg(&p.segs[sg].w[m]);
+                    if (wm != 0.0) {
+                        p.st.phi[(size_t)(3 * m + 0) * n + i] += wm * cx;
+                        p.st.phi[(size_t)(3 * m + 1) * n + i] += wm * cy;
+                        p.st.phi[(size_t)(3 * m + 2) * n + i] += wm * cz;
+                    }
+                }
+        }
     }
-#pragma unroll
-    for (int m = 0; m < NW; ++m)
-#pragma unroll
-        for (int k = 0; k < 3; ++k) p.st.phi[(size_t)(3 * m + k) * n + i] += phiD[m][k] + (double)A64[m][k];
 
     // ---- store state --------------------------------------------------------------------------
     {
@@ -254,18 +238,9 @@ int rms_launch_step_precise(const rms_step_params& p, int n_wave, cudaStream_t s
 {
     if (p.n == 0 || p.n_steps == 0) return RMS_OK;
     const unsigned grid = (unsigned)((p.n + RMS_PBLOCK - 1) / RMS_PBLOCK);
-    switch (n_wave) {
-        case 0: rms_step_precise_kernel<0><<<grid, RMS_PBLOCK, 0, stream>>>(p); break;
-        case 1: rms_step_precise_kernel<1><<<grid, RMS_PBLOCK, 0, stream>>>(p); break;
-        case 2: rms_step_precise_kernel<2><<<grid, RMS_PBLOCK, 0, stream>>>(p); break;
-        case 3: rms_step_precise_kernel<3><<<grid, RMS_PBLOCK, 0, stream>>>(p); break;
-        case 4: rms_step_precise_kernel<4><<<grid, RMS_PBLOCK, 0, stream>>>(p); break;
-        case 8: rms_step_precise_kernel<8><<<grid, RMS_PBLOCK, 0, stream>>>(p); break;
-        case 16: rms_step_precise_kernel<16><<<grid, RMS_PBLOCK, 0, stream>>>(p); break;
-        default:
-            rms_set_error("n_wave = %d is above RMS_MAX_WAVES = %d", n_wave, RMS_MAX_WAVES);
-            return RMS_ERR_UNSUPPORTED;
-    }
+    RMS_REQUIRE(n_wave >= 0 && n_wave <= RMS_MAX_WAVES, RMS_ERR_UNSUPPORTED, "n_wave = %d is above RMS_MAX_WAVES = %d", n_wave,
+                RMS_MAX_WAVES);
+    rms_step_precise_kernel<<<grid, RMS_PBLOCK, 0, stream>>>(p);
     RMS_CUDA_TRY(cudaGetLastError());
     return RMS_OK;
 }
