@@ -127,8 +127,9 @@ int rms_walkers_destroy(rms_walkers* w);
  *             moments are taken (host)
  * flags       RMS_RUN_LABEL_GATHER: test faces by gathering the neighbour's uint16 label (the paper's
  *             lookup table) instead of the neighbourhood lattice.
- *             RMS_RUN_GENERAL_KERNEL: impermeable runs with integer-valued piecewise-constant waveforms
- *             normally take the specialised kernel (csrc/rms_step_fast.cu); this flag forces the general one.
+ *             RMS_RUN_GENERAL_KERNEL: impermeable or weakly permeable runs with piecewise-constant waveforms (rectangular
+ *             lobes of any amplitude, segments of >= 32 steps on average) normally take the specialised kernel
+ *             (csrc/rms_step_fast.cu); this flag forces the general one.
  *             RMS_RUN_FP64: direction, hop, in-voxel offsets, hit order and phase in fp64 instead of fp32, for runs
  *             of more than a few 1e4 steps whose trajectories must stay on those of an fp64 reference
  *             (csrc/rms_step_precise.cu says why fp32 cannot).  Two thirds of the fp32 speed for impermeable

@@ -155,8 +155,9 @@ __device__ __forceinline__ float rms_uni(uint32_t w) { return (float)(w >> 8) * 
 struct rms_segment {          // a run of steps on which every waveform is constant (integer valued)
     uint32_t n;               // steps in the segment
     uint32_t flags;           // bit 0: some w != 0 ; bit 1: some remaining weight != 0 inside the segment
-    int32_t w[RMS_MAX_WAVES];
-    int32_t wrem_end[RMS_MAX_WAVES];  // sum of w over the steps of this launch after the segment
+    float wf[RMS_MAX_WAVES];          // the constant value of each waveform on the segment (specialised kernels)
+    int32_t w[RMS_MAX_WAVES];         // the same as integers, and ...
+    int32_t wrem_end[RMS_MAX_WAVES];  // ... the sum of w over the steps of this launch after the segment (general kernel, CONST mode)
 };
 
 enum { RMS_WMODE_CONST = 0, RMS_WMODE_TABLE = 1 };

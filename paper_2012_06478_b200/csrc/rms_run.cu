@@ -149,8 +149,11 @@ extern "C" int rms_run(const rms_substrate* s, rms_walkers* w, const rms_run_des
     // RMS_RUN_FP64: the specialised fp64 kernel serves the impermeable / neighbourhood-lattice / integer-waveform case,
     // the general fp64 kernel (table-driven waveforms, label gathers) everything else
     const bool fp64 = (d->flags & RMS_RUN_FP64) != 0;
-    bool const_mode = wave_is_integer(d->wave, (size_t)nW * nT) && !(fp64 && (permeable || lat != RMS_LAT_FACES));
-    for (size_t i = 0; const_mode && i < suf.size(); ++i) const_mode = fabs(suf[i]) < 1048576.0;   // int32 event sums: <= 1024 steps x 2^20 between flushes
+    // integer-valued waveforms: the general kernel's exact int32 path (CONST mode)
+    bool int_mode = wave_is_integer(d->wave, (size_t)nW * nT);
+    for (size_t i = 0; int_mode && i < suf.size(); ++i) int_mode = fabs(suf[i]) < 1048576.0;   // int32 event sums: <= 64 steps x 2^20 between flushes
+    // piecewise-constant waveforms (any amplitudes), segments of >= 32 steps on average: the specialised kernels
+    bool const_mode = true;
 
     // launch boundaries: snapshots and the end of the call
     std::vector<int64_t> bounds;
@@ -176,10 +179,13 @@ extern "C" int rms_run(const rms_substrate* s, rms_walkers* w, const rms_run_des
                 memset(&sg, 0, sizeof sg);
                 sg.n = (uint32_t)(e - j);
                 for (int m = 0; m < nW; ++m) {
-                    sg.w[m] = (int32_t)d->wave[(size_t)m * nT + j];
-                    sg.wrem_end[m] = (int32_t)llrint(suf[(size_t)m * (nT + 1) + e] - suf[(size_t)m * (nT + 1) + b]);
-                    if (sg.w[m] != 0) sg.flags |= 3u;
-                    if (sg.wrem_end[m] != 0) sg.flags |= 2u;
+                    sg.wf[m] = d->wave[(size_t)m * nT + j];
+                    if (int_mode) {
+                        sg.w[m] = (int32_t)d->wave[(size_t)m * nT + j];
+                        sg.wrem_end[m] = (int32_t)llrint(suf[(size_t)m * (nT + 1) + e] - suf[(size_t)m * (nT + 1) + b]);
+                        if (sg.wrem_end[m] != 0) sg.flags |= 2u;
+                    }
+                    if (sg.wf[m] != 0.f) sg.flags |= 3u;
                 }
                 segs.push_back(sg);
                 j = e;
@@ -187,9 +193,20 @@ extern "C" int rms_run(const rms_substrate* s, rms_walkers* w, const rms_run_des
             seg_range.push_back({first, segs.size() - first});
             a = b;
         }
-        if (segs.size() > (1u << 20)) { const_mode = false; segs.clear(); seg_range.clear(); }
+        if (segs.size() > (1u << 20) || (int64_t)segs.size() > nT / 32 + (int64_t)bounds.size() + 16) {
+            const_mode = false; segs.clear(); seg_range.clear();
+        }
     }
-    const int wmode = const_mode ? RMS_WMODE_CONST : RMS_WMODE_TABLE;
+    // which step kernel: specialised (fp32 / fp64) needs piecewise-constant waveforms and the neighbourhood lattice; the general
+    // fp32 kernel runs its CONST mode on integer-valued piecewise-constant waveforms, its TABLE mode otherwise; the general
+    // fp64 kernel is table driven
+    const bool nbr_fp32 = (!permeable && lat == RMS_LAT_FACES) || fast_permeable;
+    const bool use_fast = !fp64 && const_mode && nbr_fp32 && !(d->flags & RMS_RUN_GENERAL_KERNEL);
+    const bool use_precise = fp64 && const_mode && !permeable && lat == RMS_LAT_FACES;
+    const bool use_general = !use_fast && !use_precise;
+    const int wmode = (use_general && !fp64 && const_mode && int_mode) ? RMS_WMODE_CONST : RMS_WMODE_TABLE;
+    const bool need_segs = use_fast || use_precise || wmode == RMS_WMODE_CONST;
+    const bool need_table = use_general && wmode == RMS_WMODE_TABLE;
 
     // ---- device scratch: tables | segments or wave tables | q vectors | result sums -------------------
     const int nQ = nW * nG * nD;
@@ -200,12 +217,13 @@ extern "C" int rms_run(const rms_substrate* s, rms_walkers* w, const rms_run_des
     DeviceBuf b_tabs, b_segs, b_wave, b_wsuf, b_q, b_res, b_dirs, b_order;
     RMS_CUDA_TRY(rms_malloc((void**)&b_tabs.p, tabs.size() * sizeof(float)));
     RMS_CUDA_TRY(cudaMemcpyAsync(b_tabs.p, tabs.data(), tabs.size() * sizeof(float), cudaMemcpyHostToDevice, stream));
-    if (const_mode) {
+    if (need_segs) {
         if (!segs.empty()) {
             RMS_CUDA_TRY(rms_malloc((void**)&b_segs.p, segs.size() * sizeof(rms_segment)));
             RMS_CUDA_TRY(cudaMemcpyAsync(b_segs.p, segs.data(), segs.size() * sizeof(rms_segment), cudaMemcpyHostToDevice, stream));
         }
-    } else if (nW > 0 && nT > 0) {
+    }
+    if (need_table && nW > 0 && nT > 0) {
         RMS_CUDA_TRY(rms_malloc((void**)&b_wave.p, (size_t)nWk * nT * sizeof(float)));
         if (nWk > nW) RMS_CUDA_TRY(cudaMemsetAsync(b_wave.p, 0, (size_t)nWk * nT * sizeof(float), stream));
         RMS_CUDA_TRY(cudaMemcpyAsync(b_wave.p, d->wave, (size_t)nW * nT * sizeof(float), cudaMemcpyHostToDevice, stream));
@@ -284,10 +302,11 @@ extern "C" int rms_run(const rms_substrate* s, rms_walkers* w, const rms_run_des
                 sp.wtot[m] = S[a] - S[b];
                 sp.wsuf_end[m] = S[b];
             }
-            if (const_mode) {
+            if (need_segs) {
                 sp.n_seg = (int)seg_range[li].second;
                 sp.segs = b_segs.as<rms_segment>() + seg_range[li].first;
-            } else {
+            }
+            if (need_table) {
                 sp.n_seg = 1;
                 sp.wave = b_wave.as<float>() ? b_wave.as<float>() + a : nullptr;
                 // wsuf element 0 must be the suffix sum that includes the first step of this launch: S[a]
@@ -295,14 +314,10 @@ extern "C" int rms_run(const rms_substrate* s, rms_walkers* w, const rms_run_des
             }
             cudaEvent_t e0 = evs.make(), e1 = evs.make();
             RMS_CUDA_TRY(cudaEventRecord(e0, stream));
-            const bool special = !permeable && lat == RMS_LAT_FACES && wmode == RMS_WMODE_CONST;
-            const bool special_perm = fast_permeable && wmode == RMS_WMODE_CONST;
-            if (fp64)
-                rc = special ? rms_launch_step_precise(sp, nW, stream) : rms_launch_step_precise_general(sp, nWk, stream);
-            else if ((special || special_perm) && !(d->flags & RMS_RUN_GENERAL_KERNEL))
-                rc = rms_launch_step_fast(sp, nW, permeable, stream);
-            else
-                rc = rms_launch_step(sp, nWk, wmode, lat, permeable, stream);
+            if (use_precise) rc = rms_launch_step_precise(sp, nW, stream);
+            else if (fp64) rc = rms_launch_step_precise_general(sp, nWk, stream);
+            else if (use_fast) rc = rms_launch_step_fast(sp, nW, permeable, stream);
+            else rc = rms_launch_step(sp, nWk, wmode, lat, permeable, stream);
             if (rc != RMS_OK) return rc;
             RMS_CUDA_TRY(cudaEventRecord(e1, stream));
             step_ev.push_back({e0, e1});

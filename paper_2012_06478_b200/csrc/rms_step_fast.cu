@@ -1,6 +1,6 @@
 // rms_step_fast.cu -- H2..H5 for the throughput-critical case: impermeable or weakly permeable membranes (512 P <= 64,
-// i.e. P <= 1/8: the paper's regime P << 1; see rms_permeable_step below) and piecewise-constant,
-// integer-valued gradient waveforms (PGSE and every other rectangular-lobe sequence).  Same method and
+// i.e. P <= 1/8: the paper's regime P << 1; see rms_permeable_step below) and piecewise-constant
+// gradient waveforms (PGSE and every other rectangular-lobe sequence, any number of them).  Same method and
 // the same numbers as the general kernel of rms_step.cu (section 2.2 steps 2-4; corner
 // reflector of Fig.2; elastic collision P:90), organised for the B200 instruction pipes:
 //
@@ -394,7 +394,7 @@ __global__ void __launch_bounds__(RMS_FBLOCK, RMS_FMINB) rms_step_fast_kernel(co
                 SFx = SFy = SFz = 0.f; Ax = Ay = Az = 0;
                 if (seg_weighted)
                     for (int m = 0; m < p.n_wave; ++m) {
-                        const double wm = (double)__ldg(&p.segs[sg].w[m]);
+                        const double wm = (double)__ldg(&p.segs[sg].wf[m]);
                         if (wm != 0.0) {
                             p.st.phi[(size_t)(3 * m + 0) * n + i] += wm * cx;
                             p.st.phi[(size_t)(3 * m + 1) * n + i] += wm * cy;

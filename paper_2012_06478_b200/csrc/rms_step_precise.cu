@@ -194,7 +194,7 @@ __global__ void __launch_bounds__(RMS_PBLOCK) rms_step_precise_kernel(const __gr
             SFx = SFy = SFz = 0.0; Ax = Ay = Az = 0; netx = nety = netz = 0;
             if (p.segs[sg].flags & 1u)
                 for (int m = 0; m < p.n_wave; ++m) {
-                    const double wm = (double)__ldg(&p.segs[sg].w[m]);
+                    const double wm = (double)__ldg(&p.segs[sg].wf[m]);
                     if (wm != 0.0) {
                         p.st.phi[(size_t)(3 * m + 0) * n + i] += wm * cx;
                         p.st.phi[(size_t)(3 * m + 1) * n + i] += wm * cy;

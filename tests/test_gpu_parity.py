@@ -183,7 +183,7 @@ def test_four_integer_waveforms_odd_boundaries_and_chunks(rms):
 def test_sequence_sweep_many_waveforms_on_one_set_of_trajectories(rms, n_wave):
     # S: section 8(f) N1 -- a sweep of PGSE timings (the paper's Delta = delta series) evaluated on the same
     # trajectories in one run: 6 waveforms run on the 8-waveform kernel padded with zero weights, 16 on the 16-waveform one;
-    # specialised fp32 kernel, general kernel (one extra non-integer waveform -> table mode) and fp64
+    # specialised fp32 and fp64 kernels (integer and non-integer amplitudes), general kernel through RMS_RUN_GENERAL_KERNEL
     sub = ri.single_cylinder(20, 6.5, 0.1)
     nT = 640
     wave = np.zeros((n_wave, nT), np.float32)
@@ -202,11 +202,13 @@ def test_sequence_sweep_many_waveforms_on_one_set_of_trajectories(rms, n_wave):
         if flags == 8:
             assert rep["n_diff"] == 0
     wave2 = wave.copy()
-    wave2[n_wave - 1] *= 0.5                                     # non-integer -> table mode, general kernels
+    wave2[n_wave - 1] *= 0.37                                    # non-integer amplitudes: still piecewise constant, same kernels
     seq2 = ri.Sequence(dt_ms=2e-4, n_steps=nT, wave=wave2, gamp=gamp, dirs=ri.fibonacci_dirs(4), snap_steps=np.array([nT]))
     o2 = oracle_run(sub, seq2, n, 17)
     for flags in (0, 8):
-        print("waves", n_wave, "table mode, flags", flags, compare(gpu_run(sub, seq2, n, 17, flags=flags), o2, n))
+        print("waves", n_wave, "non-integer amplitudes, flags", flags, compare(gpu_run(sub, seq2, n, 17, flags=flags), o2, n))
+    print("waves", n_wave, "general kernel, table mode", compare(gpu_run(sub, seq2, n, 17, flags=2), o2, n))
+    print("waves", n_wave, "general kernel, const mode", compare(gpu_run(sub, seq, n, 17, flags=2), o, n))
 
 
 @pytest.mark.parametrize("dims", [(5, 7, 3), (1, 1, 9), (2, 3, 4)])
