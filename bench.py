@@ -36,7 +36,7 @@ sys.path.insert(0, str(ROOT))
 ALGORITHMIC_INSTR_PER_STEP = 80.0
 N_SM, LANES_PER_SM = 148, 128          # B200: 4 schedulers x 32 lanes per SM, one warp instruction per clock each
 # DRAM traffic of the step kernel per launch from the committed ncu capture (profiles/), or None.
-NCU_TRAFFIC_BYTES_PER_LAUNCH = 47.81e9   # profiles/r1c_step_kernels_ncu.md: 46.49 GB read + 1.32 GB written
+NCU_TRAFFIC_BYTES_PER_LAUNCH = 62.27e9   # profiles/r1d_step_fast_ncu.md: 60.41 GB read + 1.86 GB written
 
 
 def parse_args():
