@@ -30,6 +30,8 @@
  *   run, cylinder        short-time Mitra law D(t)/D0 = 1 - 4/(3 sqrt(pi)) (S_x/V) sqrt(D0 t)
  *                        with S_x/V counted on the staircase surface of the lattice cylinder
  *   run, encounters      membrane encounters per step = surface * step / 4
+ *   run, absorbing walls surviving fraction between plates = Brownstein-Tarr series (Eq.4; R = rho S/V)
+ *   run, rejection sampl. D_parallel = D0 (1 - 3/16 S/V ds) between plates (Eq.B.2), uniform density
  * Parity unpinned: wide-pulse signals inside voxelised cylinders / axons have
  *   no closed form; they are pinned only through the pieces above.
  */
@@ -210,6 +212,7 @@ typedef struct {
     const double* s; /* [n_labels] */
     const double* P; /* [n_labels^2] */
     const double* Q; /* [n_labels^2] saturation probability P_MT, or NULL (no absorbing membranes) */
+    int rejection;   /* 1: rejection sampling instead of elastic collision (Appendix B) */
 } lattice_t;
 
 static int wrap(int64_t a, int n) { int64_t m = a % n; return (int)(m < 0 ? m + n : m); }
@@ -243,6 +246,9 @@ static void step_core(const lattice_t* lat, int32_t vox[3], double off[3], uint1
                       int* n_enc, int* n_perm, int* n_clamp)
 {
     uint16_t L = *label;
+    const uint16_t L_in = L;
+    const int32_t v_in[3] = { vox[0], vox[1], vox[2] };
+    const int n_perm_in = *n_perm;
     double r[3], p[3];
     int done[3] = { 0, 0, 0 };
     int e = 0;
@@ -289,6 +295,13 @@ static void step_core(const lattice_t* lat, int32_t vox[3], double off[3], uint1
                 for (int k = 0; k < 3; ++k) r[k] *= scale;
                 L = Ln;
             }
+        } else if (lat->rejection) {
+            /* rejection sampling (Appendix B): a step that meets a membrane it does not cross is cancelled and
+             * the walker does not move for the step */
+            vox[0] = v_in[0]; vox[1] = v_in[1]; vox[2] = v_in[2];
+            *label = L_in;
+            *n_perm = n_perm_in; /* a permeation earlier in the cancelled step did not happen either */
+            return;
         } else {
             r[kstar] = -r[kstar]; /* elastic collision on the face plane */
         }
@@ -309,7 +322,7 @@ int rms_oracle_step(int nx, int ny, int nz, const uint16_t* labels, int n_labels
                     int32_t vox[3], double off[3], uint16_t* label, const double u[3], const double up[3],
                     int32_t counts[3])
 {
-    lattice_t lat = { nx, ny, nz, labels, n_labels, s, P, NULL };
+    lattice_t lat = { nx, ny, nz, labels, n_labels, s, P, NULL, 0 };
     int ne = 0, np = 0, nc = 0;
     perm_src_t ps = { 0, 0, 0, 0, 0, 1, { up[0], up[1], up[2] } };
     step_core(&lat, vox, off, label, u, &ps, NULL, NULL, &ne, &np, &nc);
@@ -469,7 +482,7 @@ int rms_oracle_run(
     const float* D, const float* T2, const float* kappa, const float* rho, const uint16_t* label_class, int n_classes,
     uint64_t n_walkers, uint64_t first_id, const uint8_t* label_allowed, uint64_t seed,
     double dt_ms, int64_t n_steps, int n_wave, const float* wave, int n_g, const double* gamp,
-    int n_dir, const double* dirs, int n_snap, const int64_t* snap_steps, int n_threads,
+    int n_dir, const double* dirs, int n_snap, const int64_t* snap_steps, int n_threads, int interaction,
     double* sum_alpha, double* sig_re, double* sig_im, double* m2, double* m4, double* snap_alpha,
     uint64_t* class_flow, uint64_t* counters,
     int32_t* final_vox, double* final_off, uint16_t* final_label,
@@ -497,6 +510,19 @@ int rms_oracle_run(
     if (!s_tab || !P_tab || !inv_T2 || (rho && !Q_tab)) { free(s_tab); free(P_tab); free(inv_T2); free(Q_tab); return ORC_ERR_OOM; }
     int st = rms_oracle_tables(n_labels, D, kappa, voxel_um, dt_ms, s_tab, P_tab);
     if (st == ORC_OK && rho) st = rms_oracle_mt_table(n_labels, D, rho, dt_ms, Q_tab);
+    if (st == ORC_OK && interaction == 1 && kappa) {
+        /* rejection sampling has its own permeation probability: P_T / (1 - P_T) = kappa ds / D0 C_d (Appendix B.1,
+         * generalised to 3d with Eq.2a); the paper derives it for equal diffusivities on both sides only */
+        for (int a = 0; a < n_labels && st == ORC_OK; ++a)
+            for (int b = 0; b < n_labels; ++b) {
+                double k = (double)kappa[a * n_labels + b];
+                if (a == b || k == 0.0 || isinf(k)) continue;
+                if (D[a] != D[b]) { st = ORC_ERR_ARG; break; }
+                double A = k * sqrt(6.0 * dt_ms / (double)D[a]) * (2.0 / 3.0);
+                P_tab[a * n_labels + b] = (double)(float)(A / (1.0 + A));
+            }
+    }
+    if (interaction != 0 && interaction != 1) st = ORC_ERR_ARG;
     if (st != ORC_OK) { free(s_tab); free(P_tab); free(inv_T2); free(Q_tab); return st; }
     for (int a = 0; a < n_labels; ++a) {
         double t2 = T2 ? (double)T2[a] : 0.0;
@@ -506,7 +532,7 @@ int rms_oracle_run(
     job_t job;
     memset(&job, 0, sizeof job);
     job.lat.nx = nx; job.lat.ny = ny; job.lat.nz = nz; job.lat.labels = labels; job.lat.n_labels = n_labels;
-    job.lat.s = s_tab; job.lat.P = P_tab; job.lat.Q = Q_tab;
+    job.lat.s = s_tab; job.lat.P = P_tab; job.lat.Q = Q_tab; job.lat.rejection = interaction == 1;
     job.voxel_um = voxel_um; job.inv_T2 = inv_T2; job.label_class = label_class; job.n_classes = n_classes;
     job.n_walkers = n_walkers; job.first_id = first_id; job.seed = seed; job.label_allowed = label_allowed;
     job.dt = dt_ms; job.n_steps = n_steps; job.n_wave = n_wave; job.wave = wave; job.n_g = n_g; job.gamp = gamp;

@@ -137,8 +137,9 @@ def normalise(raw, dt_ms, snap_steps):
     return out
 
 
-def run(sub, seq, n_walkers, seed, first_id=0, n_threads=1, per_walker=False):
-    """Whole path on the CPU: init -> steps -> sums.  `sub`, `seq` are rms_inputs.Substrate / Sequence."""
+def run(sub, seq, n_walkers, seed, first_id=0, n_threads=1, per_walker=False, interaction=0):
+    """Whole path on the CPU: init -> steps -> sums.  `sub`, `seq` are rms_inputs.Substrate / Sequence.
+    interaction: 0 = elastic collision (the paper's method), 1 = rejection sampling (its Appendix B)."""
     lib = _load()
     labels = np.ascontiguousarray(sub.labels, np.uint16)
     nz, ny, nx = labels.shape
@@ -174,7 +175,7 @@ def run(sub, seq, n_walkers, seed, first_id=0, n_threads=1, per_walker=False):
         C.c_uint64(n_walkers), C.c_uint64(first_id), _p(allowed, C.c_uint8), C.c_uint64(seed),
         C.c_double(seq.dt_ms), C.c_int64(n_steps), C.c_int(n_wave), _p(wave, C.c_float), C.c_int(n_g),
         _p(gamp, C.c_double), C.c_int(n_dir), _p(dirs, C.c_double), C.c_int(n_snap), _p(snaps, C.c_int64),
-        C.c_int(n_threads),
+        C.c_int(n_threads), C.c_int(interaction),
         _p(r["sum_alpha"], C.c_double), _p(r["sig_re"], C.c_double), _p(r["sig_im"], C.c_double),
         _p(r["m2"], C.c_double), _p(r["m4"], C.c_double), _p(r["snap_alpha"], C.c_double),
         _p(r["class_flow"], C.c_uint64), _p(counters, C.c_uint64),

@@ -372,3 +372,35 @@ def test_absorbing_walls_follow_the_surface_relaxation_series(rho, n_steps):
     r1 = oracle.run(sub, seq, 2000, seed=41, n_threads=THREADS, per_walker=True)
     assert np.array_equal(r0["final_vox"], r1["final_vox"]) and np.array_equal(r0["final_off"], r1["final_off"])
     assert r0["n_saturations"] == 0 and r1["n_saturations"] > 0 and np.isinf(r1["relax"]).sum() == r1["n_saturations"]
+
+
+# ------------------------------------------------------------------ rejection sampling (Appendix B)
+def test_rejection_sampling_bias_of_the_parallel_diffusivity_eq_b2():
+    """P:84 and Appendix B: a step that meets a membrane is cancelled.  Between impermeable plates the density stays
+    uniform, the transverse long-time <X^2> -> a^2/6 as for any reflecting wall, and the diffusivity PARALLEL to the
+    plates is biased to D0 (1 - 3/16 (S/V) ds) (Eq.B.2), S/V = 2/a -- while elastic collision leaves it at D0."""
+    a_vox, D0 = 10, 2.0
+    sub = ri.slabs(a_vox, 3, (4, 4), LP, D_extra=D0, D_intra=D0, place="extra")
+    n_steps, n_w = 2000, 200_000
+    seq = _narrow(n_steps, np.eye(3))
+    ds = math.sqrt(6 * D0 * DT)
+    a = a_vox * LP
+    bias = 3.0 / 16.0 * (2.0 / a) * ds
+    assert 0.015 < bias < 0.02
+    se = math.sqrt(2.0 / n_w)
+    rs = oracle.run(sub, seq, n_w, seed=51, n_threads=THREADS, interaction=1, per_walker=True)
+    ec = oracle.run(sub, seq, n_w, seed=51, n_threads=THREADS, interaction=0)
+    for k in (1, 2):                                           # y and z are parallel to the plates
+        assert abs(rs["D"][0][k] / D0 - (1 - bias)) < 0.15 * bias + 3 * se, (rs["D"][0], bias)
+        assert abs(ec["D"][0][k] / D0 - 1) < 3 * se
+        # same seed, same hop directions: the Monte Carlo noise is common to both runs and the difference isolates the bias
+        assert abs((ec["D"][0][k] - rs["D"][0][k]) / D0 - bias) < 0.1 * bias, (ec["D"][0], rs["D"][0], bias)
+    t = n_steps * DT                                           # D t / a^2 = 0.8: the transverse MSD has reached a^2 / 6
+    assert abs(rs["msd"][0][0] / (a * a / 6) - 1) < 0.03
+    # uniform density across the gap (chi^2 over the a_vox columns)
+    x = (rs["final_vox"][:, 0] % (a_vox + 3))
+    counts = np.bincount(x, minlength=a_vox + 3)[:a_vox]
+    assert counts.sum() == n_w
+    chi2 = ((counts - n_w / a_vox) ** 2 / (n_w / a_vox)).sum()
+    assert chi2 < 30, counts                                   # 9 degrees of freedom
+    assert rs["n_encounters"] > 0 and rs["n_permeations"] == 0
