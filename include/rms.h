@@ -136,6 +136,13 @@ int rms_walkers_destroy(rms_walkers* w);
  *             substrates with integer-valued piecewise-constant waveforms; a plain, slower kernel otherwise.
  *             RMS_RUN_NO_ORDERING: on large lattices the walkers are dealt to the threads in the order of the
  *             lattice cell they sit in (cache locality; results do not depend on it); this flag keeps id order.
+ *             RMS_RUN_REJECTION_SAMPLING: the paper's other membrane interaction (Appendix B): a
+ *             step that meets a membrane it does not cross is cancelled and the walker stays where it was for
+ *             that step, instead of the elastic collision.  The permeation probability is then Appendix B.1's
+ *             P_T = A / (1 + A), A = kappa sqrt(6 dt / D) 2/3, defined for equal D on both sides:
+ *             RMS_ERR_UNSUPPORTED for a finite non-zero kappa between unequal D.  Runs in the general kernels
+ *             (fp32, or fp64 with RMS_RUN_FP64); biased near membranes by Eq.B.2, which is why elastic
+ *             collision is the default.
  *
  * A second rms_run on the same walkers continues the trajectories (the random numbers are keyed on the
  * absolute step), so long runs may be chunked; phases and T2 weights keep accumulating.
@@ -158,6 +165,7 @@ int rms_walkers_destroy(rms_walkers* w);
 #define RMS_RUN_GENERAL_KERNEL 2u
 #define RMS_RUN_NO_ORDERING 4u
 #define RMS_RUN_FP64 8u
+#define RMS_RUN_REJECTION_SAMPLING 16u
 
 typedef struct {
     double dt_ms;               /* Table 1: dt */

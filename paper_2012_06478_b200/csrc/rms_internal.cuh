@@ -181,6 +181,7 @@ struct rms_step_params {
     const float* PMT;         // [n_labels^2] saturation probability at an encounter a -> b (Eq.4, R20), or NULL
     const float* rate;        // [n_labels] dt / T2
     int n_labels;
+    int rejection;            // 1: rejection sampling instead of elastic collision (R21; general kernels only)
     uint32_t t_ceil;          // ceil(512 max P(a->b)) over the membranes: coarse random bits at or above it cannot permeate
     uint32_t step0;           // steps done before this launch
     uint32_t n_steps;         // steps of this launch
@@ -223,7 +224,8 @@ int rms_launch_moments(const rms_reduce_params& p, double* d_m2, double* d_m4, d
 #define RMS_SIG_SMALL_CLASSES 8
 int rms_launch_signal(const rms_reduce_params& p, int n_wave, int nq, const double* d_qv, const int* d_qwave, double* d_re,
                       double* d_im, double* d_sum_alpha, const uint32_t* order_by_class, cudaStream_t stream, unsigned* n_launches);
-int rms_compute_tables(const rms_substrate* s, double dt, std::vector<float>& s_tab, std::vector<float>& P_tab);
+int rms_compute_tables(const rms_substrate* s, double dt, std::vector<float>& s_tab, std::vector<float>& P_tab,
+                       bool rejection_sampling = false);
 int rms_walkers_reserve_waves(rms_walkers* w, int n_wave, cudaStream_t stream);
 // rms_sched.cu: order[t] = walker index, sorted by the lattice cell the walker sits in (z-major), so that the
 // threads of a warp and the blocks resident at one time gather neighbouring words.  d_order: [n] device.

@@ -97,7 +97,8 @@ extern "C" int rms_run(const rms_substrate* s, rms_walkers* w, const rms_run_des
 
     // ---- H0 (run-time part): tables from (D, kappa, T2, dt) ---------------------------------------
     std::vector<float> s_tab, P_tab;
-    int rc = rms_compute_tables(s, d->dt_ms, s_tab, P_tab);
+    const bool rs = (d->flags & RMS_RUN_REJECTION_SAMPLING) != 0;   // P:84, Appendix B (R21)
+    int rc = rms_compute_tables(s, d->dt_ms, s_tab, P_tab, rs);
     if (rc != RMS_OK) return rc;
     const bool mt = !s->rho.empty();             // absorbing membranes (Eq.4)
     std::vector<float> tabs((size_t)nL * 2 + (size_t)nL * nL * (mt ? 2 : 1));
@@ -123,7 +124,7 @@ extern "C" int rms_run(const rms_substrate* s, rms_walkers* w, const rms_run_des
         }
     }
     const bool want_labels = (d->flags & RMS_RUN_LABEL_GATHER) != 0;
-    if (mt) permeable = true;                    // absorbing membranes are handled where labels are read: the general kernels
+    if (mt || rs) permeable = true;              // absorbing membranes and cancelled steps are handled where labels are read: the general kernels
     const int lat = (!permeable && s->d_nbr && !want_labels) ? RMS_LAT_FACES : RMS_LAT_LABELS;
     // permeable runs with P << 1 also take the specialised kernel: ceil(512 P_max) bounds the coarse random
     // bits that can permeate at all (rms_step_fast.cu)
@@ -132,7 +133,7 @@ extern "C" int rms_run(const rms_substrate* s, rms_walkers* w, const rms_run_des
         for (int b = 0; b < nL; ++b)
             if (a != b) t_max = std::max(t_max, h_P512[(size_t)a * nL + b]);
     const uint32_t t_ceil = (uint32_t)ceilf(t_max);
-    const bool fast_permeable = permeable && !mt && s->d_nbr && !want_labels && t_ceil <= 64u;
+    const bool fast_permeable = permeable && !mt && !rs && s->d_nbr && !want_labels && t_ceil <= 64u;
 
     const int nWk = rms_kernel_waves(nW);        // waveforms the step kernel is compiled for; the extra ones carry zero weight
     rc = rms_walkers_reserve_waves(w, nWk, stream);
@@ -274,6 +275,7 @@ extern "C" int rms_run(const rms_substrate* s, rms_walkers* w, const rms_run_des
     sp.s_tab = b_tabs.as<float>(); sp.rate = sp.s_tab + nL; sp.P512 = sp.rate + nL; sp.n_labels = nL;
     sp.PMT = mt ? sp.P512 + (size_t)nL * nL : nullptr;
     sp.t_ceil = t_ceil;
+    sp.rejection = rs ? 1 : 0;
     sp.counters = w->d_counters; sp.n_wave = nW; sp.wave_stride = nT; sp.wsuf_stride = nT + 1;
 
     rms_reduce_params rp;

@@ -244,6 +244,13 @@ __global__ void __launch_bounds__(RMS_BLOCK) rms_step_kernel(const __grid_consta
                         float px = fx, py = fy, pz = fz;
                         bool dx = false, dy = false, dz = false, saturated = false;
                         int e = 0;
+                        // rejection sampling (R21): what a cancelled step has to put back
+                        const int wx_in = wx, wy_in = wy, wz_in = wz, dIx_in = dIx, dIy_in = dIy, dIz_in = dIz;
+                        const uint32_t L_in = L, j_rate_in = j_rate;
+                        const float s_in = s, rate_in = rate, relax_in = relax;
+                        const unsigned n_perm_in = n_perm;
+                        int ev[3] = {0, 0, 0}, n_ev = 0;                // face passages of this step: +-(axis + 1)
+                        bool cancelled = false;
                         uint32_t v0 = 0, v1 = 0, v2 = 0, v3 = 0;
                         bool have_v = false;
                         uint32_t m0 = 0, m1 = 0, m2 = 0, m3 = 0;
@@ -317,6 +324,7 @@ __global__ void __launch_bounds__(RMS_BLOCK) rms_step_kernel(const __grid_consta
                                 if (isx) wx = nwk; else if (isy) wy = nwk; else wz = nwk;
                                 const int sg1 = neg ? -1 : 1;
                                 if (isx) dIx += sg1; else if (isy) dIy += sg1; else dIz += sg1;
+                                ev[n_ev++] = sg1 * (isx ? 1 : (isy ? 2 : 3));
                                 if (NW > 0 && acc_rem) {
                                     if (WMODE == RMS_WMODE_CONST) {
 #pragma unroll
@@ -345,11 +353,40 @@ __global__ void __launch_bounds__(RMS_BLOCK) rms_step_kernel(const __grid_consta
                                     s = s_new;
                                     L = Ln;
                                 }
+                            } else if (p.rejection) {
+                                cancelled = true;                       // rejection sampling: the walker does not move for the step
+                                break;
                             } else {
                                 pk = plane;
                                 if (isx) rx = -rx; else if (isy) ry = -ry; else rz = -rz;   // elastic collision
                             }
                             if (isx) { px = pk; dx = true; } else if (isy) { py = pk; dy = true; } else { pz = pk; dz = true; }
+                        }
+                        if (cancelled) {
+                            // undo the face passages of the cancelled step (voxel, displacement, event-driven phase part, label)
+                            for (int q = 0; q < n_ev; ++q) {
+                                const int ax = (ev[q] < 0 ? -ev[q] : ev[q]) - 1;
+                                const bool ng = ev[q] < 0;
+                                if (NW > 0 && acc_rem) {
+                                    if (WMODE == RMS_WMODE_CONST) {
+#pragma unroll
+                                        for (int m = 0; m < NW; ++m) {
+                                            const int v = ng ? -wrem[m] : wrem[m];
+                                            if (ax == 0) A32[m][0] -= v; else if (ax == 1) A32[m][1] -= v; else A32[m][2] -= v;
+                                        }
+                                    } else {
+#pragma unroll
+                                        for (int m = 0; m < NW; ++m) {
+                                            double v = p.wsuf[(size_t)m * p.wsuf_stride + (j - p.step0)] - p.wsuf_end[m];
+                                            v = ng ? -v : v;
+                                            if (ax == 0) Ad[m][0] -= v; else if (ax == 1) Ad[m][1] -= v; else Ad[m][2] -= v;
+                                        }
+                                    }
+                                }
+                            }
+                            wx = wx_in; wy = wy_in; wz = wz_in; dIx = dIx_in; dIy = dIy_in; dIz = dIz_in;
+                            L = L_in; s = s_in; rate = rate_in; relax = relax_in; j_rate = j_rate_in; n_perm = n_perm_in;
+                            px = fx; py = fy; pz = fz; rx = 0.f; ry = 0.f; rz = 0.f;
                         }
                         const float gx = px + rx, gy = py + ry, gz = pz + rz;
                         fx = fminf(fmaxf(gx, 0.f), RMS_ONE_MINUS);

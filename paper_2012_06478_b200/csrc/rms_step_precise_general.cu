@@ -76,6 +76,13 @@ __global__ void __launch_bounds__(RMS_GBLOCK) rms_step_precise_general_kernel(co
         bool have_v = false;
         uint32_t m0 = 0, m1 = 0, m2 = 0, m3 = 0;
         bool have_m = false, saturated = false;
+        // rejection sampling (R21): what a cancelled step has to put back
+        const int wx_in = wx, wy_in = wy, wz_in = wz, dIx_in = dIx, dIy_in = dIy, dIz_in = dIz;
+        const uint32_t L_in = L;
+        const double s_in = s, rate_in = rate;
+        const unsigned n_perm_in = n_perm;
+        int ev[3] = {0, 0, 0}, n_ev = 0;
+        bool cancelled = false;
 #pragma unroll 1
         for (int it = 0; it < 3; ++it) {
             const double gx = px + rx, gy = py + ry, gz = pz + rz;
@@ -130,6 +137,7 @@ __global__ void __launch_bounds__(RMS_GBLOCK) rms_step_precise_general_kernel(co
                 if (isx) wx = nwk; else if (isy) wy = nwk; else wz = nwk;
                 const int sg1 = neg ? -1 : 1;
                 if (isx) dIx += sg1; else if (isy) dIy += sg1; else dIz += sg1;
+                ev[n_ev++] = sg1 * (isx ? 1 : (isy ? 2 : 3));
 #pragma unroll
                 for (int m = 0; m < NW; ++m) {
                     double v = p.wsuf[(size_t)m * p.wsuf_stride + t] - p.wsuf_end[m];
@@ -144,11 +152,28 @@ __global__ void __launch_bounds__(RMS_GBLOCK) rms_step_precise_general_kernel(co
                     rate = (double)__ldg(p.rate + Ln);
                     L = Ln;
                 }
+            } else if (p.rejection) {
+                cancelled = true;                                              // rejection sampling: the walker does not move for the step
+                break;
             } else {
                 pk = plane;
                 if (isx) rx = -rx; else if (isy) ry = -ry; else rz = -rz;      // elastic collision
             }
             if (isx) { px = pk; dx = true; } else if (isy) { py = pk; dy = true; } else { pz = pk; dz = true; }
+        }
+        if (cancelled) {
+            for (int q = 0; q < n_ev; ++q) {
+                const int ax = (ev[q] < 0 ? -ev[q] : ev[q]) - 1;
+#pragma unroll
+                for (int m = 0; m < NW; ++m) {
+                    double v = p.wsuf[(size_t)m * p.wsuf_stride + t] - p.wsuf_end[m];
+                    v = ev[q] < 0 ? -v : v;
+                    if (ax == 0) Ad[m][0] -= v; else if (ax == 1) Ad[m][1] -= v; else Ad[m][2] -= v;
+                }
+            }
+            wx = wx_in; wy = wy_in; wz = wz_in; dIx = dIx_in; dIy = dIy_in; dIz = dIz_in;
+            L = L_in; s = s_in; rate = rate_in; n_perm = n_perm_in;
+            px = fx; py = fy; pz = fz; rx = 0.0; ry = 0.0; rz = 0.0;
         }
         const double one_minus = 0.99999999999999988898;
         const double gx = px + rx, gy = py + ry, gz = pz + rz;

@@ -327,7 +327,10 @@ extern "C" int rms_substrate_get_info(const rms_substrate* s, rms_substrate_info
 }
 
 // Eq.1 and Eq.3, Eq.C.15 for kappa = inf; fp64 on the host, rounded once to fp32.
-int rms_compute_tables(const rms_substrate* s, double dt, std::vector<float>& s_tab, std::vector<float>& P_tab)
+// Rejection sampling has its own permeation probability, P_T / (1 - P_T) = kappa ds / D C_d (Appendix B.1 with Eq.2a),
+// which the paper derives for equal diffusivities on both sides only (R21).
+int rms_compute_tables(const rms_substrate* s, double dt, std::vector<float>& s_tab, std::vector<float>& P_tab,
+                       bool rejection_sampling)
 {
     const int nL = s->n_labels;
     const double C3 = 2.0 / 3.0;
@@ -351,6 +354,12 @@ int rms_compute_tables(const rms_substrate* s, double dt, std::vector<float>& s_
                     P = 0;
                 } else if (isinf(k)) {
                     P = fmin(1.0, sqrt(Db / Da));
+                } else if (rejection_sampling) {
+                    RMS_REQUIRE(Da == Db, RMS_ERR_UNSUPPORTED,
+                                "rejection sampling with a permeable membrane between unequal diffusivities (labels %d, %d): "
+                                "Appendix B.1 gives P_T for equal D only", a, b);
+                    const double A = k * sqrt(6.0 * dt / Da) * C3;
+                    P = A / (1.0 + A);
                 } else {
                     const double Aab = k * sqrt(6.0 * dt / Da) * C3, Aba = k * sqrt(6.0 * dt / Db) * C3;
                     P = Aab / (1.0 + 0.5 * (Aab + Aba));

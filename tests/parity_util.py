@@ -12,10 +12,10 @@ def gpu_run(cfg_sub, cfg_seq, n_walkers, seed, first_id=0, flags=0, read_walkers
     return rms.simulate(cfg_sub, cfg_seq, n_walkers, seed, first_id=first_id, flags=flags, read_walkers=read_walkers)
 
 
-def oracle_run(cfg_sub, cfg_seq, n_walkers, seed, first_id=0):
+def oracle_run(cfg_sub, cfg_seq, n_walkers, seed, first_id=0, interaction=0):
     import oracle
     return oracle.run(cfg_sub, cfg_seq, n_walkers, seed, first_id=first_id, n_threads=oracle.rms_oracle.default_threads(),
-                      per_walker=True)
+                      per_walker=True, interaction=interaction)
 
 
 def compare(g, o, n_walkers, tol_s=TOL_S, tol_m=TOL_MOMENT, same_voxel=TOL_SAME_VOXEL, check_init=True, strict_s=False):
@@ -26,7 +26,8 @@ def compare(g, o, n_walkers, tol_s=TOL_S, tol_m=TOL_MOMENT, same_voxel=TOL_SAME_
     part company there for good; north_star allows 0.1 % of the walkers to do so.  Each such walker can move
     S by at most 2/N, which at the small N of most cases here is above 1e-4 by itself: those cases bound
     |dS| by 1e-4 + 2 n_diff / N (the agreeing walkers must agree to 1e-4) and widen the moment tolerances in
-    the same way; strict_s=True, used at full size where N is large, applies the plain tolerances
+    the same way (under rejection sampling every membrane met is such a discontinuity: a grazing step is cancelled
+    whole or not at all); strict_s=True, used at full size where N is large, applies the plain tolerances
     (DESIGN.md "Tolerances")."""
     rep = {}
     w = g["walkers"]
@@ -34,6 +35,9 @@ def compare(g, o, n_walkers, tol_s=TOL_S, tol_m=TOL_MOMENT, same_voxel=TOL_SAME_
         assert np.array_equal(w["vox0"], o["init_vox"])
         assert np.array_equal(w["off0"].astype(np.float64), o["init_off"])
     same = np.all(w["vox"] == o["final_vox"], axis=1)
+    # a walker that parted company may by chance end in the voxel of its twin (likely on the few-voxel periodic lattices
+    # of the small cases): offsets 0.01 voxel apart are no rounding difference, so it counts as diverged all the same
+    same &= np.abs(w["off"].astype(np.float64) - o["final_off"]).max(axis=1) < 0.01
     rep["same_voxel"] = float(same.mean())
     rep["n_diff"] = int((~same).sum())
     assert rep["same_voxel"] >= same_voxel, rep

@@ -440,6 +440,43 @@ def test_absorbing_membranes_magnetisation_transfer(rms):
     assert e.value.code == -3          # RMS_ERR_P_RANGE: P_MT > 1
 
 
+def test_rejection_sampling_interaction(rms):
+    """S: section 8(f) N4 -- the paper's other membrane interaction (Appendix B; R21): a step that meets a membrane it
+    does not cross is cancelled.  Impermeable cylinder (integer and non-integer waveforms: both modes of the fp32 general
+    kernel), equal-D permeable slabs with T2 contrast (P_T = A / (1 + A)), and an absorbing wall on top; fp32 and fp64,
+    against the oracle run with interaction = 1.  The elastic-collision result must differ (the flag is not a no-op)."""
+    import dataclasses
+    RS = rms.binding.RMS_RUN_REJECTION_SAMPLING
+    n = 20000
+    cyl = ri.single_cylinder(24, 8.5, 0.1)
+    seq = ri.pgse_sequence(2e-4, 1500, 0.1, 0.15, [0.0, 2.0], np.eye(3), snap_steps=[500, 1500])
+    o = oracle_run(cyl, seq, n, 31, interaction=1)
+    o_ecs = oracle_run(cyl, seq, n, 31)
+    assert np.abs(o["S"] - o_ecs["S"]).max() > 1e-3
+    for flags in (RS, RS | 8):
+        g = gpu_run(cyl, seq, n, 31, flags=flags)
+        print("rejection sampling, cylinder, flags", flags, compare(g, o, n))
+        assert g["n_encounters"] > n and g["n_permeations"] == 0
+    seq_f = dataclasses.replace(seq, wave=(seq.wave * 0.37).astype(np.float32))            # table-driven waveform
+    o = oracle_run(cyl, seq_f, n, 32, interaction=1)
+    for flags in (RS, RS | 8):
+        print("rejection sampling, non-integer waveform, flags", flags, compare(gpu_run(cyl, seq_f, n, 32, flags=flags), o, n))
+    sl = ri.slabs(6, 5, (3, 2), 0.1, D_extra=2.0, D_intra=2.0, kappa_membrane=4.0, T2_extra=0.3, T2_intra=0.6)
+    sl = dataclasses.replace(sl, rho=np.array([[0.0, 0.4], [0.2, 0.0]], np.float32))
+    seq = ri.pgse_sequence(2e-4, 800, 0.05, 0.08, [0.0, 5.0], ri.fibonacci_dirs(4), snap_steps=[399, 800])
+    o = oracle_run(sl, seq, n, 33, interaction=1)
+    for flags in (RS, RS | 8):
+        g = gpu_run(sl, seq, n, 33, flags=flags)
+        rep = compare(g, o, n)
+        print("rejection sampling, permeable + absorbing slabs, flags", flags, rep, "permeations", g["n_permeations"], o["n_permeations"])
+        assert g["n_permeations"] > 1000 and abs(g["n_permeations"] - o["n_permeations"]) <= 4 * rep["n_diff"] + 2
+        assert abs(g["n_saturations"] - o["n_saturations"]) <= 2 * rep["n_diff"] + 2
+    bad = ri.slabs(6, 5, (3, 2), 0.1, D_extra=2.0, D_intra=1.0, kappa_membrane=4.0)
+    with pytest.raises(rms.RmsError) as e:
+        gpu_run(bad, seq, 10, 1, flags=RS)
+    assert e.value.code == -7          # RMS_ERR_UNSUPPORTED: Appendix B.1 gives P_T for equal D only
+
+
 def test_degenerate_and_ragged_cases(rms):
     # one walker; 1, 2, 3 steps with a snapshot on every step; no waveform / no directions; hop of 0.99 voxel (three
     # interactions in most steps); a single-voxel pore (every face a membrane: the corner reflector of Fig.2)
