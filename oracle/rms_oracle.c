@@ -31,6 +31,9 @@
  *                        with S_x/V counted on the staircase surface of the lattice cylinder
  *   run, encounters      membrane encounters per step = surface * step / 4
  *   run, absorbing walls surviving fraction between plates = Brownstein-Tarr series (Eq.4; R = rho S/V)
+ *   run, T1 / mixing time alpha = exp(-(t_T2/T2 + t_mix/T1)) exactly per impermeable compartment (Eq.5);
+ *                        T1 = T2 reproduces the run without a mixing time; well-mixed permeable slabs:
+ *                        1 - <alpha> = f_b t_mix / T1_b to first order, for either starting compartment
  *   run, rejection sampl. D_parallel = D0 (1 - 3/16 S/V ds) between plates (Eq.B.2), uniform density
  * Parity unpinned: wide-pulse signals inside voxelised cylinders / axons have
  *   no closed form; they are pinned only through the pieces above.
@@ -360,6 +363,8 @@ typedef struct {
     lattice_t lat;
     double voxel_um;
     const double* inv_T2; /* [n_labels], 0 = no relaxation */
+    const double* inv_T1; /* [n_labels], 0 = no relaxation; used in the mixing time */
+    int64_t mix_first, mix_steps; /* steps mix_first .. mix_first + mix_steps - 1 (1-based) are the mixing time */
     const uint16_t* label_class;
     int n_classes;
     /* walkers */
@@ -435,7 +440,9 @@ static void* run_part(void* arg)
                 for (int k = 0; k < 3; ++k) Phi[3 * m + k] += w * dx[k];
             }
             /* Eq.5: whole dt to the compartment at the end of the hop (R12) */
-            R += j->dt * j->inv_T2[L]; /* (stays +inf once saturated) */
+            /* stimulated echo: during the mixing time the magnetisation is along B0 and Eq.5 runs with T1 (R22) */
+            int mixing = i >= j->mix_first && i < j->mix_first + j->mix_steps;
+            R += j->dt * (mixing ? j->inv_T1[L] : j->inv_T2[L]); /* (stays +inf once saturated) */
 
             while (snap < j->n_snap && j->snap_steps[snap] == i) {
                 double alpha = exp(-R);
@@ -483,6 +490,7 @@ int rms_oracle_run(
     uint64_t n_walkers, uint64_t first_id, const uint8_t* label_allowed, uint64_t seed,
     double dt_ms, int64_t n_steps, int n_wave, const float* wave, int n_g, const double* gamp,
     int n_dir, const double* dirs, int n_snap, const int64_t* snap_steps, int n_threads, int interaction,
+    const float* T1, int64_t mix_first, int64_t mix_steps,
     double* sum_alpha, double* sig_re, double* sig_im, double* m2, double* m4, double* snap_alpha,
     uint64_t* class_flow, uint64_t* counters,
     int32_t* final_vox, double* final_off, uint16_t* final_label,
@@ -505,7 +513,8 @@ int rms_oracle_run(
 
     double* s_tab = (double*)malloc(sizeof(double) * n_labels);
     double* P_tab = (double*)malloc(sizeof(double) * (size_t)n_labels * n_labels);
-    double* inv_T2 = (double*)malloc(sizeof(double) * n_labels);
+    double* inv_T2 = (double*)malloc(sizeof(double) * 2 * n_labels);
+    double* inv_T1 = inv_T2 ? inv_T2 + n_labels : NULL;
     double* Q_tab = rho ? (double*)malloc(sizeof(double) * (size_t)n_labels * n_labels) : NULL;
     if (!s_tab || !P_tab || !inv_T2 || (rho && !Q_tab)) { free(s_tab); free(P_tab); free(inv_T2); free(Q_tab); return ORC_ERR_OOM; }
     int st = rms_oracle_tables(n_labels, D, kappa, voxel_um, dt_ms, s_tab, P_tab);
@@ -523,17 +532,20 @@ int rms_oracle_run(
             }
     }
     if (interaction != 0 && interaction != 1) st = ORC_ERR_ARG;
+    if (mix_steps < 0 || (mix_steps > 0 && (mix_first < 1 || mix_first + mix_steps - 1 > n_steps))) st = ORC_ERR_ARG;
     if (st != ORC_OK) { free(s_tab); free(P_tab); free(inv_T2); free(Q_tab); return st; }
     for (int a = 0; a < n_labels; ++a) {
         double t2 = T2 ? (double)T2[a] : 0.0;
         inv_T2[a] = (t2 > 0.0 && !isinf(t2)) ? 1.0 / t2 : 0.0; /* T2 <= 0 or inf: no relaxation */
+        double t1 = T1 ? (double)T1[a] : 0.0;
+        inv_T1[a] = (t1 > 0.0 && !isinf(t1)) ? 1.0 / t1 : 0.0; /* likewise; T1 = NULL: no relaxation in the mixing time */
     }
 
     job_t job;
     memset(&job, 0, sizeof job);
     job.lat.nx = nx; job.lat.ny = ny; job.lat.nz = nz; job.lat.labels = labels; job.lat.n_labels = n_labels;
     job.lat.s = s_tab; job.lat.P = P_tab; job.lat.Q = Q_tab; job.lat.rejection = interaction == 1;
-    job.voxel_um = voxel_um; job.inv_T2 = inv_T2; job.label_class = label_class; job.n_classes = n_classes;
+    job.voxel_um = voxel_um; job.inv_T2 = inv_T2; job.inv_T1 = inv_T1; job.mix_first = mix_first; job.mix_steps = mix_steps; job.label_class = label_class; job.n_classes = n_classes;
     job.n_walkers = n_walkers; job.first_id = first_id; job.seed = seed; job.label_allowed = label_allowed;
     job.dt = dt_ms; job.n_steps = n_steps; job.n_wave = n_wave; job.wave = wave; job.n_g = n_g; job.gamp = gamp;
     job.n_dir = n_dir; job.dirs = dirs; job.n_snap = n_snap; job.snap_steps = snap_steps;

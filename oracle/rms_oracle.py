@@ -149,6 +149,9 @@ def run(sub, seq, n_walkers, seed, first_id=0, n_threads=1, per_walker=False, in
     kappa = np.ascontiguousarray(sub.kappa, np.float32)
     rho = getattr(sub, "rho", None)
     rho = None if rho is None else np.ascontiguousarray(rho, np.float32)
+    T1 = getattr(sub, "T1", None)
+    T1 = None if T1 is None else np.ascontiguousarray(T1, np.float32)
+    mix_first, mix_steps = int(getattr(seq, "mix_first_step", 0)), int(getattr(seq, "mix_n_steps", 0))
     lclass = np.ascontiguousarray(sub.label_class, np.uint16)
     allowed = np.ascontiguousarray(sub.label_allowed, np.uint8)
     wave = np.ascontiguousarray(seq.wave, np.float32)
@@ -175,7 +178,7 @@ def run(sub, seq, n_walkers, seed, first_id=0, n_threads=1, per_walker=False, in
         C.c_uint64(n_walkers), C.c_uint64(first_id), _p(allowed, C.c_uint8), C.c_uint64(seed),
         C.c_double(seq.dt_ms), C.c_int64(n_steps), C.c_int(n_wave), _p(wave, C.c_float), C.c_int(n_g),
         _p(gamp, C.c_double), C.c_int(n_dir), _p(dirs, C.c_double), C.c_int(n_snap), _p(snaps, C.c_int64),
-        C.c_int(n_threads), C.c_int(interaction),
+        C.c_int(n_threads), C.c_int(interaction), _p(T1, C.c_float), C.c_int64(mix_first), C.c_int64(mix_steps),
         _p(r["sum_alpha"], C.c_double), _p(r["sig_re"], C.c_double), _p(r["sig_im"], C.c_double),
         _p(r["m2"], C.c_double), _p(r["m4"], C.c_double), _p(r["snap_alpha"], C.c_double),
         _p(r["class_flow"], C.c_uint64), _p(counters, C.c_uint64),

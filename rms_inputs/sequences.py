@@ -56,6 +56,8 @@ class Sequence:
     b_nominal: np.ndarray = field(default_factory=lambda: np.zeros(0))  # [n_g] ms/um^2, for reports
     delta_ms: float = 0.0
     Delta_ms: float = 0.0
+    mix_first_step: int = 0     # stimulated echo: steps mix_first_step .. mix_first_step + mix_n_steps - 1 (1-based) are the
+    mix_n_steps: int = 0        # mixing time, relaxing with T1 instead of T2 (0 steps: none)
 
 
 def pgse_sequence(dt_ms: float, n_steps: int, delta_ms: float, Delta_ms: float, b, dirs, snap_steps=None) -> Sequence:

@@ -22,6 +22,7 @@ class Substrate:
     label_allowed: np.ndarray          # [n_labels] uint8: 1 = walkers are placed here
     meta: dict = field(default_factory=dict)
     rho: np.ndarray | None = None      # [n_labels, n_labels] float32, um/ms: surface relaxivity (absorbing membranes), or None
+    T1: np.ndarray | None = None       # [n_labels] float32, ms: relaxation during a mixing time (stimulated echo), or None
 
     @property
     def n_labels(self) -> int:

@@ -404,3 +404,56 @@ def test_rejection_sampling_bias_of_the_parallel_diffusivity_eq_b2():
     chi2 = ((counts - n_w / a_vox) ** 2 / (n_w / a_vox)).sum()
     assert chi2 < 30, counts                                   # 9 degrees of freedom
     assert rs["n_encounters"] > 0 and rs["n_permeations"] == 0
+
+
+# ------------------------------------------------------------------ T1 during a mixing time (stimulated echo)
+def test_t1_weight_during_the_mixing_time_of_a_stimulated_echo():
+    """in a stimulated echo the weight of Eq.5 runs with T1 of the compartment the walker is in during the mixing
+    time and with T2 outside it (reading R22).  Exact per impermeable compartment, identical to the plain run for
+    T1 = T2, and in well-mixed permeable slabs 1 - <alpha> = f_b t_mix / T1_b to first order whichever side a walker
+    started on (the label of the moment counts, not the initial one)."""
+    import dataclasses
+    n_steps, n_w = 500, 4000
+    seq0 = _narrow(n_steps, np.eye(3))
+    seq = dataclasses.replace(seq0, mix_first_step=101, mix_n_steps=250)          # steps 101..350
+    t_mix, t_te = 250 * DT, 250 * DT
+    sub = ri.uniform_lattice((6, 6, 6), LP, D_extra=2.0, T2_extra=0.0625)
+    sub = dataclasses.replace(sub, T1=np.array([0.25], np.float32))
+    r = oracle.run(sub, seq, n_w, seed=27)
+    assert math.isclose(r["sum_alpha"][0], n_w * math.exp(-(t_te / 0.0625 + t_mix / 0.25)), rel_tol=1e-12)
+    # one step of mixing time at the very start / the very end: the window is 1-based and inclusive
+    for first in (1, n_steps):
+        r1 = oracle.run(sub, dataclasses.replace(seq0, mix_first_step=first, mix_n_steps=1), 50, seed=27)
+        assert math.isclose(r1["sum_alpha"][0], 50 * math.exp(-((n_steps - 1) * DT / 0.0625 + DT / 0.25)), rel_tol=1e-12)
+    # no T1 given: no relaxation in the mixing time
+    r = oracle.run(dataclasses.replace(sub, T1=None), seq, n_w, seed=27)
+    assert math.isclose(r["sum_alpha"][0], n_w * math.exp(-t_te / 0.0625), rel_tol=1e-12)
+    # impermeable plates, each class with its own T2 and T1; the snapshot inside the window sees part of it
+    sl = ri.slabs(5, 7, (3, 3), LP, D_extra=2.0, D_intra=1.0, T2_extra=0.03125, T2_intra=0.125)
+    sl = dataclasses.replace(sl, T1=np.array([0.5, 0.25], np.float32))
+    seq_s = dataclasses.replace(seq, snap_steps=np.array([200, n_steps], np.int64))
+    r = oracle.run(sl, seq_s, n_w, seed=27)
+    n0, n1 = r["class_flow"][1, 0, 0], r["class_flow"][1, 1, 1]
+    assert n0 + n1 == n_w
+    assert math.isclose(r["sum_alpha"][0], n0 * math.exp(-(t_te / 0.03125 + t_mix / 0.5)), rel_tol=1e-12)
+    assert math.isclose(r["sum_alpha"][1], n1 * math.exp(-(t_te / 0.125 + t_mix / 0.25)), rel_tol=1e-12)
+    assert math.isclose(r["snap_alpha"][0, 1], n1 * math.exp(-(100 * DT / 0.125 + 100 * DT / 0.25)), rel_tol=1e-12)
+    # T1 = T2: the mixing time changes nothing
+    same = dataclasses.replace(sl, T1=sl.T2.copy())
+    ra, rb = oracle.run(same, seq_s, n_w, seed=27), oracle.run(sl, seq0, n_w, seed=27)
+    assert np.array_equal(ra["sum_alpha"], rb["sum_alpha"])
+    # permeable, equal D (uniform density), relaxation in the mixing time only and in compartment b only
+    n_steps, n_w = 3000, 40000
+    seq = dataclasses.replace(_narrow(n_steps, np.eye(3)), mix_first_step=2001, mix_n_steps=1000)
+    t_mix = 1000 * DT
+    ex = ri.slabs(5, 7, (3, 3), LP, D_extra=2.0, D_intra=2.0, kappa_membrane=30.0)
+    T1b = 4.0
+    ex = dataclasses.replace(ex, T1=np.array([np.inf, T1b], np.float32))
+    r = oracle.run(ex, seq, n_w, seed=29, n_threads=THREADS)
+    f_b = 7 / 12
+    x = f_b * t_mix / T1b
+    assert r["n_permeations"] > 10000 and 0.02 < x < 0.04
+    n_cls = r["class_flow"][0].sum(axis=1)
+    for c in (0, 1):        # well mixed after 2000 steps (exchange time ~ a / (2 kappa) = 0.01 ms << 0.4 ms): both classes alike
+        loss = 1 - r["sum_alpha"][c] / n_cls[c]
+        assert abs(loss - x) < 0.04 * x + x * x, (c, loss, x)
