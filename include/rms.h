@@ -56,6 +56,8 @@ typedef struct rms_walkers rms_walkers;     /* opaque */
  * rho          [n_labels*n_labels] surface relaxivity um/ms of the membrane met by a walker in label a towards label b
  *              (absorbing membrane / magnetisation transfer): the encounter saturates the walker
  *              (alpha_rho = 0, Eq.4) with probability rho_ab ds_a / D_a C_d; NULL = none (host)
+ * T1           [n_labels] ms, the relaxation time during the mixing time of a stimulated echo (see
+ *              rms_run_desc.mix_first_step); +inf or <= 0 means no relaxation; NULL = none (host)
  * label_class  [n_labels] uint16 output compartment class of each label, < n_classes <= 65535; NULL = all 0 (host).
  *              Two classes (extra / intra-cellular) are the usual choice; class = label gives per-cell outputs.
  * flags        RMS_LABELS_ON_DEVICE | RMS_ADOPT_DEVICE_PTR | RMS_NO_BRICKS | RMS_LAYOUT_X_FASTEST | RMS_LAYOUT_Z_FASTEST | RMS_LAYOUT_AUTO
@@ -85,6 +87,7 @@ typedef struct {
     const uint16_t* label_class;
     int32_t n_classes;
     uint32_t flags;
+    const float* T1;
 } rms_substrate_desc;
 
 int rms_substrate_create(const rms_substrate_desc* desc, void* cuda_stream, rms_substrate** out);
@@ -144,6 +147,11 @@ int rms_walkers_destroy(rms_walkers* w);
  *             (fp32, or fp64 with RMS_RUN_FP64); biased near membranes by Eq.B.2, which is why elastic
  *             collision is the default.
  *
+ * mix_first_step, mix_n_steps  the mixing time of a stimulated echo: in these steps Eq.5 runs with the T1 of
+ *             the compartment the walker is in, in all others with its T2.  The window lies inside 1..n_steps
+ *             (RMS_ERR_ARG otherwise); the caller keeps the waveforms at 0 there (the stored magnetisation
+ *             collects no phase; not enforced).  The window edges become launch boundaries, nothing else changes.
+ *
  * A second rms_run on the same walkers continues the trajectories (the random numbers are keyed on the
  * absolute step), so long runs may be chunked; phases and T2 weights keep accumulating.
  *
@@ -179,6 +187,8 @@ typedef struct {
     int32_t n_snap;
     const int64_t* snap_steps;
     uint32_t flags;
+    int64_t mix_first_step;     /* stimulated echo: steps mix_first_step .. mix_first_step + mix_n_steps - 1 */
+    int64_t mix_n_steps;        /* of this call (1-based) relax with T1 instead of T2; 0 = no mixing time            */
 } rms_run_desc;
 
 typedef struct {

@@ -30,11 +30,12 @@ def simulate(sub, seq, n_walkers, seed, first_id=0, flags=0, substrate_flags=0, 
     """
     labels = device_labels if device_labels is not None else sub.labels
     S = B.rms_substrate_create(labels, sub.voxel_um, sub.D, sub.T2, sub.kappa, sub.label_class, sub.n_classes,
-                               flags=substrate_flags, stream=stream, rho=getattr(sub, "rho", None))
+                               flags=substrate_flags, stream=stream, rho=getattr(sub, "rho", None), T1=getattr(sub, "T1", None))
     W = None
     try:
         W = B.rms_walkers_init(S, n_walkers, first_id, sub.label_allowed, seed, stream=stream)
-        r = B.rms_run(S, W, seq.dt_ms, seq.n_steps, seq.wave, seq.gamp, seq.dirs, seq.snap_steps, flags=flags, stream=stream)
+        r = B.rms_run(S, W, seq.dt_ms, seq.n_steps, seq.wave, seq.gamp, seq.dirs, seq.snap_steps, flags=flags, stream=stream,
+                      mix_first_step=getattr(seq, "mix_first_step", 0), mix_n_steps=getattr(seq, "mix_n_steps", 0))
         if read_walkers:
             r["walkers"] = W.read(stream=stream)
         r["substrate_info"] = S.info()

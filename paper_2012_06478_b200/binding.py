@@ -45,7 +45,8 @@ class RmsError(RuntimeError):
 class SubstrateDesc(C.Structure):
     _fields_ = [("nx", C.c_int32), ("ny", C.c_int32), ("nz", C.c_int32), ("voxel_um", C.c_double),
                 ("labels", C.c_void_p), ("n_labels", C.c_int32), ("D", C.c_void_p), ("T2", C.c_void_p),
-                ("kappa", C.c_void_p), ("rho", C.c_void_p), ("label_class", C.c_void_p), ("n_classes", C.c_int32), ("flags", C.c_uint32)]
+                ("kappa", C.c_void_p), ("rho", C.c_void_p), ("label_class", C.c_void_p), ("n_classes", C.c_int32), ("flags", C.c_uint32),
+                ("T1", C.c_void_p)]
 
 
 class SubstrateInfo(C.Structure):
@@ -57,7 +58,8 @@ class SubstrateInfo(C.Structure):
 class RunDesc(C.Structure):
     _fields_ = [("dt_ms", C.c_double), ("n_steps", C.c_int64), ("n_wave", C.c_int32), ("wave", C.c_void_p),
                 ("n_g", C.c_int32), ("gamp", C.c_void_p), ("n_dir", C.c_int32), ("dirs", C.c_void_p),
-                ("n_snap", C.c_int32), ("snap_steps", C.c_void_p), ("flags", C.c_uint32)]
+                ("n_snap", C.c_int32), ("snap_steps", C.c_void_p), ("flags", C.c_uint32),
+                ("mix_first_step", C.c_int64), ("mix_n_steps", C.c_int64)]
 
 
 class Result(C.Structure):
@@ -151,7 +153,7 @@ class Substrate:
 
 
 def rms_substrate_create(labels, voxel_um, D, T2=None, kappa=None, label_class=None, n_classes=1, flags=0,
-                         stream=None, rho=None) -> Substrate:
+                         stream=None, rho=None, T1=None) -> Substrate:
     """labels: numpy uint16 (nz, ny, nx) on the host, or a torch.uint16/int16 CUDA tensor of that shape
     (then the lattice is adopted in place, no copy)."""
     lib = load_library()
@@ -173,8 +175,9 @@ def rms_substrate_create(labels, voxel_um, D, T2=None, kappa=None, label_class=N
     kappa = _host(kappa, np.float32)
     label_class = _host(label_class, np.uint16)
     rho = _host(rho, np.float32)
+    T1 = _host(T1, np.float32)
     d = SubstrateDesc(nx, ny, nz, float(voxel_um), lab_ptr, int(D.size), _ptr(D), _ptr(T2), _ptr(kappa), _ptr(rho), _ptr(label_class),
-                      int(n_classes), int(flags))
+                      int(n_classes), int(flags), _ptr(T1))
     h = C.c_void_p()
     _check(lib.rms_substrate_create(C.byref(d), _stream_ptr(stream), C.byref(h)))
     adopt = bool(flags & RMS_ADOPT_DEVICE_PTR)
@@ -221,7 +224,7 @@ def rms_walkers_init(substrate: Substrate, n_walkers, first_walker_id=0, label_a
 
 
 def rms_run(substrate: Substrate, walkers: Walkers, dt_ms, n_steps, wave=None, gamp=None, dirs=None, snap_steps=None,
-            flags=0, stream=None) -> dict:
+            flags=0, stream=None, mix_first_step=0, mix_n_steps=0) -> dict:
     """Returns a dict of numpy arrays named as in rms_result (include/rms.h)."""
     wave = _host(wave, np.float32)
     gamp = _host(gamp, np.float64)
@@ -239,7 +242,7 @@ def rms_run(substrate: Substrate, walkers: Walkers, dt_ms, n_steps, wave=None, g
              class_flow=np.zeros((n_snap, nC, nC), np.uint64), S_re=np.zeros((n_wave, n_g, n_dir)),
              S_im=np.zeros((n_wave, n_g, n_dir)), Dapp=np.zeros((n_snap, n_dir)), Kapp=np.zeros((n_snap, n_dir)))
     d = RunDesc(float(dt_ms), int(n_steps), n_wave, _ptr(wave), n_g, _ptr(gamp), n_dir, _ptr(dirs), n_snap, _ptr(snaps),
-                int(flags))
+                int(flags), int(mix_first_step), int(mix_n_steps))
     res = Result()
     for k in ("sum_alpha", "sig_re", "sig_im", "m2", "m4", "snap_alpha", "class_flow", "S_re", "S_im", "Dapp", "Kapp"):
         setattr(res, k, r[k].ctypes.data)

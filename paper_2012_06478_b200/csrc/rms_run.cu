@@ -101,11 +101,16 @@ extern "C" int rms_run(const rms_substrate* s, rms_walkers* w, const rms_run_des
     int rc = rms_compute_tables(s, d->dt_ms, s_tab, P_tab, rs);
     if (rc != RMS_OK) return rc;
     const bool mt = !s->rho.empty();             // absorbing membranes (Eq.4)
-    std::vector<float> tabs((size_t)nL * 2 + (size_t)nL * nL * (mt ? 2 : 1));
+    // stimulated echo (R22): the steps of the mixing time relax with T1; its edges become launch boundaries
+    const int64_t mix0 = d->mix_first_step, mixN = d->mix_n_steps;
+    RMS_REQUIRE(mixN >= 0 && (mixN == 0 || (mix0 >= 1 && mix0 + mixN - 1 <= nT)), RMS_ERR_ARG,
+                "mixing time (steps %lld .. %lld) must lie inside 1 .. n_steps", (long long)mix0, (long long)(mix0 + mixN - 1));
+    std::vector<float> tabs((size_t)nL * 3 + (size_t)nL * nL * (mt ? 2 : 1));
     float* h_s = tabs.data();
     float* h_rate = h_s + nL;
     float* h_P512 = h_rate + nL;
     float* h_PMT = h_P512 + (size_t)nL * nL;
+    float* h_rate1 = h_PMT + (mt ? (size_t)nL * nL : 0);       // dt / T1
     if (mt)       // P_MT(a->b) = rho_ab ds_a / D_a C_d, C_3 = 2/3 (R20), fp64 then rounded once to fp32 (R6)
         for (int a = 0; a < nL; ++a)
             for (int b = 0; b < nL; ++b) {
@@ -118,6 +123,8 @@ extern "C" int rms_run(const rms_substrate* s, rms_walkers* w, const rms_run_des
         h_s[a] = s_tab[a];
         const float t2 = s->T2[a];
         h_rate[a] = (t2 > 0 && isfinite(t2)) ? (float)(d->dt_ms / (double)t2) : 0.f;
+        const float t1 = s->T1.empty() ? 0.f : s->T1[a];
+        h_rate1[a] = (t1 > 0 && isfinite(t1)) ? (float)(d->dt_ms / (double)t1) : 0.f;
         for (int b = 0; b < nL; ++b) {
             h_P512[(size_t)a * nL + b] = 512.f * P_tab[(size_t)a * nL + b];
             if (a != b && P_tab[(size_t)a * nL + b] > 0.f) permeable = true;
@@ -160,6 +167,12 @@ extern "C" int rms_run(const rms_substrate* s, rms_walkers* w, const rms_run_des
     std::vector<int64_t> bounds;
     for (int i = 0; i < nS; ++i) bounds.push_back(d->snap_steps[i]);
     if (bounds.empty() || bounds.back() != nT) bounds.push_back(nT);
+    if (mixN > 0) {
+        if (mix0 > 1) bounds.push_back(mix0 - 1);
+        bounds.push_back(mix0 + mixN - 1);
+        std::sort(bounds.begin(), bounds.end());
+        bounds.erase(std::unique(bounds.begin(), bounds.end()), bounds.end());
+    }
 
     std::vector<rms_segment> segs;
     std::vector<std::pair<size_t, size_t>> seg_range;   // per launch: [first, count)
@@ -274,6 +287,8 @@ extern "C" int rms_run(const rms_substrate* s, rms_walkers* w, const rms_run_des
     sp.st = w->a; sp.n = n; sp.first_id = w->first_id; sp.rk = rms_make_keys(w->seed);
     sp.s_tab = b_tabs.as<float>(); sp.rate = sp.s_tab + nL; sp.P512 = sp.rate + nL; sp.n_labels = nL;
     sp.PMT = mt ? sp.P512 + (size_t)nL * nL : nullptr;
+    const float* rate_T2 = sp.rate;
+    const float* rate_T1 = sp.P512 + (size_t)nL * nL * (mt ? 2 : 1);
     sp.t_ceil = t_ceil;
     sp.rejection = rs ? 1 : 0;
     sp.counters = w->d_counters; sp.n_wave = nW; sp.wave_stride = nT; sp.wsuf_stride = nT + 1;
@@ -297,6 +312,8 @@ extern "C" int rms_run(const rms_substrate* s, rms_walkers* w, const rms_run_des
                 if (rc != RMS_OK) return rc;
                 sp.order = b_order.as<uint32_t>();
             }
+            const bool mixing = mixN > 0 && a + 1 >= mix0 && b <= mix0 + mixN - 1;
+            sp.rate = mixing ? rate_T1 : rate_T2;
             sp.step0 = (uint32_t)(w->steps_done + (uint64_t)a);
             sp.n_steps = (uint32_t)(b - a);
             for (int m = 0; m < nW; ++m) {

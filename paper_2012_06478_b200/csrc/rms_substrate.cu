@@ -218,6 +218,7 @@ extern "C" int rms_substrate_create(const rms_substrate_desc* d, void* cuda_stre
     if (d->kappa) s->kappa.assign(d->kappa, d->kappa + (size_t)nL * nL); else s->kappa.assign((size_t)nL * nL, 0.f);
     if (d->label_class) s->label_class.assign(d->label_class, d->label_class + nL); else s->label_class.assign(nL, 0);
     if (any_rho) s->rho.assign(d->rho, d->rho + (size_t)nL * nL);
+    if (d->T1) s->T1.assign(d->T1, d->T1 + nL);
     s->all_impermeable = all_imp;
 
     int rc = RMS_OK;

@@ -477,6 +477,41 @@ def test_rejection_sampling_interaction(rms):
     assert e.value.code == -7          # RMS_ERR_UNSUPPORTED: Appendix B.1 gives P_T for equal D only
 
 
+def test_t1_weighting_in_the_mixing_time_of_a_stimulated_echo(rms):
+    """S: section 8(f) N3, second half -- P:135 (R22): the steps of the mixing time relax with T1 of the walker's compartment.
+    Impermeable cylinder (specialised kernels), permeable slabs with D, T2 and T1 contrast (general kernels) and weakly
+    permeable ones (the redo path of the specialised kernel); snapshots inside the window; windows touching step 1 and
+    the last step; fp32 and fp64."""
+    import dataclasses
+    n = 20000
+    cyl = dataclasses.replace(ri.single_cylinder(24, 8.5, 0.1), T1=np.array([0.9, 0.4], np.float32))
+    cyl = dataclasses.replace(cyl, T2=np.array([0.3, 0.15], np.float32))
+    base = ri.pgse_sequence(2e-4, 1500, 0.06, 0.24, [0.0, 2.0], np.eye(3), snap_steps=[500, 900, 1500])   # lobes 1..300, 1201..1500
+    for first, cnt in ((301, 900), (1, 1500), (1500, 1), (700, 1)):
+        seq = dataclasses.replace(base, mix_first_step=first, mix_n_steps=cnt)
+        if cnt == 1500:
+            seq = dataclasses.replace(seq, wave=np.zeros_like(base.wave))
+        o = oracle_run(cyl, seq, n, 41)
+        for flags in (0, 2, 8):
+            g = gpu_run(cyl, seq, n, 41, flags=flags)
+            print("stimulated echo, cylinder, window", first, cnt, "flags", flags, compare(g, o, n))
+    o_t2 = oracle_run(cyl, base, n, 41)
+    assert abs(o["sum_alpha"].sum() / o_t2["sum_alpha"].sum() - 1) > 1e-4                     # the window is not a no-op
+    for kappa, name in ((4.0, "permeable"), (0.05, "weakly permeable")):
+        sl = ri.slabs(6, 5, (3, 2), 0.1, D_extra=2.0, D_intra=1.0, kappa_membrane=kappa, T2_extra=0.3, T2_intra=0.6)
+        sl = dataclasses.replace(sl, T1=np.array([1.5, 0.2], np.float32))
+        seq = ri.pgse_sequence(2e-4, 800, 0.03, 0.13, [0.0, 5.0], ri.fibonacci_dirs(4), snap_steps=[399, 800])  # lobes 1..150, 651..800
+        seq = dataclasses.replace(seq, mix_first_step=151, mix_n_steps=500)
+        o = oracle_run(sl, seq, n, 43)
+        for flags in (0, 2, 8):
+            g = gpu_run(sl, seq, n, 43, flags=flags)
+            print("stimulated echo,", name, "slabs, flags", flags, compare(g, o, n), "permeations", g["n_permeations"])
+            assert g["n_permeations"] > 100
+    with pytest.raises(rms.RmsError) as e:
+        gpu_run(cyl, dataclasses.replace(base, mix_first_step=1400, mix_n_steps=200), 10, 1)
+    assert e.value.code == -1          # RMS_ERR_ARG: the window leaves 1 .. n_steps
+
+
 def test_degenerate_and_ragged_cases(rms):
     # one walker; 1, 2, 3 steps with a snapshot on every step; no waveform / no directions; hop of 0.99 voxel (three
     # interactions in most steps); a single-voxel pore (every face a membrane: the corner reflector of Fig.2)
