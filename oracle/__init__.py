@@ -12,5 +12,6 @@ from .rms_oracle import (  # noqa: F401
     init_walker,
     run,
     normalise,
+    tensor_signal,
     OracleError,
 )

@@ -34,6 +34,8 @@
  *   run, T1 / mixing time alpha = exp(-(t_T2/T2 + t_mix/T1)) exactly per impermeable compartment (Eq.5);
  *                        T1 = T2 reproduces the run without a mixing time; well-mixed permeable slabs:
  *                        1 - <alpha> = f_b t_mix / T1_b to first order, for either starting compartment
+ *   tensor_signal (rms_oracle.py)  waveform on one axis rotated onto n = scalar waveform along n (same walkers, 1e-12);
+ *                        free walk: <e^{-i phi}> = prod_k sinc(c ds |W_k|), W_k the vector suffix sums of g
  *   run, rejection sampl. D_parallel = D0 (1 - 3/16 S/V ds) between plates (Eq.B.2), uniform density
  * Parity unpinned: wide-pulse signals inside voxelised cylinders / axons have
  *   no closed form; they are pinned only through the pieces above.

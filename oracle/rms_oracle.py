@@ -193,5 +193,40 @@ def run(sub, seq, n_walkers, seed, first_id=0, n_threads=1, per_walker=False, in
     return normalise(r, seq.dt_ms, snaps)
 
 
+def tensor_signal(sub, seq, r):
+    """Eq.7 for gradient waveforms that change direction in time (B-tensor encoding; the paper's "arbitrary diffusion gradient
+    waveforms"; reading R23 in DESIGN.md), from the per-walker phase vectors of run(..., per_walker=True).
+
+    A tensor waveform t drives the gradient axes x, y, z with the scalar waveforms seq.tensor_waves[t] = (m_x, m_y, m_z)
+    (-1: axis off); with the rotation R_k (seq.rots[k], g_lab = R_k g) and the amplitude seq.tensor_gamp[t, g] the phase
+    of Eq.7 is phi = gamp dt l_p sum_a (R_k e_a) . Phi_{m_a}, Phi_m = sum_i w_m[i] (x_i - x_0) in voxels.
+    Returns tsig_re/tsig_im [n_tensor, n_g, n_rot, n_classes] (by class of the initial label) and tS [n_tensor, n_g, n_rot]."""
+    tw = np.asarray(seq.tensor_waves, np.int64).reshape(-1, 3)
+    tg = np.asarray(seq.tensor_gamp, np.float64).reshape(tw.shape[0], -1)
+    rots = np.asarray(seq.rots, np.float64).reshape(-1, 3, 3)
+    nC = int(sub.n_classes)
+    iv = r["init_vox"]
+    lab0 = np.asarray(sub.labels)[iv[:, 2], iv[:, 1], iv[:, 0]]
+    cls0 = np.asarray(sub.label_class)[lab0]
+    alpha = np.exp(-r["relax"])
+    phi = r["phi"]                                            # [n_walkers, n_wave, 3]
+    re = np.zeros((tw.shape[0], tg.shape[1], rots.shape[0], nC))
+    im = np.zeros_like(re)
+    for t in range(tw.shape[0]):
+        for k in range(rots.shape[0]):
+            proj = np.zeros(phi.shape[0])
+            for a in range(3):
+                if tw[t, a] >= 0:
+                    proj += phi[:, tw[t, a], :] @ rots[k][:, a]       # (R_k e_a) . Phi_{m_a}
+            for g in range(tg.shape[1]):
+                ph = tg[t, g] * seq.dt_ms * sub.voxel_um * proj
+                for c in range(nC):
+                    sel = cls0 == c
+                    re[t, g, k, c] = np.sum(alpha[sel] * np.cos(ph[sel]))
+                    im[t, g, k, c] = -np.sum(alpha[sel] * np.sin(ph[sel]))
+    tS = (re.sum(-1) + 1j * im.sum(-1)) / r["sum_alpha"].sum()
+    return dict(tsig_re=re, tsig_im=im, tS=tS)
+
+
 def default_threads() -> int:
     return len(os.sched_getaffinity(0))

@@ -58,6 +58,9 @@ class Sequence:
     Delta_ms: float = 0.0
     mix_first_step: int = 0     # stimulated echo: steps mix_first_step .. mix_first_step + mix_n_steps - 1 (1-based) are the
     mix_n_steps: int = 0        # mixing time, relaxing with T1 instead of T2 (0 steps: none)
+    tensor_waves: np.ndarray | None = None   # [n_tensor, 3] int32: scalar waveform on gradient axis x, y, z (-1: off)
+    tensor_gamp: np.ndarray | None = None    # [n_tensor, n_g] float64, rad/(ms um)
+    rots: np.ndarray | None = None           # [n_rot, 3, 3] float64: g_lab = R g
 
 
 def pgse_sequence(dt_ms: float, n_steps: int, delta_ms: float, Delta_ms: float, b, dirs, snap_steps=None) -> Sequence:

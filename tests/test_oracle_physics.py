@@ -457,3 +457,65 @@ def test_t1_weight_during_the_mixing_time_of_a_stimulated_echo():
     for c in (0, 1):        # well mixed after 2000 steps (exchange time ~ a / (2 kappa) = 0.01 ms << 0.4 ms): both classes alike
         loss = 1 - r["sum_alpha"][c] / n_cls[c]
         assert abs(loss - x) < 0.04 * x + x * x, (c, loss, x)
+
+
+# ------------------------------------------------------------------ gradient waveforms that change direction (B-tensor encoding)
+def _rotation_to(n):
+    """Rotation matrix whose first column is the unit vector n (so R e_x = n)."""
+    n = np.asarray(n, float) / np.linalg.norm(n)
+    a = np.array([1.0, 0.0, 0.0]) if abs(n[0]) < 0.9 else np.array([0.0, 1.0, 0.0])
+    u = np.cross(n, a); u /= np.linalg.norm(u)
+    return np.stack([n, u, np.cross(n, u)], axis=1)
+
+
+def test_tensor_encoding_reduces_to_linear_encoding_and_matches_the_free_walk_product():
+    """P:336 "arbitrary diffusion gradient waveforms" (reading R23): phi = gamp dt l_p sum_a (R e_a) . Phi_{m_a}.
+    (i) a waveform on the x gradient axis rotated by R equals the scalar waveform along n = R e_x, and components
+    (n_x w, n_y w, n_z w) with R = 1 do too -- same walkers, so to rounding; a transposed R or swapped axes fail.
+    (ii) free diffusion, three orthogonal lobes pairs one after the other (spherical encoding): for hops of fixed length ds
+    in isotropic directions <e^{-i phi}> = prod_k sinc(c ds |W_k|), W_k = sum_{i >= k} g_i the vector suffix sums."""
+    import dataclasses
+    n = np.array([0.48, -0.6, 0.64])
+    n_steps, n_w = 120, 6000
+    w = ri.pgse_wave(n_steps, 30, 80)
+    comp = np.stack([w, n[0] * w, n[1] * w, n[2] * w]).astype(np.float32)
+    R = _rotation_to(n)
+    assert np.allclose(R.T @ R, np.eye(3)) and np.allclose(R[:, 0], n) and not np.allclose(R, R.T)
+    sub = ri.single_cylinder(16, 5.5, LP)
+    G = 1500.0
+    seq = ri.Sequence(dt_ms=DT, n_steps=n_steps, wave=comp, gamp=np.full((4, 1), G), dirs=n[None], snap_steps=np.array([n_steps]),
+                      tensor_waves=np.array([[0, -1, -1], [1, 2, 3]], np.int32), tensor_gamp=np.array([[G], [G]]),
+                      rots=np.stack([R, np.eye(3)]))
+    r = oracle.run(sub, seq, n_w, seed=61, n_threads=THREADS, per_walker=True)
+    t = oracle.tensor_signal(sub, seq, r)
+    lin = r["S"][0, 0, 0]                                     # scalar waveform w along n
+    assert abs(lin) < 0.98                                    # a real attenuation
+    assert abs(t["tS"][0, 0, 0] - lin) < 1e-12                # x-axis waveform rotated onto n
+    # the float32 components n_a w carry a 6e-8 relative rounding of n_a
+    assert abs(t["tS"][1, 0, 1] - lin) < 1e-6
+    assert abs(t["tS"][0, 0, 1] - lin) > 1e-3                 # unrotated: along x, a different signal
+    assert np.allclose(t["tsig_re"].sum(-1) / r["sum_alpha"].sum(), t["tS"].real)
+    # (ii) free diffusion
+    n_steps, n_w = 90, 200_000
+    lobes = np.zeros((3, n_steps), np.float32)
+    for a in range(3):
+        lobes[a, 30 * a:30 * a + 10] = 1.0
+        lobes[a, 30 * a + 20:30 * a + 30] = -1.0
+    free = ri.uniform_lattice((8, 8, 8), LP, D_extra=2.0)
+    G = 3000.0
+    Rz = np.array([[0.6, -0.8, 0.0], [0.8, 0.6, 0.0], [0.0, 0.0, 1.0]])
+    seq = ri.Sequence(dt_ms=DT, n_steps=n_steps, wave=lobes, gamp=np.zeros((3, 1)), dirs=np.eye(3), snap_steps=np.array([n_steps]),
+                      tensor_waves=np.array([[0, 1, 2], [0, 0, -1]], np.int32), tensor_gamp=np.array([[G], [G]]),
+                      rots=np.stack([np.eye(3), Rz]))
+    r = oracle.run(free, seq, n_w, seed=62, n_threads=THREADS, per_walker=True)
+    t = oracle.tensor_signal(free, seq, r)
+    ds = math.sqrt(6 * 2.0 * DT)
+    for ti, axes in enumerate(([0, 1, 2], [0, 0, -1])):
+        g = np.stack([lobes[m] if m >= 0 else np.zeros(n_steps) for m in axes], axis=1).astype(float)   # [n_steps, 3]
+        W = np.cumsum(g[::-1], axis=0)[::-1]                  # suffix sums: hop k moves every later position
+        x = G * DT * ds * np.linalg.norm(W, axis=1)           # rotation invariant
+        expect = np.prod(np.sinc(x / np.pi))
+        assert 0.3 < expect < 0.9
+        for k in range(2):
+            assert abs(t["tS"][ti, 0, k].real - expect) < 4 / math.sqrt(n_w), (ti, k, t["tS"][ti, 0, k], expect)
+            assert abs(t["tS"][ti, 0, k].imag) < 4 / math.sqrt(n_w)
