@@ -152,6 +152,15 @@ int rms_walkers_destroy(rms_walkers* w);
  *             (RMS_ERR_ARG otherwise); the caller keeps the waveforms at 0 there (the stored magnetisation
  *             collects no phase; not enforced).  The window edges become launch boundaries, nothing else changes.
  *
+ * n_tensor, tensor_waves [n_tensor*3], tensor_gamp [n_tensor*n_g], n_rot, rots [n_rot*9] (all host)
+ *             gradient waveforms whose direction changes in time ("arbitrary diffusion gradient waveforms", P:336;
+ *             B-tensor encoding; R23).  Tensor waveform t drives the gradient axes x, y, z with the scalar
+ *             waveforms tensor_waves[3t + a] of this run (an index into wave, or -1: axis off); rots[9k + 3b + a] is
+ *             row b, column a of the matrix R_k that takes the waveform's frame to the lattice frame (g_lab = R_k g).
+ *             Phase: phi = tensor_gamp[t*n_g + g] dt l_p sum_a (R_k e_a) . Phi_{m_a} with the same per-waveform phase
+ *             vectors Phi_m the scalar signals use, so tensor signals cost nothing in the walk.  RMS_ERR_ARG for an
+ *             index outside [-1, n_wave).
+ *
  * A second rms_run on the same walkers continues the trajectories (the random numbers are keyed on the
  * absolute step), so long runs may be chunked; phases and T2 weights keep accumulating.
  *
@@ -189,6 +198,11 @@ typedef struct {
     uint32_t flags;
     int64_t mix_first_step;     /* stimulated echo: steps mix_first_step .. mix_first_step + mix_n_steps - 1 */
     int64_t mix_n_steps;        /* of this call (1-based) relax with T1 instead of T2; 0 = no mixing time            */
+    int32_t n_tensor;           /* gradient waveforms that change direction (B-tensor encoding), see above           */
+    const int32_t* tensor_waves;
+    const double* tensor_gamp;
+    int32_t n_rot;
+    const double* rots;
 } rms_run_desc;
 
 typedef struct {
@@ -208,6 +222,10 @@ typedef struct {
     double kernel_ms;           /* device time of the step kernels of this call (CUDA events)          */
     double total_ms;            /* device time of everything this call enqueued                         */
     uint32_t n_launches;        /* kernels launched by this call                                        */
+    double* tsig_re;            /* [n_tensor][n_g][n_rot][n_classes] sum alpha cos(phi), -sum alpha sin(phi) of the  */
+    double* tsig_im;            /* tensor waveforms, and                                                             */
+    double* tS_re;              /* [n_tensor][n_g][n_rot] their Eq.7 signal, classes pooled; any may be NULL          */
+    double* tS_im;
 } rms_result;
 
 int rms_run(const rms_substrate* s, rms_walkers* w, const rms_run_desc* desc, void* cuda_stream, rms_result* out);

@@ -12,6 +12,7 @@ from . import binding as B
 
 RAW_SUMS = ("sum_alpha", "sig_re", "sig_im", "m2", "m4", "snap_alpha", "class_flow")
 COUNTERS = ("n_encounters", "n_permeations", "n_clamps", "n_saturations")
+TENSOR_SUMS = ("tsig_re", "tsig_im")          # present when the run had tensor waveforms
 
 
 def shard_range(rank: int, world: int, n_walkers: int):
@@ -35,7 +36,9 @@ def simulate(sub, seq, n_walkers, seed, first_id=0, flags=0, substrate_flags=0, 
     try:
         W = B.rms_walkers_init(S, n_walkers, first_id, sub.label_allowed, seed, stream=stream)
         r = B.rms_run(S, W, seq.dt_ms, seq.n_steps, seq.wave, seq.gamp, seq.dirs, seq.snap_steps, flags=flags, stream=stream,
-                      mix_first_step=getattr(seq, "mix_first_step", 0), mix_n_steps=getattr(seq, "mix_n_steps", 0))
+                      mix_first_step=getattr(seq, "mix_first_step", 0), mix_n_steps=getattr(seq, "mix_n_steps", 0),
+                      tensor_waves=getattr(seq, "tensor_waves", None), tensor_gamp=getattr(seq, "tensor_gamp", None),
+                      rots=getattr(seq, "rots", None))
         if read_walkers:
             r["walkers"] = W.read(stream=stream)
         r["substrate_info"] = S.info()
@@ -52,7 +55,7 @@ def simulate(sub, seq, n_walkers, seed, first_id=0, flags=0, substrate_flags=0, 
 
 def merge_results(parts, t_ms):
     """Sum the raw sums of several walker-id shards and normalise again (rms_normalise, H8)."""
-    out = {k: np.sum([p[k] for p in parts], axis=0) for k in RAW_SUMS}
+    out = {k: np.sum([p[k] for p in parts], axis=0) for k in RAW_SUMS + TENSOR_SUMS if k in parts[0]}
     for k in COUNTERS:
         out[k] = int(sum(p[k] for p in parts))
     return B.rms_normalise(out, t_ms)
@@ -66,7 +69,9 @@ def allreduce_result(r, t_ms, group=None):
 
     dev = "cuda" if dist.get_backend(group) == "nccl" else "cpu"
     out = dict(r)
-    for k in RAW_SUMS:
+    for k in RAW_SUMS + TENSOR_SUMS:
+        if k not in r:
+            continue
         a = np.ascontiguousarray(r[k])
         t = torch.from_numpy(a.astype(np.float64 if a.dtype != np.uint64 else np.int64)).to(dev)
         dist.all_reduce(t, op=dist.ReduceOp.SUM, group=group)

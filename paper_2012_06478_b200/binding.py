@@ -59,7 +59,9 @@ class RunDesc(C.Structure):
     _fields_ = [("dt_ms", C.c_double), ("n_steps", C.c_int64), ("n_wave", C.c_int32), ("wave", C.c_void_p),
                 ("n_g", C.c_int32), ("gamp", C.c_void_p), ("n_dir", C.c_int32), ("dirs", C.c_void_p),
                 ("n_snap", C.c_int32), ("snap_steps", C.c_void_p), ("flags", C.c_uint32),
-                ("mix_first_step", C.c_int64), ("mix_n_steps", C.c_int64)]
+                ("mix_first_step", C.c_int64), ("mix_n_steps", C.c_int64),
+                ("n_tensor", C.c_int32), ("tensor_waves", C.c_void_p), ("tensor_gamp", C.c_void_p),
+                ("n_rot", C.c_int32), ("rots", C.c_void_p)]
 
 
 class Result(C.Structure):
@@ -67,7 +69,8 @@ class Result(C.Structure):
                 ("m4", C.c_void_p), ("snap_alpha", C.c_void_p), ("class_flow", C.c_void_p), ("S_re", C.c_void_p),
                 ("S_im", C.c_void_p), ("Dapp", C.c_void_p), ("Kapp", C.c_void_p), ("n_encounters", C.c_uint64),
                 ("n_permeations", C.c_uint64), ("n_clamps", C.c_uint64), ("n_saturations", C.c_uint64), ("kernel_ms", C.c_double),
-                ("total_ms", C.c_double), ("n_launches", C.c_uint32)]
+                ("total_ms", C.c_double), ("n_launches", C.c_uint32),
+                ("tsig_re", C.c_void_p), ("tsig_im", C.c_void_p), ("tS_re", C.c_void_p), ("tS_im", C.c_void_p)]
 
 
 class WalkerState(C.Structure):
@@ -224,7 +227,7 @@ def rms_walkers_init(substrate: Substrate, n_walkers, first_walker_id=0, label_a
 
 
 def rms_run(substrate: Substrate, walkers: Walkers, dt_ms, n_steps, wave=None, gamp=None, dirs=None, snap_steps=None,
-            flags=0, stream=None, mix_first_step=0, mix_n_steps=0) -> dict:
+            flags=0, stream=None, mix_first_step=0, mix_n_steps=0, tensor_waves=None, tensor_gamp=None, rots=None) -> dict:
     """Returns a dict of numpy arrays named as in rms_result (include/rms.h)."""
     wave = _host(wave, np.float32)
     gamp = _host(gamp, np.float64)
@@ -237,20 +240,34 @@ def rms_run(substrate: Substrate, walkers: Walkers, dt_ms, n_steps, wave=None, g
     n_dir = 0 if dirs is None else dirs.size // 3
     n_snap = 0 if snaps is None else snaps.size
     nC = substrate.n_classes
+    tw = _host(tensor_waves, np.int32)
+    tg = _host(tensor_gamp, np.float64)
+    rots = _host(rots, np.float64)
+    n_tensor = 0 if tw is None else tw.size // 3
+    n_rot = 0 if rots is None else rots.size // 9
+    if n_tensor and (tg is None or tg.size != n_tensor * n_g):
+        raise ValueError("tensor_gamp must have shape [n_tensor, n_g]")
     r = dict(sum_alpha=np.zeros(nC), sig_re=np.zeros((n_wave, n_g, n_dir, nC)), sig_im=np.zeros((n_wave, n_g, n_dir, nC)),
              m2=np.zeros((n_snap, n_dir, nC)), m4=np.zeros((n_snap, n_dir, nC)), snap_alpha=np.zeros((n_snap, nC)),
              class_flow=np.zeros((n_snap, nC, nC), np.uint64), S_re=np.zeros((n_wave, n_g, n_dir)),
              S_im=np.zeros((n_wave, n_g, n_dir)), Dapp=np.zeros((n_snap, n_dir)), Kapp=np.zeros((n_snap, n_dir)))
     d = RunDesc(float(dt_ms), int(n_steps), n_wave, _ptr(wave), n_g, _ptr(gamp), n_dir, _ptr(dirs), n_snap, _ptr(snaps),
-                int(flags), int(mix_first_step), int(mix_n_steps))
+                int(flags), int(mix_first_step), int(mix_n_steps), n_tensor, _ptr(tw), _ptr(tg), n_rot, _ptr(rots))
     res = Result()
-    for k in ("sum_alpha", "sig_re", "sig_im", "m2", "m4", "snap_alpha", "class_flow", "S_re", "S_im", "Dapp", "Kapp"):
+    keys = ["sum_alpha", "sig_re", "sig_im", "m2", "m4", "snap_alpha", "class_flow", "S_re", "S_im", "Dapp", "Kapp"]
+    if n_tensor:
+        r.update(tsig_re=np.zeros((n_tensor, n_g, n_rot, nC)), tsig_im=np.zeros((n_tensor, n_g, n_rot, nC)),
+                 tS_re=np.zeros((n_tensor, n_g, n_rot)), tS_im=np.zeros((n_tensor, n_g, n_rot)))
+        keys += ["tsig_re", "tsig_im", "tS_re", "tS_im"]
+    for k in keys:
         setattr(res, k, r[k].ctypes.data)
     _check(load_library().rms_run(substrate.handle, walkers.handle, C.byref(d), _stream_ptr(stream), C.byref(res)))
     r.update(n_encounters=int(res.n_encounters), n_permeations=int(res.n_permeations), n_clamps=int(res.n_clamps),
              n_saturations=int(res.n_saturations),
              kernel_ms=float(res.kernel_ms), total_ms=float(res.total_ms), n_launches=int(res.n_launches))
     r["S"] = r["S_re"] + 1j * r["S_im"]
+    if n_tensor:
+        r["tS"] = r["tS_re"] + 1j * r["tS_im"]
     return r
 
 
@@ -278,4 +295,11 @@ def rms_normalise(r: dict, t_ms) -> dict:
         C.c_void_p(S_im.ctypes.data), C.c_void_p(Dapp.ctypes.data), C.c_void_p(Kapp.ctypes.data)))
     out = dict(r)
     out.update(S_re=S_re, S_im=S_im, Dapp=Dapp, Kapp=Kapp, S=S_re + 1j * S_im)
+    if "tsig_re" in r:       # tensor waveforms: Eq.7 once more, no moments
+        tre, tim = _host(r["tsig_re"], np.float64), _host(r["tsig_im"], np.float64)
+        tS_re, tS_im = np.zeros(tre.shape[:-1]), np.zeros(tre.shape[:-1])
+        _check(load_library().rms_normalise(
+            C.c_int(nC), C.c_int(tre.size // nC), C.c_void_p(_ptr(arrs["sum_alpha"])), C.c_void_p(_ptr(tre)), C.c_void_p(_ptr(tim)),
+            C.c_int(0), C.c_int(0), None, None, None, None, C.c_void_p(tS_re.ctypes.data), C.c_void_p(tS_im.ctypes.data), None, None))
+        out.update(tS_re=tS_re, tS_im=tS_im, tS=tS_re + 1j * tS_im)
     return out

@@ -223,7 +223,7 @@ int rms_launch_moments(const rms_reduce_params& p, double* d_m2, double* d_m4, d
 // qv: device [nq*3] phase per unit Phi in turns; qwave: device [nq] waveform index
 // order_by_class: device [n], needed (and used) only when n_classes > RMS_SIG_SMALL_CLASSES
 #define RMS_SIG_SMALL_CLASSES 8
-int rms_launch_signal(const rms_reduce_params& p, int n_wave, int nq, const double* d_qv, const int* d_qwave, double* d_re,
+int rms_launch_signal(const rms_reduce_params& p, int n_wave, int nq, int n_terms, const double* d_qv, const int* d_qwave, double* d_re,
                       double* d_im, double* d_sum_alpha, const uint32_t* order_by_class, cudaStream_t stream, unsigned* n_launches);
 int rms_compute_tables(const rms_substrate* s, double dt, std::vector<float>& s_tab, std::vector<float>& P_tab,
                        bool rejection_sampling = false);

@@ -109,6 +109,9 @@ int rms_launch_moments(const rms_reduce_params& p, double* d_m2, double* d_m4, d
 #define SIG_TILE 256
 #define SIG_QPT 3   // q-triples per thread: a launch covers up to RED_BLOCK * SIG_QPT = 768 of them (660 in the bench)
 
+// NT = terms per q: 1 for the scalar waveforms (phi = q . Phi_m), 3 for tensor waveforms (R23: phi = sum_a q_a . Phi_{m_a},
+// a term with wave index -1 is off); qv is [q][NT][3], qwave [q][NT]
+template <int NT>
 __global__ void __launch_bounds__(RED_BLOCK) rms_signal_kernel(const rms_reduce_params p, int n_wave, int nq_l, int q_begin,
                                                                 const double* __restrict__ qv, const int* __restrict__ qwave,
                                                                 double* __restrict__ g_re, double* __restrict__ g_im,
@@ -124,15 +127,21 @@ __global__ void __launch_bounds__(RED_BLOCK) rms_signal_kernel(const rms_reduce_
 
     for (int t = threadIdx.x; t < nq_l * nC * 2 + nC; t += RED_BLOCK) s_acc[t] = 0.0;
 
-    double qx[SIG_QPT], qy[SIG_QPT], qz[SIG_QPT];
-    int qm[SIG_QPT];
+    double qx[SIG_QPT][NT], qy[SIG_QPT][NT], qz[SIG_QPT][NT];
+    int qm[SIG_QPT][NT];
+    bool qok[SIG_QPT];
 #pragma unroll
     for (int c = 0; c < SIG_QPT; ++c) {
         const int jl = c * RED_BLOCK + threadIdx.x;
         const bool ok = jl < nq_l;
         const int j = q_begin + jl;
-        qx[c] = ok ? qv[3 * j] : 0.0; qy[c] = ok ? qv[3 * j + 1] : 0.0; qz[c] = ok ? qv[3 * j + 2] : 0.0;
-        qm[c] = ok ? qwave[j] : -1;
+        qok[c] = ok;
+#pragma unroll
+        for (int t = 0; t < NT; ++t) {
+            const int jt = j * NT + t;
+            qx[c][t] = ok ? qv[3 * jt] : 0.0; qy[c][t] = ok ? qv[3 * jt + 1] : 0.0; qz[c][t] = ok ? qv[3 * jt + 2] : 0.0;
+            qm[c][t] = ok ? qwave[jt] : -1;
+        }
     }
 
     const uint64_t n_tiles = (p.n + SIG_TILE - 1) / SIG_TILE;
@@ -160,9 +169,14 @@ __global__ void __launch_bounds__(RED_BLOCK) rms_signal_kernel(const rms_reduce_
                 const double al = (double)s_alpha[w];
 #pragma unroll
                 for (int c = 0; c < SIG_QPT; ++c) {
-                    if (qm[c] < 0) continue;
-                    const double* ph = s_phi + (size_t)qm[c] * 3 * SIG_TILE + w;
-                    const double turns = qx[c] * ph[0] + qy[c] * ph[SIG_TILE] + qz[c] * ph[2 * SIG_TILE];
+                    if (!qok[c]) continue;
+                    double turns = 0.0;
+#pragma unroll
+                    for (int t = 0; t < NT; ++t) {
+                        if (NT > 1 && qm[c][t] < 0) continue;
+                        const double* ph = s_phi + (size_t)qm[c][t] * 3 * SIG_TILE + w;
+                        turns += qx[c][t] * ph[0] + qy[c][t] * ph[SIG_TILE] + qz[c][t] * ph[2 * SIG_TILE];
+                    }
                     // phase reduced in fp64 to [-pi, pi], then the hardware sine / cosine: absolute error < 5e-7 per
                     // walker (random in sign for the sine, mean +2e-8 for the cosine) against the 1e-4 tolerance on S
                     const float ph32 = (float)(6.283185307179586 * (turns - rint(turns)));
@@ -202,6 +216,7 @@ __global__ void __launch_bounds__(RED_BLOCK) rms_signal_kernel(const rms_reduce_
 // a tile of 256 consecutive walkers is one run of a class, occasionally two or three.  Thread = up to SIG_QPT
 // (waveform, b, direction) triples; sums in registers over a run; fp64 atomics into the output at the end of each run.
 // ------------------------------------------------------------------------------------------------
+template <int NT>
 __global__ void __launch_bounds__(RED_BLOCK) rms_signal_runs_kernel(const rms_reduce_params p, int n_wave, int nq_l, int q_begin,
                                                                      const double* __restrict__ qv, const int* __restrict__ qwave,
                                                                      const uint32_t* __restrict__ order, double* __restrict__ g_re,
@@ -213,15 +228,21 @@ __global__ void __launch_bounds__(RED_BLOCK) rms_signal_runs_kernel(const rms_re
     float* s_alpha = (float*)(s_phi + (size_t)n_wave * 3 * SIG_TILE);   // [SIG_TILE]
     int* s_cls = (int*)(s_alpha + SIG_TILE);                        // [SIG_TILE]
 
-    double qx[SIG_QPT], qy[SIG_QPT], qz[SIG_QPT];
-    int qm[SIG_QPT];
+    double qx[SIG_QPT][NT], qy[SIG_QPT][NT], qz[SIG_QPT][NT];
+    int qm[SIG_QPT][NT];
+    bool qok[SIG_QPT];
 #pragma unroll
     for (int c = 0; c < SIG_QPT; ++c) {
         const int jl = c * RED_BLOCK + threadIdx.x;
         const bool ok = jl < nq_l;
         const int j = q_begin + jl;
-        qx[c] = ok ? qv[3 * j] : 0.0; qy[c] = ok ? qv[3 * j + 1] : 0.0; qz[c] = ok ? qv[3 * j + 2] : 0.0;
-        qm[c] = ok ? qwave[j] : -1;
+        qok[c] = ok;
+#pragma unroll
+        for (int t = 0; t < NT; ++t) {
+            const int jt = j * NT + t;
+            qx[c][t] = ok ? qv[3 * jt] : 0.0; qy[c][t] = ok ? qv[3 * jt + 1] : 0.0; qz[c][t] = ok ? qv[3 * jt + 2] : 0.0;
+            qm[c][t] = ok ? qwave[jt] : -1;
+        }
     }
 
     const uint64_t n_tiles = (p.n + SIG_TILE - 1) / SIG_TILE;
@@ -261,9 +282,14 @@ __global__ void __launch_bounds__(RED_BLOCK) rms_signal_runs_kernel(const rms_re
             asum += al;
 #pragma unroll
             for (int c = 0; c < SIG_QPT; ++c) {
-                if (qm[c] < 0) continue;
-                const double* ph = s_phi + (size_t)qm[c] * 3 * SIG_TILE + w;
-                const double turns = qx[c] * ph[0] + qy[c] * ph[SIG_TILE] + qz[c] * ph[2 * SIG_TILE];
+                if (!qok[c]) continue;
+                double turns = 0.0;
+#pragma unroll
+                for (int t = 0; t < NT; ++t) {
+                    if (NT > 1 && qm[c][t] < 0) continue;
+                    const double* ph = s_phi + (size_t)qm[c][t] * 3 * SIG_TILE + w;
+                    turns += qx[c][t] * ph[0] + qy[c][t] * ph[SIG_TILE] + qz[c][t] * ph[2 * SIG_TILE];
+                }
                 const float ph32 = (float)(6.283185307179586 * (turns - rint(turns)));
                 float sn, cs;
                 __sincosf(ph32, &sn, &cs);
@@ -274,9 +300,12 @@ __global__ void __launch_bounds__(RED_BLOCK) rms_signal_runs_kernel(const rms_re
     }
 }
 
-int rms_launch_signal(const rms_reduce_params& p, int n_wave, int nq, const double* d_qv, const int* d_qwave, double* d_re,
+int rms_launch_signal(const rms_reduce_params& p, int n_wave, int nq, int n_terms, const double* d_qv, const int* d_qwave, double* d_re,
                       double* d_im, double* d_sum_alpha, const uint32_t* order_by_class, cudaStream_t stream, unsigned* n_launches)
 {
+    RMS_REQUIRE(n_terms == 1 || n_terms == 3, RMS_ERR_ARG, "signal reduction: 1 or 3 terms per phase");
+    auto k_runs = n_terms == 1 ? rms_signal_runs_kernel<1> : rms_signal_runs_kernel<3>;
+    auto k_sig = n_terms == 1 ? rms_signal_kernel<1> : rms_signal_kernel<3>;
     const uint64_t n_tiles = (p.n + SIG_TILE - 1) / SIG_TILE;
     const unsigned grid = (unsigned)(n_tiles < 148ull * 2 ? n_tiles : 148ull * 2);
     const int nw = n_wave > 0 ? n_wave : 1;
@@ -284,12 +313,12 @@ int rms_launch_signal(const rms_reduce_params& p, int n_wave, int nq, const doub
         RMS_REQUIRE(order_by_class, RMS_ERR_ARG, "signal reduction with many classes needs the class ordering");
         const size_t smem = (size_t)nw * 3 * SIG_TILE * sizeof(double) + SIG_TILE * (sizeof(float) + sizeof(int));
         if (smem > 48 * 1024)
-            RMS_CUDA_TRY(cudaFuncSetAttribute(rms_signal_runs_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+            RMS_CUDA_TRY(cudaFuncSetAttribute(k_runs, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         const int q_batch = RED_BLOCK * SIG_QPT;
         int q_begin = 0;
         do {
             const int nq_l = nq - q_begin < q_batch ? nq - q_begin : q_batch;
-            rms_signal_runs_kernel<<<grid, RED_BLOCK, smem, stream>>>(p, nw, nq_l > 0 ? nq_l : 0, q_begin, d_qv, d_qwave, order_by_class,
+            k_runs<<<grid, RED_BLOCK, smem, stream>>>(p, nw, nq_l > 0 ? nq_l : 0, q_begin, d_qv, d_qwave, order_by_class,
                                                                       d_re, d_im, d_sum_alpha);
             RMS_CUDA_TRY(cudaGetLastError());
             if (n_launches) ++*n_launches;
@@ -311,8 +340,8 @@ int rms_launch_signal(const rms_reduce_params& p, int n_wave, int nq, const doub
         const int nq_l = nq - q_begin < q_batch ? nq - q_begin : q_batch;
         const size_t smem = fixed + (size_t)(nq_l > 0 ? nq_l : 0) * per_q;
         if (smem > 48 * 1024)
-            RMS_CUDA_TRY(cudaFuncSetAttribute(rms_signal_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)budget));
-        rms_signal_kernel<<<grid, RED_BLOCK, smem, stream>>>(p, nw, nq_l, q_begin, d_qv, d_qwave, d_re, d_im, d_sum_alpha);
+            RMS_CUDA_TRY(cudaFuncSetAttribute(k_sig, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)budget));
+        k_sig<<<grid, RED_BLOCK, smem, stream>>>(p, nw, nq_l, q_begin, d_qv, d_qwave, d_re, d_im, d_sum_alpha);
         RMS_CUDA_TRY(cudaGetLastError());
         if (n_launches) ++*n_launches;
         q_begin += q_batch;

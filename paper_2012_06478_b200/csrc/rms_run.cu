@@ -223,7 +223,18 @@ extern "C" int rms_run(const rms_substrate* s, rms_walkers* w, const rms_run_des
     const bool need_table = use_general && wmode == RMS_WMODE_TABLE;
 
     // ---- device scratch: tables | segments or wave tables | q vectors | result sums -------------------
-    const int nQ = nW * nG * nD;
+    const int nQs = nW * nG * nD;                                    // scalar waveforms x b x direction
+    const int nTen = d->n_tensor, nR = d->n_rot;
+    RMS_REQUIRE(nTen >= 0 && nR >= 0 && nTen <= 4096 && nR <= 4096, RMS_ERR_ARG, "n_tensor and n_rot must lie in 0 .. 4096");
+    const int nQt = nTen * nG * nR;                                  // tensor waveforms x b x rotation (R23)
+    if (nQt > 0) {
+        RMS_REQUIRE(d->tensor_waves && d->tensor_gamp && d->rots, RMS_ERR_ARG, "tensor_waves, tensor_gamp and rots must be given");
+        for (int t = 0; t < 3 * nTen; ++t)
+            RMS_REQUIRE(d->tensor_waves[t] >= -1 && d->tensor_waves[t] < nW, RMS_ERR_ARG,
+                        "tensor_waves[%d] = %d is no waveform of this run", t, d->tensor_waves[t]);
+    }
+    const int nQ = nQs + nQt;
+    const int nTerms = nQt > 0 ? 3 : 1;
     const size_t n_sig = (size_t)nQ * nC, n_mom = (size_t)nS * nD * nC, n_sal = (size_t)nS * nC, n_flow = (size_t)nS * nC * nC;
     const size_t n_res_d = 2 * n_sig + 2 * n_mom + n_sal + nC;       // doubles
     RMS_REQUIRE(n_flow <= ((size_t)1 << 27) && n_res_d <= ((size_t)1 << 28), RMS_ERR_UNSUPPORTED,
@@ -245,15 +256,27 @@ extern "C" int rms_run(const rms_substrate* s, rms_walkers* w, const rms_run_des
         RMS_CUDA_TRY(cudaMemcpyAsync(b_wsuf.p, suf.data(), (size_t)nWk * (nT + 1) * sizeof(double), cudaMemcpyHostToDevice, stream));
     }
     // phase per unit Phi, in turns: gamp dt l_p n / (2 pi)   (Eq.7 with the right-endpoint rule, R11)
-    std::vector<double> qv((size_t)std::max(nQ, 1) * 3, 0.0);
-    std::vector<int> qwave(std::max(nQ, 1), 0);
+    // with tensor waveforms every q carries three (vector, waveform) terms, the scalar ones leaving two of them off
+    std::vector<double> qv((size_t)std::max(nQ, 1) * nTerms * 3, 0.0);
+    std::vector<int> qwave((size_t)std::max(nQ, 1) * nTerms, nTerms == 1 ? 0 : -1);
+    const double turn = d->dt_ms * s->voxel_um / (2.0 * 3.14159265358979323846);
     for (int m = 0; m < nW; ++m)
         for (int g = 0; g < nG; ++g)
             for (int k = 0; k < nD; ++k) {
-                const size_t q = ((size_t)m * nG + g) * nD + k;
-                const double c = d->gamp[(size_t)m * nG + g] * d->dt_ms * s->voxel_um / (2.0 * 3.14159265358979323846);
+                const size_t q = (((size_t)m * nG + g) * nD + k) * nTerms;
+                const double c = d->gamp[(size_t)m * nG + g] * turn;
                 for (int x = 0; x < 3; ++x) qv[3 * q + x] = c * d->dirs[3 * k + x];
                 qwave[q] = m;
+            }
+    for (int t = 0; t < nTen; ++t)
+        for (int g = 0; g < nG; ++g)
+            for (int k = 0; k < nR; ++k) {
+                const size_t q = ((size_t)nQs + ((size_t)t * nG + g) * nR + k) * 3;
+                const double c = d->tensor_gamp[(size_t)t * nG + g] * turn;
+                for (int ax = 0; ax < 3; ++ax) {                     // term ax: the vector R_k e_ax with the waveform on axis ax
+                    for (int x = 0; x < 3; ++x) qv[3 * (q + ax) + x] = c * d->rots[9 * k + 3 * x + ax];
+                    qwave[q + ax] = d->tensor_waves[3 * t + ax];
+                }
             }
     RMS_CUDA_TRY(rms_malloc((void**)&b_q.p, qv.size() * sizeof(double) + qwave.size() * sizeof(int)));
     RMS_CUDA_TRY(cudaMemcpyAsync(b_q.p, qv.data(), qv.size() * sizeof(double), cudaMemcpyHostToDevice, stream));
@@ -356,7 +379,7 @@ extern "C" int rms_run(const rms_substrate* s, rms_walkers* w, const rms_run_des
         rc = rms_order_by_class(s, w, b_order.as<uint32_t>(), stream, &n_launches);
         if (rc != RMS_OK) return rc;
     }
-    rc = rms_launch_signal(rp, nW, nQ, b_q.as<double>(), d_qwave, d_re, d_im, d_sum_alpha, b_order.as<uint32_t>(), stream,
+    rc = rms_launch_signal(rp, nW, nQ, nTerms, b_q.as<double>(), d_qwave, d_re, d_im, d_sum_alpha, b_order.as<uint32_t>(), stream,
                            &n_launches);
     if (rc != RMS_OK) return rc;
     RMS_CUDA_TRY(cudaEventRecord(ev_end, stream));
@@ -378,8 +401,11 @@ extern "C" int rms_run(const rms_substrate* s, rms_walkers* w, const rms_run_des
     const double* h_sal = h_m4 + n_mom;
     const double* h_sum_alpha = h_sal + n_sal;
     if (out->sum_alpha) memcpy(out->sum_alpha, h_sum_alpha, nC * sizeof(double));
-    if (out->sig_re) memcpy(out->sig_re, h_re, n_sig * sizeof(double));
-    if (out->sig_im) memcpy(out->sig_im, h_im, n_sig * sizeof(double));
+    const size_t n_sig_s = (size_t)nQs * nC, n_sig_t = (size_t)nQt * nC;
+    if (out->sig_re) memcpy(out->sig_re, h_re, n_sig_s * sizeof(double));
+    if (out->sig_im) memcpy(out->sig_im, h_im, n_sig_s * sizeof(double));
+    if (out->tsig_re) memcpy(out->tsig_re, h_re + n_sig_s, n_sig_t * sizeof(double));
+    if (out->tsig_im) memcpy(out->tsig_im, h_im + n_sig_s, n_sig_t * sizeof(double));
     if (out->m2) memcpy(out->m2, h_m2, n_mom * sizeof(double));
     if (out->m4) memcpy(out->m4, h_m4, n_mom * sizeof(double));
     if (out->snap_alpha) memcpy(out->snap_alpha, h_sal, n_sal * sizeof(double));
@@ -387,7 +413,10 @@ extern "C" int rms_run(const rms_substrate* s, rms_walkers* w, const rms_run_des
     {
         std::vector<double> t_ms(std::max(nS, 1));
         for (int sidx = 0; sidx < nS; ++sidx) t_ms[sidx] = (double)(w->steps_done + (uint64_t)d->snap_steps[sidx]) * d->dt_ms;
-        rms_normalise(nC, nQ, h_sum_alpha, h_re, h_im, nS, nD, h_sal, h_m2, h_m4, t_ms.data(), out->S_re, out->S_im, out->Dapp,
+        if (nQt > 0)      // Eq.7 for the tensor waveforms: the same normalisation, no moments
+            rms_normalise(nC, nQt, h_sum_alpha, h_re + n_sig_s, h_im + n_sig_s, 0, 0, nullptr, nullptr, nullptr, nullptr, out->tS_re,
+                          out->tS_im, nullptr, nullptr);
+        rms_normalise(nC, nQs, h_sum_alpha, h_re, h_im, nS, nD, h_sal, h_m2, h_m4, t_ms.data(), out->S_re, out->S_im, out->Dapp,
                       out->Kapp);
     }
     out->n_encounters = h_cnt[0];

@@ -512,6 +512,65 @@ def test_t1_weighting_in_the_mixing_time_of_a_stimulated_echo(rms):
     assert e.value.code == -1          # RMS_ERR_ARG: the window leaves 1 .. n_steps
 
 
+def _rotations(k, seed):
+    q, _ = np.linalg.qr(np.random.default_rng(seed).normal(size=(k, 3, 3)))
+    return q * np.sign(np.linalg.det(q))[:, None, None]
+
+
+def test_tensor_waveforms_b_tensor_encoding(rms):
+    """S: section 8(f) N1, "arbitrary g(tau) shapes (B-tensor encoding)" -- P:336 (R23): gradient waveforms that change
+    direction, phi = gamp dt l_p sum_a (R e_a) . Phi_{m_a}, evaluated in the signal reduction from the phase vectors of
+    the run's scalar waveforms.  Against oracle.tensor_signal on the same walkers: two classes (per-block sums), 13 classes
+    (class-ordered reduction), fp32 and fp64 walks, a permeable substrate with T2 contrast; the scalar signals of the same
+    run must not change; sharded runs merge."""
+    import dataclasses
+    import oracle
+    n_steps = 600
+    lobes = np.zeros((4, n_steps), np.float32)
+    for a in range(3):                       # three lobe pairs, one after the other (spherical encoding) ...
+        lobes[a, 200 * a:200 * a + 80] = 1.0
+        lobes[a, 200 * a + 110:200 * a + 190] = -1.0
+    lobes[3] = ri.pgse_wave(n_steps, 150, 400) * 0.5                        # ... and a plain pulsed gradient of half amplitude
+    tw = np.array([[0, 1, 2], [3, -1, 0], [-1, -1, -1], [1, 1, 1]], np.int32)
+    tg = np.array([[0.0, 900.0, 2500.0], [300.0, 1200.0, 2000.0], [1.0, 2.0, 3.0], [100.0, 700.0, 1500.0]])
+    rots = np.concatenate([np.eye(3)[None], _rotations(4, 3)])
+    seq = ri.Sequence(dt_ms=2e-4, n_steps=n_steps, wave=lobes, gamp=np.array([[0.0, 500.0, 1500.0]] * 4), dirs=ri.fibonacci_dirs(3),
+                      snap_steps=np.array([300, n_steps]), tensor_waves=tw, tensor_gamp=tg, rots=rots)
+    cfg = ri.make_config("cfg2", "test")
+    axons = cfg.substrate
+    nL = len(axons.D)
+    per_cell = dataclasses.replace(axons, label_class=np.arange(nL, dtype=np.uint16), n_classes=nL)
+    sl = ri.slabs(6, 5, (3, 2), 0.1, D_extra=2.0, D_intra=1.0, kappa_membrane=4.0, T2_extra=0.3, T2_intra=0.6)
+    n = 20000
+    for name, sub in (("cylinder", ri.single_cylinder(24, 8.5, 0.1)), ("axons, per-cell classes", per_cell), ("permeable slabs", sl)):
+        o = oracle_run(sub, seq, n, 71)
+        ot = oracle.tensor_signal(sub, seq, o)
+        assert np.abs(ot["tS"][0]).min() < 0.9                              # real attenuations
+        for flags in (0, 8):
+            g = gpu_run(sub, seq, n, 71, flags=flags)
+            rep = compare(g, o, n)
+            tol = 1e-4 + 2.0 * rep["n_diff"] / n
+            d = np.abs(g["tS"] - ot["tS"])
+            scale = float(o["sum_alpha"].sum())
+            d_cls = max(np.abs(g["tsig_re"] - ot["tsig_re"]).max(), np.abs(g["tsig_im"] - ot["tsig_im"]).max()) / scale
+            print("tensor waveforms,", name, "flags", flags, rep, "max |d tS|", d.max(), "per class", d_cls)
+            assert g["tS"].shape == (4, 3, 5) and g["tsig_re"].shape == (4, 3, 5, sub.n_classes)
+            assert d.max() <= tol and d_cls <= tol
+            assert np.abs(g["tS"][2] - 1.0).max() < 1e-12                   # all axes off: no phase
+    # the scalar outputs do not depend on the tensor ones riding along
+    plain = dataclasses.replace(seq, tensor_waves=None, tensor_gamp=None, rots=None)
+    g0 = gpu_run(sl, plain, n, 71)
+    g1 = gpu_run(sl, seq, n, 71)
+    assert np.abs(g0["S"] - g1["S"]).max() < 1e-12 and "tS" not in g0
+    # two shards of walker ids merge into the whole job
+    parts = [gpu_run(sl, seq, n // 2, 71, first_id=f) for f in (0, n // 2)]
+    m = rms.api.merge_results(parts, np.array([300, n_steps]) * 2e-4)
+    assert np.abs(m["tS"] - g1["tS"]).max() < 1e-12 and np.abs(m["S"] - g1["S"]).max() < 1e-12
+    with pytest.raises(rms.RmsError) as e:
+        gpu_run(sl, dataclasses.replace(seq, tensor_waves=np.array([[0, 4, 1]], np.int32), tensor_gamp=tg[:1]), 10, 1)
+    assert e.value.code == -1          # RMS_ERR_ARG: waveform 4 does not exist
+
+
 def test_degenerate_and_ragged_cases(rms):
     # one walker; 1, 2, 3 steps with a snapshot on every step; no waveform / no directions; hop of 0.99 voxel (three
     # interactions in most steps); a single-voxel pore (every face a membrane: the corner reflector of Fig.2)
