@@ -34,6 +34,10 @@
  *   run, T1 / mixing time alpha = exp(-(t_T2/T2 + t_mix/T1)) exactly per impermeable compartment (Eq.5);
  *                        T1 = T2 reproduces the run without a mixing time; well-mixed permeable slabs:
  *                        1 - <alpha> = f_b t_mix / T1_b to first order, for either starting compartment
+ *   tables, conc         equal c = Eq.3 bit for bit; P_12/P_21 = c_2 sqrt(D_2) / (c_1 sqrt(D_1)); the chain Eq.C.9-C.13-C.14;
+ *                        Eq.C.15 for kappa = inf
+ *   run, conc            initial density ~ c_L; kept by permeable membranes with D contrast; barrier-limited exchange
+ *                        rate k = 2 kappa (r^lambda / a_1 + r^(lambda-1) / a_2) between slabs
  *   tensor_signal (rms_oracle.py)  waveform on one axis rotated onto n = scalar waveform along n (same walkers, 1e-12);
  *                        free walk: <e^{-i phi}> = prod_k sinc(c ds |W_k|), W_k the vector suffix sums of g
  *   run, rejection sampl. D_parallel = D0 (1 - 3/16 S/V ds) between plates (Eq.B.2), uniform density
@@ -165,8 +169,21 @@ int rms_oracle_mt_table(int n_labels, const float* D, const float* rho, double d
 /* P[a][b] permeation probability from label a into label b.                   */
 /* Both are rounded once to fp32-representable values (R6).                    */
 /* ------------------------------------------------------------------------- */
+int rms_oracle_tables_conc(int n_labels, const float* D, const float* kappa, const float* conc, double voxel_um,
+                           double dt_ms, double* s_out, double* P_out);
+
 int rms_oracle_tables(int n_labels, const float* D, const float* kappa, double voxel_um, double dt_ms,
                       double* s_out, double* P_out)
+{
+    return rms_oracle_tables_conc(n_labels, D, kappa, NULL, voxel_um, dt_ms, s_out, P_out);
+}
+
+/* The same with a spin concentration c_L per label (Appendix C.2, Eq.C.9, C.13-C.14; Appendix C.3, Eq.C.15):
+ *   P_ab = A_ab r^lambda / (1 + alpha),  alpha = (A_ab r^lambda + A_ba r^(lambda-1)) / 2,  r = c_b / c_a,
+ *   lambda = 1 / (1 + c_b sqrt(D_b) / (c_a sqrt(D_a)))   (the paper's arg min of alpha_lambda; R24)
+ * which is Eq.C.9 with kappa_0 = kappa (1 - alpha) of Eq.C.13, and Eq.3 for r = 1.  conc = NULL: all equal. */
+int rms_oracle_tables_conc(int n_labels, const float* D, const float* kappa, const float* conc, double voxel_um,
+                           double dt_ms, double* s_out, double* P_out)
 {
     const double C3 = 2.0 / 3.0; /* Eq.2b, d = 3 */
     if (n_labels <= 0 || !D || !(voxel_um > 0) || !(dt_ms > 0)) return ORC_ERR_ARG;
@@ -185,13 +202,22 @@ int rms_oracle_tables(int n_labels, const float* D, const float* kappa, double v
             } else {
                 double k = kappa ? (double)kappa[a * n_labels + b] : 0.0;
                 double Da = D[a], Db = D[b];
+                double ca = conc ? (double)conc[a] : 1.0, cb = conc ? (double)conc[b] : 1.0;
                 if (k < 0 || k != k) return ORC_ERR_ARG;
-                if (k == 0.0) {
-                    P = 0.0;
+                if (!(ca >= 0) || !(cb >= 0) || isinf(ca) || isinf(cb)) return ORC_ERR_ARG;
+                if (k == 0.0 || ca == 0.0 || cb == 0.0) {
+                    P = 0.0; /* impermeable; nothing enters (or sits in) a medium without spins */
                 } else if (isinf(k)) {
-                    /* no membrane between media of different D: Eq.C.15 with c1 = c2 */
-                    P = sqrt(Db / Da);
+                    /* no membrane between media of different D and c: Eq.C.15 */
+                    P = cb * sqrt(Db) / (ca * sqrt(Da));
                     if (P > 1.0) P = 1.0;
+                } else if (ca != cb) {
+                    double r = cb / ca;
+                    double lam = 1.0 / (1.0 + cb * sqrt(Db) / (ca * sqrt(Da)));
+                    double Aab = k * sqrt(6.0 * dt_ms / Da) * C3 * pow(r, lam);       /* Eq.C.9a */
+                    double Aba = k * sqrt(6.0 * dt_ms / Db) * C3 * pow(r, lam - 1.0); /* Eq.C.9b */
+                    P = Aab / (1.0 + 0.5 * (Aab + Aba));                              /* Eq.C.13-C.14 */
+                    if (P > 1.0) return ORC_ERR_P_RANGE;
                 } else {
                     double Aab = k * sqrt(6.0 * dt_ms / Da) * C3; /* kappa ds_a / D_a C_d, Eq.2a */
                     double Aba = k * sqrt(6.0 * dt_ms / Db) * C3;
@@ -337,8 +363,21 @@ int rms_oracle_step(int nx, int ny, int nz, const uint16_t* labels, int n_labels
 
 /* Walker initialisation (P:151 step 1; R13): rejection sampling of a uniform voxel until its label
  * is allowed, then a uniform in-voxel offset.  Integer arithmetic: v = floor(uni(w) * n). */
+int rms_oracle_init_walker_conc(int nx, int ny, int nz, const uint16_t* labels, const uint8_t* label_allowed,
+                                const float* accept, uint64_t seed, uint64_t walker, int32_t vox[3], double off[3],
+                                uint16_t* label);
+
 int rms_oracle_init_walker(int nx, int ny, int nz, const uint16_t* labels, const uint8_t* label_allowed,
                            uint64_t seed, uint64_t walker, int32_t vox[3], double off[3], uint16_t* label)
+{
+    return rms_oracle_init_walker_conc(nx, ny, nz, labels, label_allowed, NULL, seed, walker, vox, off, label);
+}
+
+/* With spin concentrations the equilibrium density is proportional to c_L (Appendix C.2): a proposed voxel is kept
+ * with probability accept[L] = c_L / max c over the allowed labels, drawn from the spare fourth word (R24). */
+int rms_oracle_init_walker_conc(int nx, int ny, int nz, const uint16_t* labels, const uint8_t* label_allowed,
+                                const float* accept, uint64_t seed, uint64_t walker, int32_t vox[3], double off[3],
+                                uint16_t* label)
 {
     uint32_t w[4];
     for (uint32_t a = 0; a < ORC_MAX_INIT_ATTEMPTS; ++a) {
@@ -348,6 +387,7 @@ int rms_oracle_init_walker(int nx, int ny, int nz, const uint16_t* labels, const
         int z = (int)(((uint64_t)(w[2] >> 8) * (uint64_t)nz) >> 24);
         uint16_t L = labels[((size_t)z * ny + y) * nx + x];
         if (label_allowed && !label_allowed[L]) continue;
+        if (accept && !(uni(w[3]) < (double)accept[L])) continue;
         vox[0] = x; vox[1] = y; vox[2] = z;
         *label = L;
         draw(seed, walker, 0, STREAM_INIT_OFFSET, w);
@@ -372,6 +412,7 @@ typedef struct {
     /* walkers */
     uint64_t n_walkers, first_id, seed;
     const uint8_t* label_allowed;
+    const float* accept; /* [n_labels] c_L / max c, or NULL (spin concentrations, R24) */
     /* run */
     double dt;
     int64_t n_steps;
@@ -411,7 +452,8 @@ static void* run_part(void* arg)
         int32_t v0[3], v[3];
         double f0[3], f[3];
         uint16_t L0, L;
-        int st = rms_oracle_init_walker(lat->nx, lat->ny, lat->nz, lat->labels, j->label_allowed, j->seed, id, v0, f0, &L0);
+        int st = rms_oracle_init_walker_conc(lat->nx, lat->ny, lat->nz, lat->labels, j->label_allowed, j->accept, j->seed, id, v0,
+                                              f0, &L0);
         if (st != ORC_OK) { pt->status = st; break; }
         memcpy(v, v0, sizeof v); memcpy(f, f0, sizeof f); L = L0;
         int c0 = j->label_class ? j->label_class[L0] : 0;
@@ -492,7 +534,7 @@ int rms_oracle_run(
     uint64_t n_walkers, uint64_t first_id, const uint8_t* label_allowed, uint64_t seed,
     double dt_ms, int64_t n_steps, int n_wave, const float* wave, int n_g, const double* gamp,
     int n_dir, const double* dirs, int n_snap, const int64_t* snap_steps, int n_threads, int interaction,
-    const float* T1, int64_t mix_first, int64_t mix_steps,
+    const float* T1, int64_t mix_first, int64_t mix_steps, const float* conc,
     double* sum_alpha, double* sig_re, double* sig_im, double* m2, double* m4, double* snap_alpha,
     uint64_t* class_flow, uint64_t* counters,
     int32_t* final_vox, double* final_off, uint16_t* final_label,
@@ -519,7 +561,18 @@ int rms_oracle_run(
     double* inv_T1 = inv_T2 ? inv_T2 + n_labels : NULL;
     double* Q_tab = rho ? (double*)malloc(sizeof(double) * (size_t)n_labels * n_labels) : NULL;
     if (!s_tab || !P_tab || !inv_T2 || (rho && !Q_tab)) { free(s_tab); free(P_tab); free(inv_T2); free(Q_tab); return ORC_ERR_OOM; }
-    int st = rms_oracle_tables(n_labels, D, kappa, voxel_um, dt_ms, s_tab, P_tab);
+    int st = rms_oracle_tables_conc(n_labels, D, kappa, conc, voxel_um, dt_ms, s_tab, P_tab);
+    float* accept = NULL;
+    if (st == ORC_OK && conc) { /* initial density proportional to c_L over the allowed labels (R24) */
+        double cmax = 0.0;
+        for (int a = 0; a < n_labels; ++a)
+            if ((!label_allowed || label_allowed[a]) && (double)conc[a] > cmax) cmax = (double)conc[a];
+        accept = (float*)malloc(sizeof(float) * n_labels);
+        if (!accept) st = ORC_ERR_OOM;
+        else if (!(cmax > 0.0)) st = ORC_ERR_NO_SPACE;
+        else for (int a = 0; a < n_labels; ++a) accept[a] = (float)((double)conc[a] / cmax);
+        if (st == ORC_OK && interaction == 1) st = ORC_ERR_ARG; /* Appendix B.1 has no concentrations */
+    }
     if (st == ORC_OK && rho) st = rms_oracle_mt_table(n_labels, D, rho, dt_ms, Q_tab);
     if (st == ORC_OK && interaction == 1 && kappa) {
         /* rejection sampling has its own permeation probability: P_T / (1 - P_T) = kappa ds / D0 C_d (Appendix B.1,
@@ -535,7 +588,7 @@ int rms_oracle_run(
     }
     if (interaction != 0 && interaction != 1) st = ORC_ERR_ARG;
     if (mix_steps < 0 || (mix_steps > 0 && (mix_first < 1 || mix_first + mix_steps - 1 > n_steps))) st = ORC_ERR_ARG;
-    if (st != ORC_OK) { free(s_tab); free(P_tab); free(inv_T2); free(Q_tab); return st; }
+    if (st != ORC_OK) { free(s_tab); free(P_tab); free(inv_T2); free(Q_tab); free(accept); return st; }
     for (int a = 0; a < n_labels; ++a) {
         double t2 = T2 ? (double)T2[a] : 0.0;
         inv_T2[a] = (t2 > 0.0 && !isinf(t2)) ? 1.0 / t2 : 0.0; /* T2 <= 0 or inf: no relaxation */
@@ -548,7 +601,7 @@ int rms_oracle_run(
     job.lat.nx = nx; job.lat.ny = ny; job.lat.nz = nz; job.lat.labels = labels; job.lat.n_labels = n_labels;
     job.lat.s = s_tab; job.lat.P = P_tab; job.lat.Q = Q_tab; job.lat.rejection = interaction == 1;
     job.voxel_um = voxel_um; job.inv_T2 = inv_T2; job.inv_T1 = inv_T1; job.mix_first = mix_first; job.mix_steps = mix_steps; job.label_class = label_class; job.n_classes = n_classes;
-    job.n_walkers = n_walkers; job.first_id = first_id; job.seed = seed; job.label_allowed = label_allowed;
+    job.n_walkers = n_walkers; job.first_id = first_id; job.seed = seed; job.label_allowed = label_allowed; job.accept = accept;
     job.dt = dt_ms; job.n_steps = n_steps; job.n_wave = n_wave; job.wave = wave; job.n_g = n_g; job.gamp = gamp;
     job.n_dir = n_dir; job.dirs = dirs; job.n_snap = n_snap; job.snap_steps = snap_steps;
     job.final_vox = final_vox; job.final_off = final_off; job.final_label = final_label;
@@ -608,6 +661,6 @@ done:
         free(parts[t].sum_alpha); free(parts[t].sig_re); free(parts[t].sig_im); free(parts[t].m2);
         free(parts[t].m4); free(parts[t].snap_alpha); free(parts[t].class_flow);
     }
-    free(parts); free(tids); free(s_tab); free(P_tab); free(inv_T2); free(Q_tab);
+    free(parts); free(tids); free(s_tab); free(P_tab); free(inv_T2); free(Q_tab); free(accept);
     return status;
 }

@@ -69,15 +69,16 @@ def direction(wa: int, wb: int):
     return u
 
 
-def tables(D, kappa, voxel_um, dt_ms):
-    """(s[n_labels], P[n_labels, n_labels]) of Eq.1 and Eq.3."""
+def tables(D, kappa, voxel_um, dt_ms, conc=None):
+    """(s[n_labels], P[n_labels, n_labels]) of Eq.1 and Eq.3; with spin concentrations conc[n_labels], Eq.C.9 / C.13."""
     D = np.ascontiguousarray(D, np.float32)
     n = D.size
     kappa = None if kappa is None else np.ascontiguousarray(kappa, np.float32).reshape(n, n)
+    conc = None if conc is None else np.ascontiguousarray(conc, np.float32)
     s = np.zeros(n)
     P = np.zeros((n, n))
-    st = _load().rms_oracle_tables(C.c_int(n), _p(D, C.c_float), _p(kappa, C.c_float), C.c_double(voxel_um),
-                                   C.c_double(dt_ms), _p(s, C.c_double), _p(P, C.c_double))
+    st = _load().rms_oracle_tables_conc(C.c_int(n), _p(D, C.c_float), _p(kappa, C.c_float), _p(conc, C.c_float),
+                                        C.c_double(voxel_um), C.c_double(dt_ms), _p(s, C.c_double), _p(P, C.c_double))
     if st:
         raise OracleError(st)
     return s, P
@@ -152,6 +153,8 @@ def run(sub, seq, n_walkers, seed, first_id=0, n_threads=1, per_walker=False, in
     T1 = getattr(sub, "T1", None)
     T1 = None if T1 is None else np.ascontiguousarray(T1, np.float32)
     mix_first, mix_steps = int(getattr(seq, "mix_first_step", 0)), int(getattr(seq, "mix_n_steps", 0))
+    conc = getattr(sub, "conc", None)
+    conc = None if conc is None else np.ascontiguousarray(conc, np.float32)
     lclass = np.ascontiguousarray(sub.label_class, np.uint16)
     allowed = np.ascontiguousarray(sub.label_allowed, np.uint8)
     wave = np.ascontiguousarray(seq.wave, np.float32)
@@ -179,6 +182,7 @@ def run(sub, seq, n_walkers, seed, first_id=0, n_threads=1, per_walker=False, in
         C.c_double(seq.dt_ms), C.c_int64(n_steps), C.c_int(n_wave), _p(wave, C.c_float), C.c_int(n_g),
         _p(gamp, C.c_double), C.c_int(n_dir), _p(dirs, C.c_double), C.c_int(n_snap), _p(snaps, C.c_int64),
         C.c_int(n_threads), C.c_int(interaction), _p(T1, C.c_float), C.c_int64(mix_first), C.c_int64(mix_steps),
+        _p(conc, C.c_float),
         _p(r["sum_alpha"], C.c_double), _p(r["sig_re"], C.c_double), _p(r["sig_im"], C.c_double),
         _p(r["m2"], C.c_double), _p(r["m4"], C.c_double), _p(r["snap_alpha"], C.c_double),
         _p(r["class_flow"], C.c_uint64), _p(counters, C.c_uint64),

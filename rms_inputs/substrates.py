@@ -23,6 +23,7 @@ class Substrate:
     meta: dict = field(default_factory=dict)
     rho: np.ndarray | None = None      # [n_labels, n_labels] float32, um/ms: surface relaxivity (absorbing membranes), or None
     T1: np.ndarray | None = None       # [n_labels] float32, ms: relaxation during a mixing time (stimulated echo), or None
+    conc: np.ndarray | None = None     # [n_labels] float32: relative spin concentration (Appendix C.2), or None = all equal
 
     @property
     def n_labels(self) -> int:

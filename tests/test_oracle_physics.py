@@ -519,3 +519,76 @@ def test_tensor_encoding_reduces_to_linear_encoding_and_matches_the_free_walk_pr
         for k in range(2):
             assert abs(t["tS"][ti, 0, k].real - expect) < 4 / math.sqrt(n_w), (ti, k, t["tS"][ti, 0, k], expect)
             assert abs(t["tS"][ti, 0, k].imag) < 4 / math.sqrt(n_w)
+
+
+# ------------------------------------------------------------------ spin concentrations (Appendix C.2-C.3)
+def test_spin_concentration_tables_eq_c9_c13_c15():
+    """Eq.C.9 with the bias correction of Eq.C.13-C.14, lambda = arg min alpha_lambda (reading R24): equal concentrations
+    give back Eq.3 bit for bit; P_12 / P_21 = c_2 sqrt(D_2) / (c_1 sqrt(D_1)) (equilibrium); the table satisfies the
+    paper's chain P_12 = kappa_0 ds_1/D_1 C_d r^lambda, kappa_0 = kappa (1 - alpha), alpha = (P_12 + P_21)/2; kappa = inf is
+    Baxter-Frank, Eq.C.15."""
+    D = np.array([2.0, 1.0, 0.5], np.float32)
+    c = np.array([1.0, 0.5, 0.8], np.float32)
+    kap = np.array([[0, 5.0, np.inf], [5.0, 0, 0.0], [np.inf, 0.0, 0]], np.float32)
+    s0, P0 = oracle.tables(D, kap, LP, DT)
+    s1, P1 = oracle.tables(D, kap, LP, DT, conc=np.full(3, 0.7, np.float32))
+    assert np.array_equal(P0, P1) and np.array_equal(s0, s1)
+    _, P = oracle.tables(D, kap, LP, DT, conc=c)
+    want_ratio = c[1] * math.sqrt(D[1]) / (c[0] * math.sqrt(D[0]))
+    assert abs(P[0, 1] / P[1, 0] - want_ratio) < 1e-6 and P[1, 2] == 0 and P[2, 1] == 0
+    alpha = 0.5 * (P[0, 1] + P[1, 0])                                       # Eq.C.14
+    kappa0 = 5.0 * (1 - alpha)                                              # Eq.C.13
+    lam = 1 / (1 + want_ratio)
+    ds = [math.sqrt(6 * float(d) * DT) for d in D]
+    r = c[1] / c[0]
+    assert abs(P[0, 1] - kappa0 * ds[0] / D[0] * (2 / 3) * r ** lam) < 2e-7            # Eq.C.9a
+    assert abs(P[1, 0] - kappa0 * ds[1] / D[1] * (2 / 3) * r ** (lam - 1)) < 2e-7      # Eq.C.9b
+    assert 0.03 < alpha < 0.3                                               # the correction is not negligible here
+    # Eq.C.15: from the high-flux side (0: c sqrt(D) = 1.41) into 2 (0.57), and back with certainty
+    assert abs(P[0, 2] - c[2] * math.sqrt(D[2]) / (c[0] * math.sqrt(D[0]))) < 1e-7 and P[2, 0] == 1.0
+    # a medium without spins is closed
+    _, Pz = oracle.tables(D, kap, LP, DT, conc=np.array([1.0, 0.0, 1.0], np.float32))
+    assert Pz[0, 1] == 0 and Pz[1, 0] == 0
+
+
+def test_spin_concentration_initial_density_equilibrium_and_exchange_rate():
+    """(i) walkers are placed with density proportional to c_L (R24); (ii) that density is kept by a permeable membrane
+    with D contrast (the P ratio of Eq.C.9); (iii) barrier-limited exchange between two slabs (kappa a / D = 0.05) from all
+    walkers in slab 1: N_1(t)/N = f + (1 - f) exp(-k t), k = 2 kappa (r^lambda / a_1 + r^(lambda-1) / a_2),
+    f = c_1 a_1 / (c_1 a_1 + c_2 a_2) -- a wrong or swapped lambda moves k by 20 %."""
+    import dataclasses
+    wa, wb = 5, 7
+    c = np.array([1.0, 0.4], np.float32)
+    sub = ri.slabs(wa, wb, (3, 3), LP, D_extra=2.0, D_intra=1.0, kappa_membrane=30.0)
+    sub = dataclasses.replace(sub, conc=c)
+    n_w, n_steps = 120_000, 600
+    r = oracle.run(sub, _narrow(n_steps, np.eye(3), snaps=[1, n_steps]), n_w, seed=71, n_threads=THREADS, per_walker=True)
+    f_a = c[0] * wa / (c[0] * wa + c[1] * wb)
+    se = math.sqrt(f_a * (1 - f_a) / n_w)
+    x0 = np.mod(r["init_vox"][:, 0], wa + wb)
+    assert abs(np.mean(x0 < wa) - f_a) < 4 * se                             # (i)
+    for lo, hi in ((0, wa), (wa, wa + wb)):                                 # uniform inside each slab
+        cnt = np.bincount(x0, minlength=wa + wb)[lo:hi]
+        assert ((cnt - cnt.mean()) ** 2 / cnt.mean()).sum() < (hi - lo - 1) + 5 * math.sqrt(2 * (hi - lo - 1))
+    x = np.mod(r["final_vox"][:, 0], wa + wb)
+    assert r["n_permeations"] > 20_000
+    assert abs(np.mean(x < wa) - f_a) < 4 * se, (np.mean(x < wa), f_a)      # (ii)
+    # (iii)
+    a_vox, D, kappa = 5, 2.0, 0.2
+    a = a_vox * LP
+    sub = ri.slabs(a_vox, a_vox, (3, 3), LP, D_extra=D, D_intra=D, kappa_membrane=kappa, place="extra")
+    sub = dataclasses.replace(sub, conc=np.array([1.0, 0.5], np.float32))
+    snaps = [1000, 2500, 5000]
+    n_w = 60_000
+    r = oracle.run(sub, _narrow(5000, np.eye(3), snaps=snaps), n_w, seed=72, n_threads=THREADS)
+    rr, lam = 0.5, 1 / (1 + 0.5)
+    k = 2 * kappa * (rr ** lam + rr ** (lam - 1)) / a
+    f = 1 / (1 + rr)
+    for s, n in enumerate(snaps):
+        got = r["class_flow"][s, 0, 0] / n_w
+        th = f + (1 - f) * math.exp(-k * n * DT)
+        k_bad = 2 * kappa * (rr + 1.0) / a                                  # lambda = 1 instead
+        th_bad = f + (1 - f) * math.exp(-k_bad * n * DT)
+        assert abs(got - th) < 4 * math.sqrt(0.25 / n_w) + 0.005, (n, got, th)
+        if n <= 2500:
+            assert abs(got - th_bad) > 0.015, (n, got, th_bad)
