@@ -58,6 +58,10 @@ typedef struct rms_walkers rms_walkers;     /* opaque */
  *              (alpha_rho = 0, Eq.4) with probability rho_ab ds_a / D_a C_d; NULL = none (host)
  * T1           [n_labels] ms, the relaxation time during the mixing time of a stimulated echo (see
  *              rms_run_desc.mix_first_step); +inf or <= 0 means no relaxation; NULL = none (host)
+ * conc         [n_labels] relative spin concentration c_L >= 0 of each label (Appendix C.2-C.3), NULL = all equal (host).
+ *              Between labels of different c the permeation probability is Eq.C.9 with the correction of Eq.C.13 and
+ *              lambda = arg min alpha_lambda (Eq.C.15 for kappa = +inf), and rms_walkers_init places walkers with a
+ *              density proportional to c_L (R24).  Equal concentrations change nothing.
  * label_class  [n_labels] uint16 output compartment class of each label, < n_classes <= 65535; NULL = all 0 (host).
  *              Two classes (extra / intra-cellular) are the usual choice; class = label gives per-cell outputs.
  * flags        RMS_LABELS_ON_DEVICE | RMS_ADOPT_DEVICE_PTR | RMS_NO_BRICKS | RMS_LAYOUT_X_FASTEST | RMS_LAYOUT_Z_FASTEST | RMS_LAYOUT_AUTO
@@ -88,6 +92,7 @@ typedef struct {
     int32_t n_classes;
     uint32_t flags;
     const float* T1;
+    const float* conc;
 } rms_substrate_desc;
 
 int rms_substrate_create(const rms_substrate_desc* desc, void* cuda_stream, rms_substrate** out);

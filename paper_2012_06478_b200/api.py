@@ -31,7 +31,7 @@ def simulate(sub, seq, n_walkers, seed, first_id=0, flags=0, substrate_flags=0, 
     """
     labels = device_labels if device_labels is not None else sub.labels
     S = B.rms_substrate_create(labels, sub.voxel_um, sub.D, sub.T2, sub.kappa, sub.label_class, sub.n_classes,
-                               flags=substrate_flags, stream=stream, rho=getattr(sub, "rho", None), T1=getattr(sub, "T1", None))
+                               flags=substrate_flags, stream=stream, rho=getattr(sub, "rho", None), T1=getattr(sub, "T1", None), conc=getattr(sub, "conc", None))
     W = None
     try:
         W = B.rms_walkers_init(S, n_walkers, first_id, sub.label_allowed, seed, stream=stream)

@@ -46,7 +46,7 @@ class SubstrateDesc(C.Structure):
     _fields_ = [("nx", C.c_int32), ("ny", C.c_int32), ("nz", C.c_int32), ("voxel_um", C.c_double),
                 ("labels", C.c_void_p), ("n_labels", C.c_int32), ("D", C.c_void_p), ("T2", C.c_void_p),
                 ("kappa", C.c_void_p), ("rho", C.c_void_p), ("label_class", C.c_void_p), ("n_classes", C.c_int32), ("flags", C.c_uint32),
-                ("T1", C.c_void_p)]
+                ("T1", C.c_void_p), ("conc", C.c_void_p)]
 
 
 class SubstrateInfo(C.Structure):
@@ -156,7 +156,7 @@ class Substrate:
 
 
 def rms_substrate_create(labels, voxel_um, D, T2=None, kappa=None, label_class=None, n_classes=1, flags=0,
-                         stream=None, rho=None, T1=None) -> Substrate:
+                         stream=None, rho=None, T1=None, conc=None) -> Substrate:
     """labels: numpy uint16 (nz, ny, nx) on the host, or a torch.uint16/int16 CUDA tensor of that shape
     (then the lattice is adopted in place, no copy)."""
     lib = load_library()
@@ -179,8 +179,9 @@ def rms_substrate_create(labels, voxel_um, D, T2=None, kappa=None, label_class=N
     label_class = _host(label_class, np.uint16)
     rho = _host(rho, np.float32)
     T1 = _host(T1, np.float32)
+    conc = _host(conc, np.float32)
     d = SubstrateDesc(nx, ny, nz, float(voxel_um), lab_ptr, int(D.size), _ptr(D), _ptr(T2), _ptr(kappa), _ptr(rho), _ptr(label_class),
-                      int(n_classes), int(flags), _ptr(T1))
+                      int(n_classes), int(flags), _ptr(T1), _ptr(conc))
     h = C.c_void_p()
     _check(lib.rms_substrate_create(C.byref(d), _stream_ptr(stream), C.byref(h)))
     adopt = bool(flags & RMS_ADOPT_DEVICE_PTR)

@@ -62,6 +62,7 @@ struct rms_substrate {
     int NX = 0, NY = 0, NZ = 0;          // padded dims (n + 2)
     uint64_t n_membrane_faces = 0;
     std::vector<float> D, T2, kappa;     // host copies of the per-label tables
+    std::vector<float> conc;             // per label, relative spin concentration (Appendix C.2; R24); empty = all equal
     std::vector<float> T1;               // per label, mixing time of a stimulated echo; empty = none
     std::vector<float> rho;              // surface relaxivity per label pair (absorbing membranes, Eq.4); empty = none
     std::vector<uint16_t> label_class;

@@ -196,6 +196,9 @@ extern "C" int rms_substrate_create(const rms_substrate_desc* d, void* cuda_stre
             }
     }
 
+    if (d->conc)
+        for (int a = 0; a < nL; ++a)
+            RMS_REQUIRE(d->conc[a] >= 0 && isfinite(d->conc[a]), RMS_ERR_ARG, "conc[%d] is negative, infinite or NaN", a);
     bool any_rho = false;
     if (d->rho)
         for (size_t i = 0; i < (size_t)nL * nL; ++i) {
@@ -219,6 +222,7 @@ extern "C" int rms_substrate_create(const rms_substrate_desc* d, void* cuda_stre
     if (d->label_class) s->label_class.assign(d->label_class, d->label_class + nL); else s->label_class.assign(nL, 0);
     if (any_rho) s->rho.assign(d->rho, d->rho + (size_t)nL * nL);
     if (d->T1) s->T1.assign(d->T1, d->T1 + nL);
+    if (d->conc) s->conc.assign(d->conc, d->conc + nL);
     s->all_impermeable = all_imp;
 
     int rc = RMS_OK;
@@ -351,10 +355,20 @@ int rms_compute_tables(const rms_substrate* s, double dt, std::vector<float>& s_
                 P = 1.0;
             } else {
                 const double k = s->kappa[(size_t)a * nL + b], Da = s->D[a], Db = s->D[b];
-                if (k == 0) {
-                    P = 0;
+                const double ca = s->conc.empty() ? 1.0 : (double)s->conc[a], cb = s->conc.empty() ? 1.0 : (double)s->conc[b];
+                if (k == 0 || ca == 0 || cb == 0) {
+                    P = 0;                               // impermeable; nothing enters (or sits in) a medium without spins
                 } else if (isinf(k)) {
-                    P = fmin(1.0, sqrt(Db / Da));
+                    P = fmin(1.0, cb * sqrt(Db) / (ca * sqrt(Da)));      // Eq.C.15
+                } else if (ca != cb) {
+                    // Eq.C.9 with kappa_0 = kappa (1 - alpha) of Eq.C.13-C.14, lambda = arg min alpha_lambda (R24)
+                    RMS_REQUIRE(!rejection_sampling, RMS_ERR_UNSUPPORTED,
+                                "rejection sampling with unequal spin concentrations (labels %d, %d)", a, b);
+                    const double r = cb / ca, lam = 1.0 / (1.0 + cb * sqrt(Db) / (ca * sqrt(Da)));
+                    const double Aab = k * sqrt(6.0 * dt / Da) * C3 * pow(r, lam), Aba = k * sqrt(6.0 * dt / Db) * C3 * pow(r, lam - 1.0);
+                    P = Aab / (1.0 + 0.5 * (Aab + Aba));
+                    RMS_REQUIRE(P <= 1.0, RMS_ERR_P_RANGE,
+                                "Eq.C.9 gives P = %.4g > 1 from label %d into %d: lower kappa or dt (P:624)", P, a, b);
                 } else if (rejection_sampling) {
                     RMS_REQUIRE(Da == Db, RMS_ERR_UNSUPPORTED,
                                 "rejection sampling with a permeable membrane between unequal diffusivities (labels %d, %d): "

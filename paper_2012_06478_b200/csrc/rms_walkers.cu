@@ -6,9 +6,11 @@
 #define RMS_MAX_INIT_ATTEMPTS (1u << 20)
 
 // One thread per walker.  Proposal a = 0,1,..: voxel = floor(uni(w) * n) per axis from Philox(walker, a, INIT),
-// accepted iff its label is allowed; offset from Philox(walker, 0, INIT_OFFSET) (R13).
+// accepted iff its label is allowed; offset from Philox(walker, 0, INIT_OFFSET) (R13).  With spin concentrations
+// (Appendix C.2; R24) the proposal is kept with probability accept[L] = c_L / max c, against uni of the spare fourth word.
 __global__ void __launch_bounds__(256) rms_init_kernel(const uint16_t* __restrict__ labels, int nx, int ny, int nz,
-                                                        const uint8_t* __restrict__ allowed, rms_walker_arrays st, uint64_t n,
+                                                        const uint8_t* __restrict__ allowed, const float* __restrict__ accept,
+                                                        rms_walker_arrays st, uint64_t n,
                                                         uint64_t first_id, rms_philox_keys rk, int n_phi,
                                                         unsigned long long* __restrict__ counters)
 {
@@ -26,7 +28,10 @@ __global__ void __launch_bounds__(256) rms_init_kernel(const uint16_t* __restric
         y = (int)__umulhi(w1 & 0xFFFFFF00u, (uint32_t)ny);
         z = (int)__umulhi(w2 & 0xFFFFFF00u, (uint32_t)nz);
         L = labels[((size_t)z * ny + y) * nx + x];
-        if (!allowed || allowed[L]) { ok = true; break; }
+        if (allowed && !allowed[L]) continue;
+        if (accept && !(rms_uni(w3) < accept[L])) continue;
+        ok = true;
+        break;
     }
     if (!ok) atomicAdd(&counters[3], 1ull);
     rms_philox(rk, id_lo, id_hi, 0u, RMS_STREAM_INIT_OFFSET, w0, w1, w2, w3);
@@ -64,6 +69,16 @@ extern "C" int rms_walkers_init(const rms_substrate* s, uint64_t n_walkers, uint
     const size_t a4 = align_up(n * 4, 256);
     const size_t total = 20 * a4 + 256;
     uint8_t* d_allowed = nullptr;
+    float* d_accept = nullptr;
+    std::vector<float> h_accept;
+    if (!s->conc.empty()) {      // initial density proportional to c_L over the allowed labels (R24)
+        double cmax = 0.0;
+        for (int a = 0; a < s->n_labels; ++a)
+            if ((!label_allowed || label_allowed[a]) && (double)s->conc[a] > cmax) cmax = (double)s->conc[a];
+        RMS_REQUIRE(cmax > 0.0, RMS_ERR_NO_SPACE, "every allowed label has spin concentration 0");
+        h_accept.resize(s->n_labels);
+        for (int a = 0; a < s->n_labels; ++a) h_accept[a] = (float)((double)s->conc[a] / cmax);
+    }
     int rc = RMS_OK;
     unsigned long long h_cnt[8] = {0};
 #define W_TRY(expr)                                                                                      \
@@ -96,7 +111,11 @@ extern "C" int rms_walkers_init(const rms_substrate* s, uint64_t n_walkers, uint
         W_TRY(rms_malloc((void**)&d_allowed, s->n_labels));
         W_TRY(cudaMemcpyAsync(d_allowed, label_allowed, s->n_labels, cudaMemcpyHostToDevice, stream));
     }
-    rms_init_kernel<<<(unsigned)((n + 255) / 256), 256, 0, stream>>>(s->d_labels, s->nx, s->ny, s->nz, d_allowed, w->a, n,
+    if (!h_accept.empty()) {
+        W_TRY(rms_malloc((void**)&d_accept, s->n_labels * sizeof(float)));
+        W_TRY(cudaMemcpyAsync(d_accept, h_accept.data(), s->n_labels * sizeof(float), cudaMemcpyHostToDevice, stream));
+    }
+    rms_init_kernel<<<(unsigned)((n + 255) / 256), 256, 0, stream>>>(s->d_labels, s->nx, s->ny, s->nz, d_allowed, d_accept, w->a, n,
                                                                       first_walker_id, rms_make_keys(seed),
                                                                       3 * w->n_wave_alloc, w->d_counters);
     W_TRY(cudaGetLastError());
@@ -104,6 +123,8 @@ extern "C" int rms_walkers_init(const rms_substrate* s, uint64_t n_walkers, uint
     W_TRY(cudaStreamSynchronize(stream));
     if (d_allowed) rms_free(d_allowed);
     d_allowed = nullptr;
+    if (d_accept) rms_free(d_accept);
+    d_accept = nullptr;
     if (h_cnt[3] != 0) {
         rms_set_error("%llu walkers found no voxel with an allowed label in 2^20 proposals", h_cnt[3]);
         rc = RMS_ERR_NO_SPACE;
@@ -113,6 +134,7 @@ extern "C" int rms_walkers_init(const rms_substrate* s, uint64_t n_walkers, uint
     return RMS_OK;
 fail:
     if (d_allowed) rms_free(d_allowed);
+    if (d_accept) rms_free(d_accept);
     rms_walkers_destroy(w);
     return rc;
 #undef W_TRY

@@ -571,6 +571,43 @@ def test_tensor_waveforms_b_tensor_encoding(rms):
     assert e.value.code == -1          # RMS_ERR_ARG: waveform 4 does not exist
 
 
+def test_spin_concentrations_permeation_and_placement(rms):
+    """S: section 8(f) N4, "concentration-dependent (Eq.C.9)" and Baxter-Frank (Eq.C.15) -- Appendix C.2-C.3 (R24): per-label spin
+    concentrations change the permeation table and the initial density.  Tables against the oracle's (fp32-rounded on
+    both sides: identical), placement bit exact, the walk on slabs with D, T2 and concentration contrast (general and
+    specialised-with-redo kernels, fp64), on a lattice of random labels with kappa = inf pairs, and a label without
+    spins that is allowed but never populated."""
+    import dataclasses
+    import oracle
+    n = 20000
+    seq = ri.pgse_sequence(2e-4, 800, 0.05, 0.08, [0.0, 5.0], ri.fibonacci_dirs(4), snap_steps=[399, 800])
+    for kappa, name in ((4.0, "permeable"), (0.05, "weakly permeable")):
+        sl = ri.slabs(6, 5, (3, 2), 0.1, D_extra=2.0, D_intra=1.0, kappa_membrane=kappa, T2_extra=0.3, T2_intra=0.6, place="all")
+        sl = dataclasses.replace(sl, conc=np.array([1.0, 0.4], np.float32))
+        o = oracle_run(sl, seq, n, 81)
+        _, P = oracle.tables(sl.D, sl.kappa, sl.voxel_um, seq.dt_ms, conc=sl.conc)
+        S = rms.binding.rms_substrate_create(sl.labels, sl.voxel_um, sl.D, sl.T2, sl.kappa, sl.label_class, sl.n_classes, conc=sl.conc)
+        _, Pg = S.tables(seq.dt_ms)
+        S.destroy()
+        assert np.array_equal(Pg.astype(np.float64), P) and P[0, 1] != P[1, 0]
+        n_intra = int((o["init_vox"][:, 0] % 11 >= 6).sum())
+        assert abs(n_intra / n - 0.4 * 5 / (6 + 0.4 * 5)) < 0.015                    # density ~ c
+        for flags in (0, 2, 8):
+            g = gpu_run(sl, seq, n, 81, flags=flags)
+            print("spin concentrations,", name, "slabs, flags", flags, compare(g, o, n), "permeations", g["n_permeations"])
+            assert g["n_permeations"] == o["n_permeations"] or flags != 8
+    rl = ri.random_lattice((12, 11, 10), n_labels=5, seed=9, D_extra=2.0, D_intra=1.2, place="all")
+    kap = np.full((5, 5), 3.0, np.float32); kap[0, 1] = kap[1, 0] = np.inf; kap[2, 3] = kap[3, 2] = np.inf
+    rl = dataclasses.replace(rl, kappa=kap, conc=np.array([1.0, 0.7, 0.5, 0.5, 0.0], np.float32))
+    o = oracle_run(rl, seq, n, 82)
+    assert not np.any(o["final_label"] == 4) and o["n_permeations"] > 10000
+    for flags in (0, 8):
+        print("spin concentrations, random labels, flags", flags, compare(gpu_run(rl, seq, n, 82, flags=flags), o, n))
+    with pytest.raises(rms.RmsError) as e:
+        gpu_run(dataclasses.replace(rl, conc=np.array([1.0, -1.0, 1, 1, 1], np.float32)), seq, 10, 1)
+    assert e.value.code == -1          # RMS_ERR_ARG
+
+
 def test_degenerate_and_ragged_cases(rms):
     # one walker; 1, 2, 3 steps with a snapshot on every step; no waveform / no directions; hop of 0.99 voxel (three
     # interactions in most steps); a single-voxel pore (every face a membrane: the corner reflector of Fig.2)
