@@ -40,6 +40,8 @@
  *                        rate k = 2 kappa (r^lambda / a_1 + r^(lambda-1) / a_2) between slabs
  *   tensor_signal (rms_oracle.py)  waveform on one axis rotated onto n = scalar waveform along n (same walkers, 1e-12);
  *                        free walk: <e^{-i phi}> = prod_k sinc(c ds |W_k|), W_k the vector suffix sums of g
+ *   run, ERL             between plates: density (1 + h/ds)/2 within ds of a wall (Eq.A.1), gap narrowed by ds/8 per side
+ *                        (Eq.A.8), D_parallel = D0 (1 + S/V ds / 16) (Eq.A.9)
  *   run, rejection sampl. D_parallel = D0 (1 - 3/16 S/V ds) between plates (Eq.B.2), uniform density
  * Parity unpinned: wide-pulse signals inside voxelised cylinders / axons have
  *   no closed form; they are pinned only through the pieces above.
@@ -84,7 +86,8 @@ void rms_oracle_philox4x32_10(const uint32_t ctr[4], const uint32_t key[2], uint
 }
 
 /* Counter layout (R2): key = (seed_lo, seed_hi); ctr = (walker_lo, walker_hi, index, stream). */
-enum { STREAM_INIT = 0, STREAM_DIR = 1, STREAM_PERM = 2, STREAM_INIT_OFFSET = 3, STREAM_MT = 4 };
+enum { STREAM_INIT = 0, STREAM_DIR = 1, STREAM_PERM = 2, STREAM_INIT_OFFSET = 3, STREAM_MT = 4, STREAM_ERL = 5 };
+#define ORC_MAX_ERL_ATTEMPTS 4096u /* R25 */
 
 static void draw(uint64_t seed, uint64_t walker, uint32_t index, uint32_t stream, uint32_t out[4])
 {
@@ -243,7 +246,7 @@ typedef struct {
     const double* s; /* [n_labels] */
     const double* P; /* [n_labels^2] */
     const double* Q; /* [n_labels^2] saturation probability P_MT, or NULL (no absorbing membranes) */
-    int rejection;   /* 1: rejection sampling instead of elastic collision (Appendix B) */
+    int rejection;   /* 1: rejection sampling (Appendix B), 2: equal-step-length random leap (Appendix A) */
 } lattice_t;
 
 static int wrap(int64_t a, int n) { int64_t m = a % n; return (int)(m < 0 ? m + n : m); }
@@ -274,8 +277,9 @@ static double mt_uniform(mt_src_t* ms, int e)
 
 static void step_core(const lattice_t* lat, int32_t vox[3], double off[3], uint16_t* label,
                       const double u[3], perm_src_t* ps, mt_src_t* ms, int* saturated,
-                      int* n_enc, int* n_perm, int* n_clamp)
+                      int* n_enc, int* n_perm, int* n_clamp, int* cancelled)
 {
+    if (cancelled) *cancelled = 0;
     uint16_t L = *label;
     const uint16_t L_in = L;
     const int32_t v_in[3] = { vox[0], vox[1], vox[2] };
@@ -332,6 +336,7 @@ static void step_core(const lattice_t* lat, int32_t vox[3], double off[3], uint1
             vox[0] = v_in[0]; vox[1] = v_in[1]; vox[2] = v_in[2];
             *label = L_in;
             *n_perm = n_perm_in; /* a permeation earlier in the cancelled step did not happen either */
+            if (cancelled) *cancelled = 1;
             return;
         } else {
             r[kstar] = -r[kstar]; /* elastic collision on the face plane */
@@ -356,7 +361,7 @@ int rms_oracle_step(int nx, int ny, int nz, const uint16_t* labels, int n_labels
     lattice_t lat = { nx, ny, nz, labels, n_labels, s, P, NULL, 0 };
     int ne = 0, np = 0, nc = 0;
     perm_src_t ps = { 0, 0, 0, 0, 0, 1, { up[0], up[1], up[2] } };
-    step_core(&lat, vox, off, label, u, &ps, NULL, NULL, &ne, &np, &nc);
+    step_core(&lat, vox, off, label, u, &ps, NULL, NULL, &ne, &np, &nc, NULL);
     counts[0] = ne; counts[1] = np; counts[2] = nc;
     return ORC_OK;
 }
@@ -470,7 +475,16 @@ static void* run_part(void* arg)
             perm_src_t ps = { j->seed, id, i, wa, wb, 0, { 0, 0, 0 } };
             mt_src_t ms = { j->seed, id, i, 0, { 0, 0, 0 } };
             int sat = 0;
-            step_core(lat, v, f, &L, u, &ps, &ms, &sat, &ne, &np, &nc);
+            int cancelled = 0;
+            step_core(lat, v, f, &L, u, &ps, &ms, &sat, &ne, &np, &nc, &cancelled);
+            /* equal-step-length random leap (R25): a cancelled step is tried again in a new direction, drawn
+             * from the stream ERL of this step and attempt, until it meets no membrane */
+            for (uint32_t a = 1; lat->rejection == 2 && cancelled && a < ORC_MAX_ERL_ATTEMPTS; ++a) {
+                uint32_t w4[4];
+                draw(j->seed, id, (uint32_t)i, STREAM_ERL | (a << 8), w4);
+                rms_oracle_direction(w4[0], w4[1], u);
+                step_core(lat, v, f, &L, u, &ps, &ms, &sat, &ne, &np, &nc, &cancelled);
+            }
             if (sat && !isinf(R)) { R = INFINITY; pt->counters[4] += 1; } /* Eq.4: alpha_rho = 0 from here on */
             pt->counters[0] += (uint64_t)ne; pt->counters[1] += (uint64_t)np; pt->counters[2] += (uint64_t)nc;
             if ((uint64_t)ne > pt->counters[3]) pt->counters[3] = (uint64_t)ne;
@@ -586,7 +600,13 @@ int rms_oracle_run(
                 P_tab[a * n_labels + b] = (double)(float)(A / (1.0 + A));
             }
     }
-    if (interaction != 0 && interaction != 1) st = ORC_ERR_ARG;
+    if (interaction < 0 || interaction > 2) st = ORC_ERR_ARG;
+    if (st == ORC_OK && interaction == 2) {
+        /* ERL is defined for impermeable, non-absorbing membranes: a face is a wall (P = 0) or no membrane (P = 1) */
+        if (rho) st = ORC_ERR_ARG;
+        for (int a = 0; a < n_labels * n_labels && st == ORC_OK; ++a)
+            if (P_tab[a] > 0.0 && P_tab[a] < 1.0) st = ORC_ERR_ARG;
+    }
     if (mix_steps < 0 || (mix_steps > 0 && (mix_first < 1 || mix_first + mix_steps - 1 > n_steps))) st = ORC_ERR_ARG;
     if (st != ORC_OK) { free(s_tab); free(P_tab); free(inv_T2); free(Q_tab); free(accept); return st; }
     for (int a = 0; a < n_labels; ++a) {
@@ -599,7 +619,7 @@ int rms_oracle_run(
     job_t job;
     memset(&job, 0, sizeof job);
     job.lat.nx = nx; job.lat.ny = ny; job.lat.nz = nz; job.lat.labels = labels; job.lat.n_labels = n_labels;
-    job.lat.s = s_tab; job.lat.P = P_tab; job.lat.Q = Q_tab; job.lat.rejection = interaction == 1;
+    job.lat.s = s_tab; job.lat.P = P_tab; job.lat.Q = Q_tab; job.lat.rejection = interaction; /* 0 elastic collision, 1 rejection sampling, 2 ERL */
     job.voxel_um = voxel_um; job.inv_T2 = inv_T2; job.inv_T1 = inv_T1; job.mix_first = mix_first; job.mix_steps = mix_steps; job.label_class = label_class; job.n_classes = n_classes;
     job.n_walkers = n_walkers; job.first_id = first_id; job.seed = seed; job.label_allowed = label_allowed; job.accept = accept;
     job.dt = dt_ms; job.n_steps = n_steps; job.n_wave = n_wave; job.wave = wave; job.n_g = n_g; job.gamp = gamp;

@@ -140,7 +140,8 @@ def normalise(raw, dt_ms, snap_steps):
 
 def run(sub, seq, n_walkers, seed, first_id=0, n_threads=1, per_walker=False, interaction=0):
     """Whole path on the CPU: init -> steps -> sums.  `sub`, `seq` are rms_inputs.Substrate / Sequence.
-    interaction: 0 = elastic collision (the paper's method), 1 = rejection sampling (its Appendix B)."""
+    interaction: 0 = elastic collision (the paper's method), 1 = rejection sampling (its Appendix B), 2 = equal-step-length
+    random leap (its Appendix A)."""
     lib = _load()
     labels = np.ascontiguousarray(sub.labels, np.uint16)
     nz, ny, nx = labels.shape

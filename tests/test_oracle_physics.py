@@ -592,3 +592,56 @@ def test_spin_concentration_initial_density_equilibrium_and_exchange_rate():
         assert abs(got - th) < 4 * math.sqrt(0.25 / n_w) + 0.005, (n, got, th)
         if n <= 2500:
             assert abs(got - th_bad) > 0.015, (n, got, th_bad)
+
+
+# ------------------------------------------------------------------ equal-step-length random leap (Appendix A)
+def test_equal_step_length_random_leap_density_and_biases_eq_a1_a8_a9():
+    """P:80 and Appendix A (reading R25): a step that meets a membrane is cancelled and tried again in a new direction.
+    Between impermeable plates: the density within ds of a wall falls to rho(h) ~ (1 + h/ds)/2 (Eq.A.1, d = 3); the
+    long-time transverse MSD is that of a gap narrowed by ds/8 on each side (Eq.A.8); the diffusivity parallel to the
+    plates is raised to D0 (1 + S/V ds / 16) (Eq.A.9) -- elastic collision shows none of the three."""
+    D0 = 2.0
+    ds_vox = math.sqrt(6 * D0 * DT) / LP                       # 0.49 voxel
+    # density and pore shrinkage: a gap of 10 voxels
+    a_vox = 10
+    sub = ri.slabs(a_vox, 3, (4, 4), LP, D_extra=D0, D_intra=D0, place="extra")
+    n_steps, n_w = 2500, 200_000                               # D t / a^2 = 1: equilibrated, MSD at its plateau
+    seq = _narrow(n_steps, np.eye(3))
+    erl = oracle.run(sub, seq, n_w, seed=91, n_threads=THREADS, interaction=2, per_walker=True)
+    ec = oracle.run(sub, seq, n_w // 2, seed=91, n_threads=THREADS, interaction=0, per_walker=True)
+    assert erl["n_permeations"] == 0 and erl["n_encounters"] > 0
+
+    def wall_distance(r):
+        x = np.mod(r["final_vox"][:, 0], a_vox + 3) + r["final_off"][:, 0]
+        assert x.min() >= 0 and x.max() <= a_vox
+        return np.minimum(x, a_vox - x)
+
+    h = wall_distance(erl)
+    bulk = np.mean((h > 1.0) & (h <= 3.0)) / 2.0               # walkers per voxel of distance, away from the walls
+    for lo, hi in ((0.0, 0.5), (0.5, 1.0)):                    # Eq.A.1 averaged over the two halves of the layer
+        want = 0.5 * (1 + 0.5 * (lo + hi))
+        got = np.mean((h > lo * ds_vox) & (h <= hi * ds_vox)) / ((hi - lo) * ds_vox) / bulk
+        assert abs(got - want) < 0.03, (lo, hi, got, want)
+    h = wall_distance(ec)
+    got = np.mean(h <= ds_vox) / ds_vox / (np.mean((h > 1.0) & (h <= 3.0)) / 2.0)
+    assert abs(got - 1.0) < 0.03                               # elastic collision: uniform up to the wall
+    a = a_vox * LP
+    shrunk = a - 2 * (ds_vox * LP) / 8                         # Eq.A.8, d = 3
+    assert abs(ec["msd"][0][0] / (a * a / 6) - 1) < 0.01
+    assert abs(erl["msd"][0][0] / (shrunk ** 2 / 6) - 1) < 0.008, (erl["msd"][0][0], shrunk ** 2 / 6, a * a / 6)
+    assert (a * a - shrunk ** 2) / (a * a) > 0.02              # the effect is three times the tolerance
+    # parallel diffusivity: a narrower gap makes the bias larger; increments after equilibration
+    a_vox = 4
+    sub = ri.slabs(a_vox, 3, (4, 4), LP, D_extra=D0, D_intra=D0, place="extra")
+    n_w = 300_000
+    seq = _narrow(2000, np.eye(3), snaps=[1000, 2000])
+    erl = oracle.run(sub, seq, n_w, seed=92, n_threads=THREADS, interaction=2)
+    ec = oracle.run(sub, seq, n_w, seed=92, n_threads=THREADS, interaction=0)
+    bias = (2.0 / (a_vox * LP)) * (ds_vox * LP) / 16.0         # Eq.A.9 with S/V = 2/a
+    assert 0.014 < bias < 0.017
+    se = math.sqrt(2.0 / n_w)
+    for k in (1, 2):
+        d_erl = (erl["msd"][1][k] - erl["msd"][0][k]) / (2 * 1000 * DT) / D0
+        d_ec = (ec["msd"][1][k] - ec["msd"][0][k]) / (2 * 1000 * DT) / D0
+        assert abs(d_ec - 1) < 4 * se * math.sqrt(2), d_ec
+        assert abs(d_erl - (1 + bias)) < 0.2 * bias + 4 * se * math.sqrt(2), (d_erl, 1 + bias)
