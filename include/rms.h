@@ -151,6 +151,11 @@ int rms_walkers_destroy(rms_walkers* w);
  *             RMS_ERR_UNSUPPORTED for a finite non-zero kappa between unequal D.  Runs in the general kernels
  *             (fp32, or fp64 with RMS_RUN_FP64); biased near membranes by Eq.B.2, which is why elastic
  *             collision is the default.
+ *             RMS_RUN_ERL: equal-step-length random leap, the paper's third comparison interaction (PAPER.md lines 80,
+ *             340, Appendix A): a step that meets a membrane is cancelled and tried again in a new direction until it
+ *             meets none (at most 4095 retries, then the walker stays put for the step).  Impermeable, non-absorbing
+ *             membranes only (kappa 0 or +inf, no rho: RMS_ERR_UNSUPPORTED otherwise).  General kernels; depletes the
+ *             density within a hop length of the membranes (Eq.A.1), hence not the default.
  *
  * mix_first_step, mix_n_steps  the mixing time of a stimulated echo: in these steps Eq.5 runs with the T1 of
  *             the compartment the walker is in, in all others with its T2.  The window lies inside 1..n_steps
@@ -188,6 +193,7 @@ int rms_walkers_destroy(rms_walkers* w);
 #define RMS_RUN_NO_ORDERING 4u
 #define RMS_RUN_FP64 8u
 #define RMS_RUN_REJECTION_SAMPLING 16u
+#define RMS_RUN_ERL 32u
 
 typedef struct {
     double dt_ms;               /* Table 1: dt */

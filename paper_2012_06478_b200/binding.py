@@ -27,6 +27,7 @@ RMS_RUN_GENERAL_KERNEL = 2
 RMS_RUN_NO_ORDERING = 4
 RMS_RUN_FP64 = 8
 RMS_RUN_REJECTION_SAMPLING = 16
+RMS_RUN_ERL = 32
 
 STATUS = {0: "RMS_OK", -1: "RMS_ERR_ARG", -2: "RMS_ERR_STEP_TOO_LARGE", -3: "RMS_ERR_P_RANGE", -4: "RMS_ERR_NO_SPACE",
           -5: "RMS_ERR_OOM", -6: "RMS_ERR_CUDA", -7: "RMS_ERR_UNSUPPORTED"}

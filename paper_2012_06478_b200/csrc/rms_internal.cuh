@@ -97,7 +97,8 @@ struct rms_walkers {
 // ------------------------------------------------------------------------------------------------
 // random numbers: Philox4x32-10, key = (seed_lo, seed_hi), counter = (walker_lo, walker_hi, index, stream)
 // ------------------------------------------------------------------------------------------------
-enum { RMS_STREAM_INIT = 0, RMS_STREAM_DIR = 1, RMS_STREAM_PERM = 2, RMS_STREAM_INIT_OFFSET = 3, RMS_STREAM_MT = 4 };
+enum { RMS_STREAM_INIT = 0, RMS_STREAM_DIR = 1, RMS_STREAM_PERM = 2, RMS_STREAM_INIT_OFFSET = 3, RMS_STREAM_MT = 4, RMS_STREAM_ERL = 5 };
+#define RMS_MAX_ERL_ATTEMPTS 4096u   // R25
 
 #define RMS_PHILOX_M0 0xD2511F53u
 #define RMS_PHILOX_M1 0xCD9E8D57u
@@ -183,7 +184,7 @@ struct rms_step_params {
     const float* PMT;         // [n_labels^2] saturation probability at an encounter a -> b (Eq.4, R20), or NULL
     const float* rate;        // [n_labels] dt / T2
     int n_labels;
-    int rejection;            // 1: rejection sampling instead of elastic collision (R21; general kernels only)
+    int rejection;            // 1: rejection sampling (R21), 2: equal-step-length random leap (R25); general kernels only
     uint32_t t_ceil;          // ceil(512 max P(a->b)) over the membranes: coarse random bits at or above it cannot permeate
     uint32_t step0;           // steps done before this launch
     uint32_t n_steps;         // steps of this launch

@@ -97,9 +97,16 @@ extern "C" int rms_run(const rms_substrate* s, rms_walkers* w, const rms_run_des
 
     // ---- H0 (run-time part): tables from (D, kappa, T2, dt) ---------------------------------------
     std::vector<float> s_tab, P_tab;
-    const bool rs = (d->flags & RMS_RUN_REJECTION_SAMPLING) != 0;   // P:84, Appendix B (R21)
-    int rc = rms_compute_tables(s, d->dt_ms, s_tab, P_tab, rs);
+    const bool erl = (d->flags & RMS_RUN_ERL) != 0;                  // P:80, Appendix A (R25)
+    const bool rs = (d->flags & RMS_RUN_REJECTION_SAMPLING) != 0 || erl;   // P:84, Appendix B (R21); both cancel steps
+    RMS_REQUIRE(!(erl && (d->flags & RMS_RUN_REJECTION_SAMPLING)), RMS_ERR_ARG, "RMS_RUN_ERL and RMS_RUN_REJECTION_SAMPLING exclude each other");
+    RMS_REQUIRE(!(erl && !s->rho.empty()), RMS_ERR_UNSUPPORTED, "equal-step-length random leap with absorbing membranes (P:80 rules it out)");
+    int rc = rms_compute_tables(s, d->dt_ms, s_tab, P_tab, rs && !erl);
     if (rc != RMS_OK) return rc;
+    if (erl)    // a face is a wall or no membrane: the paper rules ERL out for exchange
+        for (size_t t = 0; t < P_tab.size(); ++t)
+            RMS_REQUIRE(!(P_tab[t] > 0.f && P_tab[t] < 1.f), RMS_ERR_UNSUPPORTED,
+                        "equal-step-length random leap with a permeable membrane (labels %d, %d)", (int)(t / nL), (int)(t % nL));
     const bool mt = !s->rho.empty();             // absorbing membranes (Eq.4)
     // stimulated echo (R22): the steps of the mixing time relax with T1; its edges become launch boundaries
     const int64_t mix0 = d->mix_first_step, mixN = d->mix_n_steps;
@@ -313,7 +320,7 @@ extern "C" int rms_run(const rms_substrate* s, rms_walkers* w, const rms_run_des
     const float* rate_T2 = sp.rate;
     const float* rate_T1 = sp.P512 + (size_t)nL * nL * (mt ? 2 : 1);
     sp.t_ceil = t_ceil;
-    sp.rejection = rs ? 1 : 0;
+    sp.rejection = erl ? 2 : (rs ? 1 : 0);
     sp.counters = w->d_counters; sp.n_wave = nW; sp.wave_stride = nT; sp.wsuf_stride = nT + 1;
 
     rms_reduce_params rp;

@@ -241,8 +241,17 @@ __global__ void __launch_bounds__(RMS_BLOCK) rms_step_kernel(const __grid_consta
                         fx = gx; fy = gy; fz = gz;
                     } else {
                         // ---------------- permeable / variable D: the interaction loop written out (LABELS only) ----
+                        bool saturated = false;
+                        // equal-step-length random leap (R25): a cancelled attempt is followed by another in a new direction
+#pragma unroll 1
+                        for (uint32_t attempt = 0;; ++attempt) {
+                        if (attempt) {
+                            uint32_t e0, e1, e2, e3;
+                            rms_philox(p.rk, id_lo, id_hi, j + 1u, RMS_STREAM_ERL | (attempt << 8), e0, e1, e2, e3);
+                            rms_hop(e0, e1, s, rx, ry, rz);
+                        }
                         float px = fx, py = fy, pz = fz;
-                        bool dx = false, dy = false, dz = false, saturated = false;
+                        bool dx = false, dy = false, dz = false;
                         int e = 0;
                         // rejection sampling (R21): what a cancelled step has to put back
                         const int wx_in = wx, wy_in = wy, wz_in = wz, dIx_in = dIx, dIy_in = dIy, dIz_in = dIz;
@@ -388,11 +397,14 @@ __global__ void __launch_bounds__(RMS_BLOCK) rms_step_kernel(const __grid_consta
                             L = L_in; s = s_in; rate = rate_in; relax = relax_in; j_rate = j_rate_in; n_perm = n_perm_in;
                             px = fx; py = fy; pz = fz; rx = 0.f; ry = 0.f; rz = 0.f;
                         }
+                        if (cancelled && p.rejection == 2 && attempt + 1u < RMS_MAX_ERL_ATTEMPTS) continue;
                         const float gx = px + rx, gy = py + ry, gz = pz + rz;
                         fx = fminf(fmaxf(gx, 0.f), RMS_ONE_MINUS);
                         fy = fminf(fmaxf(gy, 0.f), RMS_ONE_MINUS);
                         fz = fminf(fmaxf(gz, 0.f), RMS_ONE_MINUS);
                         n_clamp += (fx != gx) + (fy != gy) + (fz != gz);
+                        break;
+                        }
                         if (saturated && relax != RMS_INF) {   // alpha_rho = 0 from here on (Eq.4); the walk goes on
                             relax = RMS_INF;
                             ++n_sat;

@@ -58,16 +58,21 @@ __global__ void __launch_bounds__(RMS_GBLOCK) rms_step_precise_general_kernel(co
         const uint32_t j = p.step0 + t;                      // steps done before this one
         uint32_t r0, r1, r2, r3;
         rms_philox(p.rk, id_lo, id_hi, j >> 1, RMS_STREAM_DIR, r0, r1, r2, r3);
-        const uint32_t wa = (j & 1u) ? r2 : r0, wb = (j & 1u) ? r3 : r1;
+        uint32_t wa = (j & 1u) ? r2 : r0, wb = (j & 1u) ? r3 : r1;
+        double w_now[NWA];
+#pragma unroll
+        for (int m = 0; m < NW; ++m) w_now[m] = (double)__ldg(p.wave + (size_t)m * p.wave_stride + t);
+        const double one_minus = 0.99999999999999988898;
+        bool sat_step = false;
+        // equal-step-length random leap (R25): a cancelled attempt is followed by another in a new direction
+#pragma unroll 1
+        for (uint32_t attempt = 0;; ++attempt) {
         // direction (R4): z = sym(wa), azimuth pi sym(wb)
         const double z = (double)rms_sym(wa);
         double sn, cs;
         sincos(PI * (double)rms_sym(wb), &sn, &cs);
         const double rho = sqrt(1.0 - z * z);
         double rx = s * (rho * cs), ry = s * (rho * sn), rz = s * z;
-        double w_now[NWA];
-#pragma unroll
-        for (int m = 0; m < NW; ++m) w_now[m] = (double)__ldg(p.wave + (size_t)m * p.wave_stride + t);
 
         double px = fx, py = fy, pz = fz;
         bool dx = false, dy = false, dz = false;
@@ -175,12 +180,21 @@ __global__ void __launch_bounds__(RMS_GBLOCK) rms_step_precise_general_kernel(co
             L = L_in; s = s_in; rate = rate_in; n_perm = n_perm_in;
             px = fx; py = fy; pz = fz; rx = 0.0; ry = 0.0; rz = 0.0;
         }
-        const double one_minus = 0.99999999999999988898;
-        const double gx = px + rx, gy = py + ry, gz = pz + rz;
-        fx = fmin(fmax(gx, 0.0), one_minus); fy = fmin(fmax(gy, 0.0), one_minus); fz = fmin(fmax(gz, 0.0), one_minus);
-        n_clamp += (fx != gx) + (fy != gy) + (fz != gz);
+        if (!(cancelled && p.rejection == 2 && attempt + 1u < RMS_MAX_ERL_ATTEMPTS)) {
+            const double gx = px + rx, gy = py + ry, gz = pz + rz;
+            fx = fmin(fmax(gx, 0.0), one_minus); fy = fmin(fmax(gy, 0.0), one_minus); fz = fmin(fmax(gz, 0.0), one_minus);
+            n_clamp += (fx != gx) + (fy != gy) + (fz != gz);
+            if (saturated) sat_step = true;
+            break;
+        }
+        {
+            uint32_t e0, e1, e2, e3;
+            rms_philox(p.rk, id_lo, id_hi, j + 1u, RMS_STREAM_ERL | ((attempt + 1u) << 8), e0, e1, e2, e3);
+            wa = e0; wb = e1;
+        }
+        }
         relax += rate;                                                        // whole dt to the label at the end of the hop (R12)
-        if (saturated && !dead) {                                             // alpha_rho = 0 from here on (Eq.4); the walk goes on
+        if (sat_step && !dead) {                                              // alpha_rho = 0 from here on (Eq.4); the walk goes on
             relax = __longlong_as_double(0x7ff0000000000000ll);
             dead = true;
             ++n_sat;

@@ -608,6 +608,49 @@ def test_spin_concentrations_permeation_and_placement(rms):
     assert e.value.code == -1          # RMS_ERR_ARG
 
 
+def test_equal_step_length_random_leap_interaction(rms):
+    """S: section 8(f) N4 -- ERL, the paper's third interaction (Appendix A; R25): a step that meets a membrane is
+    cancelled and retried in a new direction.  Impermeable cylinder (integer and non-integer waveforms), the reduced axon
+    substrate, a lattice of random labels with kappa = inf pairs (passages before the cancelling face are undone) and a
+    hop of 0.9 voxel (many retries); fp32 and fp64, against the oracle's interaction = 2."""
+    import dataclasses
+    ERL = rms.binding.RMS_RUN_ERL
+    n = 20000
+    cyl = ri.single_cylinder(24, 8.5, 0.1)
+    seq = ri.pgse_sequence(2e-4, 1500, 0.1, 0.15, [0.0, 2.0], np.eye(3), snap_steps=[500, 1500])
+    o = oracle_run(cyl, seq, n, 95, interaction=2)
+    assert np.abs(o["S"] - oracle_run(cyl, seq, n, 95, interaction=1)["S"]).max() > 1e-3       # not rejection sampling
+    for flags in (ERL, ERL | 8):
+        g = gpu_run(cyl, seq, n, 95, flags=flags)
+        print("ERL, cylinder, flags", flags, compare(g, o, n))
+        assert g["n_encounters"] == o["n_encounters"] or flags == ERL
+    seq_f = dataclasses.replace(seq, wave=(seq.wave * 0.37).astype(np.float32))
+    o = oracle_run(cyl, seq_f, n, 96, interaction=2)
+    for flags in (ERL, ERL | 8):
+        print("ERL, non-integer waveform, flags", flags, compare(gpu_run(cyl, seq_f, n, 96, flags=flags), o, n))
+    cfg = ri.make_config("cfg2", "test")
+    seq_a = dataclasses.replace(cfg.sequence)
+    o = oracle_run(cfg.substrate, seq_a, 4000, 97, interaction=2)
+    for flags in (ERL, ERL | 8):
+        print("ERL, axons, flags", flags, compare(gpu_run(cfg.substrate, seq_a, 4000, 97, flags=flags), o, 4000))
+    hop = 0.9 ** 2 * 0.01 / (6 * 2e-4)
+    rl = ri.random_lattice((12, 11, 10), n_labels=4, seed=9, D_extra=hop, D_intra=hop, place="all")
+    kap = np.zeros((4, 4), np.float32); kap[0, 1] = kap[1, 0] = np.inf; kap[2, 3] = kap[3, 2] = np.inf
+    rl = dataclasses.replace(rl, kappa=kap)
+    seq_r = ri.pgse_sequence(2e-4, 400, 0.02, 0.04, [0.0, 20.0], np.eye(3), snap_steps=[400])
+    o = oracle_run(rl, seq_r, n, 98, interaction=2)
+    assert o["n_permeations"] > 1000 and o["n_encounters"] > 5 * n * 400 // 10
+    for flags in (ERL, ERL | 8):
+        g = gpu_run(rl, seq_r, n, 98, flags=flags)
+        rep = compare(g, o, n)
+        print("ERL, random labels, hop 0.9 voxel, flags", flags, rep, "permeations", g["n_permeations"], o["n_permeations"])
+        assert abs(g["n_permeations"] - o["n_permeations"]) <= 8 * rep["n_diff"] + 2
+    perm = ri.slabs(6, 5, (3, 2), 0.1, D_extra=2.0, D_intra=2.0, kappa_membrane=4.0)
+    with pytest.raises(rms.RmsError) as e:
+        gpu_run(perm, seq, 10, 1, flags=ERL)
+    assert e.value.code == -7          # RMS_ERR_UNSUPPORTED: the paper rules ERL out for exchange
+
+
 def test_degenerate_and_ragged_cases(rms):
     # one walker; 1, 2, 3 steps with a snapshot on every step; no waveform / no directions; hop of 0.99 voxel (three
     # interactions in most steps); a single-voxel pore (every face a membrane: the corner reflector of Fig.2)
