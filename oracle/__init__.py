@@ -13,5 +13,6 @@ from .rms_oracle import (  # noqa: F401
     run,
     normalise,
     tensor_signal,
+    volume_weighted_signal,
     OracleError,
 )

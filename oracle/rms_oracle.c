@@ -40,6 +40,8 @@
  *                        rate k = 2 kappa (r^lambda / a_1 + r^(lambda-1) / a_2) between slabs
  *   tensor_signal (rms_oracle.py)  waveform on one axis rotated onto n = scalar waveform along n (same walkers, 1e-12);
  *                        free walk: <e^{-i phi}> = prod_k sinc(c ds |W_k|), W_k the vector suffix sums of g
+ *   run, label_weight    label counts ~ w_L V_L; w_L = 1/V_L: equal walkers per cell, and the volume-weighted sum of the
+ *                        per-cell signals (volume_weighted_signal, rms_oracle.py) = the uniform-density signal
  *   run, ERL             between plates: density (1 + h/ds)/2 within ds of a wall (Eq.A.1), gap narrowed by ds/8 per side
  *                        (Eq.A.8), D_parallel = D0 (1 + S/V ds / 16) (Eq.A.9)
  *   run, rejection sampl. D_parallel = D0 (1 - 3/16 S/V ds) between plates (Eq.B.2), uniform density
@@ -548,7 +550,7 @@ int rms_oracle_run(
     uint64_t n_walkers, uint64_t first_id, const uint8_t* label_allowed, uint64_t seed,
     double dt_ms, int64_t n_steps, int n_wave, const float* wave, int n_g, const double* gamp,
     int n_dir, const double* dirs, int n_snap, const int64_t* snap_steps, int n_threads, int interaction,
-    const float* T1, int64_t mix_first, int64_t mix_steps, const float* conc,
+    const float* T1, int64_t mix_first, int64_t mix_steps, const float* conc, const float* label_weight,
     double* sum_alpha, double* sig_re, double* sig_im, double* m2, double* m4, double* snap_alpha,
     uint64_t* class_flow, uint64_t* counters,
     int32_t* final_vox, double* final_off, uint16_t* final_label,
@@ -577,15 +579,21 @@ int rms_oracle_run(
     if (!s_tab || !P_tab || !inv_T2 || (rho && !Q_tab)) { free(s_tab); free(P_tab); free(inv_T2); free(Q_tab); return ORC_ERR_OOM; }
     int st = rms_oracle_tables_conc(n_labels, D, kappa, conc, voxel_um, dt_ms, s_tab, P_tab);
     float* accept = NULL;
-    if (st == ORC_OK && conc) { /* initial density proportional to c_L over the allowed labels (R24) */
-        double cmax = 0.0;
-        for (int a = 0; a < n_labels; ++a)
-            if ((!label_allowed || label_allowed[a]) && (double)conc[a] > cmax) cmax = (double)conc[a];
+    if (st == ORC_OK && (conc || label_weight)) {
+        /* initial density proportional to c_L (R24) times the caller's placement weight of the label (walkers per
+         * axon; R26), over the allowed labels */
+        double wmax = 0.0;
         accept = (float*)malloc(sizeof(float) * n_labels);
         if (!accept) st = ORC_ERR_OOM;
-        else if (!(cmax > 0.0)) st = ORC_ERR_NO_SPACE;
-        else for (int a = 0; a < n_labels; ++a) accept[a] = (float)((double)conc[a] / cmax);
-        if (st == ORC_OK && interaction == 1) st = ORC_ERR_ARG; /* Appendix B.1 has no concentrations */
+        for (int a = 0; a < n_labels && st == ORC_OK; ++a) {
+            double w = (conc ? (double)conc[a] : 1.0) * (label_weight ? (double)label_weight[a] : 1.0);
+            if (!(w >= 0.0) || isinf(w)) st = ORC_ERR_ARG;
+            if ((!label_allowed || label_allowed[a]) && w > wmax) wmax = w;
+        }
+        if (st == ORC_OK && !(wmax > 0.0)) st = ORC_ERR_NO_SPACE;
+        for (int a = 0; a < n_labels && st == ORC_OK; ++a)
+            accept[a] = (float)((conc ? (double)conc[a] : 1.0) * (label_weight ? (double)label_weight[a] : 1.0) / wmax);
+        if (st == ORC_OK && conc && interaction == 1) st = ORC_ERR_ARG; /* Appendix B.1 has no concentrations */
     }
     if (st == ORC_OK && rho) st = rms_oracle_mt_table(n_labels, D, rho, dt_ms, Q_tab);
     if (st == ORC_OK && interaction == 1 && kappa) {

@@ -138,7 +138,17 @@ def normalise(raw, dt_ms, snap_steps):
     return out
 
 
-def run(sub, seq, n_walkers, seed, first_id=0, n_threads=1, per_walker=False, interaction=0):
+def volume_weighted_signal(r, class_volume):
+    """Signal of all cells from per-cell runs with any number of walkers per cell (PAPER.md lines 258-266, "volume-weighted sum";
+    reading R26): S = sum_c V_c S_c / sum_c V_c over the classes that hold walkers, S_c = sig_c / sum_alpha_c (Eq.7 per class)."""
+    V = np.asarray(class_volume, np.float64)
+    sa = r["sum_alpha"]
+    use = sa > 0
+    S_c = (r["sig_re"][..., use] + 1j * r["sig_im"][..., use]) / sa[use]
+    return (S_c * V[use]).sum(-1) / V[use].sum()
+
+
+def run(sub, seq, n_walkers, seed, first_id=0, n_threads=1, per_walker=False, interaction=0, label_weight=None):
     """Whole path on the CPU: init -> steps -> sums.  `sub`, `seq` are rms_inputs.Substrate / Sequence.
     interaction: 0 = elastic collision (the paper's method), 1 = rejection sampling (its Appendix B), 2 = equal-step-length
     random leap (its Appendix A)."""
@@ -156,6 +166,7 @@ def run(sub, seq, n_walkers, seed, first_id=0, n_threads=1, per_walker=False, in
     mix_first, mix_steps = int(getattr(seq, "mix_first_step", 0)), int(getattr(seq, "mix_n_steps", 0))
     conc = getattr(sub, "conc", None)
     conc = None if conc is None else np.ascontiguousarray(conc, np.float32)
+    label_weight = None if label_weight is None else np.ascontiguousarray(label_weight, np.float32)
     lclass = np.ascontiguousarray(sub.label_class, np.uint16)
     allowed = np.ascontiguousarray(sub.label_allowed, np.uint8)
     wave = np.ascontiguousarray(seq.wave, np.float32)
@@ -183,7 +194,7 @@ def run(sub, seq, n_walkers, seed, first_id=0, n_threads=1, per_walker=False, in
         C.c_double(seq.dt_ms), C.c_int64(n_steps), C.c_int(n_wave), _p(wave, C.c_float), C.c_int(n_g),
         _p(gamp, C.c_double), C.c_int(n_dir), _p(dirs, C.c_double), C.c_int(n_snap), _p(snaps, C.c_int64),
         C.c_int(n_threads), C.c_int(interaction), _p(T1, C.c_float), C.c_int64(mix_first), C.c_int64(mix_steps),
-        _p(conc, C.c_float),
+        _p(conc, C.c_float), _p(label_weight, C.c_float),
         _p(r["sum_alpha"], C.c_double), _p(r["sig_re"], C.c_double), _p(r["sig_im"], C.c_double),
         _p(r["m2"], C.c_double), _p(r["m4"], C.c_double), _p(r["snap_alpha"], C.c_double),
         _p(r["class_flow"], C.c_uint64), _p(counters, C.c_uint64),

@@ -645,3 +645,42 @@ def test_equal_step_length_random_leap_density_and_biases_eq_a1_a8_a9():
         d_ec = (ec["msd"][1][k] - ec["msd"][0][k]) / (2 * 1000 * DT) / D0
         assert abs(d_ec - 1) < 4 * se * math.sqrt(2), d_ec
         assert abs(d_erl - (1 + bias)) < 0.2 * bias + 4 * se * math.sqrt(2), (d_erl, 1 + bias)
+
+
+# ------------------------------------------------------------------ walkers per cell and the volume-weighted sum
+def test_placement_weights_and_volume_weighted_sum():
+    """The paper runs a fixed number of walkers per axon and adds the axons' signals up by volume (reading R26).
+    A placement weight w_L makes the density proportional to w_L: label counts follow w_L V_L; with w_L = 1 / V_L every
+    cell gets the same number of walkers, and the volume-weighted sum of the per-cell signals is the signal of the
+    uniform-density run."""
+    import dataclasses
+    cfg = ri.make_config("cfg2", "test")
+    sub = cfg.substrate
+    nL = sub.n_labels
+    vol = np.bincount(sub.labels.ravel(), minlength=nL).astype(float)
+    intra = np.nonzero(np.asarray(sub.label_allowed) != 0)[0]
+    assert intra.size >= 8 and vol[intra].max() / vol[intra].min() > 1.5
+    per_cell = dataclasses.replace(sub, label_class=np.arange(nL, dtype=np.uint16), n_classes=nL)
+    seq = ri.pgse_sequence(DT, 1500, 0.1, 0.15, [0.0, 1.0, 3.0], np.eye(3)[:2], snap_steps=[1500])
+    n_w = 60_000
+    w = np.zeros(nL, np.float32); w[intra] = (1.0 / vol[intra]).astype(np.float32)
+    eq = oracle.run(per_cell, seq, n_w, seed=33, n_threads=THREADS, label_weight=w, per_walker=True)
+    counts = np.bincount(eq["final_label"], minlength=nL)[intra]
+    assert counts.sum() == n_w
+    chi2 = ((counts - n_w / intra.size) ** 2 / (n_w / intra.size)).sum()
+    assert chi2 < (intra.size - 1) + 5 * math.sqrt(2 * (intra.size - 1)), counts     # equal walkers per cell
+    w2 = np.zeros(nL, np.float32); w2[intra] = np.linspace(0.2, 1.0, intra.size)
+    r2 = oracle.run(per_cell, seq, n_w, seed=34, n_threads=THREADS, label_weight=w2, per_walker=True)
+    c2 = np.bincount(r2["init_vox"][:, 0] * 0 + sub.labels[r2["init_vox"][:, 2], r2["init_vox"][:, 1], r2["init_vox"][:, 0]],
+                     minlength=nL)[intra]
+    exp = n_w * (w2[intra] * vol[intra]) / (w2[intra] * vol[intra]).sum()
+    assert ((c2 - exp) ** 2 / exp).sum() < (intra.size - 1) + 5 * math.sqrt(2 * (intra.size - 1))
+    uni = oracle.run(per_cell, seq, n_w, seed=35, n_threads=THREADS)
+    S_vw = oracle.volume_weighted_signal(eq, vol)
+    assert S_vw.shape == uni["S"].shape and abs(uni["S"][0, 2, 0]) < 0.97
+    assert np.abs(S_vw - uni["S"]).max() < 5 / math.sqrt(n_w)
+    # with uniform density the volume-weighted sum is the pooled signal up to the sampling of the walker numbers
+    assert np.abs(oracle.volume_weighted_signal(uni, vol) - uni["S"]).max() < 5 / math.sqrt(n_w)
+    # the plain average over cells is something else: the weighting matters
+    plain = ((eq["sig_re"] + 1j * eq["sig_im"])[..., intra] / eq["sum_alpha"][intra]).mean(-1)
+    assert np.abs(plain - uni["S"]).max() > 3 * np.abs(S_vw - uni["S"]).max()
