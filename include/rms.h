@@ -121,6 +121,18 @@ int rms_walkers_init(const rms_substrate* s, uint64_t n_walkers, uint64_t first_
                      const uint8_t* label_allowed, uint64_t seed, void* cuda_stream, rms_walkers** out);
 int rms_walkers_destroy(rms_walkers* w);
 
+/* The same with a placement weight per label (walkers per axon; R26): the density of walkers in an
+ * allowed label L is proportional to label_weight[L] >= 0 (times its spin concentration, if the substrate has them), so
+ * label_weight[L] = 1 / V_L (rms_substrate_label_volumes) gives every cell the same expected number of walkers.
+ * label_weight [n_labels] host; NULL = all 1, which is rms_walkers_init.  Errors as rms_walkers_init; RMS_ERR_ARG for a
+ * negative, infinite or NaN weight, RMS_ERR_NO_SPACE if every allowed label has weight 0. */
+int rms_walkers_init_weighted(const rms_substrate* s, uint64_t n_walkers, uint64_t first_walker_id,
+                              const uint8_t* label_allowed, const float* label_weight, uint64_t seed, void* cuda_stream,
+                              rms_walkers** out);
+
+/* Voxels per label, counted on the device.  voxels_out [n_labels] host.  Errors: RMS_ERR_ARG, RMS_ERR_OOM, RMS_ERR_CUDA. */
+int rms_substrate_label_volumes(const rms_substrate* s, void* cuda_stream, uint64_t* voxels_out);
+
 /* ------------------------------------------------------------------------------------------------
  * rms_run -- advance every walker by n_steps Monte Carlo steps (2.2 steps 2-4: fixed-length
  * hop sqrt(6 D dt) in a random direction; at a voxel face between unlike labels elastic reflection or
@@ -271,6 +283,12 @@ int rms_tables(const rms_substrate* s, double dt_ms, float* s_out, float* P_out)
 int rms_normalise(int n_classes, int n_q, const double* sum_alpha, const double* sig_re, const double* sig_im,
                   int n_snap, int n_dir, const double* snap_alpha, const double* m2, const double* m4,
                   const double* t_ms, double* S_re, double* S_im, double* Dapp, double* Kapp);
+
+/* The signal of all cells from per-cell sums taken with any number of walkers per cell ("volume-weighted sum", P:266;
+ * DESIGN.md R26): S = sum_c V_c S_c / sum_c V_c over the classes with sum_alpha > 0, S_c = sig_c / sum_alpha_c (Eq.7 within
+ * class c).  class_volume [n_classes], the other arrays as in rms_result.  Pure host function. */
+int rms_volume_weighted_signal(int n_classes, int n_q, const double* class_volume, const double* sum_alpha,
+                               const double* sig_re, const double* sig_im, double* S_re, double* S_im);
 
 /* Measured ceiling for the label / neighbourhood gathers of the walk (the second roofline candidate): random
  * gathers of elem_bytes (2 or 4) from a zero-filled device table of table_bytes (48 MB sits in the L2, 1 GB does not),

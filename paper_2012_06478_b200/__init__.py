@@ -15,5 +15,8 @@ from .binding import (  # noqa: F401
     rms_run,
     rms_substrate_create,
     rms_walkers_init,
+    rms_walkers_init_weighted,
+    rms_substrate_label_volumes,
+    rms_volume_weighted_signal,
 )
 from .api import simulate, shard_range  # noqa: F401

@@ -23,7 +23,7 @@ def shard_range(rank: int, world: int, n_walkers: int):
 
 
 def simulate(sub, seq, n_walkers, seed, first_id=0, flags=0, substrate_flags=0, device_labels=None, read_walkers=False,
-             stream=None, keep=None):
+             stream=None, keep=None, label_weight=None):
     """rms_substrate_create -> rms_walkers_init -> rms_run (-> rms_walkers_read); returns the result dict.
 
     device_labels: optional 16-bit CUDA tensor (nz, ny, nx) already resident in HBM (adopted, not copied).
@@ -34,7 +34,10 @@ def simulate(sub, seq, n_walkers, seed, first_id=0, flags=0, substrate_flags=0, 
                                flags=substrate_flags, stream=stream, rho=getattr(sub, "rho", None), T1=getattr(sub, "T1", None), conc=getattr(sub, "conc", None))
     W = None
     try:
-        W = B.rms_walkers_init(S, n_walkers, first_id, sub.label_allowed, seed, stream=stream)
+        if label_weight is None:
+            W = B.rms_walkers_init(S, n_walkers, first_id, sub.label_allowed, seed, stream=stream)
+        else:
+            W = B.rms_walkers_init_weighted(S, n_walkers, first_id, sub.label_allowed, label_weight, seed, stream=stream)
         r = B.rms_run(S, W, seq.dt_ms, seq.n_steps, seq.wave, seq.gamp, seq.dirs, seq.snap_steps, flags=flags, stream=stream,
                       mix_first_step=getattr(seq, "mix_first_step", 0), mix_n_steps=getattr(seq, "mix_n_steps", 0),
                       tensor_waves=getattr(seq, "tensor_waves", None), tensor_gamp=getattr(seq, "tensor_gamp", None),

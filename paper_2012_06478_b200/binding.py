@@ -34,6 +34,7 @@ STATUS = {0: "RMS_OK", -1: "RMS_ERR_ARG", -2: "RMS_ERR_STEP_TOO_LARGE", -3: "RMS
 
 EXPORTS = ("rms_substrate_create", "rms_substrate_destroy", "rms_substrate_get_info", "rms_walkers_init",
            "rms_walkers_destroy", "rms_run", "rms_walkers_read", "rms_walkers_steps_done", "rms_tables", "rms_normalise",
+           "rms_walkers_init_weighted", "rms_substrate_label_volumes", "rms_volume_weighted_signal",
            "rms_memory_trim", "rms_gather_probe", "rms_last_error", "rms_version")
 
 
@@ -226,6 +227,40 @@ def rms_walkers_init(substrate: Substrate, n_walkers, first_walker_id=0, label_a
     _check(load_library().rms_walkers_init(substrate.handle, C.c_uint64(n_walkers), C.c_uint64(first_walker_id),
                                            C.c_void_p(_ptr(allowed)), C.c_uint64(seed), _stream_ptr(stream), C.byref(h)))
     return Walkers(h, int(n_walkers), substrate)
+
+
+def rms_walkers_init_weighted(substrate: Substrate, n_walkers, first_walker_id=0, label_allowed=None, label_weight=None, seed=0,
+                              stream=None) -> Walkers:
+    allowed = _host(label_allowed, np.uint8)
+    weight = _host(label_weight, np.float32)
+    for a in (allowed, weight):
+        if a is not None and a.size != substrate.n_labels:
+            raise ValueError("label_allowed and label_weight must have n_labels entries")
+    h = C.c_void_p()
+    _check(load_library().rms_walkers_init_weighted(substrate.handle, C.c_uint64(n_walkers), C.c_uint64(first_walker_id),
+                                                    C.c_void_p(_ptr(allowed)), C.c_void_p(_ptr(weight)), C.c_uint64(seed),
+                                                    _stream_ptr(stream), C.byref(h)))
+    return Walkers(h, int(n_walkers), substrate)
+
+
+def rms_substrate_label_volumes(substrate: Substrate, stream=None) -> np.ndarray:
+    out = np.zeros(substrate.n_labels, np.uint64)
+    _check(load_library().rms_substrate_label_volumes(substrate.handle, _stream_ptr(stream), C.c_void_p(out.ctypes.data)))
+    return out
+
+
+def rms_volume_weighted_signal(r: dict, class_volume) -> np.ndarray:
+    """S = sum_c V_c S_c / sum_c V_c from the per-class sums of a result dict (rms_volume_weighted_signal in include/rms.h)."""
+    nC = r["sum_alpha"].size
+    V = _host(class_volume, np.float64)
+    if V.size != nC:
+        raise ValueError("class_volume must have n_classes entries")
+    arrs = {k: _host(r[k], np.float64) for k in ("sum_alpha", "sig_re", "sig_im")}
+    S_re, S_im = np.zeros(r["sig_re"].shape[:-1]), np.zeros(r["sig_re"].shape[:-1])
+    _check(load_library().rms_volume_weighted_signal(
+        C.c_int(nC), C.c_int(arrs["sig_re"].size // nC), C.c_void_p(_ptr(V)), C.c_void_p(_ptr(arrs["sum_alpha"])),
+        C.c_void_p(_ptr(arrs["sig_re"])), C.c_void_p(_ptr(arrs["sig_im"])), C.c_void_p(S_re.ctypes.data), C.c_void_p(S_im.ctypes.data)))
+    return S_re + 1j * S_im
 
 
 def rms_run(substrate: Substrate, walkers: Walkers, dt_ms, n_steps, wave=None, gamp=None, dirs=None, snap_steps=None,

@@ -34,6 +34,28 @@ bool wave_is_integer(const float* wave, size_t count)
 
 // H8: Eq.7 S = <alpha e^{-i phi}> / <alpha>, and the narrow-pulse D, K of P:174 with both moments
 // normalised by <alpha> (R14).  Classes are pooled.  Pure host arithmetic on the reduced sums.
+extern "C" int rms_volume_weighted_signal(int n_classes, int n_q, const double* class_volume, const double* sum_alpha,
+                                          const double* sig_re, const double* sig_im, double* S_re, double* S_im)
+{
+    RMS_REQUIRE(n_classes > 0 && n_q >= 0 && class_volume && sum_alpha, RMS_ERR_ARG, "rms_volume_weighted_signal: bad arguments");
+    RMS_REQUIRE(n_q == 0 || (sig_re && sig_im), RMS_ERR_ARG, "rms_volume_weighted_signal: null signal sums");
+    double vol = 0.0;
+    for (int c = 0; c < n_classes; ++c)
+        if (sum_alpha[c] > 0.0) vol += class_volume[c];
+    RMS_REQUIRE(vol > 0.0, RMS_ERR_ARG, "rms_volume_weighted_signal: no class holds both walkers and volume");
+    for (int q = 0; q < n_q; ++q) {
+        double re = 0.0, im = 0.0;
+        for (int c = 0; c < n_classes; ++c)
+            if (sum_alpha[c] > 0.0) {
+                re += class_volume[c] * sig_re[(size_t)q * n_classes + c] / sum_alpha[c];
+                im += class_volume[c] * sig_im[(size_t)q * n_classes + c] / sum_alpha[c];
+            }
+        if (S_re) S_re[q] = re / vol;
+        if (S_im) S_im[q] = im / vol;
+    }
+    return RMS_OK;
+}
+
 extern "C" int rms_normalise(int n_classes, int n_q, const double* sum_alpha, const double* sig_re, const double* sig_im,
                              int n_snap, int n_dir, const double* snap_alpha, const double* m2, const double* m4,
                              const double* t_ms, double* S_re, double* S_im, double* Dapp, double* Kapp)

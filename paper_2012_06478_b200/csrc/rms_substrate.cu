@@ -318,6 +318,59 @@ extern "C" int rms_substrate_destroy(rms_substrate* s)
     return RMS_OK;
 }
 
+// Voxels per label (rms_substrate_label_volumes): grid-stride pass over the uint16 lattice; a warp adds each distinct
+// label of its 32 voxels once (match_any), into a shared-memory histogram when the labels fit, else into global memory.
+#define RMS_VOL_SMEM_LABELS 8192
+__global__ void __launch_bounds__(256) rms_label_volumes_kernel(const uint16_t* __restrict__ labels, uint64_t n_vox, int n_labels,
+                                                                 unsigned long long* __restrict__ out)
+{
+    __shared__ unsigned int hist[RMS_VOL_SMEM_LABELS];
+    const bool in_smem = n_labels <= RMS_VOL_SMEM_LABELS;
+    if (in_smem)
+        for (int t = threadIdx.x; t < n_labels; t += blockDim.x) hist[t] = 0u;
+    __syncthreads();
+    const uint64_t stride = (uint64_t)gridDim.x * blockDim.x;
+    const uint64_t n_round = (n_vox + 31) / 32 * 32;                 // whole warps stay in the loop together
+    for (uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n_round; i += stride) {
+        const bool ok = i < n_vox;
+        const unsigned L = ok ? labels[i] : 0xFFFFFFFFu;
+        const unsigned peers = __match_any_sync(0xFFFFFFFFu, L);
+        if (ok && (threadIdx.x & 31) == (unsigned)(__ffs(peers) - 1)) {
+            if (in_smem) atomicAdd(&hist[L], (unsigned)__popc(peers));
+            else atomicAdd(&out[L], (unsigned long long)__popc(peers));
+        }
+    }
+    __syncthreads();
+    if (in_smem)
+        for (int t = threadIdx.x; t < n_labels; t += blockDim.x)
+            if (hist[t]) atomicAdd(&out[t], (unsigned long long)hist[t]);
+}
+
+extern "C" int rms_substrate_label_volumes(const rms_substrate* s, void* cuda_stream, uint64_t* voxels_out)
+{
+    RMS_REQUIRE(s && voxels_out, RMS_ERR_ARG, "rms_substrate_label_volumes: null argument");
+    cudaStream_t stream = (cudaStream_t)cuda_stream;
+    unsigned long long* d_out = nullptr;
+    RMS_CUDA_TRY(rms_malloc((void**)&d_out, (size_t)s->n_labels * sizeof(unsigned long long)));
+    cudaError_t e = cudaMemsetAsync(d_out, 0, (size_t)s->n_labels * sizeof(unsigned long long), stream);
+    if (e == cudaSuccess) {
+        // a block's shared counters are 32 bit: at most 2^32 - 1 voxels per block
+        const uint64_t per_block = 1ull << 24;
+        unsigned grid = (unsigned)std::min<uint64_t>(std::max<uint64_t>((s->n_vox + per_block - 1) / per_block, 148ull * 8), 1u << 20);
+        rms_label_volumes_kernel<<<grid, 256, 0, stream>>>(s->d_labels, s->n_vox, s->n_labels, d_out);
+        e = cudaGetLastError();
+    }
+    if (e == cudaSuccess)
+        e = cudaMemcpyAsync(voxels_out, d_out, (size_t)s->n_labels * sizeof(unsigned long long), cudaMemcpyDeviceToHost, stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(stream);
+    rms_free(d_out);
+    if (e != cudaSuccess) {
+        rms_set_error("rms_substrate_label_volumes failed: %s", cudaGetErrorString(e));
+        return e == cudaErrorMemoryAllocation ? RMS_ERR_OOM : RMS_ERR_CUDA;
+    }
+    return RMS_OK;
+}
+
 extern "C" int rms_substrate_get_info(const rms_substrate* s, rms_substrate_info* out)
 {
     RMS_REQUIRE(s && out, RMS_ERR_ARG, "rms_substrate_get_info: null argument");

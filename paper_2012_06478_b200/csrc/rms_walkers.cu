@@ -1,5 +1,6 @@
 // rms_walkers.cu -- H1: walker initialisation and the state arrays / read-back hook.
 #include <string.h>
+#include <cmath>
 
 #include "rms_internal.cuh"
 
@@ -52,6 +53,13 @@ static size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 extern "C" int rms_walkers_init(const rms_substrate* s, uint64_t n_walkers, uint64_t first_walker_id,
                                 const uint8_t* label_allowed, uint64_t seed, void* cuda_stream, rms_walkers** out)
 {
+    return rms_walkers_init_weighted(s, n_walkers, first_walker_id, label_allowed, nullptr, seed, cuda_stream, out);
+}
+
+extern "C" int rms_walkers_init_weighted(const rms_substrate* s, uint64_t n_walkers, uint64_t first_walker_id,
+                                         const uint8_t* label_allowed, const float* label_weight, uint64_t seed,
+                                         void* cuda_stream, rms_walkers** out)
+{
     RMS_REQUIRE(s && out, RMS_ERR_ARG, "rms_walkers_init: null substrate or output");
     *out = nullptr;
     RMS_REQUIRE(n_walkers > 0 && n_walkers < (1ull << 31), RMS_ERR_ARG, "n_walkers must be in 1..2^31-1");
@@ -71,13 +79,19 @@ extern "C" int rms_walkers_init(const rms_substrate* s, uint64_t n_walkers, uint
     uint8_t* d_allowed = nullptr;
     float* d_accept = nullptr;
     std::vector<float> h_accept;
-    if (!s->conc.empty()) {      // initial density proportional to c_L over the allowed labels (R24)
-        double cmax = 0.0;
-        for (int a = 0; a < s->n_labels; ++a)
-            if ((!label_allowed || label_allowed[a]) && (double)s->conc[a] > cmax) cmax = (double)s->conc[a];
-        RMS_REQUIRE(cmax > 0.0, RMS_ERR_NO_SPACE, "every allowed label has spin concentration 0");
+    if (!s->conc.empty() || label_weight) {
+        // initial density proportional to c_L (R24) times the caller's placement weight (R26), over the allowed labels
+        auto weight = [&](int a) {
+            return (s->conc.empty() ? 1.0 : (double)s->conc[a]) * (label_weight ? (double)label_weight[a] : 1.0);
+        };
+        double wmax = 0.0;
+        for (int a = 0; a < s->n_labels; ++a) {
+            RMS_REQUIRE(weight(a) >= 0.0 && std::isfinite(weight(a)), RMS_ERR_ARG, "label_weight[%d] is negative, infinite or NaN", a);
+            if ((!label_allowed || label_allowed[a]) && weight(a) > wmax) wmax = weight(a);
+        }
+        RMS_REQUIRE(wmax > 0.0, RMS_ERR_NO_SPACE, "every allowed label has placement weight or spin concentration 0");
         h_accept.resize(s->n_labels);
-        for (int a = 0; a < s->n_labels; ++a) h_accept[a] = (float)((double)s->conc[a] / cmax);
+        for (int a = 0; a < s->n_labels; ++a) h_accept[a] = (float)(weight(a) / wmax);
     }
     int rc = RMS_OK;
     unsigned long long h_cnt[8] = {0};

@@ -651,6 +651,43 @@ def test_equal_step_length_random_leap_interaction(rms):
     assert e.value.code == -7          # RMS_ERR_UNSUPPORTED: the paper rules ERL out for exchange
 
 
+def test_walkers_per_axon_placement_and_volume_weighted_sum(rms):
+    """S: section 8(f) N2, "volume-weighted sums; walkers-per-axon placement" -- P:258-266 (R26): placement weights per label
+    (bit exact against the oracle), the voxel count per label on the device, and the volume-weighted sum of the per-cell
+    signals; with w_L = 1 / V_L every axon gets the same expected number of walkers."""
+    import dataclasses
+    import oracle
+    cfg = ri.make_config("cfg2", "test")
+    sub = cfg.substrate
+    nL = sub.n_labels
+    vol = np.bincount(sub.labels.ravel(), minlength=nL)
+    intra = np.nonzero(np.asarray(sub.label_allowed) != 0)[0]
+    per_cell = dataclasses.replace(sub, label_class=np.arange(nL, dtype=np.uint16), n_classes=nL)
+    S = rms.rms_substrate_create(per_cell.labels, per_cell.voxel_um, per_cell.D, per_cell.T2, per_cell.kappa, per_cell.label_class, nL)
+    assert np.array_equal(rms.rms_substrate_label_volumes(S), vol.astype(np.uint64))
+    S.destroy()
+    big = ri.random_lattice((70, 33, 41), n_labels=9000, seed=4)            # more labels than the shared-memory histogram holds
+    S = rms.rms_substrate_create(big.labels, big.voxel_um, big.D, big.T2, big.kappa, big.label_class, big.n_classes)
+    assert np.array_equal(rms.rms_substrate_label_volumes(S), np.bincount(big.labels.ravel(), minlength=9000).astype(np.uint64))
+    S.destroy()
+    w = np.zeros(nL, np.float32); w[intra] = (1.0 / vol[intra]).astype(np.float32)
+    seq = ri.pgse_sequence(2e-4, 1500, 0.1, 0.15, [0.0, 1.0, 3.0], np.eye(3)[:2], snap_steps=[1500])
+    n = 30000
+    o = oracle.run(per_cell, seq, n, 37, n_threads=oracle.rms_oracle.default_threads(), per_walker=True, label_weight=w)
+    for flags in (0, 8):
+        g = rms.simulate(per_cell, seq, n, 37, flags=flags, read_walkers=True, label_weight=w)
+        rep = compare(g, o, n)                                               # includes the bit-exact placement
+        got = rms.rms_volume_weighted_signal(g, vol.astype(float))
+        want = oracle.volume_weighted_signal(o, vol.astype(float))
+        print("walkers per axon, flags", flags, rep, "max |d S_vw|", np.abs(got - want).max())
+        assert np.abs(got - want).max() <= 1e-4 + 2.0 * rep["n_diff"] / n
+    counts = np.bincount(g["walkers"]["label"], minlength=nL)[intra]
+    assert counts.sum() == n and counts.min() > 0.8 * n / intra.size and counts.max() < 1.2 * n / intra.size
+    with pytest.raises(rms.RmsError) as e:
+        rms.simulate(per_cell, seq, 10, 1, label_weight=np.zeros(nL, np.float32))
+    assert e.value.code == -4          # RMS_ERR_NO_SPACE
+
+
 def test_degenerate_and_ragged_cases(rms):
     # one walker; 1, 2, 3 steps with a snapshot on every step; no waveform / no directions; hop of 0.99 voxel (three
     # interactions in most steps); a single-voxel pore (every face a membrane: the corner reflector of Fig.2)

@@ -74,6 +74,19 @@ def test_rms_normalise_is_eq7_and_the_narrow_pulse_moments(rms):
     assert np.allclose(out["Kapp"], x4 / x2 ** 2 - 3.0, rtol=1e-13)                        # K, both moments over <a> (R14)
 
 
+def test_rms_volume_weighted_signal_is_the_volume_weighted_sum_of_per_class_signals(rms):
+    rng = np.random.default_rng(6)
+    nC, nW, nG, nD = 5, 2, 3, 4
+    r = dict(sum_alpha=np.array([7.0, 0.0, 3.0, 11.0, 2.0]), sig_re=rng.normal(size=(nW, nG, nD, nC)), sig_im=rng.normal(size=(nW, nG, nD, nC)))
+    V = np.array([10.0, 99.0, 1.0, 4.0, 6.0])
+    use = r["sum_alpha"] > 0                                                              # class 1 holds no walkers: left out
+    want = (((r["sig_re"] + 1j * r["sig_im"])[..., use] / r["sum_alpha"][use]) * V[use]).sum(-1) / V[use].sum()   # P:266, R26
+    got = rms.binding.rms_volume_weighted_signal(r, V)
+    assert got.shape == (nW, nG, nD) and np.allclose(got, want, rtol=1e-14)
+    with pytest.raises(rms.RmsError):
+        rms.binding.rms_volume_weighted_signal(dict(r, sum_alpha=np.zeros(nC)), V)
+
+
 def test_shard_range_partitions_the_walker_ids(rms):
     for n, world in ((10, 3), (1_000_000, 8), (7, 8), (0, 2)):
         got = [rms.api.shard_range(r, world, n) for r in range(world)]
