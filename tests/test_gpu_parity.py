@@ -129,6 +129,30 @@ def test_chunked_run_continues_the_same_trajectories(rms):
     print("chunked", rep)
 
 
+def test_chunked_run_with_a_comparison_interaction_and_a_mixing_time(rms):
+    """The random numbers of the retries (R25) are keyed on the absolute step and the mixing time (R22) is given per call: three
+    calls -- the middle one all mixing time, its T1 weight and the ERL retries included -- equal the oracle's single run."""
+    import dataclasses
+    sub = dataclasses.replace(ri.single_cylinder(24, 8.5, 0.1), T2=np.array([0.3, 0.15], np.float32), T1=np.array([0.9, 0.4], np.float32))
+    seq = ri.pgse_sequence(2e-4, 900, 0.06, 0.12, [0.0, 2.0], np.eye(3), snap_steps=[900])     # lobes 1..300, 601..900
+    seq = dataclasses.replace(seq, mix_first_step=301, mix_n_steps=300)
+    n = 6000
+    for interaction, flag in ((2, rms.binding.RMS_RUN_ERL), (1, rms.binding.RMS_RUN_REJECTION_SAMPLING)):
+        o = oracle_run(sub, seq, n, 19, interaction=interaction)
+        for fp in (0, 8):
+            S = rms.rms_substrate_create(sub.labels, sub.voxel_um, sub.D, sub.T2, sub.kappa, sub.label_class, sub.n_classes, T1=sub.T1)
+            W = rms.rms_walkers_init(S, n, 0, sub.label_allowed, 19)
+            enc = 0
+            for a, b, mix in ((0, 301, (301, 1)), (301, 599, (1, 298)), (599, 900, (1, 1))):     # odd cuts; window 301..600 split over all three
+                r = rms.rms_run(S, W, seq.dt_ms, b - a, seq.wave[:, a:b], seq.gamp, seq.dirs, [b - a], flags=flag | fp,
+                                mix_first_step=mix[0], mix_n_steps=mix[1])
+                enc += r["n_encounters"]
+            r["n_encounters"] = enc
+            r["walkers"] = W.read()
+            print("chunked, interaction", interaction, "fp64" if fp else "fp32", compare(r, o, n))
+            W.destroy(); S.destroy()
+
+
 def test_general_waveform_table_mode_and_two_waves(rms):
     # non-integer gradient shapes (sine, trapezoid) take the table path; two waveforms share one trajectory set
     sub = ri.single_cylinder(24, 7.5, 0.1)
