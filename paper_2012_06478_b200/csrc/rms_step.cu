@@ -62,7 +62,9 @@ __device__ __forceinline__ float rms_hit_time(bool cross, float f, float r)
     return cross ? __fdividef((r > 0.f ? 1.f : 0.f) - f, r) : RMS_INF;
 }
 
-template <int NW, int WMODE, int LAT, bool PERM>
+// PERM: 0 impermeable (per-axis outcome), 1 the interaction loop written out (permeation, D contrast), 2 the same with the
+// absorbing membranes (Eq.4) and the bookkeeping of a cancelled step (rejection sampling, ERL) compiled in
+template <int NW, int WMODE, int LAT, int PERM>
 __global__ void __launch_bounds__(RMS_BLOCK) rms_step_kernel(const __grid_constant__ rms_step_params p)
 {
     const uint64_t t_global = (uint64_t)blockIdx.x * RMS_BLOCK + threadIdx.x;
@@ -242,10 +244,11 @@ __global__ void __launch_bounds__(RMS_BLOCK) rms_step_kernel(const __grid_consta
                     } else {
                         // ---------------- permeable / variable D: the interaction loop written out (LABELS only) ----
                         bool saturated = false;
+                        constexpr bool REJ = PERM == 2;
                         // equal-step-length random leap (R25): a cancelled attempt is followed by another in a new direction
 #pragma unroll 1
                         for (uint32_t attempt = 0;; ++attempt) {
-                        if (attempt) {
+                        if (REJ && attempt) {
                             uint32_t e0, e1, e2, e3;
                             rms_philox(p.rk, id_lo, id_hi, j + 1u, RMS_STREAM_ERL | (attempt << 8), e0, e1, e2, e3);
                             rms_hop(e0, e1, s, rx, ry, rz);
@@ -288,7 +291,7 @@ __global__ void __launch_bounds__(RMS_BLOCK) rms_step_kernel(const __grid_consta
                             bool pass = true;
                             if (Ln != L) {
                                 ++n_enc;
-                                if (p.PMT) {   // absorbing membrane (Eq.4, R20): the encounter saturates the walker with P_MT
+                                if (REJ && p.PMT) {   // absorbing membrane (Eq.4, R20): the encounter saturates the walker with P_MT
                                     const float Q = __ldg(p.PMT + (size_t)L * p.n_labels + Ln);
                                     if (Q > 0.f) {
                                         if (!have_m) {
@@ -333,7 +336,7 @@ __global__ void __launch_bounds__(RMS_BLOCK) rms_step_kernel(const __grid_consta
                                 if (isx) wx = nwk; else if (isy) wy = nwk; else wz = nwk;
                                 const int sg1 = neg ? -1 : 1;
                                 if (isx) dIx += sg1; else if (isy) dIy += sg1; else dIz += sg1;
-                                ev[n_ev++] = sg1 * (isx ? 1 : (isy ? 2 : 3));
+                                if (REJ) ev[n_ev++] = sg1 * (isx ? 1 : (isy ? 2 : 3));
                                 if (NW > 0 && acc_rem) {
                                     if (WMODE == RMS_WMODE_CONST) {
 #pragma unroll
@@ -362,7 +365,7 @@ __global__ void __launch_bounds__(RMS_BLOCK) rms_step_kernel(const __grid_consta
                                     s = s_new;
                                     L = Ln;
                                 }
-                            } else if (p.rejection) {
+                            } else if (REJ && p.rejection) {
                                 cancelled = true;                       // rejection sampling: the walker does not move for the step
                                 break;
                             } else {
@@ -371,7 +374,7 @@ __global__ void __launch_bounds__(RMS_BLOCK) rms_step_kernel(const __grid_consta
                             }
                             if (isx) { px = pk; dx = true; } else if (isy) { py = pk; dy = true; } else { pz = pk; dz = true; }
                         }
-                        if (cancelled) {
+                        if (REJ && cancelled) {
                             // undo the face passages of the cancelled step (voxel, displacement, event-driven phase part, label)
                             for (int q = 0; q < n_ev; ++q) {
                                 const int ax = (ev[q] < 0 ? -ev[q] : ev[q]) - 1;
@@ -397,7 +400,7 @@ __global__ void __launch_bounds__(RMS_BLOCK) rms_step_kernel(const __grid_consta
                             L = L_in; s = s_in; rate = rate_in; relax = relax_in; j_rate = j_rate_in; n_perm = n_perm_in;
                             px = fx; py = fy; pz = fz; rx = 0.f; ry = 0.f; rz = 0.f;
                         }
-                        if (cancelled && p.rejection == 2 && attempt + 1u < RMS_MAX_ERL_ATTEMPTS) continue;
+                        if (REJ && cancelled && p.rejection == 2 && attempt + 1u < RMS_MAX_ERL_ATTEMPTS) continue;
                         const float gx = px + rx, gy = py + ry, gz = pz + rz;
                         fx = fminf(fmaxf(gx, 0.f), RMS_ONE_MINUS);
                         fy = fminf(fmaxf(gy, 0.f), RMS_ONE_MINUS);
@@ -405,7 +408,7 @@ __global__ void __launch_bounds__(RMS_BLOCK) rms_step_kernel(const __grid_consta
                         n_clamp += (fx != gx) + (fy != gy) + (fz != gz);
                         break;
                         }
-                        if (saturated && relax != RMS_INF) {   // alpha_rho = 0 from here on (Eq.4); the walk goes on
+                        if (REJ && saturated && relax != RMS_INF) {   // alpha_rho = 0 from here on (Eq.4); the walk goes on
                             relax = RMS_INF;
                             ++n_sat;
                         }
@@ -479,12 +482,14 @@ template <int NW, int WMODE>
 static int launch_nw(const rms_step_params& p, int lat, bool permeable, cudaStream_t stream)
 {
     const unsigned grid = (unsigned)((p.n + RMS_BLOCK - 1) / RMS_BLOCK);
-    if (permeable)
-        rms_step_kernel<NW, WMODE, RMS_LAT_LABELS, true><<<grid, RMS_BLOCK, 0, stream>>>(p);
+    if (permeable && (p.rejection || p.PMT))
+        rms_step_kernel<NW, WMODE, RMS_LAT_LABELS, 2><<<grid, RMS_BLOCK, 0, stream>>>(p);
+    else if (permeable)
+        rms_step_kernel<NW, WMODE, RMS_LAT_LABELS, 1><<<grid, RMS_BLOCK, 0, stream>>>(p);
     else if (lat == RMS_LAT_FACES)
-        rms_step_kernel<NW, WMODE, RMS_LAT_FACES, false><<<grid, RMS_BLOCK, 0, stream>>>(p);
+        rms_step_kernel<NW, WMODE, RMS_LAT_FACES, 0><<<grid, RMS_BLOCK, 0, stream>>>(p);
     else
-        rms_step_kernel<NW, WMODE, RMS_LAT_LABELS, false><<<grid, RMS_BLOCK, 0, stream>>>(p);
+        rms_step_kernel<NW, WMODE, RMS_LAT_LABELS, 0><<<grid, RMS_BLOCK, 0, stream>>>(p);
     RMS_CUDA_TRY(cudaGetLastError());
     return RMS_OK;
 }

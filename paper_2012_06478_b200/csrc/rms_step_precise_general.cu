@@ -11,7 +11,8 @@ namespace {
 __device__ __forceinline__ bool rms_outside_g(double g) { return (uint32_t)__double2hiint(g) >= 0x3FF00000u; }   // g >= 1 or g < 0
 }
 
-template <int NW>
+// REJ: the absorbing membranes (Eq.4) and the bookkeeping of a cancelled step (rejection sampling, ERL) compiled in
+template <int NW, bool REJ>
 __global__ void __launch_bounds__(RMS_GBLOCK) rms_step_precise_general_kernel(const __grid_constant__ rms_step_params p)
 {
     const uint64_t t_global = (uint64_t)blockIdx.x * RMS_GBLOCK + threadIdx.x;
@@ -113,7 +114,7 @@ __global__ void __launch_bounds__(RMS_GBLOCK) rms_step_precise_general_kernel(co
             bool pass = true;
             if (Ln != L) {                                                     // a membrane
                 ++n_enc;
-                if (p.PMT) {   // absorbing membrane (Eq.4, R20): the encounter saturates the walker with probability P_MT
+                if (REJ && p.PMT) {   // absorbing membrane (Eq.4, R20): the encounter saturates the walker with probability P_MT
                     const float Q = __ldg(p.PMT + (size_t)L * p.n_labels + Ln);
                     if (Q > 0.f) {
                         if (!have_m) { rms_philox(p.rk, id_lo, id_hi, j + 1u, RMS_STREAM_MT, m0, m1, m2, m3); have_m = true; }
@@ -142,7 +143,7 @@ __global__ void __launch_bounds__(RMS_GBLOCK) rms_step_precise_general_kernel(co
                 if (isx) wx = nwk; else if (isy) wy = nwk; else wz = nwk;
                 const int sg1 = neg ? -1 : 1;
                 if (isx) dIx += sg1; else if (isy) dIy += sg1; else dIz += sg1;
-                ev[n_ev++] = sg1 * (isx ? 1 : (isy ? 2 : 3));
+                if (REJ) ev[n_ev++] = sg1 * (isx ? 1 : (isy ? 2 : 3));
 #pragma unroll
                 for (int m = 0; m < NW; ++m) {
                     double v = p.wsuf[(size_t)m * p.wsuf_stride + t] - p.wsuf_end[m];
@@ -157,7 +158,7 @@ __global__ void __launch_bounds__(RMS_GBLOCK) rms_step_precise_general_kernel(co
                     rate = (double)__ldg(p.rate + Ln);
                     L = Ln;
                 }
-            } else if (p.rejection) {
+            } else if (REJ && p.rejection) {
                 cancelled = true;                                              // rejection sampling: the walker does not move for the step
                 break;
             } else {
@@ -166,7 +167,7 @@ __global__ void __launch_bounds__(RMS_GBLOCK) rms_step_precise_general_kernel(co
             }
             if (isx) { px = pk; dx = true; } else if (isy) { py = pk; dy = true; } else { pz = pk; dz = true; }
         }
-        if (cancelled) {
+        if (REJ && cancelled) {
             for (int q = 0; q < n_ev; ++q) {
                 const int ax = (ev[q] < 0 ? -ev[q] : ev[q]) - 1;
 #pragma unroll
@@ -180,7 +181,7 @@ __global__ void __launch_bounds__(RMS_GBLOCK) rms_step_precise_general_kernel(co
             L = L_in; s = s_in; rate = rate_in; n_perm = n_perm_in;
             px = fx; py = fy; pz = fz; rx = 0.0; ry = 0.0; rz = 0.0;
         }
-        if (!(cancelled && p.rejection == 2 && attempt + 1u < RMS_MAX_ERL_ATTEMPTS)) {
+        if (!(REJ && cancelled && p.rejection == 2 && attempt + 1u < RMS_MAX_ERL_ATTEMPTS)) {
             const double gx = px + rx, gy = py + ry, gz = pz + rz;
             fx = fmin(fmax(gx, 0.0), one_minus); fy = fmin(fmax(gy, 0.0), one_minus); fz = fmin(fmax(gz, 0.0), one_minus);
             n_clamp += (fx != gx) + (fy != gy) + (fz != gz);
@@ -194,7 +195,7 @@ __global__ void __launch_bounds__(RMS_GBLOCK) rms_step_precise_general_kernel(co
         }
         }
         relax += rate;                                                        // whole dt to the label at the end of the hop (R12)
-        if (sat_step && !dead) {                                              // alpha_rho = 0 from here on (Eq.4); the walk goes on
+        if (REJ && sat_step && !dead) {                                              // alpha_rho = 0 from here on (Eq.4); the walk goes on
             relax = __longlong_as_double(0x7ff0000000000000ll);
             dead = true;
             ++n_sat;
@@ -239,13 +240,13 @@ int rms_launch_step_precise_general(const rms_step_params& p, int n_wave, cudaSt
     if (p.n == 0 || p.n_steps == 0) return RMS_OK;
     const unsigned grid = (unsigned)((p.n + RMS_GBLOCK - 1) / RMS_GBLOCK);
     switch (n_wave) {
-        case 0: rms_step_precise_general_kernel<0><<<grid, RMS_GBLOCK, 0, stream>>>(p); break;
-        case 1: rms_step_precise_general_kernel<1><<<grid, RMS_GBLOCK, 0, stream>>>(p); break;
-        case 2: rms_step_precise_general_kernel<2><<<grid, RMS_GBLOCK, 0, stream>>>(p); break;
-        case 3: rms_step_precise_general_kernel<3><<<grid, RMS_GBLOCK, 0, stream>>>(p); break;
-        case 4: rms_step_precise_general_kernel<4><<<grid, RMS_GBLOCK, 0, stream>>>(p); break;
-        case 8: rms_step_precise_general_kernel<8><<<grid, RMS_GBLOCK, 0, stream>>>(p); break;
-        case 16: rms_step_precise_general_kernel<16><<<grid, RMS_GBLOCK, 0, stream>>>(p); break;
+        case 0: if (p.rejection || p.PMT) rms_step_precise_general_kernel<0, true><<<grid, RMS_GBLOCK, 0, stream>>>(p); else rms_step_precise_general_kernel<0, false><<<grid, RMS_GBLOCK, 0, stream>>>(p); break;
+        case 1: if (p.rejection || p.PMT) rms_step_precise_general_kernel<1, true><<<grid, RMS_GBLOCK, 0, stream>>>(p); else rms_step_precise_general_kernel<1, false><<<grid, RMS_GBLOCK, 0, stream>>>(p); break;
+        case 2: if (p.rejection || p.PMT) rms_step_precise_general_kernel<2, true><<<grid, RMS_GBLOCK, 0, stream>>>(p); else rms_step_precise_general_kernel<2, false><<<grid, RMS_GBLOCK, 0, stream>>>(p); break;
+        case 3: if (p.rejection || p.PMT) rms_step_precise_general_kernel<3, true><<<grid, RMS_GBLOCK, 0, stream>>>(p); else rms_step_precise_general_kernel<3, false><<<grid, RMS_GBLOCK, 0, stream>>>(p); break;
+        case 4: if (p.rejection || p.PMT) rms_step_precise_general_kernel<4, true><<<grid, RMS_GBLOCK, 0, stream>>>(p); else rms_step_precise_general_kernel<4, false><<<grid, RMS_GBLOCK, 0, stream>>>(p); break;
+        case 8: if (p.rejection || p.PMT) rms_step_precise_general_kernel<8, true><<<grid, RMS_GBLOCK, 0, stream>>>(p); else rms_step_precise_general_kernel<8, false><<<grid, RMS_GBLOCK, 0, stream>>>(p); break;
+        case 16: if (p.rejection || p.PMT) rms_step_precise_general_kernel<16, true><<<grid, RMS_GBLOCK, 0, stream>>>(p); else rms_step_precise_general_kernel<16, false><<<grid, RMS_GBLOCK, 0, stream>>>(p); break;
         default:
             rms_set_error("n_wave = %d is above RMS_MAX_WAVES = %d", n_wave, RMS_MAX_WAVES);
             return RMS_ERR_UNSUPPORTED;
