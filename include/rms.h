@@ -147,7 +147,7 @@ int rms_substrate_label_volumes(const rms_substrate* s, void* cuda_stream, uint6
  *             moments are taken (host)
  * flags       RMS_RUN_LABEL_GATHER: test faces by gathering the neighbour's uint16 label (the paper's
  *             lookup table) instead of the neighbourhood lattice.
- *             RMS_RUN_GENERAL_KERNEL: impermeable or weakly permeable runs with piecewise-constant waveforms (rectangular
+ *             RMS_RUN_GENERAL_KERNEL: impermeable or permeable runs with piecewise-constant waveforms (rectangular
  *             lobes of any amplitude, segments of >= 32 steps on average) normally take the specialised kernel
  *             (csrc/rms_step_fast.cu); this flag forces the general one.
  *             RMS_RUN_FP64: direction, hop, in-voxel offsets, hit order and phase in fp64 instead of fp32, for runs

@@ -34,6 +34,13 @@ bool wave_is_integer(const float* wave, size_t count)
 
 // H8: Eq.7 S = <alpha e^{-i phi}> / <alpha>, and the narrow-pulse D, K of P:174 with both moments
 // normalised by <alpha> (R14).  Classes are pooled.  Pure host arithmetic on the reduced sums.
+// Permeable runs take the specialised kernel when ceil(512 P_max) is at most this.  Measured on the cfg3 lattice (1e6 walkers
+// x 1e4 steps, general kernel 176 ms): 65 / 71 / 81 / 90 / 102 / 112 ms at 512 P_max = 0.2 / 23 / 73 / 130 / 213 / 292 -- the
+// redo of a step that may permeate is cheaper than the general kernel at any P, so the bound is the largest possible.
+#ifndef RMS_FAST_PERM_TCEIL
+#define RMS_FAST_PERM_TCEIL 512u
+#endif
+
 extern "C" int rms_volume_weighted_signal(int n_classes, int n_q, const double* class_volume, const double* sum_alpha,
                                           const double* sig_re, const double* sig_im, double* S_re, double* S_im)
 {
@@ -169,7 +176,7 @@ extern "C" int rms_run(const rms_substrate* s, rms_walkers* w, const rms_run_des
         for (int b = 0; b < nL; ++b)
             if (a != b) t_max = std::max(t_max, h_P512[(size_t)a * nL + b]);
     const uint32_t t_ceil = (uint32_t)ceilf(t_max);
-    const bool fast_permeable = permeable && !mt && !rs && s->d_nbr && !want_labels && t_ceil <= 64u;
+    const bool fast_permeable = permeable && !mt && !rs && s->d_nbr && !want_labels && t_ceil <= RMS_FAST_PERM_TCEIL;
 
     const int nWk = rms_kernel_waves(nW);        // waveforms the step kernel is compiled for; the extra ones carry zero weight
     rc = rms_walkers_reserve_waves(w, nWk, stream);

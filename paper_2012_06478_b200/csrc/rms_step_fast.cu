@@ -1,5 +1,5 @@
-// rms_step_fast.cu -- H2..H5 for the throughput-critical case: impermeable or weakly permeable membranes (512 P <= 64,
-// i.e. P <= 1/8: the paper's regime P << 1; see rms_permeable_step below) and piecewise-constant
+// rms_step_fast.cu -- H2..H5 for the throughput-critical case: impermeable or permeable membranes (built for the
+// paper's regime P << 1, and measured to stay ahead of the general kernel at any P; see rms_permeable_step below) and piecewise-constant
 // gradient waveforms (PGSE and every other rectangular-lobe sequence, any number of them).  Same method and
 // the same numbers as the general kernel of rms_step.cu (section 2.2 steps 2-4; corner
 // reflector of Fig.2; elastic collision P:90), organised for the B200 instruction pipes:
