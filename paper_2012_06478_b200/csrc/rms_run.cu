@@ -175,8 +175,10 @@ extern "C" int rms_run(const rms_substrate* s, rms_walkers* w, const rms_run_des
     for (int a = 0; a < nL; ++a)
         for (int b = 0; b < nL; ++b)
             if (a != b) t_max = std::max(t_max, h_P512[(size_t)a * nL + b]);
-    const uint32_t t_ceil = (uint32_t)ceilf(t_max);
-    const bool fast_permeable = permeable && !mt && !rs && s->d_nbr && !want_labels && t_ceil <= RMS_FAST_PERM_TCEIL;
+    const uint32_t t_ceil_P = (uint32_t)ceilf(t_max);
+    // absorbing membranes: the saturation draw belongs to every membrane met, so every such step is redone (t_ceil = 512)
+    const uint32_t t_ceil = mt ? 512u : t_ceil_P;
+    const bool fast_permeable = permeable && !rs && s->d_nbr && !want_labels && t_ceil <= RMS_FAST_PERM_TCEIL;
 
     const int nWk = rms_kernel_waves(nW);        // waveforms the step kernel is compiled for; the extra ones carry zero weight
     rc = rms_walkers_reserve_waves(w, nWk, stream);

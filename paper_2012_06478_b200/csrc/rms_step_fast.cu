@@ -78,7 +78,9 @@ __device__ __noinline__ uint2 rms_fold_ghost(int lin, uint32_t wraps, int nx, in
 // redone here by the interaction loop written out (the same arithmetic as rms_step.cu: labels gathered from the
 // uint16 lattice, hop rescaled on entering a compartment of different D, R7).  Rare, so out of line.
 //   st  = { fx, fy, fz, s }           in: offsets before the hop, hop length;  out: offsets after it, new hop length
-//   ist = { lin, wraps, L, dAx, dAy, dAz, n_enc, n_perm }   in: lin, wraps, L;  out: all (dA = net voxel move per axis)
+//   ist = { lin, wraps, L, dAx, dAy, dAz, n_enc, n_perm, saturated }   in: lin, wraps, L;  out: all (dA = net voxel move per axis)
+// Absorbing membranes (Eq.4; R20) ride on the same path: their saturation draw belongs to every membrane met, so a run with
+// a rho table sets ceil(512 P_max) to 512 and every step that meets a membrane comes here.
 // ------------------------------------------------------------------------------------------------------------------
 __device__ __noinline__ void rms_permeable_step(const rms_step_params* pp, uint32_t id_lo, uint32_t id_hi, uint32_t j,
                                                 uint32_t wa, uint32_t wb, float rx, float ry, float rz, float* st, int* ist)
@@ -103,6 +105,8 @@ __device__ __noinline__ void rms_permeable_step(const rms_step_params* pp, uint3
     int e = 0, n_enc = 0, n_perm = 0;
     uint32_t v0 = 0, v1 = 0, v2 = 0, v3 = 0;
     bool have_v = false;
+    uint32_t m0 = 0, m1 = 0, m2 = 0, m3 = 0;
+    bool have_m = false, saturated = false;
     for (int it = 0; it < 3; ++it) {
         float t3[3];
         bool any = false;
@@ -125,6 +129,13 @@ __device__ __noinline__ void rms_permeable_step(const rms_step_params* pp, uint3
         bool pass = true;
         if (Ln != L) {
             ++n_enc;
+            if (p.PMT) {                                                     // Eq.4: the encounter saturates the walker with P_MT
+                const float Q = __ldg(p.PMT + (size_t)L * p.n_labels + Ln);
+                if (Q > 0.f) {
+                    if (!have_m) { rms_philox(p.rk, id_lo, id_hi, j + 1u, RMS_STREAM_MT, m0, m1, m2, m3); have_m = true; }
+                    if (rms_uni(e == 0 ? m0 : (e == 1 ? m1 : m2)) < Q) saturated = true;
+                }
+            }
             const float T = __ldg(p.P512 + (size_t)L * p.n_labels + Ln);     // 512 P(L -> Ln), Eq.3
             if (T >= 512.f) pass = true;
             else if (T <= 0.f) pass = false;
@@ -166,7 +177,7 @@ __device__ __noinline__ void rms_permeable_step(const rms_step_params* pp, uint3
     ist[1] = (int)((uint32_t)ist[1] + (uint32_t)wr[0] + ((uint32_t)wr[1] << 10) + ((uint32_t)wr[2] << 20));
     ist[2] = (int)L;
     ist[3] = dA[0]; ist[4] = dA[1]; ist[5] = dA[2];
-    ist[6] = n_enc; ist[7] = n_perm;
+    ist[6] = n_enc; ist[7] = n_perm; ist[8] = saturated ? 1 : 0;
 }
 
 }  // namespace
@@ -207,7 +218,7 @@ __global__ void __launch_bounds__(RMS_FBLOCK, RMS_FMINB) rms_step_fast_kernel(co
     float s = p.s_tab[L];
     float rate = p.rate[L], relax = p.st.relax[i];
     uint32_t j_rate = p.step0;                  // steps up to here are already in `relax`
-    unsigned n_perm = 0;
+    unsigned n_perm = 0, n_sat = 0;
     const uint32_t t_ceil = PERM ? p.t_ceil : 0u;   // permeation needs coarse bits below ceil(512 P_max)
 
     const int SX = XFAST ? 1 : p.SX, SY = p.SY, SZ = p.SZ;      // x fastest (the default order): unit stride known at compile time
@@ -299,12 +310,16 @@ __global__ void __launch_bounds__(RMS_FBLOCK, RMS_FMINB) rms_step_fast_kernel(co
             if (PERM && (redo & 1u)) {
                 // a membrane of this step may be permeated: redo the step by the written-out interaction loop
                 float st[4] = {fx, fy, fz, s};
-                int ist[8] = {lin, (int)wraps, (int)L, 0, 0, 0, 0, 0};
+                int ist[9] = {lin, (int)wraps, (int)L, 0, 0, 0, 0, 0, 0};
                 rms_permeable_step(&p, id_lo, id_hi, jj, wa, wb, rx, ry, rz, st, ist);
                 gx = st[0]; gy = st[1]; gz = st[2];
                 lin = ist[0]; wraps = (uint32_t)ist[1];
                 Ax += ist[3] * remK; Ay += ist[4] * remK; Az += ist[5] * remK;
                 n_enc += (unsigned)ist[6]; n_perm += (unsigned)ist[7];
+                if (ist[8] && relax != __int_as_float(0x7f800000)) {   // alpha_rho = 0 from here on (Eq.4); the walk goes on
+                    relax = __int_as_float(0x7f800000);
+                    ++n_sat;
+                }
                 if ((uint32_t)ist[2] != L) {
                     // Eq.5: the whole dt of this step goes to the compartment at the end of the hop (R12)
                     relax = fmaf(rate, (float)(jj - j_rate), relax);
@@ -431,9 +446,11 @@ __global__ void __launch_bounds__(RMS_FBLOCK, RMS_FMINB) rms_step_fast_kernel(co
     const unsigned mask = __activemask();
     n_enc = __reduce_add_sync(mask, n_enc);
     if (PERM) n_perm = __reduce_add_sync(mask, n_perm);
+    if (PERM) n_sat = __reduce_add_sync(mask, n_sat);
     if ((threadIdx.x & 31) == (unsigned)(__ffs(mask) - 1)) {
         if (n_enc) atomicAdd(&p.counters[0], (unsigned long long)n_enc);
         if (PERM && n_perm) atomicAdd(&p.counters[1], (unsigned long long)n_perm);
+        if (PERM && n_sat) atomicAdd(&p.counters[4], (unsigned long long)n_sat);
     }
 }
 
