@@ -53,7 +53,17 @@ struct rms_substrate {
     // shell.  Bit (dx+1) + 3 (dy+1) + 9 (dz+1), d in {-1,0,1}^3, = the voxel at that offset carries the SAME
     // label as this voxel (bit 13 = the voxel itself = 1); a face towards +-k is a membrane iff the
     // bit of the face neighbour is 0.  Bit 27 (RMS_NBR_GHOST) = ghost voxel.
+    // Built on demand (rms_substrate_ensure_nbr): the fp64 specialised kernel and the general kernel's face-bit mode read it;
+    // the fp32 specialised kernel reads the octant lattice below.
     uint32_t* d_nbr = nullptr;
+    // octant lattice (rms_substrate_create, unless RMS_NO_BRICKS): one 64-bit word per padded voxel = 8 bytes, one per octant
+    // of hop directions.  Byte o, o = [hop_x < 0] 4 + [hop_y < 0] 2 + [hop_z < 0], holds the same-label bits of the 2x2x2
+    // block a hop of that octant can reach: bit c (c = 4 [moved in x] + 2 [moved in y] + [moved in z], 1..7) = the voxel at
+    // (sigma_x [c & 4], sigma_y [c & 2], sigma_z [c & 1]) carries the label of this voxel; bit 0 = ghost voxel.  The 26
+    // neighbours appear in 4 (faces), 2 (edges) and 1 (corners) of the bytes: the redundancy buys a one-instruction
+    // extraction (PRMT by the octant) of everything a hop can ask (at most three faces, all inside the block).
+    uint2* d_oct = nullptr;
+    bool want_bricks = false;            // RMS_NO_BRICKS not given: d_nbr may be built on demand
     // memory order of the neighbourhood lattice: index = X SX + Y SY + Z SZ over the padded coordinates.  The axis with
     // the fewest membrane faces normal to it (the direction the cells run along) is made the fastest one, so that
     // the 8 words of a 32-byte sector belong to one compartment; x fastest (1, NX, NX NY) or z fastest (NY NZ, NZ, 1).
@@ -174,6 +184,9 @@ struct rms_step_params {
     int nx, ny, nz;
     const uint16_t* labels;
     const uint32_t* nbr;
+    const uint2* oct;         // octant lattice (rms_substrate::d_oct), same padded geometry and strides as nbr
+    const uint32_t* lut1;     // device, [1024]: interaction outcome by (octant byte >> 1, faces reached); rms_step_fast.cu
+    const uint32_t* lut2;     // device, [8192]: the same with the hit order, for the entries lut1 marks order dependent
     int NX, NY;               // padded dims of the neighbourhood lattice
     int SX, SY, SZ;           // its strides: index = X SX + Y SY + Z SZ; SX == 1 (x fastest) or SZ == 1 (z fastest)
     rms_walker_arrays st;
@@ -204,6 +217,10 @@ struct rms_step_params {
 int rms_launch_step(const rms_step_params& p, int n_wave, int wmode, int lat, bool permeable, cudaStream_t stream);
 // RMS_LAT_FACES + RMS_WMODE_CONST only; permeable: P(a->b) << 1 expected (rms_step_fast.cu)
 int rms_launch_step_fast(const rms_step_params& p, int n_wave, bool permeable, cudaStream_t stream);
+// the two look-up tables of the specialised kernel (constants of the method, built once per device)
+int rms_fast_luts(const uint32_t** d_lut1, const uint32_t** d_lut2);
+// builds rms_substrate::d_nbr if it is not there yet (needs d_labels); rms_substrate.cu
+int rms_substrate_ensure_nbr(const rms_substrate* s, cudaStream_t stream);
 // the same in fp64 arithmetic (rms_step_precise.cu, RMS_RUN_FP64)
 int rms_launch_step_precise(const rms_step_params& p, int n_wave, cudaStream_t stream);
 // fp64, everything else: permeable / variable D / any waveform, RMS_WMODE_TABLE data, label gathers (rms_step_precise_general.cu)

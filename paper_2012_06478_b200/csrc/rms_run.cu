@@ -168,7 +168,7 @@ extern "C" int rms_run(const rms_substrate* s, rms_walkers* w, const rms_run_des
     }
     const bool want_labels = (d->flags & RMS_RUN_LABEL_GATHER) != 0;
     if (mt || rs) permeable = true;              // absorbing membranes and cancelled steps are handled where labels are read: the general kernels
-    const int lat = (!permeable && s->d_nbr && !want_labels) ? RMS_LAT_FACES : RMS_LAT_LABELS;
+    const int lat = (!permeable && s->want_bricks && !want_labels) ? RMS_LAT_FACES : RMS_LAT_LABELS;
     // permeable runs with P << 1 also take the specialised kernel: ceil(512 P_max) bounds the coarse random
     // bits that can permeate at all (rms_step_fast.cu)
     float t_max = 0.f;
@@ -178,7 +178,7 @@ extern "C" int rms_run(const rms_substrate* s, rms_walkers* w, const rms_run_des
     const uint32_t t_ceil_P = (uint32_t)ceilf(t_max);
     // absorbing membranes: the saturation draw belongs to every membrane met, so every such step is redone (t_ceil = 512)
     const uint32_t t_ceil = mt ? 512u : t_ceil_P;
-    const bool fast_permeable = permeable && !rs && s->d_nbr && !want_labels && t_ceil <= RMS_FAST_PERM_TCEIL;
+    const bool fast_permeable = permeable && !rs && s->d_oct && !want_labels && t_ceil <= RMS_FAST_PERM_TCEIL;
 
     const int nWk = rms_kernel_waves(nW);        // waveforms the step kernel is compiled for; the extra ones carry zero weight
     rc = rms_walkers_reserve_waves(w, nWk, stream);
@@ -259,6 +259,11 @@ extern "C" int rms_run(const rms_substrate* s, rms_walkers* w, const rms_run_des
     const int wmode = (use_general && !fp64 && const_mode && int_mode) ? RMS_WMODE_CONST : RMS_WMODE_TABLE;
     const bool need_segs = use_fast || use_precise || wmode == RMS_WMODE_CONST;
     const bool need_table = use_general && wmode == RMS_WMODE_TABLE;
+    // the 27-bit neighbourhood lattice serves the fp64 specialised kernel and the general kernel's face-bit mode: built on demand
+    if (use_precise || (use_general && lat == RMS_LAT_FACES)) {
+        rc = rms_substrate_ensure_nbr(s, stream);
+        if (rc != RMS_OK) return rc;
+    }
 
     // ---- device scratch: tables | segments or wave tables | q vectors | result sums -------------------
     const int nQs = nW * nG * nD;                                    // scalar waveforms x b x direction
@@ -344,7 +349,12 @@ extern "C" int rms_run(const rms_substrate* s, rms_walkers* w, const rms_run_des
     rms_step_params sp;
     memset(&sp, 0, sizeof sp);
     sp.nx = s->nx; sp.ny = s->ny; sp.nz = s->nz;
-    sp.labels = s->d_labels; sp.nbr = s->d_nbr; sp.NX = s->NX; sp.NY = s->NY; sp.SX = s->SX; sp.SY = s->SY; sp.SZ = s->SZ;
+    sp.labels = s->d_labels; sp.nbr = s->d_nbr; sp.oct = s->d_oct;
+    if (use_fast) {
+        rc = rms_fast_luts(&sp.lut1, &sp.lut2);
+        if (rc != RMS_OK) return rc;
+    }
+    sp.NX = s->NX; sp.NY = s->NY; sp.SX = s->SX; sp.SY = s->SY; sp.SZ = s->SZ;
     sp.st = w->a; sp.n = n; sp.first_id = w->first_id; sp.rk = rms_make_keys(w->seed);
     sp.s_tab = b_tabs.as<float>(); sp.rate = sp.s_tab + nL; sp.P512 = sp.rate + nL; sp.n_labels = nL;
     sp.PMT = mt ? sp.P512 + (size_t)nL * nL : nullptr;

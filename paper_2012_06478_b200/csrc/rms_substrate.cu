@@ -3,6 +3,8 @@
 #include <stdarg.h>
 #include <string.h>
 
+#include <mutex>
+
 #include "rms_internal.cuh"
 
 // ------------------------------------------------------------------------------------------------
@@ -69,12 +71,46 @@ __global__ void __launch_bounds__(256) rms_sample_faces_kernel(const uint16_t* _
 // 32 (x) x 32 (z) tile in shared memory and writes it transposed, 128 contiguous bytes per x.
 #define RMS_NBR_ZCHUNK 128
 
-template <bool ZFAST>
-__global__ void __launch_bounds__(128) rms_build_nbr_kernel(const uint16_t* __restrict__ labels, int nx, int ny, int nz,
-                                                             uint32_t* __restrict__ nbr, int SX, int SY, int SZ, int n_labels,
-                                                             unsigned long long* __restrict__ stats)
+__device__ __forceinline__ void rms_nbr_make_word(uint32_t m, bool, const uint32_t*, uint32_t& w) { w = m; }
+__device__ __forceinline__ void rms_nbr_make_word(uint32_t m, bool ghost, const uint32_t* quad, uint2& w)
 {
-    __shared__ uint32_t tile[ZFAST ? 4 : 1][ZFAST ? 32 : 1][ZFAST ? 33 : 1];
+    const uint32_t t0 = (quad[(m >> 9) & 511u] & 0xFEFEFEFEu) | (ghost ? 0x01010101u : 0u);   // bit 0: itself -> ghost flag
+    const uint32_t e = t0 | (quad[(m >> 18) & 511u] << 1);      // hop_z > 0: the plane above
+    const uint32_t f = t0 | (quad[m & 511u] << 1);              // hop_z < 0: the plane below
+    w.x = __byte_perm(e, f, 0x5140);                            // bytes o = 2 q + [hop_z < 0]
+    w.y = __byte_perm(e, f, 0x7362);
+}
+
+//
+// OCT: the word written is the 64-bit octant word of rms_substrate::d_oct instead (WORD = uint2), expanded from the 27 bits
+// through a 512-entry table in shared memory: entry [9-bit z-plane], byte q = 2 [hop_x < 0] + [hop_y < 0], even bits
+// 0, 2, 4, 6 = the plane's same-label bits at (0, 0), (0, sy), (sx, 0), (sx, sy).  The plane of the voxel gives the even
+// bits of an octant byte (not moved in z), the plane above or below, shifted by one, the odd ones.
+template <bool OCT> struct rms_nbr_word { typedef uint32_t type; };
+template <> struct rms_nbr_word<true> { typedef uint2 type; };
+
+template <bool ZFAST, bool OCT>
+__global__ void __launch_bounds__(128) rms_build_nbr_kernel(const uint16_t* __restrict__ labels, int nx, int ny, int nz,
+                                                             typename rms_nbr_word<OCT>::type* __restrict__ nbr, int SX, int SY, int SZ,
+                                                             int n_labels, unsigned long long* __restrict__ stats)
+{
+    typedef typename rms_nbr_word<OCT>::type WORD;
+    __shared__ WORD tile[ZFAST ? 4 : 1][ZFAST ? 32 : 1][ZFAST ? 33 : 1];
+    __shared__ uint32_t quad[OCT ? 512 : 1];
+    if (OCT) {
+        for (int t = threadIdx.x; t < 512; t += blockDim.x) {
+            uint32_t v = 0;
+            for (int q = 0; q < 4; ++q) {
+                const int sx = (q & 2) ? -1 : 1, sy = (q & 1) ? -1 : 1;
+                for (int xy = 0; xy < 4; ++xy) {
+                    const int dx = (xy >> 1) * sx, dy = (xy & 1) * sy;
+                    v |= ((t >> ((dx + 1) + 3 * (dy + 1))) & 1u) << (8 * q + 2 * xy);
+                }
+            }
+            quad[t] = v;
+        }
+        __syncthreads();
+    }
     const int NX = nx + 2, NY = ny + 2, NZ = nz + 2;
     const int Xt = blockIdx.x * blockDim.x + threadIdx.x;
     const bool active = Xt < NX;
@@ -100,7 +136,7 @@ __global__ void __launch_bounds__(128) rms_build_nbr_kernel(const uint16_t* __re
 #pragma unroll
             for (int k = 0; k < 9; ++k) { pa[k] = __ldg(labels + (bl + off[k])); pb[k] = __ldg(labels + (bm + off[k])); }
         }
-        uint32_t* out = nbr + ((size_t)X * SX + (size_t)Y * SY + (size_t)Z0 * SZ);
+        WORD* out = nbr + ((size_t)X * SX + (size_t)Y * SY + (size_t)Z0 * SZ);
         int Z = Z0, zi = 0, zbase = Z0;
         // one voxel: read plane z+1 into HI, compare the 27 labels with the centre of MID, write the word
 #define RMS_NBR_ONE(LO, MID, HI)                                                                              \
@@ -115,8 +151,10 @@ __global__ void __launch_bounds__(128) rms_build_nbr_kernel(const uint16_t* __re
                      ((HI[k] == L) ? (1u << (k + 18)) : 0u);                                                  \
             const bool ghost = ghost_xy | (Z == 0) | (Z == NZ - 1);                                           \
             if (ghost) m |= RMS_NBR_GHOST;                                                                    \
+            WORD word;                                                                                        \
+            rms_nbr_make_word(m, ghost, quad, word);                                                          \
             if (ZFAST) {                                                                                      \
-                tile[warp][zi][lane] = m;                                                                     \
+                tile[warp][zi][lane] = word;                                                                  \
                 if (++zi == 32 || Z == Z1 - 1) {       /* warp-uniform: flush the staged tile, transposed */  \
                     __syncwarp();                                                                             \
                     const int Xw = Xt - lane;                                                                 \
@@ -126,7 +164,7 @@ __global__ void __launch_bounds__(128) rms_build_nbr_kernel(const uint16_t* __re
                     zbase += zi; zi = 0;                                                                      \
                 }                                                                                             \
             } else {                                                                                          \
-                *out = m;                                                                                     \
+                *out = word;                                                                                  \
                 out += SZ;                                                                                    \
             }                                                                                                 \
             if (!ghost && active) {                                                                           \
@@ -258,8 +296,9 @@ extern "C" int rms_substrate_create(const rms_substrate_desc* d, void* cuda_stre
     SUB_TRY(rms_malloc((void**)&d_stats, 5 * sizeof(unsigned long long)));
     SUB_TRY(cudaMemsetAsync(d_stats, 0, 5 * sizeof(unsigned long long), stream));
     if (!(d->flags & RMS_NO_BRICKS)) {
+        s->want_bricks = true;
         s->NX = s->nx + 2; s->NY = s->ny + 2; s->NZ = s->nz + 2;
-        SUB_TRY(rms_malloc((void**)&s->d_nbr, (size_t)s->NX * s->NY * s->NZ * sizeof(uint32_t)));
+        SUB_TRY(rms_malloc((void**)&s->d_oct, (size_t)s->NX * s->NY * s->NZ * sizeof(uint2)));
         dim3 grid((s->NX + 127) / 128, s->NY, (s->NZ + RMS_NBR_ZCHUNK - 1) / RMS_NBR_ZCHUNK);
         if (grid.y > 65535u || grid.z > 65535u) {
             rms_set_error("lattice too large for the neighbourhood-lattice build (ny+2, nz+2 must be <= 65535)");
@@ -281,9 +320,9 @@ extern "C" int rms_substrate_create(const rms_substrate_desc* d, void* cuda_stre
         if (zfast) { s->SZ = 1; s->SY = s->NZ; s->SX = s->NY * s->NZ; }
         else       { s->SX = 1; s->SY = s->NX; s->SZ = s->NX * s->NY; }
         if (zfast)
-            rms_build_nbr_kernel<true><<<grid, 128, 0, stream>>>(s->d_labels, s->nx, s->ny, s->nz, s->d_nbr, s->SX, s->SY, s->SZ, nL, d_stats);
+            rms_build_nbr_kernel<true, true><<<grid, 128, 0, stream>>>(s->d_labels, s->nx, s->ny, s->nz, s->d_oct, s->SX, s->SY, s->SZ, nL, d_stats);
         else
-            rms_build_nbr_kernel<false><<<grid, 128, 0, stream>>>(s->d_labels, s->nx, s->ny, s->nz, s->d_nbr, s->SX, s->SY, s->SZ, nL, d_stats);
+            rms_build_nbr_kernel<false, true><<<grid, 128, 0, stream>>>(s->d_labels, s->nx, s->ny, s->nz, s->d_oct, s->SX, s->SY, s->SZ, nL, d_stats);
         SUB_TRY(cudaGetLastError());
     } else {
         rms_check_labels_kernel<<<148 * 8, 256, 0, stream>>>(s->d_labels, (size_t)n_vox, nL, d_stats);
@@ -313,8 +352,42 @@ extern "C" int rms_substrate_destroy(rms_substrate* s)
     if (!s) return RMS_OK;
     if (s->owns_labels && s->d_labels) rms_free((void*)s->d_labels);
     if (s->d_nbr) rms_free(s->d_nbr);
+    if (s->d_oct) rms_free(s->d_oct);
     if (s->d_label_class) rms_free(s->d_label_class);
     delete s;
+    return RMS_OK;
+}
+
+// The 27-bit neighbourhood lattice is read by the fp64 specialised kernel and by the general kernel's face-bit mode only,
+// so it is built at the first run that wants it (same padded geometry and memory order as the octant lattice).
+int rms_substrate_ensure_nbr(const rms_substrate* cs, cudaStream_t stream)
+{
+    static std::mutex mu;
+    std::lock_guard<std::mutex> lock(mu);
+    rms_substrate* s = const_cast<rms_substrate*>(cs);
+    if (s->d_nbr) return RMS_OK;
+    RMS_REQUIRE(s->want_bricks, RMS_ERR_UNSUPPORTED, "substrate was created with RMS_NO_BRICKS");
+    unsigned long long* d_stats = nullptr;
+    uint32_t* nbr = nullptr;
+    RMS_CUDA_TRY(rms_malloc((void**)&d_stats, 2 * sizeof(unsigned long long)));
+    cudaError_t e = rms_malloc((void**)&nbr, (size_t)s->NX * s->NY * s->NZ * sizeof(uint32_t));
+    if (e == cudaSuccess) e = cudaMemsetAsync(d_stats, 0, 2 * sizeof(unsigned long long), stream);
+    if (e == cudaSuccess) {
+        dim3 grid((s->NX + 127) / 128, s->NY, (s->NZ + RMS_NBR_ZCHUNK - 1) / RMS_NBR_ZCHUNK);
+        if (s->SZ == 1)
+            rms_build_nbr_kernel<true, false><<<grid, 128, 0, stream>>>(s->d_labels, s->nx, s->ny, s->nz, nbr, s->SX, s->SY, s->SZ, s->n_labels, d_stats);
+        else
+            rms_build_nbr_kernel<false, false><<<grid, 128, 0, stream>>>(s->d_labels, s->nx, s->ny, s->nz, nbr, s->SX, s->SY, s->SZ, s->n_labels, d_stats);
+        e = cudaGetLastError();
+    }
+    if (e == cudaSuccess) e = cudaStreamSynchronize(stream);   // d_stats goes back to the cache below
+    rms_free(d_stats);
+    if (e != cudaSuccess) {
+        if (nbr) rms_free(nbr);
+        rms_set_error("building the neighbourhood lattice failed: %s", cudaGetErrorString(e));
+        return e == cudaErrorMemoryAllocation ? RMS_ERR_OOM : RMS_ERR_CUDA;
+    }
+    s->d_nbr = nbr;
     return RMS_OK;
 }
 
@@ -379,8 +452,9 @@ extern "C" int rms_substrate_get_info(const rms_substrate* s, rms_substrate_info
     out->n_voxels = s->n_vox;
     out->n_membrane_faces = s->n_membrane_faces;
     out->lattice_bytes = s->n_vox * sizeof(uint16_t);
-    out->brick_bytes = s->d_nbr ? (uint64_t)s->NX * s->NY * s->NZ * sizeof(uint32_t) : 0;
-    out->has_bricks = s->d_nbr != nullptr;
+    const uint64_t n_pad = (uint64_t)s->NX * s->NY * s->NZ;
+    out->brick_bytes = (s->d_oct ? n_pad * sizeof(uint2) : 0) + (s->d_nbr ? n_pad * sizeof(uint32_t) : 0);
+    out->has_bricks = s->d_oct != nullptr;
     return RMS_OK;
 }
 
