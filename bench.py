@@ -53,6 +53,8 @@ def parse_args():
     ap.add_argument("--layout", default="x", choices=["auto", "x", "z"], help="memory order of the neighbourhood lattice")
     ap.add_argument("--waves", type=int, default=1,
                     help="number of PGSE waveforms evaluated on the same trajectories (sequence sweep, not the headline)")
+    ap.add_argument("--substrate", default="cfg4", choices=["cfg4", "cfg3"],
+                    help="cfg3: the permeable, D- and T2-contrast variant of the lattice with walkers in every label (not the headline)")
     ap.add_argument("--fp64", action="store_true", help="RMS_RUN_FP64: the step kernel in fp64 arithmetic (not the headline)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -163,6 +165,8 @@ class ClockSampler:
 def make_workload(args):
     import rms_inputs as ri
     cfg = ri.make_config("cfg4", args.scale, n_walkers=args.walkers, n_steps=args.mc_steps, n_dir=args.dirs)
+    if args.substrate == "cfg3":
+        cfg.substrate = ri.make_config("cfg3", args.scale).substrate
     if args.waves > 1:      # sequence sweep: waveform m has delta = Delta / (m + 1) ... all on one set of trajectories
         seq = cfg.sequence
         n = seq.n_steps

@@ -8,8 +8,12 @@
 // of it (L2 reuse).  Walkers drift apart by sqrt(6 D t); rms_run re-sorts at every launch boundary.
 #include "rms_internal.cuh"
 
+#ifndef RMS_CELL_XY
 #define RMS_CELL_XY 8
+#endif
+#ifndef RMS_CELL_Z
 #define RMS_CELL_Z 16
+#endif
 
 namespace {
 
@@ -121,7 +125,11 @@ int rms_order_walkers(const rms_substrate* s, const rms_walkers* w, uint32_t* d_
     cudaError_t e = cudaMemsetAsync(d_count, 0, n_tiles * 4096 * sizeof(uint32_t), stream);
     if (e == cudaSuccess) {
         const unsigned grid = (unsigned)((w->n + 255) / 256);
+#ifdef RMS_CELL_ORDER_Z
+        const bool zfast = RMS_CELL_ORDER_Z != 0;
+#else
         const bool zfast = s->SZ == 1 && s->SX != 1;
+#endif
         rms_cell_hist_kernel<<<grid, 256, 0, stream>>>(w->a, w->n, cx, cy, cz, zfast, d_count);
         rms_cell_scan_kernel<<<1, 1024, 0, stream>>>((uint4*)d_count, (uint32_t)n_tiles);
         rms_cell_scatter_kernel<<<grid, 256, 0, stream>>>(w->a, w->n, cx, cy, cz, zfast, d_count, d_order);
