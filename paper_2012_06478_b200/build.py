@@ -14,7 +14,7 @@ from pathlib import Path
 PKG = Path(__file__).resolve().parent
 CSRC = PKG / "csrc"
 LIB = PKG / "librms_b200.so"
-SOURCES = ["rms_memory.cu", "rms_probe.cu", "rms_sched.cu", "rms_substrate.cu", "rms_walkers.cu", "rms_step.cu", "rms_step_fast.cu", "rms_step_precise.cu", "rms_step_precise_general.cu", "rms_reduce.cu", "rms_run.cu"]
+SOURCES = ["rms_memory.cu", "rms_probe.cu", "rms_sched.cu", "rms_substrate.cu", "rms_walkers.cu", "rms_step.cu", "rms_step_fast.cu", "rms_step_precise_general.cu", "rms_reduce.cu", "rms_run.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC", "--threads", "0"]
 

@@ -53,8 +53,8 @@ struct rms_substrate {
     // shell.  Bit (dx+1) + 3 (dy+1) + 9 (dz+1), d in {-1,0,1}^3, = the voxel at that offset carries the SAME
     // label as this voxel (bit 13 = the voxel itself = 1); a face towards +-k is a membrane iff the
     // bit of the face neighbour is 0.  Bit 27 (RMS_NBR_GHOST) = ghost voxel.
-    // Built on demand (rms_substrate_ensure_nbr): the fp64 specialised kernel and the general kernel's face-bit mode read it;
-    // the fp32 specialised kernel reads the octant lattice below.
+    // Built on demand (rms_substrate_ensure_nbr): only the general fp32 kernel's face-bit mode reads it; the specialised
+    // kernel (fp32 and fp64 directions) reads the octant lattice below.
     uint32_t* d_nbr = nullptr;
     // octant lattice (rms_substrate_create, unless RMS_NO_BRICKS): one 64-bit word per padded voxel = 8 bytes, one per octant
     // of hop directions.  Byte o, o = [hop_x < 0] 4 + [hop_y < 0] 2 + [hop_z < 0], holds the same-label bits of the 2x2x2
@@ -216,13 +216,11 @@ struct rms_step_params {
 
 int rms_launch_step(const rms_step_params& p, int n_wave, int wmode, int lat, bool permeable, cudaStream_t stream);
 // RMS_LAT_FACES + RMS_WMODE_CONST only; permeable: P(a->b) << 1 expected (rms_step_fast.cu)
-int rms_launch_step_fast(const rms_step_params& p, int n_wave, bool permeable, cudaStream_t stream);
+int rms_launch_step_fast(const rms_step_params& p, int n_wave, bool permeable, bool fp64, cudaStream_t stream);
 // the two look-up tables of the specialised kernel (constants of the method, built once per device)
 int rms_fast_luts(const uint32_t** d_lut1, const uint32_t** d_lut2);
 // builds rms_substrate::d_nbr if it is not there yet (needs d_labels); rms_substrate.cu
 int rms_substrate_ensure_nbr(const rms_substrate* s, cudaStream_t stream);
-// the same in fp64 arithmetic (rms_step_precise.cu, RMS_RUN_FP64)
-int rms_launch_step_precise(const rms_step_params& p, int n_wave, cudaStream_t stream);
 // fp64, everything else: permeable / variable D / any waveform, RMS_WMODE_TABLE data, label gathers (rms_step_precise_general.cu)
 int rms_launch_step_precise_general(const rms_step_params& p, int n_wave, cudaStream_t stream);
 

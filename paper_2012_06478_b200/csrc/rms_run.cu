@@ -192,8 +192,9 @@ extern "C" int rms_run(const rms_substrate* s, rms_walkers* w, const rms_run_des
         double* S = &suf[(size_t)m * (nT + 1)];
         for (int64_t j = nT; j >= 1; --j) { acc += (double)d->wave[(size_t)m * nT + (j - 1)]; S[j - 1] = acc; }
     }
-    // RMS_RUN_FP64: the specialised fp64 kernel serves the impermeable / neighbourhood-lattice / integer-waveform case,
-    // the general fp64 kernel (table-driven waveforms, label gathers) everything else
+    // RMS_RUN_FP64: the specialised kernel with fp64 directions and 2^-63 fixed-point offsets serves every run it serves in fp32
+    // (piecewise-constant waveforms; impermeable, permeable, absorbing), the general fp64 kernel (table-driven waveforms,
+    // label gathers, rejection sampling, ERL) everything else
     const bool fp64 = (d->flags & RMS_RUN_FP64) != 0;
     // integer-valued waveforms: the general kernel's exact int32 path (CONST mode)
     bool int_mode = wave_is_integer(d->wave, (size_t)nW * nT);
@@ -253,14 +254,14 @@ extern "C" int rms_run(const rms_substrate* s, rms_walkers* w, const rms_run_des
     // fp32 kernel runs its CONST mode on integer-valued piecewise-constant waveforms, its TABLE mode otherwise; the general
     // fp64 kernel is table driven
     const bool nbr_fp32 = (!permeable && lat == RMS_LAT_FACES) || fast_permeable;
-    const bool use_fast = !fp64 && const_mode && nbr_fp32 && !(d->flags & RMS_RUN_GENERAL_KERNEL);
-    const bool use_precise = fp64 && const_mode && !permeable && lat == RMS_LAT_FACES;
-    const bool use_general = !use_fast && !use_precise;
+    // (RMS_RUN_FP64 on the specialised kernel: its direction arithmetic in fp64, rms_step_fast.cu)
+    const bool use_fast = const_mode && nbr_fp32 && !(d->flags & RMS_RUN_GENERAL_KERNEL);
+    const bool use_general = !use_fast;
     const int wmode = (use_general && !fp64 && const_mode && int_mode) ? RMS_WMODE_CONST : RMS_WMODE_TABLE;
-    const bool need_segs = use_fast || use_precise || wmode == RMS_WMODE_CONST;
+    const bool need_segs = use_fast || wmode == RMS_WMODE_CONST;
     const bool need_table = use_general && wmode == RMS_WMODE_TABLE;
-    // the 27-bit neighbourhood lattice serves the fp64 specialised kernel and the general kernel's face-bit mode: built on demand
-    if (use_precise || (use_general && lat == RMS_LAT_FACES)) {
+    // the 27-bit neighbourhood lattice serves the general fp32 kernel's face-bit mode only: built on demand
+    if (use_general && !fp64 && lat == RMS_LAT_FACES) {
         rc = rms_substrate_ensure_nbr(s, stream);
         if (rc != RMS_OK) return rc;
     }
@@ -404,9 +405,8 @@ extern "C" int rms_run(const rms_substrate* s, rms_walkers* w, const rms_run_des
             }
             cudaEvent_t e0 = evs.make(), e1 = evs.make();
             RMS_CUDA_TRY(cudaEventRecord(e0, stream));
-            if (use_precise) rc = rms_launch_step_precise(sp, nW, stream);
+            if (use_fast) rc = rms_launch_step_fast(sp, nW, permeable, fp64, stream);
             else if (fp64) rc = rms_launch_step_precise_general(sp, nWk, stream);
-            else if (use_fast) rc = rms_launch_step_fast(sp, nW, permeable, stream);
             else rc = rms_launch_step(sp, nWk, wmode, lat, permeable, stream);
             if (rc != RMS_OK) return rc;
             RMS_CUDA_TRY(cudaEventRecord(e1, stream));

@@ -352,28 +352,47 @@ def test_fp64_mode_stays_on_the_oracle_trajectories_over_a_long_run(rms):
     ~1e-6 voxel of and fall below 99.9 % same-voxel long before this; fp64 positions differ
     from the oracle's by ~1e-13 and must hold the plain tolerances."""
     cfg = ri.make_config("cfg2", "test")
-    n, n_steps = 2000, 200_000
+    n, n_steps = 20_000, 200_000
     seq = ri.pgse_sequence(cfg.sequence.dt_ms, n_steps, 10.0, 25.0, np.linspace(0.0, 10.0, 5), ri.fibonacci_dirs(12),
                            snap_steps=[50_001, 100_000, n_steps])
     o = oracle_run(cfg.substrate, seq, n, cfg.seed)
     g64 = gpu_run(cfg.substrate, seq, n, cfg.seed, flags=8)
     rep = compare(g64, o, n)
     print("fp64 200k steps", rep)
-    assert rep["n_diff"] <= 1 and rep["max_offset_diff"] < 1e-6          # offsets are read back as fp32
+    assert rep["n_diff"] <= 2 and rep["max_offset_diff"] < 1e-6          # offsets are read back as fp32
     g32 = gpu_run(cfg.substrate, seq, n, cfg.seed)
     same32 = float(np.all(g32["walkers"]["vox"] == o["final_vox"], axis=1).mean())
     print("fp32 same-voxel fraction at 200k steps:", same32)
     assert rep["same_voxel"] >= same32
 
 
+def test_fp32_accuracy_envelope_on_the_axon_substrate(rms):
+    """The fp32 path (fp32 direction arithmetic, exact fixed-point positions) parts company with the oracle only where a hop
+    passes a convex membrane corner within its position error; the share of walkers that have done
+    so grows like steps^1.5.  The measured curve on the reduced axon substrate, less a margin, so that a change that
+    costs accuracy (a cheaper square root, sine or conversion) is caught even where it still passes 99.9 % on one case."""
+    cfg = ri.make_config("cfg2", "test")
+    n = 50_000
+    for n_steps, floor in ((10_000, 0.9997), (40_000, 0.997)):
+        seq = ri.pgse_sequence(cfg.sequence.dt_ms, n_steps, 0.2 * n_steps * cfg.sequence.dt_ms, 0.5 * n_steps * cfg.sequence.dt_ms,
+                               [0.0, 4.0], np.eye(3), snap_steps=[n_steps])
+        o = oracle_run(cfg.substrate, seq, n, cfg.seed)
+        g = gpu_run(cfg.substrate, seq, n, cfg.seed)
+        same = float(np.all(g["walkers"]["vox"] == o["final_vox"], axis=1).mean())
+        print("fp32 same-voxel fraction at", n_steps, "steps:", same)
+        assert same >= floor, (n_steps, same)
+
+
 def test_fp64_mode_general_kernel_permeable_and_table_waveforms(rms):
     # RMS_RUN_FP64 outside the specialised case: permeable + D contrast + T2 (cfg3 reduced), and a non-integer waveform
     c3 = ri.make_config("cfg3", "test")
-    g = gpu_run(c3.substrate, c3.sequence, c3.n_walkers, c3.seed, flags=8)
-    o = oracle_run(c3.substrate, c3.sequence, c3.n_walkers, c3.seed)
-    rep = compare(g, o, c3.n_walkers)
-    print("fp64 cfg3 reduced", rep)
-    assert rep["n_diff"] == 0 and rep["perm_diff"] == 0 and g["n_permeations"] > 0
+    n3 = 100_000
+    o = oracle_run(c3.substrate, c3.sequence, n3, c3.seed)
+    for flags in (8, 8 | 2):       # the specialised kernel with fp64 directions (redo path for permeations); the general fp64 kernel
+        g = gpu_run(c3.substrate, c3.sequence, n3, c3.seed, flags=flags)
+        rep = compare(g, o, n3)
+        print("fp64 cfg3 reduced, flags", flags, rep)
+        assert rep["n_diff"] <= 2 and rep["perm_diff"] <= 2 and g["n_permeations"] > 0
     sub = ri.single_cylinder(24, 7.5, 0.1)
     n_steps = 801
     t = (np.arange(n_steps) + 1.0) / n_steps
@@ -387,15 +406,17 @@ def test_fp64_mode_general_kernel_permeable_and_table_waveforms(rms):
     assert rep["n_diff"] == 0
 
 
-@pytest.mark.parametrize("name,n_ids", [("cfg1", 20_000), ("cfg2", 2_000), ("cfg3", 4_000)])
+@pytest.mark.parametrize("name,n_ids", [("cfg1", 100_000), ("cfg2", 10_000), ("cfg3", 100_000)])
 def test_full_length_configs_in_fp64_on_a_sample_of_walker_ids(rms, name, n_ids):
     """BASELINE.json configs 1-3 at their full lattice size and full number of steps (85,000 / 500,000 / 50,000), on
-    the first n_ids walker ids (what the oracle finishes in seconds; trajectories depend on (seed, id) only, so
-    the sample is exactly the corresponding slice of the full job), in RMS_RUN_FP64: plain tolerances."""
+    the first n_ids walker ids -- cfg1 whole (all of its 1e5 walkers), cfg3 and cfg2 on 10 % and 1 % of theirs (what the
+    oracle finishes in under a minute; trajectories depend on (seed, id) only, so the sample is exactly the corresponding
+    slice of the full job) -- in RMS_RUN_FP64: plain tolerances."""
     import torch
     cfg = ri.make_config(name, "full")
     labels_dev = torch.from_numpy(cfg.substrate.labels.view(np.int16)).cuda()
     g = rms.simulate(cfg.substrate, cfg.sequence, n_ids, cfg.seed, flags=8, device_labels=labels_dev, read_walkers=True)
+    g["_sub"], g["_seq"] = cfg.substrate, cfg.sequence
     o = oracle_run(cfg.substrate, cfg.sequence, n_ids, cfg.seed)
     rep = compare(g, o, n_ids)
     print("full length", name, cfg.sequence.n_steps, "steps", rep, "kernel_ms", g["kernel_ms"])
