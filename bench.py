@@ -35,8 +35,13 @@ sys.path.insert(0, str(ROOT))
 # Algorithmic thread-instructions per walker-step, frozen in DESIGN.md ("Roofline") before tuning.
 ALGORITHMIC_INSTR_PER_STEP = 80.0
 N_SM, LANES_PER_SM = 148, 128          # B200: 4 schedulers x 32 lanes per SM, one warp instruction per clock each
-# DRAM traffic of the step kernel per launch from the committed ncu capture (profiles/), or None.
-NCU_TRAFFIC_BYTES_PER_LAUNCH = 62.27e9   # profiles/r1d_step_fast_ncu.md: 60.41 GB read + 1.86 GB written
+# DRAM traffic of the step kernel per launch (dram__bytes_read.sum + dram__bytes_write.sum of one `ncu --set full` capture),
+# by the configuration that was captured; a run of any other configuration reports traffic = null.
+# key: (substrate, lattice, layout, walkers, mc_steps, fp64)
+NCU_CAPTURES = {
+    ("cfg4", "facemask", "x", 1_000_000, 10_000, False): {"bytes": 78.50e9, "source": "profiles/r2a_step_fast_ncu.md (commit 8a3974e)"},
+    ("cfg4", "facemask", "z", 1_000_000, 10_000, False): {"bytes": 39.28e9, "source": "profiles/r2a_step_fast_ncu.md (commit 8a3974e)"},
+}
 
 
 def parse_args():
@@ -184,7 +189,7 @@ def workload_config(args, cfg, extra=None):
          "walkers_per_gpu": args.walkers, "mc_steps": args.mc_steps, "dt_ms": cfg.sequence.dt_ms,
          "directions": int(cfg.sequence.dirs.shape[0]), "b_values": int(cfg.sequence.gamp.shape[1]),
          "lattice_path": args.lattice, "layout": args.layout, "pass": "rms_substrate_create + rms_walkers_init + rms_run",
-         "l2": "inputs larger than L2 (label lattice 1.0 GB + neighbourhood lattice 2.0 GB vs 126 MB L2)" if args.scale == "full"
+         "l2": "inputs larger than L2 (label lattice 1.0 GB + octant lattice 4.0 GB vs 126 MB L2)" if args.scale == "full"
          else "reduced test lattice (fits L2) -- not a valid bench configuration"}
     if extra:
         c.update(extra)
@@ -213,7 +218,7 @@ def run_reference(args):
     line = {"impl": "reference", "metric": "walker_steps_per_s", "value": value, "unit": "walker-steps/s", "n_gpus": args.gpus,
             "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * total / len(times), "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": workload_config(args, cfg, {"sample": f"first {sample} walker ids x {args.mc_steps} steps per step"}),
+            "config": workload_config(args, cfg),
             "cpu_baseline": {"value": value, "unit": "walker-steps/s", "cores": threads, "kind": "oracle",
                              "sample": f"first {sample} walker ids x {args.mc_steps} steps"},
             "e2e": {"value": value, "unit": "walker-steps/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
@@ -366,21 +371,24 @@ def main():
     peak_ginstr = N_SM * LANES_PER_SM * sm_mhz * 1e6 / 1e9
     k_ms_per_launch = kernel_ms / args.steps
     achieved_ginstr = ALGORITHMIC_INSTR_PER_STEP * n_walkers * mc_steps / (k_ms_per_launch * 1e-3) / 1e9
-    roofline = {"bound": "alu", "kernel": ("rms_step_precise_kernel" if args.fp64 else "rms_step_fast_kernel") if args.lattice == "facemask" else "rms_step_kernel", "achieved": achieved_ginstr, "peak": peak_ginstr,
+    cap = NCU_CAPTURES.get((args.substrate, args.lattice, args.layout, n_walkers, mc_steps, bool(args.fp64))) if args.waves == 1 else None
+    traffic = cap["bytes"] if cap else None
+    roofline = {"bound": "alu", "kernel": "rms_step_fast_kernel" if args.lattice == "facemask" else "rms_step_kernel",
+                "achieved": achieved_ginstr, "peak": peak_ginstr,
                 "unit": "Ginstr/s (thread-instructions)", "frac": achieved_ginstr / peak_ginstr,
-                "traffic": NCU_TRAFFIC_BYTES_PER_LAUNCH,
+                "traffic": traffic, "traffic_source": cap["source"] if cap else None,
                 "algorithmic_instr_per_walker_step": ALGORITHMIC_INSTR_PER_STEP, "kernel_ms_per_launch": k_ms_per_launch,
                 "kernel_share_of_step": kernel_ms / dev_ms,
                 "peak_source": f"148 SM x 128 lanes x SM clock measured during the run ({sm_mhz:.0f} MHz; "
                                f"MEASURED_PEAKS.json present: {peaks_file.exists()})"}
 
     # second roofline candidate: random-gather ceilings measured on this GPU, against the gather rate of the
-    # step kernel (0.68 voxel changes per walker-step, one 4-byte word each)
+    # step kernel (0.68 voxel changes per walker-step, one 8-byte octant word each)
     try:
         g_l2 = rms.binding.rms_gather_probe(48 << 20, 4, 2048)
         g_hbm = rms.binding.rms_gather_probe(2 << 30, 4, 512)
         k_rate = 0.68 * n_walkers * mc_steps / (k_ms_per_launch * 1e-3)
-        k_dram = (NCU_TRAFFIC_BYTES_PER_LAUNCH / 32.0) / (k_ms_per_launch * 1e-3) if NCU_TRAFFIC_BYTES_PER_LAUNCH else None
+        k_dram = (traffic / 32.0) / (k_ms_per_launch * 1e-3) if traffic else None
         roofline["gather"] = {"kernel_gathers_per_s": k_rate, "kernel_dram_sectors_per_s": k_dram,
                               "ceiling_l2_resident_48MB": g_l2, "ceiling_hbm_2GB": g_hbm,
                               "dram_sectors_frac_of_hbm_ceiling": (k_dram / g_hbm) if k_dram else None,

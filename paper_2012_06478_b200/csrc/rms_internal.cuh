@@ -37,7 +37,8 @@ void rms_set_error(const char* fmt, ...);
 // device memory (rms_memory.cu): caching allocator behind every handle
 // ------------------------------------------------------------------------------------------------
 cudaError_t rms_malloc(void** p, size_t bytes);
-void rms_free(void* p);
+void rms_free(void* p);                                  // the work on the block has completed
+void rms_free_async(void* p, cudaStream_t stream);       // the work on the block is queued on `stream`
 
 // ------------------------------------------------------------------------------------------------
 // handles
@@ -98,6 +99,7 @@ struct rms_walkers {
     const rms_substrate* sub = nullptr;
     uint64_t n = 0, first_id = 0, seed = 0;
     uint64_t steps_done = 0;
+    bool poisoned = false;     // a run failed after its first launch: the walkers are part-way through it (rms_run refuses them)
     int n_wave_alloc = 0;
     rms_walker_arrays a{};
     void* d_block = nullptr;   // one allocation behind all arrays but phi

@@ -8,16 +8,26 @@
 
 namespace {
 
-struct DeviceBuf {   // frees on scope exit
+struct DeviceBuf {   // frees on scope exit; work on the block may still be queued on the stream (error returns)
     void* p = nullptr;
-    ~DeviceBuf() { if (p) rms_free(p); }
+    cudaStream_t stream = nullptr;
+    ~DeviceBuf() { if (p) rms_free_async(p, stream); }
     template <class T> T* as() { return (T*)p; }
+};
+
+// A failure after the first launch leaves the walkers advanced by part of the run while steps_done is not: a later run would
+// reuse Philox step indices on moved walkers.  The guard waits for the queued work and marks the handle unusable.
+struct RunGuard {
+    rms_walkers* w;
+    cudaStream_t stream;
+    bool armed = false;
+    ~RunGuard() { if (armed) { cudaStreamSynchronize(stream); w->poisoned = true; } }
 };
 
 struct Events {
     std::vector<cudaEvent_t> ev;
     ~Events() { for (auto e : ev) cudaEventDestroy(e); }
-    cudaEvent_t make() { cudaEvent_t e = nullptr; cudaEventCreate(&e); ev.push_back(e); return e; }
+    cudaEvent_t make() { cudaEvent_t e = nullptr; if (cudaEventCreate(&e) != cudaSuccess) e = nullptr; else ev.push_back(e); return e; }
 };
 
 // Is every weight an integer small enough for the exact int32 path (piecewise-constant gradients such as PGSE)?
@@ -100,6 +110,7 @@ extern "C" int rms_run(const rms_substrate* s, rms_walkers* w, const rms_run_des
 {
     RMS_REQUIRE(s && w && d && out, RMS_ERR_ARG, "rms_run: null argument");
     RMS_REQUIRE(w->sub == s, RMS_ERR_ARG, "rms_run: walkers were initialised on another substrate");
+    RMS_REQUIRE(!w->poisoned, RMS_ERR_ARG, "rms_run: an earlier run on these walkers failed part-way; initialise them again");
     RMS_REQUIRE(d->n_steps >= 0, RMS_ERR_ARG, "n_steps is negative");
     RMS_REQUIRE(d->n_wave >= 0 && d->n_g >= 0 && d->n_dir >= 0 && d->n_snap >= 0, RMS_ERR_ARG, "negative count in rms_run_desc");
     RMS_REQUIRE(d->n_wave <= RMS_MAX_WAVES, RMS_ERR_UNSUPPORTED, "n_wave = %d is above RMS_MAX_WAVES = %d", d->n_wave,
@@ -206,6 +217,14 @@ extern "C" int rms_run(const rms_substrate* s, rms_walkers* w, const rms_run_des
     std::vector<int64_t> bounds;
     for (int i = 0; i < nS; ++i) bounds.push_back(d->snap_steps[i]);
     if (bounds.empty() || bounds.back() != nT) bounds.push_back(nT);
+    {
+        // the general kernels count box wraps in 10-bit fields per launch (+-511 per axis): on a lattice a few voxels wide a
+        // long launch is split so that no walker can wrap more often than that (hop < 1 voxel per step)
+        const int64_t max_launch = 511ll * std::min(s->nx, std::min(s->ny, s->nz));
+        for (int64_t b = max_launch; b < nT; b += max_launch) bounds.push_back(b);
+        std::sort(bounds.begin(), bounds.end());
+        bounds.erase(std::unique(bounds.begin(), bounds.end()), bounds.end());
+    }
     if (mixN > 0) {
         if (mix0 > 1) bounds.push_back(mix0 - 1);
         bounds.push_back(mix0 + mixN - 1);
@@ -284,6 +303,7 @@ extern "C" int rms_run(const rms_substrate* s, rms_walkers* w, const rms_run_des
     RMS_REQUIRE(n_flow <= ((size_t)1 << 27) && n_res_d <= ((size_t)1 << 28), RMS_ERR_UNSUPPORTED,
                 "n_classes = %d with %d snapshots, %d signals: the result arrays would exceed 1-2 GB", nC, nS, nQ);
     DeviceBuf b_tabs, b_segs, b_wave, b_wsuf, b_q, b_res, b_dirs, b_order;
+    for (DeviceBuf* b : {&b_tabs, &b_segs, &b_wave, &b_wsuf, &b_q, &b_res, &b_dirs, &b_order}) b->stream = stream;
     RMS_CUDA_TRY(rms_malloc((void**)&b_tabs.p, tabs.size() * sizeof(float)));
     RMS_CUDA_TRY(cudaMemcpyAsync(b_tabs.p, tabs.data(), tabs.size() * sizeof(float), cudaMemcpyHostToDevice, stream));
     if (need_segs) {
@@ -347,6 +367,7 @@ extern "C" int rms_run(const rms_substrate* s, rms_walkers* w, const rms_run_des
     RMS_CUDA_TRY(cudaEventRecord(ev_begin, stream));
     unsigned n_launches = 0;
 
+    RunGuard guard{w, stream};
     rms_step_params sp;
     memset(&sp, 0, sizeof sp);
     sp.nx = s->nx; sp.ny = s->ny; sp.nz = s->nz;
@@ -405,6 +426,7 @@ extern "C" int rms_run(const rms_substrate* s, rms_walkers* w, const rms_run_des
             }
             cudaEvent_t e0 = evs.make(), e1 = evs.make();
             RMS_CUDA_TRY(cudaEventRecord(e0, stream));
+            guard.armed = true;
             if (use_fast) rc = rms_launch_step_fast(sp, nW, permeable, fp64, stream);
             else if (fp64) rc = rms_launch_step_precise_general(sp, nWk, stream);
             else rc = rms_launch_step(sp, nWk, wmode, lat, permeable, stream);
@@ -477,6 +499,7 @@ extern "C" int rms_run(const rms_substrate* s, rms_walkers* w, const rms_run_des
     out->kernel_ms = ms;
     out->total_ms = tot;
     out->n_launches = n_launches;
+    guard.armed = false;
     w->steps_done += (uint64_t)nT;
     return RMS_OK;
 }

@@ -108,7 +108,7 @@ int rms_order_by_class(const rms_substrate* s, const rms_walkers* w, uint32_t* d
         e = cudaGetLastError();
         if (n_launches) *n_launches += 3;
     }
-    rms_free(d_count);
+    rms_free_async(d_count, stream);
     RMS_CUDA_TRY(e);
     return RMS_OK;
 }
@@ -136,8 +136,8 @@ int rms_order_walkers(const rms_substrate* s, const rms_walkers* w, uint32_t* d_
         e = cudaGetLastError();
         if (n_launches) *n_launches += 3;
     }
-    // the block goes back to the cache; later work on this stream is ordered after the kernels above
-    rms_free(d_count);
+    // the block goes back to the cache with an event behind the kernels above
+    rms_free_async(d_count, stream);
     RMS_CUDA_TRY(e);
     return RMS_OK;
 }

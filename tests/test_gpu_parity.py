@@ -280,6 +280,25 @@ def test_free_box_wraps_many_times(rms):
     assert np.abs(g["walkers"]["vox"]).max() > 8               # really left the box
 
 
+def test_one_voxel_wide_lattice_over_200k_steps_wrap_counters(rms):
+    """A (1, 1, 9) lattice without membranes, 200,000 steps: a walker wraps the 1-voxel axes ~+-250 times (sigma) and more than
+    +-511 times for ~4 % of the walkers; the general kernels count wraps per launch in 10-bit fields, so rms_run must split
+    the run.  Default path (specialised kernel) and the general fp32 / fp64 kernels against the oracle."""
+    sub = ri.uniform_lattice((1, 1, 9), 0.1, D_extra=8.0)           # hop of 0.98 voxel: sigma = 253 voxels after 200,000 steps
+    n, n_steps = 5_000, 200_000
+    seq = ri.pgse_sequence(2e-4, n_steps, 10.0, 20.0, [0.0, 0.05], np.eye(3), snap_steps=[n_steps])
+    o = oracle_run(sub, seq, n, 13)
+    assert np.abs(o["final_vox"][:, 0]).max() > 511
+    for flags in (0, 2, 8 | 2):
+        g = gpu_run(sub, seq, n, 13, flags=flags)
+        # free diffusion: no membrane, no discontinuity -- every walker stays with its twin; fp32 offsets drift by ~1e-5
+        same = np.all(g["walkers"]["vox"] == o["final_vox"], axis=1)
+        print("1x1x9, flags", flags, "same voxel", same.mean(), "max |dS|", np.abs(g["S"] - o["S"]).max(), "launches", g["n_launches"])
+        assert same.mean() >= 0.999
+        assert np.abs(g["S"] - o["S"]).max() <= 1e-4 + 2.0 * (1 - same.mean())
+        assert np.allclose(g["m2"], o["m2"], rtol=1e-4 + 8 * (1 - same.mean()))
+
+
 def test_walker_subrange_and_placement_only(rms):
     cfg = ri.make_config("cfg1", "test")
     g, o, n = _both(cfg, n_walkers=257, first_id=1000)          # ragged: 2 blocks + 1 walker
