@@ -64,6 +64,8 @@ struct rms_substrate {
     // neighbours appear in 4 (faces), 2 (edges) and 1 (corners) of the bytes: the redundancy buys a one-instruction
     // extraction (PRMT by the octant) of everything a hop can ask (at most three faces, all inside the block).
     uint2* d_oct = nullptr;
+    uint2* d_oct_alloc = nullptr;        // the allocation behind d_oct (d_oct = d_oct_alloc + oct_margin)
+    size_t oct_margin = 0;
     bool want_bricks = false;            // RMS_NO_BRICKS not given: d_nbr may be built on demand
     // memory order of the neighbourhood lattice: index = X SX + Y SY + Z SZ over the padded coordinates.  The axis with
     // the fewest membrane faces normal to it (the direction the cells run along) is made the fastest one, so that

@@ -3,6 +3,7 @@
 #include <stdarg.h>
 #include <string.h>
 
+#include <algorithm>
 #include <mutex>
 
 #include "rms_internal.cuh"
@@ -298,7 +299,11 @@ extern "C" int rms_substrate_create(const rms_substrate_desc* d, void* cuda_stre
     if (!(d->flags & RMS_NO_BRICKS)) {
         s->want_bricks = true;
         s->NX = s->nx + 2; s->NY = s->ny + 2; s->NZ = s->nz + 2;
-        SUB_TRY(rms_malloc((void**)&s->d_oct, (size_t)s->NX * s->NY * s->NZ * sizeof(uint2)));
+        // a margin on either side: the step kernel asks for the word of the voxel a hop would enter before it knows whether the
+        // walker sits on a ghost voxel, whose neighbours may lie outside the padded lattice (the value is never used then)
+        s->oct_margin = (size_t)std::max(s->NX * s->NY, s->NY * s->NZ) + (size_t)std::max(s->NX, s->NZ) + 2;
+        SUB_TRY(rms_malloc((void**)&s->d_oct_alloc, ((size_t)s->NX * s->NY * s->NZ + 2 * s->oct_margin) * sizeof(uint2)));
+        s->d_oct = s->d_oct_alloc + s->oct_margin;
         dim3 grid((s->NX + 127) / 128, s->NY, (s->NZ + RMS_NBR_ZCHUNK - 1) / RMS_NBR_ZCHUNK);
         if (grid.y > 65535u || grid.z > 65535u) {
             rms_set_error("lattice too large for the neighbourhood-lattice build (ny+2, nz+2 must be <= 65535)");
@@ -352,7 +357,7 @@ extern "C" int rms_substrate_destroy(rms_substrate* s)
     if (!s) return RMS_OK;
     if (s->owns_labels && s->d_labels) rms_free((void*)s->d_labels);
     if (s->d_nbr) rms_free(s->d_nbr);
-    if (s->d_oct) rms_free(s->d_oct);
+    if (s->d_oct_alloc) rms_free(s->d_oct_alloc);
     if (s->d_label_class) rms_free(s->d_label_class);
     delete s;
     return RMS_OK;
