@@ -39,8 +39,7 @@ N_SM, LANES_PER_SM = 148, 128          # B200: 4 schedulers x 32 lanes per SM, o
 # by the configuration that was captured; a run of any other configuration reports traffic = null.
 # key: (substrate, lattice, layout, walkers, mc_steps, fp64)
 NCU_CAPTURES = {
-    ("cfg4", "facemask", "x", 1_000_000, 10_000, False): {"bytes": 78.50e9, "source": "profiles/r2a_step_fast_ncu.md (commit 8a3974e)"},
-    ("cfg4", "facemask", "z", 1_000_000, 10_000, False): {"bytes": 39.28e9, "source": "profiles/r2a_step_fast_ncu.md (commit 8a3974e)"},
+    ("cfg4", "facemask", "x", 1_000_000, 10_000, False): {"bytes": 68.68e9, "source": "profiles/r2d_step_fast_ncu.md (68.08 GB read + 0.60 GB written)"},
 }
 
 
