@@ -806,3 +806,23 @@ def test_tables_match_oracle(rms):
     assert np.array_equal(s_g.astype(np.float64), s_o) and np.array_equal(P_g.astype(np.float64), P_o)
     info = S.info()
     assert info["n_membrane_faces"] == 0 and info["has_bricks"] == 1
+
+
+def test_philox_of_the_cuda_path_matches_curand_and_the_oracle(rms, tmp_path):
+    """K1 (S: section 8(c)): the product's Philox4x32-10 against cuRAND's Philox4_32_10 generator (a third implementation, NVIDIA's)
+    and against the oracle's, on 4096 (key, counter) pairs spread over all four counter words."""
+    import pathlib
+    import subprocess
+    import oracle
+    src = pathlib.Path(__file__).resolve().parent / "cuda" / "philox_vs_curand.cu"
+    exe = tmp_path / "philox_vs_curand"
+    subprocess.run(["nvcc", "-gencode", "arch=compute_100a,code=sm_100a", "-O2", "-std=c++17", "-o", str(exe), str(src)], check=True)
+    out = subprocess.run([str(exe)], check=True, capture_output=True, text=True).stdout.split()
+    v = np.array([int(x, 16) for x in out], np.uint64).reshape(-1, 8)
+    assert v.shape[0] == 4096 and np.array_equal(v[:, :4], v[:, 4:])
+    seed = 0x123456789ABCDEF1
+    for t in (0, 1, 77, 4095):
+        c01, c23 = (7919 * t * 1000003 + 1) & (2 ** 64 - 1), ((104729 * t << 20) + 3) & (2 ** 64 - 1)
+        ctr = [c01 & 0xFFFFFFFF, c01 >> 32, c23 & 0xFFFFFFFF, c23 >> 32]
+        ref = oracle.rms_oracle.philox4x32_10(ctr, [seed & 0xFFFFFFFF, seed >> 32])
+        assert np.array_equal(ref.astype(np.uint64), v[t, :4])
