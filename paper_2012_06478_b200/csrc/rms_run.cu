@@ -178,7 +178,7 @@ extern "C" int rms_run(const rms_substrate* s, rms_walkers* w, const rms_run_des
         }
     }
     const bool want_labels = (d->flags & RMS_RUN_LABEL_GATHER) != 0;
-    if (mt || rs) permeable = true;              // absorbing membranes and cancelled steps are handled where labels are read: the general kernels
+    if (mt || rs) permeable = true;              // absorbing membranes and cancelled steps take the kernels' permeable variants
     const int lat = (!permeable && s->want_bricks && !want_labels) ? RMS_LAT_FACES : RMS_LAT_LABELS;
     // permeable runs with P << 1 also take the specialised kernel: ceil(512 P_max) bounds the coarse random
     // bits that can permeate at all (rms_step_fast.cu)
@@ -189,7 +189,8 @@ extern "C" int rms_run(const rms_substrate* s, rms_walkers* w, const rms_run_des
     const uint32_t t_ceil_P = (uint32_t)ceilf(t_max);
     // absorbing membranes: the saturation draw belongs to every membrane met, so every such step is redone (t_ceil = 512)
     const uint32_t t_ceil = mt ? 512u : t_ceil_P;
-    const bool fast_permeable = permeable && !rs && s->d_oct && !want_labels && t_ceil <= RMS_FAST_PERM_TCEIL;
+    // (rejection sampling too: the specialised kernel cancels a step at its first uncrossed membrane; ERL stays on the general ones)
+    const bool fast_permeable = permeable && !erl && s->d_oct && !want_labels && t_ceil <= RMS_FAST_PERM_TCEIL;
 
     const int nWk = rms_kernel_waves(nW);        // waveforms the step kernel is compiled for; the extra ones carry zero weight
     rc = rms_walkers_reserve_waves(w, nWk, stream);

@@ -518,7 +518,7 @@ def test_rejection_sampling_interaction(rms):
     o = oracle_run(cyl, seq, n, 31, interaction=1)
     o_ecs = oracle_run(cyl, seq, n, 31)
     assert np.abs(o["S"] - o_ecs["S"]).max() > 1e-3
-    for flags in (RS, RS | 8):
+    for flags in (RS, RS | 8, RS | 2, RS | 2 | 8):      # specialised kernel (fp32 / fp64 directions), general kernels (fp32 / fp64)
         g = gpu_run(cyl, seq, n, 31, flags=flags)
         print("rejection sampling, cylinder, flags", flags, compare(g, o, n))
         assert g["n_encounters"] > n and g["n_permeations"] == 0
