@@ -66,16 +66,18 @@ typedef struct rms_walkers rms_walkers;     /* opaque */
  *              Two classes (extra / intra-cellular) are the usual choice; class = label gives per-cell outputs.
  * flags        RMS_LABELS_ON_DEVICE | RMS_ADOPT_DEVICE_PTR | RMS_NO_BRICKS | RMS_LAYOUT_X_FASTEST | RMS_LAYOUT_Z_FASTEST | RMS_LAYOUT_AUTO
  *
- * Derived on the device, unless RMS_NO_BRICKS: the neighbourhood lattice, one 32-bit word per voxel (plus a
- * one-voxel periodic ghost shell) whose 27 bits say which voxels of the 3x3x3 block around it carry the
- * same label -- a face is a membrane iff the labels on its two sides differ, and a hop shorter than
- * a voxel only ever meets faces inside that block.
+ * Derived on the device, unless RMS_NO_BRICKS: the octant lattice, one 64-bit word per voxel (plus a
+ * one-voxel periodic ghost shell): eight bytes, one per octant of hop directions, whose bits say which voxels
+ * of the 2x2x2 block a hop of that octant can reach carry the same label -- a face is a membrane iff the labels
+ * on its two sides differ, and a hop shorter than a voxel only ever meets faces inside that block (P:62,
+ * P:159).  8 bytes per voxel of device memory on top of the labels (4 more, on demand, for the general fp32
+ * kernel's face-bit mode).
  * Errors: RMS_ERR_ARG, RMS_ERR_OOM, RMS_ERR_CUDA.
  */
 #define RMS_LABELS_ON_DEVICE 1u
 #define RMS_ADOPT_DEVICE_PTR 2u
 #define RMS_NO_BRICKS 4u
-#define RMS_LAYOUT_X_FASTEST 8u   /* memory order of the neighbourhood lattice: x fastest (the default)                  */
+#define RMS_LAYOUT_X_FASTEST 8u   /* memory order of the octant lattice: x fastest (the default)                         */
 #define RMS_LAYOUT_Z_FASTEST 16u  /* z fastest: the 8 words of a 32-byte sector lie along z (cells elongated along z)    */
 #define RMS_LAYOUT_AUTO 24u       /* x or z, whichever axis has fewer membrane faces normal to it (sampled)              */
 
@@ -150,19 +152,20 @@ int rms_substrate_label_volumes(const rms_substrate* s, void* cuda_stream, uint6
  *             RMS_RUN_GENERAL_KERNEL: impermeable or permeable runs with piecewise-constant waveforms (rectangular
  *             lobes of any amplitude, segments of >= 32 steps on average) normally take the specialised kernel
  *             (csrc/rms_step_fast.cu); this flag forces the general one.
- *             RMS_RUN_FP64: direction, hop, in-voxel offsets, hit order and phase in fp64 instead of fp32, for runs
- *             of more than a few 1e4 steps whose trajectories must stay on those of an fp64 reference
- *             (csrc/rms_step_precise.cu says why fp32 cannot).  Two thirds of the fp32 speed for impermeable
- *             substrates with integer-valued piecewise-constant waveforms; a plain, slower kernel otherwise.
+ *             RMS_RUN_FP64: the direction of every hop in fp64 and the in-voxel offsets in 2^-63 fixed point (exact
+ *             additions), hit order and phase in fp64, for runs of more than a few 1e4 steps whose trajectories must
+ *             stay on those of an fp64 reference (DESIGN.md "Tolerances" says why fp32 directions cannot).  Three
+ *             quarters of the fp32 speed wherever the specialised kernel runs (piecewise-constant waveforms;
+ *             impermeable, permeable, absorbing, rejection sampling); a plain, slower kernel otherwise.
  *             RMS_RUN_NO_ORDERING: on large lattices the walkers are dealt to the threads in the order of the
  *             lattice cell they sit in (cache locality; results do not depend on it); this flag keeps id order.
  *             RMS_RUN_REJECTION_SAMPLING: the paper's other membrane interaction (Appendix B): a
  *             step that meets a membrane it does not cross is cancelled and the walker stays where it was for
  *             that step, instead of the elastic collision.  The permeation probability is then Appendix B.1's
  *             P_T = A / (1 + A), A = kappa sqrt(6 dt / D) 2/3, defined for equal D on both sides:
- *             RMS_ERR_UNSUPPORTED for a finite non-zero kappa between unequal D.  Runs in the general kernels
- *             (fp32, or fp64 with RMS_RUN_FP64); biased near membranes by Eq.B.2, which is why elastic
- *             collision is the default.
+ *             RMS_ERR_UNSUPPORTED for a finite non-zero kappa between unequal D.  Runs in the specialised kernel
+ *             (piecewise-constant waveforms) or the general ones, fp32 or fp64 with RMS_RUN_FP64; biased near
+ *             membranes by Eq.B.2, which is why elastic collision is the default.
  *             RMS_RUN_ERL: equal-step-length random leap, the paper's third comparison interaction (PAPER.md lines 80,
  *             340, Appendix A): a step that meets a membrane is cancelled and tried again in a new direction until it
  *             meets none (at most 4095 retries, then the walker stays put for the step).  Impermeable, non-absorbing
