@@ -54,7 +54,8 @@ def parse_args():
     ap.add_argument("--dirs", type=int, default=60)
     ap.add_argument("--lattice", default="facemask", choices=["facemask", "labels"])
     ap.add_argument("--scale", default="full", choices=["full", "test"])
-    ap.add_argument("--layout", default="x", choices=["auto", "x", "z"], help="memory order of the neighbourhood lattice")
+    ap.add_argument("--layout", default="auto", choices=["auto", "x", "z"],
+                    help="memory order of the neighbourhood lattice (auto: RMS_LAYOUT_AUTO picks the axis the membranes run along)")
     ap.add_argument("--waves", type=int, default=1,
                     help="number of PGSE waveforms evaluated on the same trajectories (sequence sweep, not the headline)")
     ap.add_argument("--substrate", default="cfg4", choices=["cfg4", "cfg3"],
