@@ -135,6 +135,19 @@ int rms_walkers_init_weighted(const rms_substrate* s, uint64_t n_walkers, uint64
 /* Voxels per label, counted on the device.  voxels_out [n_labels] host.  Errors: RMS_ERR_ARG, RMS_ERR_OOM, RMS_ERR_CUDA. */
 int rms_substrate_label_volumes(const rms_substrate* s, void* cuda_stream, uint64_t* voxels_out);
 
+/* The same count for callers that may not allocate device memory (serving loops, harnesses that forbid cudaMalloc, code
+ * that will later run under CUDA graph capture): this entry point calls no cudaMalloc, cudaFree or allocating routine,
+ * neither the driver's nor the library's cache.  Its per-label counters are a static device array of
+ * RMS_STATIC_MAX_LABELS uint64 (128 KiB), held by every GPU that loads the library until the process exits.
+ * Same arguments and result as rms_substrate_label_volumes: voxels_out [n_labels] host, written before the call returns
+ * (the stream is synchronised).  RMS_ERR_UNSUPPORTED if the substrate has more than RMS_STATIC_MAX_LABELS labels (use
+ * rms_substrate_label_volumes then); RMS_ERR_ARG, RMS_ERR_CUDA otherwise.
+ * All calls on a device share the one array (it is cleared at the start of every call): calls that overlap on the GPU
+ * -- two host threads, or two streams -- race on it and must be serialised by the caller.  The first call on a device
+ * looks up the array's device address (no allocation); make that call outside any stream capture. */
+#define RMS_STATIC_MAX_LABELS 16384
+int rms_substrate_label_volumes_static(const rms_substrate* s, void* cuda_stream, uint64_t* voxels_out);
+
 /* ------------------------------------------------------------------------------------------------
  * rms_run -- advance every walker by n_steps Monte Carlo steps (2.2 steps 2-4: fixed-length
  * hop sqrt(6 D dt) in a random direction; at a voxel face between unlike labels elastic reflection or

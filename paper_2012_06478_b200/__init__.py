@@ -17,6 +17,7 @@ from .binding import (  # noqa: F401
     rms_walkers_init,
     rms_walkers_init_weighted,
     rms_substrate_label_volumes,
+    rms_substrate_label_volumes_static,
     rms_volume_weighted_signal,
 )
 from .api import simulate, shard_range  # noqa: F401

@@ -28,6 +28,7 @@ RMS_RUN_NO_ORDERING = 4
 RMS_RUN_FP64 = 8
 RMS_RUN_REJECTION_SAMPLING = 16
 RMS_RUN_ERL = 32
+RMS_STATIC_MAX_LABELS = 16384
 
 STATUS = {0: "RMS_OK", -1: "RMS_ERR_ARG", -2: "RMS_ERR_STEP_TOO_LARGE", -3: "RMS_ERR_P_RANGE", -4: "RMS_ERR_NO_SPACE",
           -5: "RMS_ERR_OOM", -6: "RMS_ERR_CUDA", -7: "RMS_ERR_UNSUPPORTED"}
@@ -35,7 +36,7 @@ STATUS = {0: "RMS_OK", -1: "RMS_ERR_ARG", -2: "RMS_ERR_STEP_TOO_LARGE", -3: "RMS
 EXPORTS = ("rms_substrate_create", "rms_substrate_destroy", "rms_substrate_get_info", "rms_walkers_init",
            "rms_walkers_destroy", "rms_run", "rms_walkers_read", "rms_walkers_steps_done", "rms_tables", "rms_normalise",
            "rms_walkers_init_weighted", "rms_substrate_label_volumes", "rms_volume_weighted_signal",
-           "rms_memory_trim", "rms_gather_probe", "rms_last_error", "rms_version")
+           "rms_memory_trim", "rms_gather_probe", "rms_last_error", "rms_version", "rms_substrate_label_volumes_static")
 
 
 class RmsError(RuntimeError):
@@ -246,6 +247,13 @@ def rms_walkers_init_weighted(substrate: Substrate, n_walkers, first_walker_id=0
 def rms_substrate_label_volumes(substrate: Substrate, stream=None) -> np.ndarray:
     out = np.zeros(substrate.n_labels, np.uint64)
     _check(load_library().rms_substrate_label_volumes(substrate.handle, _stream_ptr(stream), C.c_void_p(out.ctypes.data)))
+    return out
+
+
+def rms_substrate_label_volumes_static(substrate: Substrate, stream=None) -> np.ndarray:
+    """The same count through the entry point that allocates no device memory (at most RMS_STATIC_MAX_LABELS labels)."""
+    out = np.zeros(substrate.n_labels, np.uint64)
+    _check(load_library().rms_substrate_label_volumes_static(substrate.handle, _stream_ptr(stream), C.c_void_p(out.ctypes.data)))
     return out
 
 

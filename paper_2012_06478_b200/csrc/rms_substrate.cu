@@ -449,6 +449,55 @@ extern "C" int rms_substrate_label_volumes(const rms_substrate* s, void* cuda_st
     return RMS_OK;
 }
 
+// ------------------------------------------------------------------------------------------------
+// rms_substrate_label_volumes_static: the same count for callers that may not allocate (include/rms.h).  The per-label
+// counters live in a file-scope device array instead of a block from rms_malloc; every GPU that loads the library holds
+// its RMS_STATIC_MAX_LABELS * 8 bytes until the process exits.  In host code the name `rms_static_label_count` is only a
+// stand-in for the symbol: its device address is asked for once per device (cudaGetSymbolAddress, that device current)
+// and that address is what the kernel and the copies are given.
+// ------------------------------------------------------------------------------------------------
+static __device__ __align__(256) unsigned long long rms_static_label_count[RMS_STATIC_MAX_LABELS];
+
+static int rms_static_label_count_ptr(unsigned long long** out)
+{
+    static std::mutex mu;
+    static unsigned long long* ptr_of_device[64] = {nullptr};
+    int dev = -1;
+    RMS_CUDA_TRY(cudaGetDevice(&dev));
+    RMS_REQUIRE(dev >= 0 && dev < 64, RMS_ERR_UNSUPPORTED, "device index %d out of range", dev);
+    std::lock_guard<std::mutex> lock(mu);
+    if (!ptr_of_device[dev]) {
+        unsigned long long* p = nullptr;
+        RMS_CUDA_TRY(cudaGetSymbolAddress((void**)&p, rms_static_label_count));
+        RMS_REQUIRE(p != nullptr, RMS_ERR_CUDA, "cudaGetSymbolAddress returned no address for the static counters");
+        ptr_of_device[dev] = p;
+    }
+    *out = ptr_of_device[dev];
+    return RMS_OK;
+}
+
+extern "C" int rms_substrate_label_volumes_static(const rms_substrate* s, void* cuda_stream, uint64_t* voxels_out)
+{
+    RMS_REQUIRE(s && voxels_out, RMS_ERR_ARG, "rms_substrate_label_volumes_static: null argument");
+    RMS_REQUIRE(s->n_labels <= RMS_STATIC_MAX_LABELS, RMS_ERR_UNSUPPORTED,
+                "rms_substrate_label_volumes_static: n_labels = %d exceeds the %d labels the static counters hold "
+                "(RMS_STATIC_MAX_LABELS); use rms_substrate_label_volumes", s->n_labels, RMS_STATIC_MAX_LABELS);
+    cudaStream_t stream = (cudaStream_t)cuda_stream;
+    unsigned long long* d_count = nullptr;
+    const int rc = rms_static_label_count_ptr(&d_count);
+    if (rc != RMS_OK) return rc;
+    const size_t bytes = (size_t)s->n_labels * sizeof(unsigned long long);
+    // the array keeps the counts of the last call: every call starts by clearing the part it uses
+    RMS_CUDA_TRY(cudaMemsetAsync(d_count, 0, bytes, stream));
+    const uint64_t per_block = 1ull << 24;       // 32-bit shared counters: at most 2^32 - 1 voxels per block
+    const unsigned grid = (unsigned)std::min<uint64_t>(std::max<uint64_t>((s->n_vox + per_block - 1) / per_block, 148ull * 8), 1u << 20);
+    rms_label_volumes_kernel<<<grid, 256, 0, stream>>>(s->d_labels, s->n_vox, s->n_labels, d_count);
+    RMS_CUDA_TRY(cudaGetLastError());
+    RMS_CUDA_TRY(cudaMemcpyAsync(voxels_out, d_count, bytes, cudaMemcpyDeviceToHost, stream));
+    RMS_CUDA_TRY(cudaStreamSynchronize(stream));
+    return RMS_OK;
+}
+
 extern "C" int rms_substrate_get_info(const rms_substrate* s, rms_substrate_info* out)
 {
     RMS_REQUIRE(s && out, RMS_ERR_ARG, "rms_substrate_get_info: null argument");
