@@ -40,6 +40,9 @@ N_SM, LANES_PER_SM = 148, 128          # B200: 4 schedulers x 32 lanes per SM, o
 # key: (substrate, lattice, layout, walkers, mc_steps, fp64)
 NCU_CAPTURES = {
     ("cfg4", "facemask", "x", 1_000_000, 10_000, False): {"bytes": 68.68e9, "source": "profiles/r2d_step_fast_ncu.md (68.08 GB read + 0.60 GB written)"},
+    # RMS_LAYOUT_AUTO picks z fastest on this lattice: the two keys name the same launch
+    ("cfg4", "facemask", "auto", 1_000_000, 10_000, False): {"bytes": 32.35e9, "source": "profiles/r2e_step_fast_ncu.md (31.75 GB read + 0.59 GB written)"},
+    ("cfg4", "facemask", "z", 1_000_000, 10_000, False): {"bytes": 32.35e9, "source": "profiles/r2e_step_fast_ncu.md (31.75 GB read + 0.59 GB written)"},
 }
 
 
