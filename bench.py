@@ -59,6 +59,8 @@ def parse_args():
     ap.add_argument("--scale", default="full", choices=["full", "test"])
     ap.add_argument("--layout", default="auto", choices=["auto", "x", "z"],
                     help="memory order of the neighbourhood lattice (auto: RMS_LAYOUT_AUTO picks the axis the membranes run along)")
+    ap.add_argument("--lattice-format", default="oct", choices=["oct", "dict"],
+                    help="oct: 8-byte octant word per voxel; dict: RMS_LATTICE_DICT, 2-byte code per voxel + dictionary of octant words")
     ap.add_argument("--waves", type=int, default=1,
                     help="number of PGSE waveforms evaluated on the same trajectories (sequence sweep, not the headline)")
     ap.add_argument("--substrate", default="cfg4", choices=["cfg4", "cfg3"],
@@ -191,7 +193,7 @@ def workload_config(args, cfg, extra=None):
          "intra_fraction": round(cfg.substrate.meta.get("intra_fraction", 0.0), 4),
          "walkers_per_gpu": args.walkers, "mc_steps": args.mc_steps, "dt_ms": cfg.sequence.dt_ms,
          "directions": int(cfg.sequence.dirs.shape[0]), "b_values": int(cfg.sequence.gamp.shape[1]),
-         "lattice_path": args.lattice, "layout": args.layout, "pass": "rms_substrate_create + rms_walkers_init + rms_run",
+         "lattice_path": args.lattice, "layout": args.layout, "lattice_format": args.lattice_format, "pass": "rms_substrate_create + rms_walkers_init + rms_run",
          "l2": "inputs larger than L2 (label lattice 1.0 GB + octant lattice 4.0 GB vs 126 MB L2)" if args.scale == "full"
          else "reduced test lattice (fits L2) -- not a valid bench configuration"}
     if extra:
@@ -301,6 +303,8 @@ def main():
     if args.fp64:
         flags |= rms.binding.RMS_RUN_FP64
     sflags = {"auto": rms.binding.RMS_LAYOUT_AUTO, "x": rms.binding.RMS_LAYOUT_X_FASTEST, "z": rms.binding.RMS_LAYOUT_Z_FASTEST}[args.layout]
+    if args.lattice_format == "dict":
+        sflags |= rms.binding.RMS_LATTICE_DICT
     t_ms = np.asarray(seq.snap_steps, np.float64) * seq.dt_ms
 
     labels_dev = torch.from_numpy(sub.labels.view(np.int16)).cuda()          # resident in HBM before timing
@@ -416,7 +420,9 @@ def main():
             "clocks": clocks, "e2e": e2e, "gpu_launches": launches, "roofline": roofline, "cpu_baseline": cpu_baseline,
             "wall_ms_per_step": 1e3 * wall / args.steps,
             "check": {"S_b_max_dir0": float(abs(r["S"][0, -1, 0])), "n_encounters": r["n_encounters"],
-                      "n_membrane_faces": r["substrate_info"]["n_membrane_faces"]}}
+                      "n_membrane_faces": r["substrate_info"]["n_membrane_faces"],
+                      "dict_entries": r["substrate_info"]["dict_entries"],
+                      "dict_escaped_voxels": r["substrate_info"]["dict_escaped_voxels"]}}
     print(json.dumps(line))
     if world > 1:
         dist.destroy_process_group()

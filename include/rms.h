@@ -64,7 +64,8 @@ typedef struct rms_walkers rms_walkers;     /* opaque */
  *              density proportional to c_L (R24).  Equal concentrations change nothing.
  * label_class  [n_labels] uint16 output compartment class of each label, < n_classes <= 65535; NULL = all 0 (host).
  *              Two classes (extra / intra-cellular) are the usual choice; class = label gives per-cell outputs.
- * flags        RMS_LABELS_ON_DEVICE | RMS_ADOPT_DEVICE_PTR | RMS_NO_BRICKS | RMS_LAYOUT_X_FASTEST | RMS_LAYOUT_Z_FASTEST | RMS_LAYOUT_AUTO
+ * flags        RMS_LABELS_ON_DEVICE | RMS_ADOPT_DEVICE_PTR | RMS_NO_BRICKS | RMS_LAYOUT_X_FASTEST | RMS_LAYOUT_Z_FASTEST | RMS_LAYOUT_AUTO |
+ *              RMS_LATTICE_DICT
  *
  * Derived on the device, unless RMS_NO_BRICKS: the octant lattice, one 64-bit word per voxel (plus a
  * one-voxel periodic ghost shell): eight bytes, one per octant of hop directions, whose bits say which voxels
@@ -80,6 +81,10 @@ typedef struct rms_walkers rms_walkers;     /* opaque */
 #define RMS_LAYOUT_X_FASTEST 8u   /* memory order of the octant lattice: x fastest (the default)                         */
 #define RMS_LAYOUT_Z_FASTEST 16u  /* z fastest: the 8 words of a 32-byte sector lie along z (cells elongated along z)    */
 #define RMS_LAYOUT_AUTO 24u       /* x or z, whichever axis has fewer membrane faces normal to it (sampled)              */
+#define RMS_LATTICE_DICT 32u      /* store a 16-bit code per voxel and the octant words of the distinct neighbourhoods in a
+                                     dictionary (2 bytes per voxel instead of 8: a quarter of the cache footprint of a walker;
+                                     one more, dependent, look-up per face reached).  Lattices with more distinct
+                                     neighbourhoods than the tables hold (independent random labels) get the octant lattice. */
 
 typedef struct {
     int32_t nx, ny, nz;
@@ -107,6 +112,8 @@ typedef struct {
     uint64_t lattice_bytes;     /* uint16 lattice on the device                                          */
     uint64_t brick_bytes;       /* neighbourhood lattice on the device (0 with RMS_NO_BRICKS)            */
     int32_t has_bricks;
+    uint32_t dict_entries;        /* RMS_LATTICE_DICT: distinct neighbourhoods in the dictionary (0: octant lattice in use) */
+    uint32_t dict_escaped_voxels; /* voxels whose neighbourhood found no free code (their words sit in a hash table)        */
 } rms_substrate_info;
 
 int rms_substrate_get_info(const rms_substrate* s, rms_substrate_info* out /* host */);
@@ -185,6 +192,11 @@ int rms_substrate_label_volumes_static(const rms_substrate* s, void* cuda_stream
  *             membranes only (kappa 0 or +inf, no rho: RMS_ERR_UNSUPPORTED otherwise).  General kernels; depletes the
  *             density within a hop length of the membranes (Eq.A.1), hence not the default.
  *
+ *             RMS_RUN_NO_SLICES: a launch of the specialised kernel over more walkers than the GPU holds at a time is cut into
+ *             time slices of ~1000 steps that are dealt to the SMs from a queue, so that the SMs do not idle while the last
+ *             blocks finish (results do not depend on it beyond the order of the fp64 phase additions); this flag keeps one
+ *             block per group of walkers for the whole launch.
+ *
  * mix_first_step, mix_n_steps  the mixing time of a stimulated echo: in these steps Eq.5 runs with the T1 of
  *             the compartment the walker is in, in all others with its T2.  The window lies inside 1..n_steps
  *             (RMS_ERR_ARG otherwise); the caller keeps the waveforms at 0 there (the stored magnetisation
@@ -222,6 +234,7 @@ int rms_substrate_label_volumes_static(const rms_substrate* s, void* cuda_stream
 #define RMS_RUN_FP64 8u
 #define RMS_RUN_REJECTION_SAMPLING 16u
 #define RMS_RUN_ERL 32u
+#define RMS_RUN_NO_SLICES 64u
 
 typedef struct {
     double dt_ms;               /* Table 1: dt */

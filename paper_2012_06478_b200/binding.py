@@ -22,12 +22,14 @@ RMS_NO_BRICKS = 4
 RMS_LAYOUT_X_FASTEST = 8
 RMS_LAYOUT_Z_FASTEST = 16
 RMS_LAYOUT_AUTO = 24
+RMS_LATTICE_DICT = 32
 RMS_RUN_LABEL_GATHER = 1
 RMS_RUN_GENERAL_KERNEL = 2
 RMS_RUN_NO_ORDERING = 4
 RMS_RUN_FP64 = 8
 RMS_RUN_REJECTION_SAMPLING = 16
 RMS_RUN_ERL = 32
+RMS_RUN_NO_SLICES = 64
 RMS_STATIC_MAX_LABELS = 16384
 
 STATUS = {0: "RMS_OK", -1: "RMS_ERR_ARG", -2: "RMS_ERR_STEP_TOO_LARGE", -3: "RMS_ERR_P_RANGE", -4: "RMS_ERR_NO_SPACE",
@@ -55,7 +57,8 @@ class SubstrateDesc(C.Structure):
 class SubstrateInfo(C.Structure):
     _fields_ = [("nx", C.c_int32), ("ny", C.c_int32), ("nz", C.c_int32), ("n_labels", C.c_int32),
                 ("n_classes", C.c_int32), ("n_voxels", C.c_uint64), ("n_membrane_faces", C.c_uint64),
-                ("lattice_bytes", C.c_uint64), ("brick_bytes", C.c_uint64), ("has_bricks", C.c_int32)]
+                ("lattice_bytes", C.c_uint64), ("brick_bytes", C.c_uint64), ("has_bricks", C.c_int32),
+                ("dict_entries", C.c_uint32), ("dict_escaped_voxels", C.c_uint32)]
 
 
 class RunDesc(C.Structure):

@@ -67,6 +67,16 @@ struct rms_substrate {
     uint2* d_oct_alloc = nullptr;        // the allocation behind d_oct (d_oct = d_oct_alloc + oct_margin)
     size_t oct_margin = 0;
     bool want_bricks = false;            // RMS_NO_BRICKS not given: d_nbr may be built on demand
+    // dictionary lattice (RMS_LATTICE_DICT; instead of d_oct): one 16-bit code per padded voxel, same geometry, strides and
+    // margin; d_dict[code] = the voxel's octant word.  Code 0 = interior voxel (all 26 neighbours carry its label), codes
+    // 1 .. RMS_DICT_ESCAPE - 1 in the order the build met the neighbourhoods, RMS_DICT_ESCAPE = the lattice has more distinct
+    // neighbourhoods than codes: the word of such a voxel is in the hash table d_esc, keyed by its padded index + 1
+    // (slot = {key, 0, word.x, word.y}, linear probing from rms_esc_hash(index) & esc_mask).
+    uint16_t* d_code = nullptr;
+    uint16_t* d_code_alloc = nullptr;
+    uint2* d_dict = nullptr;             // [RMS_DICT_ESCAPE]
+    uint4* d_esc = nullptr;
+    uint32_t esc_mask = 0, n_dict = 0, n_esc = 0;
     // memory order of the neighbourhood lattice: index = X SX + Y SY + Z SZ over the padded coordinates.  The axis with
     // the fewest membrane faces normal to it (the direction the cells run along) is made the fastest one, so that
     // the 8 words of a 32-byte sector belong to one compartment; x fastest (1, NX, NX NY) or z fastest (NY NZ, NZ, 1).
@@ -183,12 +193,21 @@ static inline int rms_kernel_waves(int n_wave) { return n_wave <= 4 ? n_wave : (
 enum { RMS_LAT_LABELS = 0, RMS_LAT_FACES = 1 };
 #define RMS_NBR_GHOST (1u << 27)
 #define RMS_NBR_SELF 13
+#define RMS_DICT_ESCAPE 0xFFFFu
+#define RMS_OCT_INTERIOR 0xFEFEFEFEu     // both halves of the octant word of an interior voxel
+#ifdef __CUDACC__
+__host__ __device__ __forceinline__ uint32_t rms_esc_hash(uint32_t lin) { return (lin * 0x9E3779B1u) >> 8; }
+#endif
 
 struct rms_step_params {
     int nx, ny, nz;
     const uint16_t* labels;
     const uint32_t* nbr;
     const uint2* oct;         // octant lattice (rms_substrate::d_oct), same padded geometry and strides as nbr
+    const uint16_t* code;     // or the dictionary lattice (rms_substrate::d_code, d_dict, d_esc): oct == NULL then
+    const uint2* dict;
+    const uint4* esc;
+    uint32_t esc_mask;
     const uint32_t* lut1;     // device, [1024]: interaction outcome by (octant byte >> 1, faces reached); rms_step_fast.cu
     const uint32_t* lut2;     // device, [8192]: the same with the hit order, for the entries lut1 marks order dependent
     int NX, NY;               // padded dims of the neighbourhood lattice
@@ -216,7 +235,14 @@ struct rms_step_params {
     int n_wave;
     unsigned long long* counters;    // [0] encounters [1] permeations [2] clamps [3] init failures [4] saturations
     const uint32_t* order;           // thread t works on walker order[t] (spatially sorted, rms_sched.cu); NULL = identity
+    // specialised kernel, time slices (rms_step_fast.cu): the first n_whole groups of walkers take one block each for all
+    // steps, the last n_sliced groups one block per slice of slice_len steps (n_slices of them, the last one shorter);
+    // sched = device [1 + n_sliced], zeroed before the launch.  n_slices <= 1: one block per group.
+    uint32_t n_slices, slice_len, n_whole, n_sliced;
+    uint32_t* sched;
 };
+// fills in the time-slice fields of p for its n walkers x n_steps (n_slices = 0: none); *sched_words = size of p.sched
+void rms_fast_slices(rms_step_params* p, size_t* sched_words);
 
 int rms_launch_step(const rms_step_params& p, int n_wave, int wmode, int lat, bool permeable, cudaStream_t stream);
 // RMS_LAT_FACES + RMS_WMODE_CONST only; permeable: P(a->b) << 1 expected (rms_step_fast.cu)

@@ -190,7 +190,7 @@ extern "C" int rms_run(const rms_substrate* s, rms_walkers* w, const rms_run_des
     // absorbing membranes: the saturation draw belongs to every membrane met, so every such step is redone (t_ceil = 512)
     const uint32_t t_ceil = mt ? 512u : t_ceil_P;
     // (rejection sampling too: the specialised kernel cancels a step at its first uncrossed membrane; ERL stays on the general ones)
-    const bool fast_permeable = permeable && !erl && s->d_oct && !want_labels && t_ceil <= RMS_FAST_PERM_TCEIL;
+    const bool fast_permeable = permeable && !erl && (s->d_oct || s->d_code) && !want_labels && t_ceil <= RMS_FAST_PERM_TCEIL;
 
     const int nWk = rms_kernel_waves(nW);        // waveforms the step kernel is compiled for; the extra ones carry zero weight
     rc = rms_walkers_reserve_waves(w, nWk, stream);
@@ -303,8 +303,8 @@ extern "C" int rms_run(const rms_substrate* s, rms_walkers* w, const rms_run_des
     const size_t n_res_d = 2 * n_sig + 2 * n_mom + n_sal + nC;       // doubles
     RMS_REQUIRE(n_flow <= ((size_t)1 << 27) && n_res_d <= ((size_t)1 << 28), RMS_ERR_UNSUPPORTED,
                 "n_classes = %d with %d snapshots, %d signals: the result arrays would exceed 1-2 GB", nC, nS, nQ);
-    DeviceBuf b_tabs, b_segs, b_wave, b_wsuf, b_q, b_res, b_dirs, b_order;
-    for (DeviceBuf* b : {&b_tabs, &b_segs, &b_wave, &b_wsuf, &b_q, &b_res, &b_dirs, &b_order}) b->stream = stream;
+    DeviceBuf b_tabs, b_segs, b_wave, b_wsuf, b_q, b_res, b_dirs, b_order, b_sched;
+    for (DeviceBuf* b : {&b_tabs, &b_segs, &b_wave, &b_wsuf, &b_q, &b_res, &b_dirs, &b_order, &b_sched}) b->stream = stream;
     RMS_CUDA_TRY(rms_malloc((void**)&b_tabs.p, tabs.size() * sizeof(float)));
     RMS_CUDA_TRY(cudaMemcpyAsync(b_tabs.p, tabs.data(), tabs.size() * sizeof(float), cudaMemcpyHostToDevice, stream));
     if (need_segs) {
@@ -373,6 +373,7 @@ extern "C" int rms_run(const rms_substrate* s, rms_walkers* w, const rms_run_des
     memset(&sp, 0, sizeof sp);
     sp.nx = s->nx; sp.ny = s->ny; sp.nz = s->nz;
     sp.labels = s->d_labels; sp.nbr = s->d_nbr; sp.oct = s->d_oct;
+    sp.code = s->d_code; sp.dict = s->d_dict; sp.esc = s->d_esc; sp.esc_mask = s->esc_mask;
     if (use_fast) {
         rc = rms_fast_luts(&sp.lut1, &sp.lut2);
         if (rc != RMS_OK) return rc;
@@ -428,6 +429,16 @@ extern "C" int rms_run(const rms_substrate* s, rms_walkers* w, const rms_run_des
             cudaEvent_t e0 = evs.make(), e1 = evs.make();
             RMS_CUDA_TRY(cudaEventRecord(e0, stream));
             guard.armed = true;
+            if (use_fast && !(d->flags & RMS_RUN_NO_SLICES)) {
+                // time slices: fill the tail of a launch of many waves of blocks (rms_step_fast.cu)
+                size_t words = 0;
+                rms_fast_slices(&sp, &words);
+                if (sp.n_slices > 1u) {
+                    if (!b_sched.p) RMS_CUDA_TRY(rms_malloc((void**)&b_sched.p, words * sizeof(uint32_t)));   // the same size at every launch
+                    RMS_CUDA_TRY(cudaMemsetAsync(b_sched.p, 0, words * sizeof(uint32_t), stream));
+                    sp.sched = b_sched.as<uint32_t>();
+                }
+            }
             if (use_fast) rc = rms_launch_step_fast(sp, nW, permeable, fp64, stream);
             else if (fp64) rc = rms_launch_step_precise_general(sp, nWk, stream);
             else rc = rms_launch_step(sp, nWk, wmode, lat, permeable, stream);

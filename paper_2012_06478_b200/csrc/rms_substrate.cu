@@ -1,6 +1,7 @@
 // rms_substrate.cu -- H0: substrate upload and the derived neighbourhood lattice (include/rms.h, rms_substrate_create).
 #include <math.h>
 #include <stdarg.h>
+#include <stdlib.h>
 #include <string.h>
 
 #include <algorithm>
@@ -87,15 +88,99 @@ __device__ __forceinline__ void rms_nbr_make_word(uint32_t m, bool ghost, const 
 // through a 512-entry table in shared memory: entry [9-bit z-plane], byte q = 2 [hop_x < 0] + [hop_y < 0], even bits
 // 0, 2, 4, 6 = the plane's same-label bits at (0, 0), (0, sy), (sx, 0), (sx, sy).  The plane of the voxel gives the even
 // bits of an octant byte (not moved in z), the plane above or below, shifted by one, the odd ones.
-template <bool OCT> struct rms_nbr_word { typedef uint32_t type; };
-template <> struct rms_nbr_word<true> { typedef uint2 type; };
+template <bool OCT, bool DICT> struct rms_nbr_word { typedef uint32_t type; };
+template <> struct rms_nbr_word<true, false> { typedef uint2 type; };
+template <> struct rms_nbr_word<true, true> { typedef uint16_t type; };
 
-template <bool ZFAST, bool OCT>
-__global__ void __launch_bounds__(128) rms_build_nbr_kernel(const uint16_t* __restrict__ labels, int nx, int ny, int nz,
-                                                             typename rms_nbr_word<OCT>::type* __restrict__ nbr, int SX, int SY, int SZ,
-                                                             int n_labels, unsigned long long* __restrict__ stats)
+// DICT: the word written is the 16-bit code of rms_substrate::d_code; the octant word goes into the dictionary.  A hash
+// table in global memory (2 MB, L2 resident) maps the 28-bit neighbourhood word (27 same-label bits + ghost flag, never 0) to
+// its code: slot = key | (code + 1) << 32, claimed with a compare-and-swap on the empty slot (0), the code published by the
+// claimant afterwards; readers of a claimed slot poll until the code is there.  Interior voxels (9 in 10) never come here, and
+// a thread remembers the last neighbourhood it looked up (cells run along its column).
+struct rms_dict_build {
+    unsigned long long* hash;
+    uint32_t hash_mask;
+    uint2* dict;
+    uint32_t dict_cap;          // codes 1 .. dict_cap - 1 are handed out, then RMS_DICT_ESCAPE
+    uint4* esc;
+    uint32_t esc_mask, esc_cap;
+    uint32_t* counters;         // [0] neighbourhoods met, [1] escaped voxels, [2] gave up (tables full)
+};
+
+__device__ __noinline__ uint32_t rms_dict_lookup(const rms_dict_build& B, uint32_t key, uint2 word, uint32_t lin)
 {
-    typedef typename rms_nbr_word<OCT>::type WORD;
+    uint32_t code = RMS_DICT_ESCAPE;
+    bool done = false;
+    uint32_t h = ((key * 0x9E3779B1u) >> 10) & B.hash_mask;
+    for (int probe = 0; probe < 4096 && !done; ++probe) {
+        volatile unsigned long long* slot = B.hash + h;
+        unsigned long long cur = *slot;
+        if (cur == 0ull) {
+            cur = atomicCAS((unsigned long long*)slot, 0ull, (unsigned long long)key);
+            if (cur == 0ull) {                                        // claimed: hand out the code, publish it
+                const uint32_t idx = atomicAdd(&B.counters[0], 1u) + 1u;
+                code = idx < B.dict_cap ? idx : RMS_DICT_ESCAPE;
+                if (code != RMS_DICT_ESCAPE) B.dict[code] = word;
+                __threadfence();
+                *slot = (unsigned long long)key | ((unsigned long long)(code + 1u) << 32);
+                done = true;
+            }
+        }
+        if (!done && (uint32_t)cur == key) {
+            while ((cur >> 32) == 0ull) cur = *slot;                 // the claimant publishes without waiting for anyone
+            code = (uint32_t)(cur >> 32) - 1u;
+            done = true;
+        }
+        h = (h + 1u) & B.hash_mask;
+    }
+    if (!done) { B.counters[2] = 1u; return RMS_DICT_ESCAPE; }
+    if (code == RMS_DICT_ESCAPE) {
+        // more neighbourhoods than codes: this voxel's word goes into the escape table under its own index
+        if (atomicAdd(&B.counters[1], 1u) >= B.esc_cap) { B.counters[2] = 1u; return code; }
+        uint32_t g = rms_esc_hash(lin) & B.esc_mask;
+        for (int probe = 0; probe < 4096; ++probe) {
+            if (atomicCAS(&B.esc[g].x, 0u, lin + 1u) == 0u) {
+                B.esc[g].z = word.x; B.esc[g].w = word.y;
+                return code;
+            }
+            g = (g + 1u) & B.esc_mask;
+        }
+        B.counters[2] = 1u;
+    }
+    return code;
+}
+
+template <bool OCT, bool DICT>
+__device__ __forceinline__ void rms_nbr_emit(uint32_t m, bool ghost, const uint32_t* quad, const rms_dict_build& B, uint32_t lin,
+                                             bool give_up, uint32_t& last_key, uint32_t& last_code,
+                                             typename rms_nbr_word<OCT, DICT>::type& w)
+{
+    if constexpr (!DICT) {
+        rms_nbr_make_word(m, ghost, quad, w);
+    } else {
+        if (m == 0x07FFFFFFu) { w = 0; return; }                      // interior, not a ghost (m carries the ghost flag)
+        if (m != last_key) {
+            if (give_up) { w = (uint16_t)RMS_DICT_ESCAPE; return; }   // the tables are full: the build is being abandoned
+            uint2 word;
+            rms_nbr_make_word(m, ghost, quad, word);
+            last_code = rms_dict_lookup(B, m, word, lin);
+            last_key = m;
+        } else if (last_code == RMS_DICT_ESCAPE) {                    // every escaped voxel has its own entry
+            uint2 word;
+            rms_nbr_make_word(m, ghost, quad, word);
+            last_code = rms_dict_lookup(B, m, word, lin);
+        }
+        w = (uint16_t)last_code;
+    }
+}
+
+template <bool ZFAST, bool OCT, bool DICT = false>
+__global__ void __launch_bounds__(128) rms_build_nbr_kernel(const uint16_t* __restrict__ labels, int nx, int ny, int nz,
+                                                             typename rms_nbr_word<OCT, DICT>::type* __restrict__ nbr, int SX, int SY, int SZ,
+                                                             int n_labels, unsigned long long* __restrict__ stats,
+                                                             const rms_dict_build dictb = rms_dict_build())
+{
+    typedef typename rms_nbr_word<OCT, DICT>::type WORD;
     __shared__ WORD tile[ZFAST ? 4 : 1][ZFAST ? 32 : 1][ZFAST ? 33 : 1];
     __shared__ uint32_t quad[OCT ? 512 : 1];
     if (OCT) {
@@ -139,6 +224,8 @@ __global__ void __launch_bounds__(128) rms_build_nbr_kernel(const uint16_t* __re
         }
         WORD* out = nbr + ((size_t)X * SX + (size_t)Y * SY + (size_t)Z0 * SZ);
         int Z = Z0, zi = 0, zbase = Z0;
+        uint32_t last_key = 0u, last_code = 0u;
+        const bool give_up = DICT && *(volatile uint32_t*)&dictb.counters[2] != 0u;
         // one voxel: read plane z+1 into HI, compare the 27 labels with the centre of MID, write the word
 #define RMS_NBR_ONE(LO, MID, HI)                                                                              \
         if (Z < Z1) {                                                                                         \
@@ -153,7 +240,7 @@ __global__ void __launch_bounds__(128) rms_build_nbr_kernel(const uint16_t* __re
             const bool ghost = ghost_xy | (Z == 0) | (Z == NZ - 1);                                           \
             if (ghost) m |= RMS_NBR_GHOST;                                                                    \
             WORD word;                                                                                        \
-            rms_nbr_make_word(m, ghost, quad, word);                                                          \
+            rms_nbr_emit<OCT, DICT>(m, ghost, quad, dictb, (uint32_t)(X * SX + Y * SY + Z * SZ), give_up, last_key, last_code, word); \
             if (ZFAST) {                                                                                      \
                 tile[warp][zi][lane] = word;                                                                  \
                 if (++zi == 32 || Z == Z1 - 1) {       /* warp-uniform: flush the staged tile, transposed */  \
@@ -266,6 +353,7 @@ extern "C" int rms_substrate_create(const rms_substrate_desc* d, void* cuda_stre
 
     int rc = RMS_OK;
     unsigned long long* d_stats = nullptr;
+    unsigned long long* d_hash = nullptr;              // the dictionary build's hash table and counters
     unsigned long long h_stats[5] = {0, 0, 0, 0, 0};   // membrane faces, bad labels, sampled faces with normal x, y, z
 #define SUB_TRY(expr)                                                                                    \
     do {                                                                                                 \
@@ -302,8 +390,7 @@ extern "C" int rms_substrate_create(const rms_substrate_desc* d, void* cuda_stre
         // a margin on either side: the step kernel asks for the word of the voxel a hop would enter before it knows whether the
         // walker sits on a ghost voxel, whose neighbours may lie outside the padded lattice (the value is never used then)
         s->oct_margin = (size_t)std::max(s->NX * s->NY, s->NY * s->NZ) + (size_t)std::max(s->NX, s->NZ) + 2;
-        SUB_TRY(rms_malloc((void**)&s->d_oct_alloc, ((size_t)s->NX * s->NY * s->NZ + 2 * s->oct_margin) * sizeof(uint2)));
-        s->d_oct = s->d_oct_alloc + s->oct_margin;
+        const size_t n_pad = (size_t)s->NX * s->NY * s->NZ;
         dim3 grid((s->NX + 127) / 128, s->NY, (s->NZ + RMS_NBR_ZCHUNK - 1) / RMS_NBR_ZCHUNK);
         if (grid.y > 65535u || grid.z > 65535u) {
             rms_set_error("lattice too large for the neighbourhood-lattice build (ny+2, nz+2 must be <= 65535)");
@@ -324,11 +411,57 @@ extern "C" int rms_substrate_create(const rms_substrate_desc* d, void* cuda_stre
         }
         if (zfast) { s->SZ = 1; s->SY = s->NZ; s->SX = s->NY * s->NZ; }
         else       { s->SX = 1; s->SY = s->NX; s->SZ = s->NX * s->NY; }
-        if (zfast)
-            rms_build_nbr_kernel<true, true><<<grid, 128, 0, stream>>>(s->d_labels, s->nx, s->ny, s->nz, s->d_oct, s->SX, s->SY, s->SZ, nL, d_stats);
-        else
-            rms_build_nbr_kernel<false, true><<<grid, 128, 0, stream>>>(s->d_labels, s->nx, s->ny, s->nz, s->d_oct, s->SX, s->SY, s->SZ, nL, d_stats);
-        SUB_TRY(cudaGetLastError());
+        bool have_dict = false;
+        if (d->flags & RMS_LATTICE_DICT) {
+            // dictionary lattice: 16-bit codes + the octant words of the distinct neighbourhoods; abandoned for the octant
+            // lattice below if the lattice has more of them than the tables hold (random labels)
+            rms_dict_build B;
+            memset(&B, 0, sizeof B);
+            B.hash_mask = (1u << 18) - 1u;
+            B.dict_cap = RMS_DICT_ESCAPE;
+            if (const char* cap = getenv("RMS_DICT_CAP")) B.dict_cap = (uint32_t)std::min(std::max(atoi(cap), 2), (int)RMS_DICT_ESCAPE);   // tests: force escapes
+            B.esc_mask = (1u << 20) - 1u;
+            B.esc_cap = 1u << 19;
+            uint32_t h_cnt[4] = {0, 0, 0, 0};
+            SUB_TRY(rms_malloc((void**)&s->d_code_alloc, (n_pad + 2 * s->oct_margin) * sizeof(uint16_t)));
+            s->d_code = s->d_code_alloc + s->oct_margin;
+            SUB_TRY(rms_malloc((void**)&s->d_dict, (size_t)RMS_DICT_ESCAPE * sizeof(uint2)));
+            SUB_TRY(rms_malloc((void**)&s->d_esc, ((size_t)B.esc_mask + 1) * sizeof(uint4)));
+            SUB_TRY(rms_malloc((void**)&d_hash, ((size_t)B.hash_mask + 1) * sizeof(unsigned long long) + 4 * sizeof(uint32_t)));
+            B.hash = d_hash; B.counters = (uint32_t*)(d_hash + B.hash_mask + 1);
+            B.dict = s->d_dict; B.esc = s->d_esc;
+            SUB_TRY(cudaMemsetAsync(d_hash, 0, ((size_t)B.hash_mask + 1) * sizeof(unsigned long long) + 4 * sizeof(uint32_t), stream));
+            SUB_TRY(cudaMemsetAsync(s->d_esc, 0, ((size_t)B.esc_mask + 1) * sizeof(uint4), stream));
+            SUB_TRY(cudaMemsetAsync(s->d_dict, 0xFE, sizeof(uint2), stream));        // code 0: the interior voxel's word
+            if (zfast)
+                rms_build_nbr_kernel<true, true, true><<<grid, 128, 0, stream>>>(s->d_labels, s->nx, s->ny, s->nz, s->d_code, s->SX, s->SY, s->SZ, nL, d_stats, B);
+            else
+                rms_build_nbr_kernel<false, true, true><<<grid, 128, 0, stream>>>(s->d_labels, s->nx, s->ny, s->nz, s->d_code, s->SX, s->SY, s->SZ, nL, d_stats, B);
+            SUB_TRY(cudaGetLastError());
+            SUB_TRY(cudaMemcpyAsync(h_cnt, B.counters, sizeof h_cnt, cudaMemcpyDeviceToHost, stream));
+            SUB_TRY(cudaStreamSynchronize(stream));
+            rms_free(d_hash);
+            d_hash = nullptr;
+            if (h_cnt[2] == 0) {
+                have_dict = true;
+                s->esc_mask = B.esc_mask;
+                s->n_dict = std::min(h_cnt[0] + 1u, B.dict_cap);
+                s->n_esc = h_cnt[1];
+            } else {
+                rms_free(s->d_code_alloc); rms_free(s->d_dict); rms_free(s->d_esc);
+                s->d_code_alloc = s->d_code = nullptr; s->d_dict = nullptr; s->d_esc = nullptr;
+                SUB_TRY(cudaMemsetAsync(d_stats, 0, 2 * sizeof(unsigned long long), stream));    // counted again below
+            }
+        }
+        if (!have_dict) {
+            SUB_TRY(rms_malloc((void**)&s->d_oct_alloc, (n_pad + 2 * s->oct_margin) * sizeof(uint2)));
+            s->d_oct = s->d_oct_alloc + s->oct_margin;
+            if (zfast)
+                rms_build_nbr_kernel<true, true><<<grid, 128, 0, stream>>>(s->d_labels, s->nx, s->ny, s->nz, s->d_oct, s->SX, s->SY, s->SZ, nL, d_stats);
+            else
+                rms_build_nbr_kernel<false, true><<<grid, 128, 0, stream>>>(s->d_labels, s->nx, s->ny, s->nz, s->d_oct, s->SX, s->SY, s->SZ, nL, d_stats);
+            SUB_TRY(cudaGetLastError());
+        }
     } else {
         rms_check_labels_kernel<<<148 * 8, 256, 0, stream>>>(s->d_labels, (size_t)n_vox, nL, d_stats);
         SUB_TRY(cudaGetLastError());
@@ -347,6 +480,7 @@ extern "C" int rms_substrate_create(const rms_substrate_desc* d, void* cuda_stre
     return RMS_OK;
 fail:
     if (d_stats) rms_free(d_stats);
+    if (d_hash) rms_free(d_hash);
     rms_substrate_destroy(s);
     return rc;
 #undef SUB_TRY
@@ -358,6 +492,9 @@ extern "C" int rms_substrate_destroy(rms_substrate* s)
     if (s->owns_labels && s->d_labels) rms_free((void*)s->d_labels);
     if (s->d_nbr) rms_free(s->d_nbr);
     if (s->d_oct_alloc) rms_free(s->d_oct_alloc);
+    if (s->d_code_alloc) rms_free(s->d_code_alloc);
+    if (s->d_dict) rms_free(s->d_dict);
+    if (s->d_esc) rms_free(s->d_esc);
     if (s->d_label_class) rms_free(s->d_label_class);
     delete s;
     return RMS_OK;
@@ -507,8 +644,11 @@ extern "C" int rms_substrate_get_info(const rms_substrate* s, rms_substrate_info
     out->n_membrane_faces = s->n_membrane_faces;
     out->lattice_bytes = s->n_vox * sizeof(uint16_t);
     const uint64_t n_pad = (uint64_t)s->NX * s->NY * s->NZ;
-    out->brick_bytes = (s->d_oct ? n_pad * sizeof(uint2) : 0) + (s->d_nbr ? n_pad * sizeof(uint32_t) : 0);
-    out->has_bricks = s->d_oct != nullptr;
+    out->brick_bytes = (s->d_oct ? n_pad * sizeof(uint2) : 0) + (s->d_nbr ? n_pad * sizeof(uint32_t) : 0) +
+                       (s->d_code ? n_pad * sizeof(uint16_t) + (size_t)RMS_DICT_ESCAPE * sizeof(uint2) + ((size_t)s->esc_mask + 1) * sizeof(uint4) : 0);
+    out->has_bricks = s->d_oct != nullptr || s->d_code != nullptr;
+    out->dict_entries = s->n_dict;
+    out->dict_escaped_voxels = s->n_esc;
     return RMS_OK;
 }
 

@@ -7,9 +7,10 @@ TOL_S = 1e-4               # |dS| absolute per b-value and direction (real and i
 TOL_MOMENT = 1e-4          # cumulants / moments, relative
 
 
-def gpu_run(cfg_sub, cfg_seq, n_walkers, seed, first_id=0, flags=0, read_walkers=True):
+def gpu_run(cfg_sub, cfg_seq, n_walkers, seed, first_id=0, flags=0, read_walkers=True, substrate_flags=0):
     import paper_2012_06478_b200 as rms
-    g = rms.simulate(cfg_sub, cfg_seq, n_walkers, seed, first_id=first_id, flags=flags, read_walkers=read_walkers)
+    g = rms.simulate(cfg_sub, cfg_seq, n_walkers, seed, first_id=first_id, flags=flags, read_walkers=read_walkers,
+                     substrate_flags=substrate_flags)
     g["_sub"], g["_seq"] = cfg_sub, cfg_seq          # for the per-walker accounting of compare()
     return g
 
