@@ -152,13 +152,13 @@ __device__ __noinline__ uint32_t rms_dict_lookup(const rms_dict_build& B, uint32
 
 template <bool OCT, bool DICT>
 __device__ __forceinline__ void rms_nbr_emit(uint32_t m, bool ghost, const uint32_t* quad, const rms_dict_build& B, uint32_t lin,
-                                             bool give_up, uint32_t& last_key, uint32_t& last_code,
+                                             bool give_up, bool active, uint32_t& last_key, uint32_t& last_code,
                                              typename rms_nbr_word<OCT, DICT>::type& w)
 {
     if constexpr (!DICT) {
         rms_nbr_make_word(m, ghost, quad, w);
     } else {
-        if (m == 0x07FFFFFFu) { w = 0; return; }                      // interior, not a ghost (m carries the ghost flag)
+        if (m == 0x07FFFFFFu || !active) { w = 0; return; }           // interior, not a ghost (m carries the ghost flag); idle lane
         if (m != last_key) {
             if (give_up) { w = (uint16_t)RMS_DICT_ESCAPE; return; }   // the tables are full: the build is being abandoned
             uint2 word;
@@ -240,7 +240,7 @@ __global__ void __launch_bounds__(128) rms_build_nbr_kernel(const uint16_t* __re
             const bool ghost = ghost_xy | (Z == 0) | (Z == NZ - 1);                                           \
             if (ghost) m |= RMS_NBR_GHOST;                                                                    \
             WORD word;                                                                                        \
-            rms_nbr_emit<OCT, DICT>(m, ghost, quad, dictb, (uint32_t)(X * SX + Y * SY + Z * SZ), give_up, last_key, last_code, word); \
+            rms_nbr_emit<OCT, DICT>(m, ghost, quad, dictb, (uint32_t)(X * SX + Y * SY + Z * SZ), give_up, active, last_key, last_code, word); \
             if (ZFAST) {                                                                                      \
                 tile[warp][zi][lane] = word;                                                                  \
                 if (++zi == 32 || Z == Z1 - 1) {       /* warp-uniform: flush the staged tile, transposed */  \
@@ -420,8 +420,10 @@ extern "C" int rms_substrate_create(const rms_substrate_desc* d, void* cuda_stre
             B.hash_mask = (1u << 18) - 1u;
             B.dict_cap = RMS_DICT_ESCAPE;
             if (const char* cap = getenv("RMS_DICT_CAP")) B.dict_cap = (uint32_t)std::min(std::max(atoi(cap), 2), (int)RMS_DICT_ESCAPE);   // tests: force escapes
-            B.esc_mask = (1u << 20) - 1u;
-            B.esc_cap = 1u << 19;
+            uint32_t esc_slots = 4096u;                                    // one slot per 8 voxels, 2^12 .. 2^20, half of them usable
+            while (esc_slots < (1u << 20) && (size_t)esc_slots * 8 < n_pad) esc_slots <<= 1;
+            B.esc_mask = esc_slots - 1u;
+            B.esc_cap = esc_slots / 2u;
             uint32_t h_cnt[4] = {0, 0, 0, 0};
             SUB_TRY(rms_malloc((void**)&s->d_code_alloc, (n_pad + 2 * s->oct_margin) * sizeof(uint16_t)));
             s->d_code = s->d_code_alloc + s->oct_margin;

@@ -356,6 +356,75 @@ def test_full_size_bench_workload_against_the_oracle(rms):
     assert g["n_launches"] >= 5 and g["kernel_ms"] > 0
 
 
+def _same_trajectories(a, b, tag, exact_relax=True):
+    """Two runs of the CUDA path that must have walked the same trajectories: positions, labels and counts bit for bit; the
+    phase and signal sums may differ by the order of their fp64 additions only."""
+    wa, wb = a["walkers"], b["walkers"]
+    for k in ("vox", "off", "label") + (("relax",) if exact_relax else ()):
+        assert np.array_equal(wa[k], wb[k]), (tag, k)
+    assert np.allclose(wa["relax"], wb["relax"], rtol=0, atol=2e-8), tag
+    assert a["n_encounters"] == b["n_encounters"] and a["n_permeations"] == b["n_permeations"], tag
+    scale = max(1e-30, float(np.abs(wa["phi"]).max()))
+    assert float(np.abs(wa["phi"] - wb["phi"]).max()) <= 1e-11 * scale, tag
+    # (relaxation sums that differ in their last fp32 bit move the weights alpha = exp(-relax) by 1e-8)
+    assert float(np.abs(a["S"] - b["S"]).max()) <= (1e-10 if exact_relax else 1e-7), tag
+    rtol = 1e-12 if exact_relax else 1e-7
+    assert np.allclose(a["m2"], b["m2"], rtol=rtol) and np.allclose(a["m4"], b["m4"], rtol=rtol), tag
+
+
+def test_time_slices_of_the_specialised_kernel_leave_the_trajectories_alone(rms):
+    """rms_step_fast.cu cuts the last one to two waves of blocks of a launch into time slices dealt from a queue.  Enough
+    walkers for a whole-range wave and a sliced part (782 groups of 512), a launch long enough to be sliced (4 slices, the
+    last one ragged, odd step count): the same run with RMS_RUN_NO_SLICES must end in the same place, fp32 and fp64,
+    impermeable and permeable (whose relaxation sums are added slice by slice: fp32 rounding), octant and dictionary
+    lattice; and the sliced permeable run holds north_star's tolerances against the oracle."""
+    NO_SLICES, DICT = rms.binding.RMS_RUN_NO_SLICES, rms.binding.RMS_LATTICE_DICT
+    n = 400_001
+    c2, c3 = ri.make_config("cfg2", "test"), ri.make_config("cfg3", "test")
+    seq = ri.pgse_sequence(2e-4, 4101, 0.2, 0.5, np.linspace(0.0, 4.0, 4), ri.fibonacci_dirs(6), snap_steps=[4101])
+    for name, sub in (("cfg2", c2.substrate), ("cfg3", c3.substrate)):
+        for flags in (0, 8):
+            for sf in (0, DICT):
+                whole = gpu_run(sub, seq, n, 11, flags=flags | NO_SLICES, substrate_flags=sf)
+                sliced = gpu_run(sub, seq, n, 11, flags=flags, substrate_flags=sf)
+                _same_trajectories(whole, sliced, (name, flags, sf), exact_relax=(name == "cfg2"))
+                if name == "cfg3" and flags == 0 and sf == 0:
+                    print("sliced cfg3 against the oracle", compare(sliced, oracle_run(sub, seq, n, 11), n))
+
+
+@pytest.mark.parametrize("dict_cap", [None, "40", "3"], ids=["full_dictionary", "escapes", "gives_up"])
+def test_dictionary_lattice_walks_the_trajectories_of_the_octant_lattice(rms, monkeypatch, dict_cap):
+    """RMS_LATTICE_DICT stores a 16-bit code per voxel and the octant words of the distinct neighbourhoods once; the words a
+    walker reads are the same, so the trajectories are those of the octant lattice bit for bit: axons (impermeable,
+    permeable), a cylinder, independent random labels, a one-voxel-wide box, both memory orders, fp32 and fp64 directions.
+    RMS_DICT_CAP (a test hook of rms_substrate_create) shrinks the dictionary: 40 codes push most boundary voxels into the
+    escape table; with 3 codes that table overflows too on some of the lattices and the build falls back to the octant lattice."""
+    DICT = rms.binding.RMS_LATTICE_DICT
+    if dict_cap:
+        monkeypatch.setenv("RMS_DICT_CAP", dict_cap)
+    c2, c3, c0 = ri.make_config("cfg2", "test"), ri.make_config("cfg3", "test"), ri.make_config("cfg0")
+    seq_r = ri.pgse_sequence(2e-4, 400, 0.02, 0.04, [0.0, 20.0], np.eye(3), snap_steps=[400])
+    cases = [("cfg2", c2.substrate, c2.sequence, 20_000), ("cfg3", c3.substrate, c3.sequence, 20_000),
+             ("cfg0", c0.substrate, c0.sequence, 5_000),
+             ("random", ri.random_lattice((12, 11, 10), n_labels=3, seed=9, place="all"), seq_r, 5_000),
+             ("1x1x9", ri.random_lattice((1, 1, 9), n_labels=2, seed=2, place="all"), seq_r, 2_000)]
+    seen = set()
+    for name, sub, seq, n in cases:
+        for layout in (rms.binding.RMS_LAYOUT_X_FASTEST, rms.binding.RMS_LAYOUT_Z_FASTEST):
+            for flags in (0, 8):
+                a = gpu_run(sub, seq, n, 5, flags=flags, substrate_flags=layout)
+                b = gpu_run(sub, seq, n, 5, flags=flags, substrate_flags=layout | DICT)
+                _same_trajectories(a, b, (name, layout, flags))
+                info = b["substrate_info"]
+                assert a["substrate_info"]["dict_entries"] == 0 and info["has_bricks"] == 1
+                seen.add("octant" if info["dict_entries"] == 0 else ("escapes" if info["dict_escaped_voxels"] else "dictionary"))
+                if dict_cap is None:
+                    assert info["dict_entries"] > 1 and info["dict_escaped_voxels"] == 0
+                    assert info["brick_bytes"] < a["substrate_info"]["brick_bytes"] or info["n_voxels"] < 100_000
+    print("lattices in use", sorted(seen))
+    assert {None: seen == {"dictionary"}, "40": "escapes" in seen, "3": "octant" in seen}[dict_cap]
+
+
 def test_general_kernel_and_id_order_agree_with_the_specialised_path(rms):
     # same inputs through the general step kernel and without spatial ordering: identical physics, so the results
     # agree with the oracle under the same tolerances, and with each other to rounding
