@@ -37,12 +37,13 @@ ALGORITHMIC_INSTR_PER_STEP = 80.0
 N_SM, LANES_PER_SM = 148, 128          # B200: 4 schedulers x 32 lanes per SM, one warp instruction per clock each
 # DRAM traffic of the step kernel per launch (dram__bytes_read.sum + dram__bytes_write.sum of one `ncu --set full` capture),
 # by the configuration that was captured; a run of any other configuration reports traffic = null.
-# key: (substrate, lattice, layout, walkers, mc_steps, fp64)
+# key: (substrate, lattice, layout, lattice_format, walkers, mc_steps, fp64)
 NCU_CAPTURES = {
-    ("cfg4", "facemask", "x", 1_000_000, 10_000, False): {"bytes": 68.68e9, "source": "profiles/r2d_step_fast_ncu.md (68.08 GB read + 0.60 GB written)"},
     # RMS_LAYOUT_AUTO picks z fastest on this lattice: the two keys name the same launch
-    ("cfg4", "facemask", "auto", 1_000_000, 10_000, False): {"bytes": 32.35e9, "source": "profiles/r2e_step_fast_ncu.md (31.75 GB read + 0.59 GB written)"},
-    ("cfg4", "facemask", "z", 1_000_000, 10_000, False): {"bytes": 32.35e9, "source": "profiles/r2e_step_fast_ncu.md (31.75 GB read + 0.59 GB written)"},
+    ("cfg4", "facemask", "auto", "oct", 1_000_000, 10_000, False): {"bytes": 45.94e9, "source": "profiles/r2f_r2g_step_fast_ncu.md, capture f (44.52 GB read + 1.43 GB written)"},
+    ("cfg4", "facemask", "z", "oct", 1_000_000, 10_000, False): {"bytes": 45.94e9, "source": "profiles/r2f_r2g_step_fast_ncu.md, capture f (44.52 GB read + 1.43 GB written)"},
+    ("cfg4", "facemask", "auto", "dict", 1_000_000, 10_000, False): {"bytes": 10.12e9, "source": "profiles/r2f_r2g_step_fast_ncu.md, capture g (8.81 GB read + 1.31 GB written)"},
+    ("cfg4", "facemask", "z", "dict", 1_000_000, 10_000, False): {"bytes": 10.12e9, "source": "profiles/r2f_r2g_step_fast_ncu.md, capture g (8.81 GB read + 1.31 GB written)"},
 }
 
 
@@ -378,7 +379,7 @@ def main():
     peak_ginstr = N_SM * LANES_PER_SM * sm_mhz * 1e6 / 1e9
     k_ms_per_launch = kernel_ms / args.steps
     achieved_ginstr = ALGORITHMIC_INSTR_PER_STEP * n_walkers * mc_steps / (k_ms_per_launch * 1e-3) / 1e9
-    cap = NCU_CAPTURES.get((args.substrate, args.lattice, args.layout, n_walkers, mc_steps, bool(args.fp64))) if args.waves == 1 else None
+    cap = NCU_CAPTURES.get((args.substrate, args.lattice, args.layout, args.lattice_format, n_walkers, mc_steps, bool(args.fp64))) if args.waves == 1 else None
     traffic = cap["bytes"] if cap else None
     roofline = {"bound": "alu", "kernel": "rms_step_fast_kernel" if args.lattice == "facemask" else "rms_step_kernel",
                 "achieved": achieved_ginstr, "peak": peak_ginstr,

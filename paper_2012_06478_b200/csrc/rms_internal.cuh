@@ -69,12 +69,13 @@ struct rms_substrate {
     bool want_bricks = false;            // RMS_NO_BRICKS not given: d_nbr may be built on demand
     // dictionary lattice (RMS_LATTICE_DICT; instead of d_oct): one 16-bit code per padded voxel, same geometry, strides and
     // margin; d_dict[code] = the voxel's octant word.  Code 0 = interior voxel (all 26 neighbours carry its label), codes
-    // 1 .. RMS_DICT_ESCAPE - 1 in the order the build met the neighbourhoods, RMS_DICT_ESCAPE = the lattice has more distinct
-    // neighbourhoods than codes: the word of such a voxel is in the hash table d_esc, keyed by its padded index + 1
-    // (slot = {key, 0, word.x, word.y}, linear probing from rms_esc_hash(index) & esc_mask).
+    // below RMS_DICT_FIXED the prismatic neighbourhoods (rms_fixed_code), codes RMS_DICT_FIXED .. RMS_DICT_TODO - 1 in the order the
+    // build met the other neighbourhoods, RMS_DICT_ESCAPE = the lattice has more distinct neighbourhoods than codes: the word
+    // of such a voxel is in the hash table d_esc, keyed by its padded index + 1 (slot = {key, 0, word.x, word.y}, linear
+    // probing from rms_esc_hash(index) & esc_mask); d_dict[RMS_DICT_ESCAPE] carries the ghost flag (rms_step_fast.cu).
     uint16_t* d_code = nullptr;
     uint16_t* d_code_alloc = nullptr;
-    uint2* d_dict = nullptr;             // [RMS_DICT_ESCAPE]
+    uint2* d_dict = nullptr;             // [RMS_DICT_ESCAPE + 1]
     uint4* d_esc = nullptr;
     uint32_t esc_mask = 0, n_dict = 0, n_esc = 0;
     // memory order of the neighbourhood lattice: index = X SX + Y SY + Z SZ over the padded coordinates.  The axis with
@@ -194,9 +195,55 @@ enum { RMS_LAT_LABELS = 0, RMS_LAT_FACES = 1 };
 #define RMS_NBR_GHOST (1u << 27)
 #define RMS_NBR_SELF 13
 #define RMS_DICT_ESCAPE 0xFFFFu
+#define RMS_DICT_TODO 0xFFFEu           // not a code (reserved)
 #define RMS_OCT_INTERIOR 0xFEFEFEFEu     // both halves of the octant word of an interior voxel
+#define RMS_DICT_FIXED 2048u              // codes below this are fixed: interior, prismatic neighbourhoods, and their ghost variants
+#define RMS_DICT_NONE 0xFFFFFFFFu
 #ifdef __CUDACC__
 __host__ __device__ __forceinline__ uint32_t rms_esc_hash(uint32_t lin) { return (lin * 0x9E3779B1u) >> 8; }
+// Codes that need no search.  0: the interior voxel (all 27 same-label bits set).  Prismatic neighbourhoods: the 27 bits do not
+// change along one lattice axis (the wall of a cell that runs along that axis: 9 in 10 boundary voxels of an axon lattice);
+// they get 1 + 256 f + pat8, f = 0 / 1 / 2 for the axis z / y / x, pat8 = the 8 neighbour bits of the 3 x 3 cross-section
+// (centre, always 1, left out).  Ghost voxels (RMS_NBR_GHOST set): the same + 1024.  RMS_DICT_NONE for any other word.
+__host__ __device__ __forceinline__ uint32_t rms_fixed_code(uint32_t word)
+{
+    const uint32_t g = (word >> 27) ? 1024u : 0u, m = word & 0x07FFFFFFu;
+    if (m == 0x07FFFFFFu) return g;
+    const uint32_t p0 = m & 511u, p1 = (m >> 9) & 511u, p2 = m >> 18;        // planes dz = -1, 0, +1
+    uint32_t q, f;
+    if (p0 == p1 && p2 == p1) { q = p1; f = 0u; }
+    else {
+        const uint32_t r0 = m & 0x01C0E07u, r1 = (m >> 3) & 0x01C0E07u, r2 = (m >> 6) & 0x01C0E07u;   // rows dy = -1, 0, +1 of the planes
+        if (r0 == r1 && r2 == r1) { q = (r1 & 7u) | ((r1 >> 6) & 0x38u) | ((r1 >> 12) & 0x1C0u); f = 1u; }
+        else {
+            const uint32_t a = m & 0x1249249u, b = (m >> 1) & 0x1249249u, c = (m >> 2) & 0x1249249u;  // dx = -1, 0, +1 of the rows
+            if (a != b || c != b) return RMS_DICT_NONE;
+            q = 0u;
+#pragma unroll
+            for (int k = 0; k < 9; ++k) q |= ((b >> (3 * k)) & 1u) << k;
+            f = 2u;
+        }
+    }
+    return g + 1u + 256u * f + ((q & 15u) | ((q >> 5) << 4));
+}
+// the neighbourhood word of a fixed code: 0, 1 .. 768, 1024, 1025 .. 1792 (0 for the unused codes in between)
+__host__ __device__ __forceinline__ uint32_t rms_fixed_word(uint32_t code)
+{
+    const uint32_t g = code >= 1024u ? RMS_NBR_GHOST : 0u;
+    code &= 1023u;
+    if (code == 0u) return g | 0x07FFFFFFu;
+    if (code > 768u) return 0u;
+    const uint32_t f = (code - 1u) >> 8, pat = (code - 1u) & 255u;
+    const uint32_t q = (pat & 15u) | 16u | ((pat >> 4) << 5);
+    uint32_t m = 0u;
+    if (f == 0u) m = q | (q << 9) | (q << 18);
+    else if (f == 1u) {
+        for (int dz = 0; dz < 3; ++dz) { const uint32_t r = (q >> (3 * dz)) & 7u; m |= (r | (r << 3) | (r << 6)) << (9 * dz); }
+    } else {
+        for (int k = 0; k < 9; ++k) if ((q >> k) & 1u) m |= 7u << (3 * k);
+    }
+    return g | m;
+}
 #endif
 
 struct rms_step_params {

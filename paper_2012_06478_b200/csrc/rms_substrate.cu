@@ -101,11 +101,12 @@ struct rms_dict_build {
     unsigned long long* hash;
     uint32_t hash_mask;
     uint2* dict;
-    uint32_t dict_cap;          // codes 1 .. dict_cap - 1 are handed out, then RMS_DICT_ESCAPE
+    uint32_t dict_cap;          // codes RMS_DICT_FIXED .. dict_cap - 1 are handed out, then RMS_DICT_ESCAPE
     uint4* esc;
     uint32_t esc_mask, esc_cap;
     uint32_t* counters;         // [0] neighbourhoods met, [1] escaped voxels, [2] gave up (tables full)
 };
+#define RMS_DICT_CACHE 2048u      // entries of a block's shared-memory cache of the hash table (key | code << 32)
 
 __device__ __noinline__ uint32_t rms_dict_lookup(const rms_dict_build& B, uint32_t key, uint2 word, uint32_t lin)
 {
@@ -118,7 +119,7 @@ __device__ __noinline__ uint32_t rms_dict_lookup(const rms_dict_build& B, uint32
         if (cur == 0ull) {
             cur = atomicCAS((unsigned long long*)slot, 0ull, (unsigned long long)key);
             if (cur == 0ull) {                                        // claimed: hand out the code, publish it
-                const uint32_t idx = atomicAdd(&B.counters[0], 1u) + 1u;
+                const uint32_t idx = atomicAdd(&B.counters[0], 1u) + RMS_DICT_FIXED;   // below: interior and prismatic codes
                 code = idx < B.dict_cap ? idx : RMS_DICT_ESCAPE;
                 if (code != RMS_DICT_ESCAPE) B.dict[code] = word;
                 __threadfence();
@@ -151,24 +152,32 @@ __device__ __noinline__ uint32_t rms_dict_lookup(const rms_dict_build& B, uint32
 }
 
 template <bool OCT, bool DICT>
-__device__ __forceinline__ void rms_nbr_emit(uint32_t m, bool ghost, const uint32_t* quad, const rms_dict_build& B, uint32_t lin,
-                                             bool give_up, bool active, uint32_t& last_key, uint32_t& last_code,
+__device__ __forceinline__ void rms_nbr_emit(uint32_t m, bool ghost, const uint32_t* quad, const rms_dict_build& B, uint32_t lin, bool active,
+                                             bool give_up, unsigned long long* cache, uint32_t& last_key, uint32_t& last_code,
                                              typename rms_nbr_word<OCT, DICT>::type& w)
 {
     if constexpr (!DICT) {
         rms_nbr_make_word(m, ghost, quad, w);
     } else {
-        if (m == 0x07FFFFFFu || !active) { w = 0; return; }           // interior, not a ghost (m carries the ghost flag); idle lane
-        if (m != last_key) {
+        // interior (m carries the ghost flag, so not a ghost) -> 0; prismatic -> its fixed code (a third of the boundary voxels
+        // of an axon lattice); the rest: the neighbourhood this thread looked up last (cells run along its column), the block's
+        // shared-memory cache of the hash table, the hash table (its latency, met at 1 voxel in 14, doubled the time of the
+        // build before the cache)
+        if (m == 0x07FFFFFFu || !active) { w = 0; return; }
+        const uint32_t pc = rms_fixed_code(m);
+        if (pc != RMS_DICT_NONE) { w = (uint16_t)pc; return; }
+        if (m != last_key || last_code == RMS_DICT_ESCAPE) {          // every escaped voxel has its own entry
             if (give_up) { w = (uint16_t)RMS_DICT_ESCAPE; return; }   // the tables are full: the build is being abandoned
-            uint2 word;
-            rms_nbr_make_word(m, ghost, quad, word);
-            last_code = rms_dict_lookup(B, m, word, lin);
+            const uint32_t c = ((m * 0x9E3779B1u) >> 7) & (RMS_DICT_CACHE - 1u);
+            const unsigned long long hit = cache[c];
+            if ((uint32_t)hit == m) last_code = (uint32_t)(hit >> 32);
+            else {
+                uint2 word;
+                rms_nbr_make_word(m, ghost, quad, word);
+                last_code = rms_dict_lookup(B, m, word, lin);
+                if (last_code != RMS_DICT_ESCAPE) cache[c] = (unsigned long long)m | ((unsigned long long)last_code << 32);
+            }
             last_key = m;
-        } else if (last_code == RMS_DICT_ESCAPE) {                    // every escaped voxel has its own entry
-            uint2 word;
-            rms_nbr_make_word(m, ghost, quad, word);
-            last_code = rms_dict_lookup(B, m, word, lin);
         }
         w = (uint16_t)last_code;
     }
@@ -183,6 +192,9 @@ __global__ void __launch_bounds__(128) rms_build_nbr_kernel(const uint16_t* __re
     typedef typename rms_nbr_word<OCT, DICT>::type WORD;
     __shared__ WORD tile[ZFAST ? 4 : 1][ZFAST ? 32 : 1][ZFAST ? 33 : 1];
     __shared__ uint32_t quad[OCT ? 512 : 1];
+    __shared__ unsigned long long cache[DICT ? RMS_DICT_CACHE : 1];   // DICT: recent (neighbourhood word, code) pairs
+    if (DICT)
+        for (int t = threadIdx.x; t < (int)RMS_DICT_CACHE; t += blockDim.x) cache[t] = 0ull;   // (OCT is set with DICT: the barrier below)
     if (OCT) {
         for (int t = threadIdx.x; t < 512; t += blockDim.x) {
             uint32_t v = 0;
@@ -226,6 +238,7 @@ __global__ void __launch_bounds__(128) rms_build_nbr_kernel(const uint16_t* __re
         int Z = Z0, zi = 0, zbase = Z0;
         uint32_t last_key = 0u, last_code = 0u;
         const bool give_up = DICT && *(volatile uint32_t*)&dictb.counters[2] != 0u;
+
         // one voxel: read plane z+1 into HI, compare the 27 labels with the centre of MID, write the word
 #define RMS_NBR_ONE(LO, MID, HI)                                                                              \
         if (Z < Z1) {                                                                                         \
@@ -240,7 +253,7 @@ __global__ void __launch_bounds__(128) rms_build_nbr_kernel(const uint16_t* __re
             const bool ghost = ghost_xy | (Z == 0) | (Z == NZ - 1);                                           \
             if (ghost) m |= RMS_NBR_GHOST;                                                                    \
             WORD word;                                                                                        \
-            rms_nbr_emit<OCT, DICT>(m, ghost, quad, dictb, (uint32_t)(X * SX + Y * SY + Z * SZ), give_up, active, last_key, last_code, word); \
+            rms_nbr_emit<OCT, DICT>(m, ghost, quad, dictb, (uint32_t)(X * SX + Y * SY + Z * SZ), active, give_up, cache, last_key, last_code, word); \
             if (ZFAST) {                                                                                      \
                 tile[warp][zi][lane] = word;                                                                  \
                 if (++zi == 32 || Z == Z1 - 1) {       /* warp-uniform: flush the staged tile, transposed */  \
@@ -277,6 +290,32 @@ __global__ void __launch_bounds__(128) rms_build_nbr_kernel(const uint16_t* __re
         if (n_faces) atomicAdd(&stats[0], (unsigned long long)n_faces);
         if (bad) atomicAdd(&stats[1], (unsigned long long)bad);
     }
+}
+
+// the fixed part of the dictionary: code 0 (interior), the prismatic codes, their ghost variants, and -- so that the step kernel needs no test
+// for it before the look-up -- the escape code, whose entry carries the ghost flag and so sends the walker to the rare path
+__global__ void __launch_bounds__(256) rms_dict_init_kernel(uint2* __restrict__ dict)
+{
+    __shared__ uint32_t quad[512];
+    for (int t = threadIdx.x; t < 512; t += blockDim.x) {
+        uint32_t v = 0;
+        for (int q = 0; q < 4; ++q) {
+            const int sx = (q & 2) ? -1 : 1, sy = (q & 1) ? -1 : 1;
+            for (int xy = 0; xy < 4; ++xy) {
+                const int dx = (xy >> 1) * sx, dy = (xy & 1) * sy;
+                v |= ((t >> ((dx + 1) + 3 * (dy + 1))) & 1u) << (8 * q + 2 * xy);
+            }
+        }
+        quad[t] = v;
+    }
+    __syncthreads();
+    for (uint32_t code = threadIdx.x; code < RMS_DICT_FIXED; code += blockDim.x) {
+        uint2 w = make_uint2(0u, 0u);
+        const uint32_t m = rms_fixed_word(code);
+        if (m) rms_nbr_make_word(m, (m & RMS_NBR_GHOST) != 0u, quad, w);
+        dict[code] = w;
+    }
+    if (threadIdx.x == 0) dict[RMS_DICT_ESCAPE] = make_uint2(0x01010101u, 0x01010101u);
 }
 
 // label check + membrane count without building the face lattice (RMS_NO_BRICKS)
@@ -389,7 +428,7 @@ extern "C" int rms_substrate_create(const rms_substrate_desc* d, void* cuda_stre
         s->NX = s->nx + 2; s->NY = s->ny + 2; s->NZ = s->nz + 2;
         // a margin on either side: the step kernel asks for the word of the voxel a hop would enter before it knows whether the
         // walker sits on a ghost voxel, whose neighbours may lie outside the padded lattice (the value is never used then)
-        s->oct_margin = (size_t)std::max(s->NX * s->NY, s->NY * s->NZ) + (size_t)std::max(s->NX, s->NZ) + 2;
+        s->oct_margin = ((size_t)std::max(s->NX * s->NY, s->NY * s->NZ) + (size_t)std::max(s->NX, s->NZ) + 2 + 7) / 8 * 8;   // (16-byte steps)
         const size_t n_pad = (size_t)s->NX * s->NY * s->NZ;
         dim3 grid((s->NX + 127) / 128, s->NY, (s->NZ + RMS_NBR_ZCHUNK - 1) / RMS_NBR_ZCHUNK);
         if (grid.y > 65535u || grid.z > 65535u) {
@@ -418,8 +457,9 @@ extern "C" int rms_substrate_create(const rms_substrate_desc* d, void* cuda_stre
             rms_dict_build B;
             memset(&B, 0, sizeof B);
             B.hash_mask = (1u << 18) - 1u;
-            B.dict_cap = RMS_DICT_ESCAPE;
-            if (const char* cap = getenv("RMS_DICT_CAP")) B.dict_cap = (uint32_t)std::min(std::max(atoi(cap), 2), (int)RMS_DICT_ESCAPE);   // tests: force escapes
+            B.dict_cap = RMS_DICT_TODO;
+            if (const char* cap = getenv("RMS_DICT_CAP"))                  // tests: force escapes
+                B.dict_cap = (uint32_t)std::min(std::max(atoi(cap) + (int)RMS_DICT_FIXED, (int)RMS_DICT_FIXED), (int)RMS_DICT_TODO);
             uint32_t esc_slots = 4096u;                                    // one slot per 8 voxels, 2^12 .. 2^20, half of them usable
             while (esc_slots < (1u << 20) && (size_t)esc_slots * 8 < n_pad) esc_slots <<= 1;
             B.esc_mask = esc_slots - 1u;
@@ -427,14 +467,15 @@ extern "C" int rms_substrate_create(const rms_substrate_desc* d, void* cuda_stre
             uint32_t h_cnt[4] = {0, 0, 0, 0};
             SUB_TRY(rms_malloc((void**)&s->d_code_alloc, (n_pad + 2 * s->oct_margin) * sizeof(uint16_t)));
             s->d_code = s->d_code_alloc + s->oct_margin;
-            SUB_TRY(rms_malloc((void**)&s->d_dict, (size_t)RMS_DICT_ESCAPE * sizeof(uint2)));
+            SUB_TRY(rms_malloc((void**)&s->d_dict, ((size_t)RMS_DICT_ESCAPE + 1) * sizeof(uint2)));
             SUB_TRY(rms_malloc((void**)&s->d_esc, ((size_t)B.esc_mask + 1) * sizeof(uint4)));
             SUB_TRY(rms_malloc((void**)&d_hash, ((size_t)B.hash_mask + 1) * sizeof(unsigned long long) + 4 * sizeof(uint32_t)));
             B.hash = d_hash; B.counters = (uint32_t*)(d_hash + B.hash_mask + 1);
             B.dict = s->d_dict; B.esc = s->d_esc;
             SUB_TRY(cudaMemsetAsync(d_hash, 0, ((size_t)B.hash_mask + 1) * sizeof(unsigned long long) + 4 * sizeof(uint32_t), stream));
             SUB_TRY(cudaMemsetAsync(s->d_esc, 0, ((size_t)B.esc_mask + 1) * sizeof(uint4), stream));
-            SUB_TRY(cudaMemsetAsync(s->d_dict, 0xFE, sizeof(uint2), stream));        // code 0: the interior voxel's word
+            rms_dict_init_kernel<<<1, 256, 0, stream>>>(s->d_dict);
+            SUB_TRY(cudaGetLastError());
             if (zfast)
                 rms_build_nbr_kernel<true, true, true><<<grid, 128, 0, stream>>>(s->d_labels, s->nx, s->ny, s->nz, s->d_code, s->SX, s->SY, s->SZ, nL, d_stats, B);
             else
@@ -447,7 +488,7 @@ extern "C" int rms_substrate_create(const rms_substrate_desc* d, void* cuda_stre
             if (h_cnt[2] == 0) {
                 have_dict = true;
                 s->esc_mask = B.esc_mask;
-                s->n_dict = std::min(h_cnt[0] + 1u, B.dict_cap);
+                s->n_dict = std::min(h_cnt[0] + RMS_DICT_FIXED, B.dict_cap);
                 s->n_esc = h_cnt[1];
             } else {
                 rms_free(s->d_code_alloc); rms_free(s->d_dict); rms_free(s->d_esc);
@@ -647,7 +688,7 @@ extern "C" int rms_substrate_get_info(const rms_substrate* s, rms_substrate_info
     out->lattice_bytes = s->n_vox * sizeof(uint16_t);
     const uint64_t n_pad = (uint64_t)s->NX * s->NY * s->NZ;
     out->brick_bytes = (s->d_oct ? n_pad * sizeof(uint2) : 0) + (s->d_nbr ? n_pad * sizeof(uint32_t) : 0) +
-                       (s->d_code ? n_pad * sizeof(uint16_t) + (size_t)RMS_DICT_ESCAPE * sizeof(uint2) + ((size_t)s->esc_mask + 1) * sizeof(uint4) : 0);
+                       (s->d_code ? n_pad * sizeof(uint16_t) + ((size_t)RMS_DICT_ESCAPE + 1) * sizeof(uint2) + ((size_t)s->esc_mask + 1) * sizeof(uint4) : 0);
     out->has_bricks = s->d_oct != nullptr || s->d_code != nullptr;
     out->dict_entries = s->n_dict;
     out->dict_escaped_voxels = s->n_esc;
