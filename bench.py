@@ -248,25 +248,27 @@ def run_sweep(args):
         dt = base.sequence.dt_ms
         seq = ri.pgse_sequence(dt, args.mc_steps, 0.4 * args.mc_steps * dt, 0.6 * args.mc_steps * dt, b, dirs,
                                snap_steps=[args.mc_steps])
-        for lattice, flags in (("facemask", 0), ("labels", rms.RMS_RUN_LABEL_GATHER)):
+        layout = {"auto": rms.binding.RMS_LAYOUT_AUTO, "x": rms.binding.RMS_LAYOUT_X_FASTEST, "z": rms.binding.RMS_LAYOUT_Z_FASTEST}[args.layout]
+        for lattice, flags, sflags in (("facemask", 0, layout), ("facemask, dictionary lattice", 0, layout | rms.binding.RMS_LATTICE_DICT),
+                                       ("labels", rms.RMS_RUN_LABEL_GATHER, layout)):
             for n_w in (100_000, 1_000_000, 10_000_000, 100_000_000):
                 if n_w > args.sweep_max_walkers:
                     continue
                 reps = 3 if n_w <= 1_000_000 else 1
-                rms.simulate(sub, seq, min(n_w, 1_000_000), base.seed, flags=flags, device_labels=labels_dev)   # warm-up
+                rms.simulate(sub, seq, min(n_w, 1_000_000), base.seed, flags=flags, substrate_flags=sflags, device_labels=labels_dev)   # warm-up
                 e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
                 torch.cuda.synchronize()
                 e0.record(stream)
                 k_ms = 0.0
                 for _ in range(reps):
-                    r = rms.simulate(sub, seq, n_w, base.seed, flags=flags, device_labels=labels_dev)
+                    r = rms.simulate(sub, seq, n_w, base.seed, flags=flags, substrate_flags=sflags, device_labels=labels_dev)
                     k_ms += r["kernel_ms"]
                 e1.record(stream)
                 torch.cuda.synchronize()
                 ms = e0.elapsed_time(e1) / reps
                 steps = float(n_w) * args.mc_steps
                 print(json.dumps({"sweep": "cfg4", "walkers": n_w, "mc_steps": args.mc_steps, "directions": n_dir,
-                                  "b_values": int(seq.gamp.shape[1]), "lattice_path": lattice, "pass_ms": ms,
+                                  "b_values": int(seq.gamp.shape[1]), "lattice_path": lattice, "layout": args.layout, "pass_ms": ms,
                                   "step_kernel_ms": k_ms / reps, "walker_steps_per_s": steps / (ms * 1e-3),
                                   "step_kernel_walker_steps_per_s": steps / (k_ms / reps * 1e-3),
                                   "issue_roofline_frac": ALGORITHMIC_INSTR_PER_STEP * steps / (k_ms / reps * 1e-3) /
