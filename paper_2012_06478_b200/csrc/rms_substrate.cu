@@ -441,7 +441,7 @@ extern "C" int rms_substrate_create(const rms_substrate_desc* d, void* cuda_stre
         // z, such as axons, give z); a sample of the lattice decides
         bool zfast = (d->flags & RMS_LAYOUT_AUTO) == RMS_LAYOUT_Z_FASTEST;
         if ((d->flags & RMS_LAYOUT_AUTO) == RMS_LAYOUT_AUTO) {
-            const int sy = s->ny >= 64 ? 4 : 1, sz = s->nz >= 64 ? 4 : 1;
+            const int sy = s->ny >= 256 ? 8 : (s->ny >= 64 ? 4 : 1), sz = s->nz >= 256 ? 8 : (s->nz >= 64 ? 4 : 1);
             rms_sample_faces_kernel<<<148 * 4, 256, 0, stream>>>(s->d_labels, s->nx, s->ny, s->nz, sy, sz, d_stats + 2);
             SUB_TRY(cudaGetLastError());
             SUB_TRY(cudaMemcpyAsync(h_stats + 2, d_stats + 2, 3 * sizeof(unsigned long long), cudaMemcpyDeviceToHost, stream));
