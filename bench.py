@@ -67,6 +67,7 @@ def parse_args():
     ap.add_argument("--substrate", default="cfg4", choices=["cfg4", "cfg3"],
                     help="cfg3: the permeable, D- and T2-contrast variant of the lattice with walkers in every label (not the headline)")
     ap.add_argument("--fp64", action="store_true", help="RMS_RUN_FP64: the step kernel in fp64 arithmetic (not the headline)")
+    ap.add_argument("--no-slices", action="store_true", help="RMS_RUN_NO_SLICES: one block per group of walkers for the whole launch (diagnostic)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--cpu-sample-walkers", type=int, default=250_000)
@@ -305,6 +306,8 @@ def main():
     flags = rms.RMS_RUN_LABEL_GATHER if args.lattice == "labels" else 0
     if args.fp64:
         flags |= rms.binding.RMS_RUN_FP64
+    if args.no_slices:
+        flags |= rms.binding.RMS_RUN_NO_SLICES
     sflags = {"auto": rms.binding.RMS_LAYOUT_AUTO, "x": rms.binding.RMS_LAYOUT_X_FASTEST, "z": rms.binding.RMS_LAYOUT_Z_FASTEST}[args.layout]
     if args.lattice_format == "dict":
         sflags |= rms.binding.RMS_LATTICE_DICT
