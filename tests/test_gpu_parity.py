@@ -374,14 +374,14 @@ def _same_trajectories(a, b, tag, exact_relax=True):
 
 def test_time_slices_of_the_specialised_kernel_leave_the_trajectories_alone(rms):
     """rms_step_fast.cu cuts the last one to two waves of blocks of a launch into time slices dealt from a queue.  Enough
-    walkers for a whole-range wave and a sliced part (782 groups of 512), a launch long enough to be sliced (4 slices, the
+    walkers for a whole-range wave and a sliced part (782 groups of 512), a launch long enough to be sliced (3 slices, the
     last one ragged, odd step count): the same run with RMS_RUN_NO_SLICES must end in the same place, fp32 and fp64,
     impermeable and permeable (whose relaxation sums are added slice by slice: fp32 rounding), octant and dictionary
     lattice; and the sliced permeable run holds north_star's tolerances against the oracle."""
     NO_SLICES, DICT = rms.binding.RMS_RUN_NO_SLICES, rms.binding.RMS_LATTICE_DICT
     n = 400_001
     c2, c3 = ri.make_config("cfg2", "test"), ri.make_config("cfg3", "test")
-    seq = ri.pgse_sequence(2e-4, 4101, 0.2, 0.5, np.linspace(0.0, 4.0, 4), ri.fibonacci_dirs(6), snap_steps=[4101])
+    seq = ri.pgse_sequence(2e-4, 6301, 0.3, 0.8, np.linspace(0.0, 4.0, 4), ri.fibonacci_dirs(6), snap_steps=[6301])
     for name, sub in (("cfg2", c2.substrate), ("cfg3", c3.substrate)):
         for flags in (0, 8):
             for sf in (0, DICT):
