@@ -287,6 +287,10 @@ struct rms_step_params {
     // sched = device [1 + n_sliced], zeroed before the launch.  n_slices <= 1: one block per group.
     uint32_t n_slices, slice_len, n_whole, n_sliced;
     uint32_t* sched;
+    // four constants of the direction arithmetic, read as constant-bank operands: written as literals, the compiler has to
+    // move each into a register again at every step (instructions with two constants) -- 4 of ~120 instructions per step
+    uint32_t k_hi7f, k_tau_or;   // 0x7F, 0x3F800080
+    float k_two, k_sin3;         // 2.0f, -2.4641574e-06f
 };
 // fills in the time-slice fields of p for its n walkers x n_steps (n_slices = 0: none); *sched_words = size of p.sched
 void rms_fast_slices(rms_step_params* p, size_t* sched_words);

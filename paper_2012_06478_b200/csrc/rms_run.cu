@@ -374,6 +374,7 @@ extern "C" int rms_run(const rms_substrate* s, rms_walkers* w, const rms_run_des
     sp.nx = s->nx; sp.ny = s->ny; sp.nz = s->nz;
     sp.labels = s->d_labels; sp.nbr = s->d_nbr; sp.oct = s->d_oct;
     sp.code = s->d_code; sp.dict = s->d_dict; sp.esc = s->d_esc; sp.esc_mask = s->esc_mask;
+    sp.k_hi7f = 0x7Fu; sp.k_tau_or = 0x3F800080u; sp.k_two = 2.0f; sp.k_sin3 = -2.4641574e-06f;
     if (use_fast) {
         rc = rms_fast_luts(&sp.lut1, &sp.lut2);
         if (rc != RMS_OK) return rc;
