@@ -67,6 +67,9 @@ def parse_args():
     ap.add_argument("--substrate", default="cfg4", choices=["cfg4", "cfg3"],
                     help="cfg3: the permeable, D- and T2-contrast variant of the lattice with walkers in every label (not the headline)")
     ap.add_argument("--fp64", action="store_true", help="RMS_RUN_FP64: the step kernel in fp64 arithmetic (not the headline)")
+    ap.add_argument("--interaction", default="ec", choices=["ec", "rs", "erl"],
+                    help="membrane interaction: elastic collision (the method, the headline), rejection sampling, equal-step-length random leap")
+    ap.add_argument("--general-kernel", action="store_true", help="RMS_RUN_GENERAL_KERNEL (diagnostic)")
     ap.add_argument("--no-slices", action="store_true", help="RMS_RUN_NO_SLICES: one block per group of walkers for the whole launch (diagnostic)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -195,7 +198,8 @@ def workload_config(args, cfg, extra=None):
          "intra_fraction": round(cfg.substrate.meta.get("intra_fraction", 0.0), 4),
          "walkers_per_gpu": args.walkers, "mc_steps": args.mc_steps, "dt_ms": cfg.sequence.dt_ms,
          "directions": int(cfg.sequence.dirs.shape[0]), "b_values": int(cfg.sequence.gamp.shape[1]),
-         "lattice_path": args.lattice, "layout": args.layout, "lattice_format": args.lattice_format, "pass": "rms_substrate_create + rms_walkers_init + rms_run",
+         "lattice_path": args.lattice, "layout": args.layout, "lattice_format": args.lattice_format,
+         "interaction": args.interaction, "pass": "rms_substrate_create + rms_walkers_init + rms_run",
          "l2": "inputs larger than L2 (label lattice 1.0 GB + octant lattice 4.0 GB vs 126 MB L2)" if args.scale == "full"
          else "reduced test lattice (fits L2) -- not a valid bench configuration"}
     if extra:
@@ -308,6 +312,9 @@ def main():
         flags |= rms.binding.RMS_RUN_FP64
     if args.no_slices:
         flags |= rms.binding.RMS_RUN_NO_SLICES
+    if args.general_kernel:
+        flags |= rms.binding.RMS_RUN_GENERAL_KERNEL
+    flags |= {"ec": 0, "rs": rms.binding.RMS_RUN_REJECTION_SAMPLING, "erl": rms.binding.RMS_RUN_ERL}[args.interaction]
     sflags = {"auto": rms.binding.RMS_LAYOUT_AUTO, "x": rms.binding.RMS_LAYOUT_X_FASTEST, "z": rms.binding.RMS_LAYOUT_Z_FASTEST}[args.layout]
     if args.lattice_format == "dict":
         sflags |= rms.binding.RMS_LATTICE_DICT
@@ -384,7 +391,8 @@ def main():
     peak_ginstr = N_SM * LANES_PER_SM * sm_mhz * 1e6 / 1e9
     k_ms_per_launch = kernel_ms / args.steps
     achieved_ginstr = ALGORITHMIC_INSTR_PER_STEP * n_walkers * mc_steps / (k_ms_per_launch * 1e-3) / 1e9
-    cap = NCU_CAPTURES.get((args.substrate, args.lattice, args.layout, args.lattice_format, n_walkers, mc_steps, bool(args.fp64))) if args.waves == 1 else None
+    cap = NCU_CAPTURES.get((args.substrate, args.lattice, args.layout, args.lattice_format, n_walkers, mc_steps, bool(args.fp64))) \
+        if args.waves == 1 and args.interaction == "ec" and not args.no_slices and not args.general_kernel else None
     traffic = cap["bytes"] if cap else None
     roofline = {"bound": "alu", "kernel": "rms_step_fast_kernel" if args.lattice == "facemask" else "rms_step_kernel",
                 "achieved": achieved_ginstr, "peak": peak_ginstr,

@@ -189,9 +189,9 @@ int rms_substrate_label_volumes_static(const rms_substrate* s, void* cuda_stream
  *             RMS_RUN_ERL: equal-step-length random leap, the paper's third comparison interaction (PAPER.md lines 80,
  *             340, Appendix A): a step that meets a membrane is cancelled and tried again in a new direction until it
  *             meets none (at most 4095 retries, then the walker stays put for the step).  Impermeable, non-absorbing
- *             membranes only (kappa 0 or +inf, no rho: RMS_ERR_UNSUPPORTED otherwise).  General kernels; depletes the
+ *             membranes only (kappa 0 or +inf, no rho: RMS_ERR_UNSUPPORTED otherwise).  Runs in the specialised kernel
+ *             (piecewise-constant waveforms, kappa 0 everywhere; fp32 or fp64) or the general ones; depletes the
  *             density within a hop length of the membranes (Eq.A.1), hence not the default.
- *
  *             RMS_RUN_NO_SLICES: a launch of the specialised kernel over more walkers than the GPU holds at a time is cut into
  *             time slices of ~1000 steps that are dealt to the SMs from a queue, so that the SMs do not idle while the last
  *             blocks finish (results do not depend on it beyond the order of the fp64 phase additions); this flag keeps one

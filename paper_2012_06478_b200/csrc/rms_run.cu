@@ -189,8 +189,9 @@ extern "C" int rms_run(const rms_substrate* s, rms_walkers* w, const rms_run_des
     const uint32_t t_ceil_P = (uint32_t)ceilf(t_max);
     // absorbing membranes: the saturation draw belongs to every membrane met, so every such step is redone (t_ceil = 512)
     const uint32_t t_ceil = mt ? 512u : t_ceil_P;
-    // (rejection sampling too: the specialised kernel cancels a step at its first uncrossed membrane; ERL stays on the general ones)
-    const bool fast_permeable = permeable && !erl && (s->d_oct || s->d_code) && !want_labels && t_ceil <= RMS_FAST_PERM_TCEIL;
+    // (rejection sampling and ERL too: the specialised kernel cancels a step at its first uncrossed membrane and, for ERL, tries again)
+    const bool fast_permeable = permeable && (s->d_oct || s->d_code) && !want_labels && t_ceil <= RMS_FAST_PERM_TCEIL &&
+                                !(erl && t_ceil_P > 0u);     // ERL across kappa = inf faces: every step would take the fp32 side path
 
     const int nWk = rms_kernel_waves(nW);        // waveforms the step kernel is compiled for; the extra ones carry zero weight
     rc = rms_walkers_reserve_waves(w, nWk, stream);

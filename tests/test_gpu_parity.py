@@ -756,19 +756,22 @@ def test_equal_step_length_random_leap_interaction(rms):
     seq = ri.pgse_sequence(2e-4, 1500, 0.1, 0.15, [0.0, 2.0], np.eye(3), snap_steps=[500, 1500])
     o = oracle_run(cyl, seq, n, 95, interaction=2)
     assert np.abs(o["S"] - oracle_run(cyl, seq, n, 95, interaction=1)["S"]).max() > 1e-3       # not rejection sampling
-    for flags in (ERL, ERL | 8):
+    # the specialised kernel (fp32, fp64 directions) and, with RMS_RUN_GENERAL_KERNEL = 2, the general ones
+    ALL = (ERL, ERL | 8, ERL | 2, ERL | 2 | 8)
+    for flags in ALL:
         g = gpu_run(cyl, seq, n, 95, flags=flags)
         print("ERL, cylinder, flags", flags, compare(g, o, n))
-        assert g["n_encounters"] == o["n_encounters"] or flags == ERL
+        assert g["n_encounters"] == o["n_encounters"] or not (flags & 8)
     seq_f = dataclasses.replace(seq, wave=(seq.wave * 0.37).astype(np.float32))
     o = oracle_run(cyl, seq_f, n, 96, interaction=2)
-    for flags in (ERL, ERL | 8):
+    for flags in ALL:
         print("ERL, non-integer waveform, flags", flags, compare(gpu_run(cyl, seq_f, n, 96, flags=flags), o, n))
     cfg = ri.make_config("cfg2", "test")
     seq_a = dataclasses.replace(cfg.sequence)
     o = oracle_run(cfg.substrate, seq_a, 100_000, 97, interaction=2)
-    for flags in (ERL, ERL | 8):
+    for flags in ALL:
         print("ERL, axons, flags", flags, compare(gpu_run(cfg.substrate, seq_a, 100_000, 97, flags=flags), o, 100_000))
+    print("ERL, axons, dictionary lattice", compare(gpu_run(cfg.substrate, seq_a, 100_000, 97, flags=ERL, substrate_flags=rms.binding.RMS_LATTICE_DICT), o, 100_000))
     hop = 0.9 ** 2 * 0.01 / (6 * 2e-4)
     rl = ri.random_lattice((12, 11, 10), n_labels=4, seed=9, D_extra=hop, D_intra=hop, place="all")
     kap = np.zeros((4, 4), np.float32); kap[0, 1] = kap[1, 0] = np.inf; kap[2, 3] = kap[3, 2] = np.inf
@@ -776,6 +779,7 @@ def test_equal_step_length_random_leap_interaction(rms):
     seq_r = ri.pgse_sequence(2e-4, 400, 0.02, 0.04, [0.0, 20.0], np.eye(3), snap_steps=[400])
     o = oracle_run(rl, seq_r, n, 98, interaction=2)
     assert o["n_permeations"] > 1000 and o["n_encounters"] > 5 * n * 400 // 10
+    # (with kappa = inf pairs ERL stays on the general kernels: the specialised one would redo every step in its fp32 side path)
     for flags in (ERL, ERL | 8):
         g = gpu_run(rl, seq_r, n, 98, flags=flags)
         rep = compare(g, o, n)
