@@ -176,7 +176,8 @@ int rms_substrate_label_volumes_static(const rms_substrate* s, void* cuda_stream
  *             additions), hit order and phase in fp64, for runs of more than a few 1e4 steps whose trajectories must
  *             stay on those of an fp64 reference (DESIGN.md "Tolerances" says why fp32 directions cannot).  Three
  *             quarters of the fp32 speed wherever the specialised kernel runs (piecewise-constant waveforms;
- *             impermeable, permeable, absorbing, rejection sampling); a plain, slower kernel otherwise.
+ *             impermeable, permeable with P << 1, rejection sampling, ERL between walls); a plain, slower fp64 kernel
+ *             otherwise (general waveforms, label gathers, absorbing membranes, faces with P = 1).
  *             RMS_RUN_NO_ORDERING: on large lattices the walkers are dealt to the threads in the order of the
  *             lattice cell they sit in (cache locality; results do not depend on it); this flag keeps id order.
  *             RMS_RUN_REJECTION_SAMPLING: the paper's other membrane interaction (Appendix B): a

@@ -190,8 +190,14 @@ extern "C" int rms_run(const rms_substrate* s, rms_walkers* w, const rms_run_des
     // absorbing membranes: the saturation draw belongs to every membrane met, so every such step is redone (t_ceil = 512)
     const uint32_t t_ceil = mt ? 512u : t_ceil_P;
     // (rejection sampling and ERL too: the specialised kernel cancels a step at its first uncrossed membrane and, for ERL, tries again)
+    // RMS_RUN_FP64: the specialised kernel with fp64 directions and 2^-63 fixed-point offsets serves every run it serves in fp32
+    // (piecewise-constant waveforms; impermeable, permeable), the general fp64 kernel (table-driven waveforms, label gathers)
+    // everything else
+    const bool fp64 = (d->flags & RMS_RUN_FP64) != 0;
+    // Where every step that meets a membrane takes the specialised kernel's side path (absorbing membranes, faces with P = 1),
+    // fp64 runs go to the general fp64 kernel: that path works on fp32 offsets, and the trajectories would be fp32 ones.
     const bool fast_permeable = permeable && (s->d_oct || s->d_code) && !want_labels && t_ceil <= RMS_FAST_PERM_TCEIL &&
-                                !(erl && t_ceil_P > 0u);     // ERL across kappa = inf faces: every step would take the fp32 side path
+                                !(erl && t_ceil_P > 0u) && !(fp64 && t_ceil >= 512u);
 
     const int nWk = rms_kernel_waves(nW);        // waveforms the step kernel is compiled for; the extra ones carry zero weight
     rc = rms_walkers_reserve_waves(w, nWk, stream);
@@ -205,10 +211,6 @@ extern "C" int rms_run(const rms_substrate* s, rms_walkers* w, const rms_run_des
         double* S = &suf[(size_t)m * (nT + 1)];
         for (int64_t j = nT; j >= 1; --j) { acc += (double)d->wave[(size_t)m * nT + (j - 1)]; S[j - 1] = acc; }
     }
-    // RMS_RUN_FP64: the specialised kernel with fp64 directions and 2^-63 fixed-point offsets serves every run it serves in fp32
-    // (piecewise-constant waveforms; impermeable, permeable, absorbing), the general fp64 kernel (table-driven waveforms,
-    // label gathers, rejection sampling, ERL) everything else
-    const bool fp64 = (d->flags & RMS_RUN_FP64) != 0;
     // integer-valued waveforms: the general kernel's exact int32 path (CONST mode)
     bool int_mode = wave_is_integer(d->wave, (size_t)nW * nT);
     for (size_t i = 0; int_mode && i < suf.size(); ++i) int_mode = fabs(suf[i]) < 1048576.0;   // int32 event sums: <= 64 steps x 2^20 between flushes
