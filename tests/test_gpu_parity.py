@@ -390,6 +390,15 @@ def test_time_slices_of_the_specialised_kernel_leave_the_trajectories_alone(rms)
                 _same_trajectories(whole, sliced, (name, flags, sf), exact_relax=(name == "cfg2"))
                 if name == "cfg3" and flags == 0 and sf == 0:
                     print("sliced cfg3 against the oracle", compare(sliced, oracle_run(sub, seq, n, 11), n))
+    # two launches (a snapshot in the middle), both long enough to be sliced: the schedule is set up again for each; and
+    # the kernel variants that can cancel a step (rejection sampling, ERL), which carry more state over a slice boundary
+    seq2 = ri.pgse_sequence(2e-4, 9000, 0.4, 1.0, np.linspace(0.0, 4.0, 3), ri.fibonacci_dirs(3), snap_steps=[4500, 9000])
+    RS, ERL = rms.binding.RMS_RUN_REJECTION_SAMPLING, rms.binding.RMS_RUN_ERL
+    for flags in (0, 8, RS, ERL | 8):
+        whole = gpu_run(c2.substrate, seq2, n, 12, flags=flags | NO_SLICES)
+        sliced = gpu_run(c2.substrate, seq2, n, 12, flags=flags)
+        assert sliced["n_launches"] == whole["n_launches"]
+        _same_trajectories(whole, sliced, ("two launches", flags))
 
 
 @pytest.mark.parametrize("dict_cap", [None, "40", "3"], ids=["full_dictionary", "escapes", "gives_up"])
