@@ -187,7 +187,7 @@ template <bool ZFAST, bool OCT, bool DICT = false>
 __global__ void __launch_bounds__(128) rms_build_nbr_kernel(const uint16_t* __restrict__ labels, int nx, int ny, int nz,
                                                              typename rms_nbr_word<OCT, DICT>::type* __restrict__ nbr, int SX, int SY, int SZ,
                                                              int n_labels, unsigned long long* __restrict__ stats,
-                                                             const rms_dict_build dictb = rms_dict_build())
+                                                             const rms_dict_build dictb = rms_dict_build(), int z_chunk0 = 0)
 {
     typedef typename rms_nbr_word<OCT, DICT>::type WORD;
     __shared__ WORD tile[ZFAST ? 4 : 1][ZFAST ? 32 : 1][ZFAST ? 33 : 1];
@@ -214,7 +214,7 @@ __global__ void __launch_bounds__(128) rms_build_nbr_kernel(const uint16_t* __re
     const bool active = Xt < NX;
     const int X = active ? Xt : NX - 1;               // idle lanes of the last block shadow the last column (ZFAST needs whole warps)
     const int Y = blockIdx.y;
-    const int Z0 = blockIdx.z * RMS_NBR_ZCHUNK, Z1 = min(NZ, Z0 + RMS_NBR_ZCHUNK);
+    const int Z0 = ((int)blockIdx.z + z_chunk0) * RMS_NBR_ZCHUNK, Z1 = min(NZ, Z0 + RMS_NBR_ZCHUNK);   // (z_chunk0: a launch per chunk)
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     unsigned n_faces = 0, bad = 0;
     if (ZFAST || active) {
@@ -329,6 +329,27 @@ __global__ void __launch_bounds__(256) rms_check_labels_kernel(const uint16_t* _
     if ((threadIdx.x & 31) == 0 && bad) atomicAdd(&stats[1], (unsigned long long)bad);
 }
 
+#define RMS_UPLOAD_SLABS 8
+// the stream the slabs of a large host lattice are uploaded on, one per device, kept for the life of the process
+static int rms_copy_stream(cudaStream_t* out)
+{
+    static std::mutex mu;
+    static cudaStream_t streams[64] = {nullptr};
+    int dev = -1;
+    RMS_CUDA_TRY(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= 64) return RMS_ERR_UNSUPPORTED;
+    std::lock_guard<std::mutex> lock(mu);
+    if (!streams[dev]) RMS_CUDA_TRY(cudaStreamCreateWithFlags(&streams[dev], cudaStreamNonBlocking));
+    *out = streams[dev];
+    return RMS_OK;
+}
+static void rms_destroy_events(cudaEvent_t ev_start, cudaEvent_t* ev_slab)
+{
+    if (ev_start) cudaEventDestroy(ev_start);
+    for (int k = 0; k < RMS_UPLOAD_SLABS; ++k)
+        if (ev_slab[k]) cudaEventDestroy(ev_slab[k]);
+}
+
 extern "C" int rms_substrate_create(const rms_substrate_desc* d, void* cuda_stream, rms_substrate** out)
 {
     RMS_REQUIRE(d && out, RMS_ERR_ARG, "rms_substrate_create: null descriptor or output");
@@ -393,6 +414,9 @@ extern "C" int rms_substrate_create(const rms_substrate_desc* d, void* cuda_stre
     int rc = RMS_OK;
     unsigned long long* d_stats = nullptr;
     unsigned long long* d_hash = nullptr;              // the dictionary build's hash table and counters
+    bool piped = false;                                // the labels arrive in slabs (below)
+    cudaStream_t copy_stream = nullptr;
+    cudaEvent_t ev_start = nullptr, ev_slab[RMS_UPLOAD_SLABS] = {nullptr};
     unsigned long long h_stats[5] = {0, 0, 0, 0, 0};   // membrane faces, bad labels, sampled faces with normal x, y, z
 #define SUB_TRY(expr)                                                                                    \
     do {                                                                                                 \
@@ -412,8 +436,27 @@ extern "C" int rms_substrate_create(const rms_substrate_desc* d, void* cuda_stre
         SUB_TRY(rms_malloc((void**)&buf, n_vox * sizeof(uint16_t)));
         s->d_labels = buf;
         s->owns_labels = true;
-        SUB_TRY(cudaMemcpyAsync(buf, d->labels, n_vox * sizeof(uint16_t),
-                                (d->flags & RMS_LABELS_ON_DEVICE) ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice, stream));
+        // Host labels of a large lattice: uploaded in slabs of z-planes on a stream of the library's own, an event behind each,
+        // so that the build below works on the planes that have arrived while the rest is still on the bus (pinned host
+        // memory; from pageable memory the copies simply do not overlap anything)
+        piped = !(d->flags & (RMS_LABELS_ON_DEVICE | RMS_NO_BRICKS | RMS_LATTICE_DICT)) && d->nz >= 4 * RMS_NBR_ZCHUNK && n_vox >= (1u << 20) &&
+                rms_copy_stream(&copy_stream) == RMS_OK;
+        if (piped) {
+            const size_t plane = (size_t)d->nx * d->ny;
+            SUB_TRY(cudaEventCreateWithFlags(&ev_start, cudaEventDisableTiming));
+            SUB_TRY(cudaEventRecord(ev_start, stream));
+            SUB_TRY(cudaStreamWaitEvent(copy_stream, ev_start, 0));
+            for (int k = 0; k < RMS_UPLOAD_SLABS; ++k) {
+                const int za = (int)((long long)d->nz * k / RMS_UPLOAD_SLABS), zb = (int)((long long)d->nz * (k + 1) / RMS_UPLOAD_SLABS);
+                SUB_TRY(cudaMemcpyAsync(buf + za * plane, d->labels + za * plane, (size_t)(zb - za) * plane * sizeof(uint16_t),
+                                        cudaMemcpyHostToDevice, copy_stream));
+                SUB_TRY(cudaEventCreateWithFlags(&ev_slab[k], cudaEventDisableTiming));
+                SUB_TRY(cudaEventRecord(ev_slab[k], copy_stream));
+            }
+        } else {
+            SUB_TRY(cudaMemcpyAsync(buf, d->labels, n_vox * sizeof(uint16_t),
+                                    (d->flags & RMS_LABELS_ON_DEVICE) ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice, stream));
+        }
     }
     {
         uint16_t* lc = nullptr;
@@ -442,7 +485,10 @@ extern "C" int rms_substrate_create(const rms_substrate_desc* d, void* cuda_stre
         bool zfast = (d->flags & RMS_LAYOUT_AUTO) == RMS_LAYOUT_Z_FASTEST;
         if ((d->flags & RMS_LAYOUT_AUTO) == RMS_LAYOUT_AUTO) {
             const int sy = s->ny >= 256 ? 8 : (s->ny >= 64 ? 4 : 1), sz = s->nz >= 256 ? 8 : (s->nz >= 64 ? 4 : 1);
-            rms_sample_faces_kernel<<<148 * 4, 256, 0, stream>>>(s->d_labels, s->nx, s->ny, s->nz, sy, sz, d_stats + 2);
+            // (labels arriving in slabs: the first slab decides)
+            if (piped) SUB_TRY(cudaStreamWaitEvent(stream, ev_slab[0], 0));
+            const int nz_sample = piped ? s->nz / RMS_UPLOAD_SLABS : s->nz;
+            rms_sample_faces_kernel<<<148 * 4, 256, 0, stream>>>(s->d_labels, s->nx, s->ny, nz_sample, sy, sz, d_stats + 2);
             SUB_TRY(cudaGetLastError());
             SUB_TRY(cudaMemcpyAsync(h_stats + 2, d_stats + 2, 3 * sizeof(unsigned long long), cudaMemcpyDeviceToHost, stream));
             SUB_TRY(cudaStreamSynchronize(stream));
@@ -499,7 +545,22 @@ extern "C" int rms_substrate_create(const rms_substrate_desc* d, void* cuda_stre
         if (!have_dict) {
             SUB_TRY(rms_malloc((void**)&s->d_oct_alloc, (n_pad + 2 * s->oct_margin) * sizeof(uint2)));
             s->d_oct = s->d_oct_alloc + s->oct_margin;
-            if (zfast)
+            if (piped) {
+                // one launch per chunk of 128 padded planes, each behind the slab that holds the last plane it reads; chunk 0
+                // reads the periodic image of the last plane and goes last
+                const dim3 grid1(grid.x, grid.y, 1);
+                for (int cc = 1; cc <= (int)grid.z; ++cc) {
+                    const int c = cc % (int)grid.z;
+                    const int z_hi = c == 0 ? s->nz - 1 : std::min(s->nz - 1, c * RMS_NBR_ZCHUNK + RMS_NBR_ZCHUNK - 1);
+                    int k = 0;
+                    while ((int)((long long)s->nz * (k + 1) / RMS_UPLOAD_SLABS) <= z_hi) ++k;
+                    SUB_TRY(cudaStreamWaitEvent(stream, ev_slab[k], 0));
+                    if (zfast)
+                        rms_build_nbr_kernel<true, true><<<grid1, 128, 0, stream>>>(s->d_labels, s->nx, s->ny, s->nz, s->d_oct, s->SX, s->SY, s->SZ, nL, d_stats, rms_dict_build(), c);
+                    else
+                        rms_build_nbr_kernel<false, true><<<grid1, 128, 0, stream>>>(s->d_labels, s->nx, s->ny, s->nz, s->d_oct, s->SX, s->SY, s->SZ, nL, d_stats, rms_dict_build(), c);
+                }
+            } else if (zfast)
                 rms_build_nbr_kernel<true, true><<<grid, 128, 0, stream>>>(s->d_labels, s->nx, s->ny, s->nz, s->d_oct, s->SX, s->SY, s->SZ, nL, d_stats);
             else
                 rms_build_nbr_kernel<false, true><<<grid, 128, 0, stream>>>(s->d_labels, s->nx, s->ny, s->nz, s->d_oct, s->SX, s->SY, s->SZ, nL, d_stats);
@@ -519,9 +580,12 @@ extern "C" int rms_substrate_create(const rms_substrate_desc* d, void* cuda_stre
         goto fail;
     }
     s->n_membrane_faces = h_stats[0];
+    rms_destroy_events(ev_start, ev_slab);
     *out = s;
     return RMS_OK;
 fail:
+    if (piped) cudaStreamSynchronize(copy_stream);     // nothing of ours may still be writing into a block that is about to be freed
+    rms_destroy_events(ev_start, ev_slab);
     if (d_stats) rms_free(d_stats);
     if (d_hash) rms_free(d_hash);
     rms_substrate_destroy(s);

@@ -434,6 +434,29 @@ def test_dictionary_lattice_walks_the_trajectories_of_the_octant_lattice(rms, mo
     assert {None: seen == {"dictionary"}, "40": "escapes" in seen, "3": "octant" in seen}[dict_cap]
 
 
+def test_host_labels_uploaded_in_slabs_give_the_lattice_of_device_labels(rms):
+    """rms_substrate_create uploads the host labels of a large lattice in slabs of z-planes on a stream of its own and builds
+    the octant lattice chunk by chunk behind them.  The full axon lattice from host memory (pageable and pinned), in both
+    memory orders and with RMS_LAYOUT_AUTO (decided on the first slab then), against the same lattice adopted from device
+    memory: same membrane count, same trajectories (walkers over the whole box, enough steps to cross faces everywhere)."""
+    import torch
+    cfg = ri.make_config("cfg4", "full")
+    sub = cfg.substrate
+    seq = ri.pgse_sequence(2e-4, 300, 0.01, 0.03, [0.0, 1.0], np.eye(3), snap_steps=[300])
+    n = 200_000
+    labels_dev = torch.from_numpy(sub.labels.view(np.int16)).cuda()
+    pinned = torch.from_numpy(sub.labels.view(np.int16)).pin_memory()
+    import dataclasses
+    sub_pinned = dataclasses.replace(sub, labels=pinned.numpy().view(np.uint16))
+    for layout in (rms.binding.RMS_LAYOUT_X_FASTEST, rms.binding.RMS_LAYOUT_Z_FASTEST, rms.binding.RMS_LAYOUT_AUTO):
+        ref = rms.simulate(sub, seq, n, 3, device_labels=labels_dev, read_walkers=True, substrate_flags=layout)
+        for name, s_host in (("pageable", sub), ("pinned", sub_pinned)):
+            g = rms.simulate(s_host, seq, n, 3, read_walkers=True, substrate_flags=layout)
+            assert g["substrate_info"]["n_membrane_faces"] == ref["substrate_info"]["n_membrane_faces"], (layout, name)
+            _same_trajectories(ref, g, (layout, name))
+    assert ref["n_encounters"] > 100_000
+
+
 def test_general_kernel_and_id_order_agree_with_the_specialised_path(rms):
     # same inputs through the general step kernel and without spatial ordering: identical physics, so the results
     # agree with the oracle under the same tolerances, and with each other to rounding
