@@ -256,7 +256,7 @@ struct rms_step_params {
     const uint4* esc;
     uint32_t esc_mask;
     const uint32_t* lut1;     // device, [1024]: interaction outcome by (octant byte >> 1, faces reached); rms_step_fast.cu
-    const uint32_t* lut2;     // device, [8192]: the same with the hit order, for the entries lut1 marks order dependent
+    const uint16_t* lut2;     // device, [240 * 8]: the outcomes by hit order of the entries lut1 marks order dependent
     int NX, NY;               // padded dims of the neighbourhood lattice
     int SX, SY, SZ;           // its strides: index = X SX + Y SY + Z SZ; SX == 1 (x fastest) or SZ == 1 (z fastest)
     rms_walker_arrays st;
@@ -299,7 +299,7 @@ int rms_launch_step(const rms_step_params& p, int n_wave, int wmode, int lat, bo
 // RMS_LAT_FACES + RMS_WMODE_CONST only; permeable: P(a->b) << 1 expected (rms_step_fast.cu)
 int rms_launch_step_fast(const rms_step_params& p, int n_wave, bool permeable, bool fp64, cudaStream_t stream);
 // the two look-up tables of the specialised kernel (constants of the method, built once per device)
-int rms_fast_luts(const uint32_t** d_lut1, const uint32_t** d_lut2);
+int rms_fast_luts(const uint32_t** d_lut1, const uint16_t** d_lut2);
 // builds rms_substrate::d_nbr if it is not there yet (needs d_labels); rms_substrate.cu
 int rms_substrate_ensure_nbr(const rms_substrate* s, cudaStream_t stream);
 // fp64, everything else: permeable / variable D / any waveform, RMS_WMODE_TABLE data, label gathers (rms_step_precise_general.cu)
