@@ -40,8 +40,8 @@ N_SM, LANES_PER_SM = 148, 128          # B200: 4 schedulers x 32 lanes per SM, o
 # key: (substrate, lattice, layout, lattice_format, walkers, mc_steps, fp64)
 NCU_CAPTURES = {
     # RMS_LAYOUT_AUTO picks z fastest on this lattice: the two keys name the same launch
-    ("cfg4", "facemask", "auto", "oct", 1_000_000, 10_000, False): {"bytes": 40.33e9, "source": "profiles/r2i_step_fast_ncu.md (39.42 GB read + 0.90 GB written)"},
-    ("cfg4", "facemask", "z", "oct", 1_000_000, 10_000, False): {"bytes": 40.33e9, "source": "profiles/r2i_step_fast_ncu.md (39.42 GB read + 0.90 GB written)"},
+    ("cfg4", "facemask", "auto", "oct", 1_000_000, 10_000, False): {"bytes": 40.94e9, "source": "profiles/r2j_step_fast_ncu.md (40.04 GB read + 0.91 GB written)"},
+    ("cfg4", "facemask", "z", "oct", 1_000_000, 10_000, False): {"bytes": 40.94e9, "source": "profiles/r2j_step_fast_ncu.md (40.04 GB read + 0.91 GB written)"},
     ("cfg4", "facemask", "auto", "dict", 1_000_000, 10_000, False): {"bytes": 10.12e9, "source": "profiles/r2f_r2g_step_fast_ncu.md, capture g (8.81 GB read + 1.31 GB written)"},
     ("cfg4", "facemask", "z", "dict", 1_000_000, 10_000, False): {"bytes": 10.12e9, "source": "profiles/r2f_r2g_step_fast_ncu.md, capture g (8.81 GB read + 1.31 GB written)"},
 }
