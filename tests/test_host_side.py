@@ -131,3 +131,18 @@ def test_allreduce_of_two_shards_over_gloo_equals_the_merged_job(rms, tmp_path):
             assert np.allclose(got[k], ref[k], rtol=1e-13), k
         assert np.array_equal(got["class_flow"], ref["class_flow"])
         assert int(got["n_encounters"]) == 21 and int(got["n_permeations"]) == 1 and int(got["n_saturations"]) == 3
+
+
+def test_fixed_codes_of_the_dictionary_lattice(tmp_path):
+    """RMS_LATTICE_DICT gives interior and prismatic neighbourhoods (and their ghost variants) codes that need no search
+    (csrc/rms_internal.cuh: rms_fixed_code / rms_fixed_word).  The host-only program tests/cuda/fixed_codes_host.cu checks that
+    every fixed code and its 27-bit word map onto each other, that a word gets a code exactly when it does not change along a
+    lattice axis (4e6 pseudo-random words, every z-invariant word), and the two interior codes."""
+    import shutil
+    import subprocess
+    if shutil.which("nvcc") is None:
+        pytest.skip("nvcc not on PATH")
+    exe = tmp_path / "fixed_codes_host"
+    subprocess.run(["nvcc", "-std=c++17", "-O1", "-Wno-deprecated-gpu-targets", "-o", str(exe), str(ROOT / "tests" / "cuda" / "fixed_codes_host.cu")], check=True)
+    out = subprocess.run([str(exe)], capture_output=True, text=True)
+    assert out.returncode == 0 and out.stdout.split()[:4] == ["bad", "0", "fixed", "1538"], out.stdout
