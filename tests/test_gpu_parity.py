@@ -455,6 +455,14 @@ def test_host_labels_uploaded_in_slabs_give_the_lattice_of_device_labels(rms):
             assert g["substrate_info"]["n_membrane_faces"] == ref["substrate_info"]["n_membrane_faces"], (layout, name)
             _same_trajectories(ref, g, (layout, name))
     assert ref["n_encounters"] > 100_000
+    # a narrow box whose plane count is no multiple of the slab or chunk sizes (one block per row, ragged last chunk and slab)
+    small = ri.random_lattice((40, 30, 1100 + 37), n_labels=3, seed=21, place="all")
+    dev = torch.from_numpy(small.labels.view(np.int16)).cuda()
+    for layout in (rms.binding.RMS_LAYOUT_X_FASTEST, rms.binding.RMS_LAYOUT_Z_FASTEST, rms.binding.RMS_LAYOUT_AUTO):
+        ref = rms.simulate(small, seq, 50_000, 4, device_labels=dev, read_walkers=True, substrate_flags=layout)
+        g = rms.simulate(small, seq, 50_000, 4, read_walkers=True, substrate_flags=layout)
+        assert g["substrate_info"]["n_membrane_faces"] == ref["substrate_info"]["n_membrane_faces"]
+        _same_trajectories(ref, g, ("narrow box", layout))
 
 
 def test_general_kernel_and_id_order_agree_with_the_specialised_path(rms):
