@@ -83,7 +83,8 @@ typedef struct rms_walkers rms_walkers;     /* opaque */
 #define RMS_LAYOUT_AUTO 24u       /* x or z, whichever axis has fewer membrane faces normal to it (sampled)              */
 #define RMS_LATTICE_DICT 32u      /* store a 16-bit code per voxel and the octant words of the distinct neighbourhoods in a
                                      dictionary (2 bytes per voxel instead of 8: a quarter of the cache footprint of a walker;
-                                     one more, dependent, look-up per face reached).  Lattices with more distinct
+                                     one more, dependent, look-up per face reached; same speed on the axon lattice, a
+                                     build a third longer).  Lattices with more distinct
                                      neighbourhoods than the tables hold (independent random labels) get the octant lattice. */
 
 typedef struct {

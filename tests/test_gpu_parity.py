@@ -454,6 +454,10 @@ def test_host_labels_uploaded_in_slabs_give_the_lattice_of_device_labels(rms):
             g = rms.simulate(s_host, seq, n, 3, read_walkers=True, substrate_flags=layout)
             assert g["substrate_info"]["n_membrane_faces"] == ref["substrate_info"]["n_membrane_faces"], (layout, name)
             _same_trajectories(ref, g, (layout, name))
+        # the dictionary lattice is built behind the slabs in the same way
+        g = rms.simulate(sub_pinned, seq, n, 3, read_walkers=True, substrate_flags=layout | rms.binding.RMS_LATTICE_DICT)
+        assert g["substrate_info"]["dict_entries"] > 60_000 and g["substrate_info"]["n_membrane_faces"] == ref["substrate_info"]["n_membrane_faces"]
+        _same_trajectories(ref, g, (layout, "dictionary lattice, pinned"))
     assert ref["n_encounters"] > 100_000
     # a narrow box whose plane count is no multiple of the slab or chunk sizes (one block per row, ragged last chunk and slab)
     small = ri.random_lattice((40, 30, 1100 + 37), n_labels=3, seed=21, place="all")
