@@ -341,7 +341,7 @@ def test_error_codes(rms):
 def test_full_size_bench_workload_against_the_oracle(rms):
     """The workload bench.py times, whole: cfg4 point on the full 500x500x2000 axon lattice, 1e6 walkers x 10,000
     steps, 60 directions x 11 b-values, in bench.py's launch configuration (device-resident labels, specialised
-    kernel, spatial ordering, RMS_LAYOUT_AUTO as bench.py's default --layout auto), against the oracle run on every one of
+    kernel, spatial ordering, RMS_LAYOUT_AUTO | RMS_LATTICE_DICT as bench.py's defaults), against the oracle run on every one of
     those walkers (about a minute of host time).
     Plain north_star tolerances: >= 99.9 % same final voxel, |dS| <= 1e-4 for all 660 (b, direction), moments 1e-4."""
     import torch
@@ -349,7 +349,8 @@ def test_full_size_bench_workload_against_the_oracle(rms):
     n = cfg.n_walkers
     labels_dev = torch.from_numpy(cfg.substrate.labels.view(np.int16)).cuda()
     g = rms.simulate(cfg.substrate, cfg.sequence, n, cfg.seed, device_labels=labels_dev, read_walkers=True,
-                     substrate_flags=rms.binding.RMS_LAYOUT_AUTO)
+                     substrate_flags=rms.binding.RMS_LAYOUT_AUTO | rms.binding.RMS_LATTICE_DICT)
+    assert g["substrate_info"]["dict_entries"] > 60_000
     o = oracle_run(cfg.substrate, cfg.sequence, n, cfg.seed)
     rep = compare(g, o, n)
     print("full-size cfg4", rep)
