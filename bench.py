@@ -42,8 +42,8 @@ NCU_CAPTURES = {
     # RMS_LAYOUT_AUTO picks z fastest on this lattice: the two keys name the same launch
     ("cfg4", "facemask", "auto", "oct", 1_000_000, 10_000, False): {"bytes": 40.94e9, "source": "profiles/r2j_step_fast_ncu.md (40.04 GB read + 0.91 GB written)"},
     ("cfg4", "facemask", "z", "oct", 1_000_000, 10_000, False): {"bytes": 40.94e9, "source": "profiles/r2j_step_fast_ncu.md (40.04 GB read + 0.91 GB written)"},
-    ("cfg4", "facemask", "auto", "dict", 1_000_000, 10_000, False): {"bytes": 6.74e9, "source": "profiles/r2k_step_fast_dict_ncu.md (5.91 GB read + 0.84 GB written)"},
-    ("cfg4", "facemask", "z", "dict", 1_000_000, 10_000, False): {"bytes": 6.74e9, "source": "profiles/r2k_step_fast_dict_ncu.md (5.91 GB read + 0.84 GB written)"},
+    ("cfg4", "facemask", "auto", "dict", 1_000_000, 10_000, False): {"bytes": 6.93e9, "source": "profiles/r2k_step_fast_dict_ncu.md (6.09 GB read + 0.84 GB written)"},
+    ("cfg4", "facemask", "z", "dict", 1_000_000, 10_000, False): {"bytes": 6.93e9, "source": "profiles/r2k_step_fast_dict_ncu.md (6.09 GB read + 0.84 GB written)"},
 }
 
 
